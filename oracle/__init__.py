@@ -1,0 +1,216 @@
+"""CPU oracle for the LIETS-QSGS growth path -- TEST INFRASTRUCTURE ONLY.
+
+ctypes binding of ``oracle/liets_oracle.c`` (plain serial C written from PAPER.md; see the header
+for citations and pins).  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
+``cpu_baseline`` / ``--impl reference`` legs may import this package.  It imports nothing from
+``paper_2602_11734_b200`` and that package imports nothing from here.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "liets_oracle.c")
+_DEPS = [_SRC, os.path.join(_HERE, "liets_oracle.h"), os.path.join(_HERE, "liets_oracle_directions.inc")]
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+OK, FRONT_EMPTY, MAX_STEPS = 0, 1, 2
+
+
+def build(force=False):
+    """Compile liboracle.so with gcc -O2 (no SIMD intrinsics, no OpenMP: the oracle is serial)."""
+    if not force and os.path.exists(_LIB) and all(os.path.getmtime(_LIB) >= os.path.getmtime(d) for d in _DEPS):
+        return _LIB
+    subprocess.check_call(["gcc", "-O2", "-std=gnu99", "-Wall", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is not None:
+        return _lib
+    L = ctypes.CDLL(build())
+    u32, u64, i64, dbl, vp, ci = (ctypes.c_uint32, ctypes.c_uint64, ctypes.c_int64, ctypes.c_double,
+                                  ctypes.c_void_p, ctypes.c_int)
+    P = ctypes.POINTER
+    L.oracle_philox4x32_10.argtypes = [P(u32), P(u32), P(u32)]
+    L.oracle_philox4x32_10.restype = None
+    L.oracle_growth_draw.argtypes = [u64, u32, u64, ci]
+    L.oracle_growth_draw.restype = u32
+    L.oracle_seed_draw.argtypes = [u64, u64]
+    L.oracle_seed_draw.restype = u32
+    L.oracle_direction.argtypes = [ci, P(ci), P(ci), P(ci), P(ci)]
+    L.oracle_direction.restype = None
+    L.oracle_prob_to_threshold.argtypes = [dbl]
+    L.oracle_prob_to_threshold.restype = u64
+    L.oracle_target_count.argtypes = [dbl, u64]
+    L.oracle_target_count.restype = u64
+    L.oracle_step_threshold.argtypes = [u64, ci, u64, u64]
+    L.oracle_step_threshold.restype = u64
+    L.oracle_new.argtypes = [ci, ci, ci, ci]
+    L.oracle_new.restype = vp
+    L.oracle_free.argtypes = [vp]
+    L.oracle_free.restype = None
+    L.oracle_set_growth.argtypes = [vp, dbl, dbl, dbl, ci]
+    L.oracle_set_growth.restype = ci
+    L.oracle_set_target.argtypes = [vp, dbl]
+    L.oracle_set_target.restype = ci
+    L.oracle_seed.argtypes = [vp, dbl, ci, u64]
+    L.oracle_seed.restype = i64
+    L.oracle_seed_explicit.argtypes = [vp, P(u64), u64, u64]
+    L.oracle_seed_explicit.restype = i64
+    L.oracle_step_full.argtypes = [vp]
+    L.oracle_step_full.restype = ci
+    L.oracle_step_list.argtypes = [vp]
+    L.oracle_step_list.restype = ci
+    L.oracle_generate.argtypes = [vp, dbl, u32, ci, P(u32)]
+    L.oracle_generate.restype = ci
+    L.oracle_grid.argtypes = [vp]
+    L.oracle_grid.restype = P(ctypes.c_uint8)
+    for name in ("oracle_n_solid", "oracle_n_front_exact", "oracle_n_target"):
+        getattr(L, name).argtypes = [vp]
+        getattr(L, name).restype = u64
+    L.oracle_step_index.argtypes = [vp]
+    L.oracle_step_index.restype = u32
+    L.oracle_rates.argtypes = [vp, P(u64), P(u64)]
+    L.oracle_rates.restype = None
+    L.oracle_permute_front.argtypes = [vp, ci, u64]
+    L.oracle_permute_front.restype = None
+    L.oracle_s2.argtypes = [vp, ci, ci, ci, ci, ci, ci, P(u64), P(u64)]
+    L.oracle_s2.restype = None
+    _lib = L
+    return L
+
+
+def philox4x32_10(ctr, key):
+    c = (ctypes.c_uint32 * 4)(*ctr)
+    k = (ctypes.c_uint32 * 2)(*key)
+    o = (ctypes.c_uint32 * 4)()
+    lib().oracle_philox4x32_10(c, k, o)
+    return tuple(int(x) for x in o)
+
+
+def growth_draw(rng_seed, t, p, d):
+    return int(lib().oracle_growth_draw(rng_seed, t, p, d))
+
+
+def seed_draw(rng_seed, v):
+    return int(lib().oracle_seed_draw(rng_seed, v))
+
+
+def direction(d):
+    a, b, c, k = ctypes.c_int(), ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    lib().oracle_direction(d, a, b, c, k)
+    return a.value, b.value, c.value, k.value
+
+
+def prob_to_threshold(p):
+    return int(lib().oracle_prob_to_threshold(p))
+
+
+def target_count(phi, N):
+    return int(lib().oracle_target_count(phi, N))
+
+
+def step_threshold(R, law, n_t, n_solid):
+    return int(lib().oracle_step_threshold(R, law, n_t, n_solid))
+
+
+def s2(grid, periodic, axis, rmax):
+    """grid: uint8 array of shape (nz, ny, nx). Returns (pairs, valid) uint64 arrays of r = 0..rmax."""
+    g = np.ascontiguousarray(grid, dtype=np.uint8)
+    nz, ny, nx = g.shape
+    pairs = np.zeros(rmax + 1, dtype=np.uint64)
+    valid = np.zeros(rmax + 1, dtype=np.uint64)
+    P64 = ctypes.POINTER(ctypes.c_uint64)
+    lib().oracle_s2(g.ctypes.data, nx, ny, nz, int(periodic), axis, rmax,
+                    pairs.ctypes.data_as(P64), valid.ctypes.data_as(P64))
+    return pairs, valid
+
+
+class Oracle:
+    """One oracle run: create -> set_growth -> seed -> step/generate -> grid()."""
+
+    def __init__(self, nx, ny, nz, periodic=False):
+        self._L = lib()
+        self.nx, self.ny, self.nz, self.periodic = nx, ny, nz, bool(periodic)
+        self.N = nx * ny * nz
+        self._h = self._L.oracle_new(nx, ny, nz, int(periodic))
+        if not self._h:
+            raise ValueError("bad dimensions")
+
+    def close(self):
+        if self._h:
+            self._L.oracle_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        self.close()
+
+    def set_growth(self, g_face, g_edge, g_corner, law=1):
+        if self._L.oracle_set_growth(self._h, g_face, g_edge, g_corner, law):
+            raise ValueError("bad growth parameters")
+
+    def set_target(self, phi):
+        if self._L.oracle_set_target(self._h, phi):
+            raise ValueError("bad target")
+
+    def seed(self, core_prob, spacing_s, rng_seed):
+        n = self._L.oracle_seed(self._h, core_prob, spacing_s, rng_seed)
+        if n < 0:
+            raise ValueError("bad seed parameters")
+        return int(n)
+
+    def seed_explicit(self, idx, rng_seed=0):
+        a = np.ascontiguousarray(idx, dtype=np.uint64)
+        n = self._L.oracle_seed_explicit(self._h, a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)), a.size, rng_seed)
+        if n < 0:
+            raise ValueError("seed index out of range")
+        return int(n)
+
+    def step(self, use_list=True):
+        rc = self._L.oracle_step_list(self._h) if use_list else self._L.oracle_step_full(self._h)
+        if rc:
+            raise RuntimeError("oracle step: state error %d" % rc)
+
+    def generate(self, phi, max_steps=100000, use_list=True):
+        steps = ctypes.c_uint32(0)
+        rc = self._L.oracle_generate(self._h, phi, max_steps, int(use_list), steps)
+        if rc < 0:
+            raise RuntimeError("oracle generate: error %d" % rc)
+        return rc, int(steps.value)
+
+    def grid(self):
+        """uint8 copy of the phase array, shape (nz, ny, nx), 1 = solid."""
+        ptr = self._L.oracle_grid(self._h)
+        return np.ctypeslib.as_array(ptr, shape=(self.N,)).reshape(self.nz, self.ny, self.nx).copy()
+
+    @property
+    def n_solid(self):
+        return int(self._L.oracle_n_solid(self._h))
+
+    @property
+    def n_front_exact(self):
+        return int(self._L.oracle_n_front_exact(self._h))
+
+    @property
+    def n_target(self):
+        return int(self._L.oracle_n_target(self._h))
+
+    @property
+    def step_index(self):
+        return int(self._L.oracle_step_index(self._h))
+
+    def rates(self):
+        a = (ctypes.c_uint64 * 26)()
+        s = (ctypes.c_uint64 * 26)()
+        self._L.oracle_rates(self._h, a, s)
+        return np.array(a[:], dtype=np.uint64), np.array(s[:], dtype=np.uint64)
+
+    def permute_front(self, how, key=0):
+        self._L.oracle_permute_front(self._h, how, key)

@@ -1,0 +1,388 @@
+/*
+ * liets_oracle.c -- CPU ORACLE for the LIETS-QSGS growth path.  TEST INFRASTRUCTURE ONLY.
+ * See liets_oracle.h for scope, citations and pins.  Plain serial C99 (+ gcc's __int128),
+ * no blocking, no fusion, no reordering beyond what the cited passage states.
+ */
+#include "liets_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ------------------------------------------------------------------------------------------
+ * Philox4x32-10 (R9).  One round:
+ *   (c0,c1,c2,c3) <- (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0));
+ * between rounds k0 += W0, k1 += W1; ten rounds.
+ * ------------------------------------------------------------------------------------------ */
+void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+    const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t prod0 = (uint64_t)M0 * (uint64_t)c0;
+        uint64_t prod1 = (uint64_t)M1 * (uint64_t)c2;
+        uint32_t n0 = (uint32_t)(prod1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)prod1;
+        uint32_t n2 = (uint32_t)(prod0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)prod0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0; k1 += W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* R9: growth draw.  key = (seed lo, seed hi); counter = (p lo, p hi, step t, d / 4);
+ * the draw of direction d is output word d % 4. */
+uint32_t oracle_growth_draw(uint64_t rng_seed, uint32_t t, uint64_t p, int d) {
+    uint32_t key[2] = { (uint32_t)(rng_seed & 0xFFFFFFFFu), (uint32_t)(rng_seed >> 32) };
+    uint32_t ctr[4] = { (uint32_t)(p & 0xFFFFFFFFu), (uint32_t)(p >> 32), t, (uint32_t)(d / 4) };
+    uint32_t out[4];
+    oracle_philox4x32_10(ctr, key, out);
+    return out[d % 4];
+}
+
+/* R9: seeding draw.  counter = ((v/4) lo, (v/4) hi, 0, 0xFFFFFFFF); draw of voxel v is word v % 4.
+ * (c3 = 0xFFFFFFFF never collides with a growth counter, whose c3 is 0..6.) */
+uint32_t oracle_seed_draw(uint64_t rng_seed, uint64_t v) {
+    uint32_t key[2] = { (uint32_t)(rng_seed & 0xFFFFFFFFu), (uint32_t)(rng_seed >> 32) };
+    uint64_t blk = v / 4;
+    uint32_t ctr[4] = { (uint32_t)(blk & 0xFFFFFFFFu), (uint32_t)(blk >> 32), 0u, 0xFFFFFFFFu };
+    uint32_t out[4];
+    oracle_philox4x32_10(ctr, key, out);
+    return out[v % 4];
+}
+
+/* ------------------------------------------------------------------------------------------
+ * R1: the 26 directions.  See DESIGN.md "Readings" R1 for the order; class = |dx|+|dy|+|dz|.
+ * ------------------------------------------------------------------------------------------ */
+#include "liets_oracle_directions.inc"
+
+void oracle_direction(int d, int* dx, int* dy, int* dz, int* cls) {
+    *dx = ORACLE_DIRS[d][0]; *dy = ORACLE_DIRS[d][1]; *dz = ORACLE_DIRS[d][2];
+    *cls = abs(*dx) + abs(*dy) + abs(*dz);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Integer thresholds (R7, R8) and Eq. (1) (R6).
+ * ------------------------------------------------------------------------------------------ */
+uint64_t oracle_prob_to_threshold(double p) {
+    if (p <= 0.0) return 0;
+    if (p >= 1.0) return (uint64_t)1 << 32;
+    return (uint64_t)floor(p * 4294967296.0 + 0.5);
+}
+
+uint64_t oracle_target_count(double phi_s, uint64_t N) {
+    double x = ceil(phi_s * (double)N);
+    if (x < 1.0) return 1;
+    if (x > (double)N) return N;
+    return (uint64_t)x;
+}
+
+/* G = G_ref (phi_s - 0.95 phi_a)/(0.05 phi_s) = G_ref (20 n_t - 19 n_solid)/n_t, clamped to [0,1]. */
+uint64_t oracle_step_threshold(uint64_t R, int law, uint64_t n_t, uint64_t n_solid) {
+    if (law == 0) return R;
+    unsigned __int128 a = (unsigned __int128)20 * n_t;
+    unsigned __int128 b = (unsigned __int128)19 * n_solid;
+    if (b >= a) return 0;
+    unsigned __int128 T = ((unsigned __int128)R * (a - b)) / n_t;
+    unsigned __int128 one = (unsigned __int128)1 << 32;
+    return (uint64_t)(T > one ? one : T);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * State
+ * ------------------------------------------------------------------------------------------ */
+struct oracle_state {
+    int nx, ny, nz, periodic;
+    uint64_t N;
+    uint8_t* grid;            /* phase array, 1 = solid, 0 = void */
+    uint64_t* front;          /* active set A */
+    uint64_t n_front, cap_front;
+    uint64_t n_solid;
+    uint32_t step;            /* t: continues across step/generate calls */
+    uint64_t rng_seed;
+    int seeded;
+    uint64_t R[4];            /* R[class], class 1..3 */
+    int law;
+    int has_target;
+    uint64_t n_t;
+    uint64_t attempts[26], successes[26];
+};
+
+oracle_state* oracle_new(int nx, int ny, int nz, int periodic) {
+    if (nx < 1 || ny < 1 || nz < 1) return NULL;
+    oracle_state* o = (oracle_state*)calloc(1, sizeof(*o));
+    o->nx = nx; o->ny = ny; o->nz = nz; o->periodic = periodic ? 1 : 0;
+    o->N = (uint64_t)nx * (uint64_t)ny * (uint64_t)nz;
+    o->grid = (uint8_t*)calloc(o->N, 1);
+    o->cap_front = 1024;
+    o->front = (uint64_t*)malloc(o->cap_front * sizeof(uint64_t));
+    return o;
+}
+
+void oracle_free(oracle_state* o) {
+    if (!o) return;
+    free(o->grid); free(o->front); free(o);
+}
+
+int oracle_set_growth(oracle_state* o, double g_face, double g_edge, double g_corner, int law) {
+    if (g_face < 0 || g_face > 1 || g_edge < 0 || g_edge > 1 || g_corner < 0 || g_corner > 1) return -1;
+    if (law != 0 && law != 1) return -1;
+    o->R[1] = oracle_prob_to_threshold(g_face);
+    o->R[2] = oracle_prob_to_threshold(g_edge);
+    o->R[3] = oracle_prob_to_threshold(g_corner);
+    o->law = law;
+    return 0;
+}
+
+int oracle_set_target(oracle_state* o, double phi_s) {
+    if (!(phi_s > 0.0) || phi_s > 1.0) return -1;
+    o->n_t = oracle_target_count(phi_s, o->N);
+    o->has_target = 1;
+    return 0;
+}
+
+static void front_push(oracle_state* o, uint64_t p) {
+    if (o->n_front == o->cap_front) {
+        o->cap_front *= 2;
+        o->front = (uint64_t*)realloc(o->front, o->cap_front * sizeof(uint64_t));
+    }
+    o->front[o->n_front++] = p;
+}
+
+/* neighbour of p in direction d: returns 1 and *q if it exists (inside a non-periodic domain,
+ * PAPER.md:53, :145; or wrapped per coordinate if periodic, "roll"; R5). */
+static int neighbour(const oracle_state* o, uint64_t p, int d, uint64_t* q) {
+    int64_t x = (int64_t)(p % (uint64_t)o->nx);
+    int64_t y = (int64_t)((p / (uint64_t)o->nx) % (uint64_t)o->ny);
+    int64_t z = (int64_t)(p / ((uint64_t)o->nx * (uint64_t)o->ny));
+    x += ORACLE_DIRS[d][0]; y += ORACLE_DIRS[d][1]; z += ORACLE_DIRS[d][2];
+    if (o->periodic) {
+        x = (x % o->nx + o->nx) % o->nx;
+        y = (y % o->ny + o->ny) % o->ny;
+        z = (z % o->nz + o->nz) % o->nz;
+    } else if (x < 0 || x >= o->nx || y < 0 || y >= o->ny || z < 0 || z >= o->nz) {
+        return 0;
+    }
+    *q = (uint64_t)x + (uint64_t)o->nx * ((uint64_t)y + (uint64_t)o->ny * (uint64_t)z);
+    return 1;
+}
+
+/* does solid cell p have at least one void neighbour (R13) */
+static int has_void_neighbour(const oracle_state* o, uint64_t p) {
+    for (int d = 0; d < 26; ++d) {
+        uint64_t q;
+        if (neighbour(o, p, d, &q) && o->grid[q] == 0) return 1;
+    }
+    return 0;
+}
+
+static void reset_run(oracle_state* o, uint64_t rng_seed) {
+    memset(o->grid, 0, o->N);
+    o->n_front = 0; o->n_solid = 0; o->step = 0; o->rng_seed = rng_seed; o->seeded = 1;
+    memset(o->attempts, 0, sizeof(o->attempts));
+    memset(o->successes, 0, sizeof(o->successes));
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Seeding and seed spacing (R11, R12).
+ * Candidates: every voxel v, ascending index, whose draw is below T_core.
+ * Spacing: scan candidates in ascending index; accept v iff every already accepted seed w has
+ * L1(v,w) >= s (per-axis min(|D|, n-|D|) if periodic).  s <= 1 accepts all.
+ * ------------------------------------------------------------------------------------------ */
+static int64_t axis_dist(int64_t a, int64_t b, int n, int periodic) {
+    int64_t d = a > b ? a - b : b - a;
+    if (periodic && n - d < d) d = n - d;
+    return d;
+}
+
+static int64_t l1_dist(const oracle_state* o, uint64_t v, uint64_t w) {
+    int64_t vx = (int64_t)(v % (uint64_t)o->nx), wx = (int64_t)(w % (uint64_t)o->nx);
+    int64_t vy = (int64_t)((v / (uint64_t)o->nx) % (uint64_t)o->ny), wy = (int64_t)((w / (uint64_t)o->nx) % (uint64_t)o->ny);
+    int64_t vz = (int64_t)(v / ((uint64_t)o->nx * (uint64_t)o->ny)), wz = (int64_t)(w / ((uint64_t)o->nx * (uint64_t)o->ny));
+    return axis_dist(vx, wx, o->nx, o->periodic) + axis_dist(vy, wy, o->ny, o->periodic) +
+           axis_dist(vz, wz, o->nz, o->periodic);
+}
+
+int64_t oracle_seed(oracle_state* o, double core_prob, int spacing_s, uint64_t rng_seed) {
+    if (core_prob < 0.0 || core_prob > 1.0 || spacing_s < 0) return -1;
+    reset_run(o, rng_seed);
+    uint64_t T_core = oracle_prob_to_threshold(core_prob);
+    for (uint64_t v = 0; v < o->N; ++v) {
+        if ((uint64_t)oracle_seed_draw(rng_seed, v) >= T_core) continue;   /* not a candidate */
+        int ok = 1;
+        if (spacing_s > 1) {
+            for (uint64_t i = 0; i < o->n_front; ++i) {                    /* accepted so far */
+                if (l1_dist(o, v, o->front[i]) < (int64_t)spacing_s) { ok = 0; break; }
+            }
+        }
+        if (ok) { o->grid[v] = 1; front_push(o, v); }
+    }
+    o->n_solid = o->n_front;       /* A_0 = seeds (R3) */
+    return (int64_t)o->n_solid;
+}
+
+int64_t oracle_seed_explicit(oracle_state* o, const uint64_t* idx, uint64_t n, uint64_t rng_seed) {
+    reset_run(o, rng_seed);
+    for (uint64_t i = 0; i < n; ++i) {
+        if (idx[i] >= o->N) return -1;
+        if (o->grid[idx[i]] == 0) { o->grid[idx[i]] = 1; front_push(o, idx[i]); }
+    }
+    o->n_solid = o->n_front;
+    return (int64_t)o->n_solid;
+}
+
+/* per-step thresholds, evaluated once from n_solid at the start of the step (R6) */
+static int step_thresholds(const oracle_state* o, uint64_t T[4]) {
+    if (!o->seeded) return -2;
+    if (o->law == 1 && !o->has_target) return -2;
+    for (int c = 1; c <= 3; ++c) T[c] = oracle_step_threshold(o->R[c], o->law, o->n_t, o->n_solid);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * One step, plain definition (Algorithm 2, keyed draws; "counted
+ * once"; PAPER.md:78 new cells act only in the next iteration):
+ *   for every p with g_t[p] = 1, every direction d, q = p + e_d: if q exists and g_t[q] = 0 and
+ *   draw(seed, t, p, d) < T_class(d) then g_{t+1}[q] = 1.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_step_full(oracle_state* o) {
+    uint64_t T[4];
+    int rc = step_thresholds(o, T);
+    if (rc) return rc;
+    uint8_t* next = (uint8_t*)malloc(o->N);
+    memcpy(next, o->grid, o->N);
+    for (uint64_t p = 0; p < o->N; ++p) {
+        if (o->grid[p] != 1) continue;
+        for (int d = 0; d < 26; ++d) {
+            uint64_t q;
+            if (!neighbour(o, p, d, &q)) continue;
+            if (o->grid[q] != 0) continue;
+            int cls = abs(ORACLE_DIRS[d][0]) + abs(ORACLE_DIRS[d][1]) + abs(ORACLE_DIRS[d][2]);
+            o->attempts[d]++;
+            if ((uint64_t)oracle_growth_draw(o->rng_seed, o->step, p, d) < T[cls]) {
+                o->successes[d]++;
+                next[q] = 1;
+            }
+        }
+    }
+    memcpy(o->grid, next, o->N);
+    free(next);
+    /* phi_a recomputed from the phase array; the front is rebuilt by definition */
+    o->n_solid = 0; o->n_front = 0;
+    for (uint64_t p = 0; p < o->N; ++p) o->n_solid += o->grid[p];
+    for (uint64_t p = 0; p < o->N; ++p)
+        if (o->grid[p] == 1 && has_void_neighbour(o, p)) front_push(o, p);
+    o->step++;
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * One step, Algorithm 3 line by line.  A_{t+1} = prune(A_t U A_new) (R4).
+ * ------------------------------------------------------------------------------------------ */
+int oracle_step_list(oracle_state* o) {
+    uint64_t T[4];
+    int rc = step_thresholds(o, T);
+    if (rc) return rc;
+    uint64_t n_old = o->n_front;                       /* sources: A at the start of the step */
+    for (int d = 0; d < 26; ++d) {                     /* line 4: for each d in directions   */
+        int cls = abs(ORACLE_DIRS[d][0]) + abs(ORACLE_DIRS[d][1]) + abs(ORACLE_DIRS[d][2]);
+        for (uint64_t i = 0; i < n_old; ++i) {
+            uint64_t p = o->front[i], q;
+            if (!neighbour(o, p, d, &q)) continue;     /* line 5: N_d inside domain          */
+            if (o->grid[q] != 0) continue;             /* line 6: C_d, still void            */
+            if ((uint64_t)oracle_growth_draw(o->rng_seed, o->step, p, d) < T[cls]) { /* line 8 */
+                o->grid[q] = 1;                        /* line 9                             */
+                front_push(o, q);                      /* line 10: A_new U {q}, once per q   */
+                o->n_solid++;
+            }
+        }
+    }
+    /* line 14: prune -- drop cells with no void neighbour (duplicates cannot occur: a cell is
+     * pushed only at its 0 -> 1 transition) */
+    uint64_t kept = 0;
+    for (uint64_t i = 0; i < o->n_front; ++i)
+        if (has_void_neighbour(o, o->front[i])) o->front[kept++] = o->front[i];
+    o->n_front = kept;
+    o->step++;
+    return 0;
+}
+
+/* while phi_a < phi_s and A not empty (R7: n_solid < n_t; R14: max_steps) */
+int oracle_generate(oracle_state* o, double phi_s, uint32_t max_steps, int use_list,
+                    uint32_t* steps_out) {
+    if (oracle_set_target(o, phi_s)) return -1;
+    if (!o->seeded) return -2;
+    uint32_t done = 0;
+    int status = ORACLE_OK;
+    for (;;) {
+        if (o->n_solid >= o->n_t) { status = ORACLE_OK; break; }
+        if (o->n_front == 0) { status = ORACLE_FRONT_EMPTY; break; }
+        if (done >= max_steps) { status = ORACLE_MAX_STEPS; break; }
+        int rc = use_list ? oracle_step_list(o) : oracle_step_full(o);
+        if (rc) return rc;
+        done++;
+    }
+    if (steps_out) *steps_out = done;
+    return status;
+}
+
+const uint8_t* oracle_grid(const oracle_state* o) { return o->grid; }
+uint64_t oracle_n_solid(const oracle_state* o) { return o->n_solid; }
+uint32_t oracle_step_index(const oracle_state* o) { return o->step; }
+uint64_t oracle_n_target(const oracle_state* o) { return o->n_t; }
+
+uint64_t oracle_n_front_exact(const oracle_state* o) {
+    uint64_t n = 0;
+    for (uint64_t p = 0; p < o->N; ++p)
+        if (o->grid[p] == 1 && has_void_neighbour(o, p)) n++;
+    return n;
+}
+
+void oracle_rates(const oracle_state* o, uint64_t attempts[26], uint64_t successes[26]) {
+    memcpy(attempts, o->attempts, sizeof(o->attempts));
+    memcpy(successes, o->successes, sizeof(o->successes));
+}
+
+void oracle_permute_front(oracle_state* o, int how, uint64_t key) {
+    uint64_t n = o->n_front;
+    if (how == 1) {
+        for (uint64_t i = 0; i < n / 2; ++i) {
+            uint64_t tmp = o->front[i]; o->front[i] = o->front[n - 1 - i]; o->front[n - 1 - i] = tmp;
+        }
+    } else if (how == 2) {                              /* Fisher-Yates with a keyed LCG */
+        uint64_t s = key * 6364136223846793005ull + 1442695040888963407ull;
+        for (uint64_t i = n; i > 1; --i) {
+            s = s * 6364136223846793005ull + 1442695040888963407ull;
+            uint64_t j = (s >> 33) % i;
+            uint64_t tmp = o->front[i - 1]; o->front[i - 1] = o->front[j]; o->front[j] = tmp;
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Two-point correlation of the void phase along one axis, exact pair counts (R16).
+ * ------------------------------------------------------------------------------------------ */
+void oracle_s2(const uint8_t* grid, int nx, int ny, int nz, int periodic, int axis, int rmax,
+               uint64_t* pairs, uint64_t* valid) {
+    int n[3] = { nx, ny, nz };
+    for (int r = 0; r <= rmax; ++r) {
+        uint64_t np = 0, nv = 0;
+        for (int z = 0; z < nz; ++z)
+            for (int y = 0; y < ny; ++y)
+                for (int x = 0; x < nx; ++x) {
+                    int c[3] = { x, y, z };
+                    c[axis] += r;
+                    if (c[axis] >= n[axis]) {
+                        if (!periodic) continue;
+                        c[axis] %= n[axis];
+                    }
+                    nv++;
+                    uint64_t a = (uint64_t)x + (uint64_t)nx * ((uint64_t)y + (uint64_t)ny * (uint64_t)z);
+                    uint64_t b = (uint64_t)c[0] + (uint64_t)nx * ((uint64_t)c[1] + (uint64_t)ny * (uint64_t)c[2]);
+                    if (grid[a] == 0 && grid[b] == 0) np++;
+                }
+        pairs[r] = np; valid[r] = nv;
+    }
+}

@@ -1,0 +1,411 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (CPU only).
+
+Each test names the pin of SURVEY.md section 8(c) / DESIGN.md it implements.  Nothing here touches
+the CUDA path: the oracle must be trustworthy before any kernel is compared with it.
+"""
+import itertools
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def coords(shape):
+    nz, ny, nx = shape
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    return x, y, z
+
+
+def axis_d(a, b, n, periodic):
+    d = np.abs(a - b)
+    return np.minimum(d, n - d) if periodic else d
+
+
+# ------------------------------------------------------------------------------------------ P1
+def test_p1_philox_known_answers():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "philox4x32_10_kat.txt")) if l[0] not in "#\n"]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(t, 16) for t in r]
+        assert oracle.philox4x32_10(v[0:4], v[4:6]) == tuple(v[6:10])
+
+
+def test_p1_draw_layout_matches_philox_block():
+    # R9: growth counter = (p lo, p hi, t, d//4), word d%4; seeding counter = (v//4, 0, 0, ~0), word v%4
+    seed = 0x0123456789ABCDEF
+    key = (seed & 0xFFFFFFFF, seed >> 32)
+    for p, t, d in [(0, 0, 0), (12345, 7, 13), (2**32 - 1, 40, 25), (2**31 + 5, 3, 22)]:
+        blk = oracle.philox4x32_10([p & 0xFFFFFFFF, p >> 32, t, d // 4], key)
+        assert oracle.growth_draw(seed, t, p, d) == blk[d % 4]
+    for v in [0, 1, 2, 3, 4, 1000003, 2**32 - 1]:
+        blk = oracle.philox4x32_10([(v // 4) & 0xFFFFFFFF, (v // 4) >> 32, 0, 0xFFFFFFFF], key)
+        assert oracle.seed_draw(seed, v) == blk[v % 4]
+
+
+def test_direction_table_is_the_26_neighbourhood():
+    ds = [oracle.direction(d) for d in range(26)]
+    vecs = [d[:3] for d in ds]
+    assert len(set(vecs)) == 26 and (0, 0, 0) not in vecs
+    assert all(max(map(abs, v)) == 1 for v in vecs)
+    cls = [d[3] for d in ds]
+    assert (cls.count(1), cls.count(2), cls.count(3)) == (6, 12, 8)       # face / edge / corner
+    assert all(c == sum(map(abs, v)) for c, v in zip(cls, vecs))
+    # R1: lexicographic in (dz, dy, dx), dz slowest
+    assert vecs == [(dx, dy, dz) for dz, dy, dx in itertools.product((-1, 0, 1), repeat=3) if (dx, dy, dz) != (0, 0, 0)]
+
+
+# ------------------------------------------------------------------------------------------ P8
+def test_p8_thresholds_against_big_integers():
+    two32 = 1 << 32
+    assert oracle.prob_to_threshold(0.0) == 0
+    assert oracle.prob_to_threshold(1.0) == two32
+    assert oracle.prob_to_threshold(0.5) == 1 << 31
+    assert oracle.prob_to_threshold(0.01) == math.floor(0.01 * two32 + 0.5)
+    rng = np.random.default_rng(5)
+    for _ in range(2000):
+        R = int(rng.integers(0, two32 + 1))
+        n_t = int(rng.integers(1, 2**32 + 1))
+        n = int(rng.integers(0, int(1.2 * n_t) + 1))
+        expect = min(two32, (R * max(0, 20 * n_t - 19 * n)) // n_t)
+        assert oracle.step_threshold(R, 1, n_t, n) == expect
+        assert oracle.step_threshold(R, 0, n_t, n) == R
+    for R in (0, 1, 42949673, two32 // 20, two32 // 20 + 1, two32):
+        for n_t in (1, 78644, 6_000_000, 858_993_460, 2**32):
+            assert oracle.step_threshold(R, 1, n_t, 0) == min(two32, 20 * R)     # 20 G_ref at phi_a = 0
+            assert oracle.step_threshold(R, 1, n_t, n_t) == R                    # G_ref at the target
+    # Eq. (1) in double precision agrees to one unit of T
+    R, n_t = oracle.prob_to_threshold(0.01), 51_200_000
+    for n in (0, 1, 999, 25_000_000, 51_199_999):
+        phi_s, phi_a = n_t / 64e6, n / 64e6
+        G = 0.01 * (phi_s - 0.95 * phi_a) / (0.05 * phi_s)
+        assert abs(oracle.step_threshold(R, 1, n_t, n) - G * two32) <= 2.0 + 1e-9 * G * two32
+
+
+def test_r7_target_count():
+    assert oracle.target_count(0.30, 64**3) == 78644
+    assert oracle.target_count(0.75, 200**3) == 6_000_000
+    assert oracle.target_count(0.8, 2**30) == 858_993_460
+    assert oracle.target_count(1.0, 1000) == 1000
+    assert oracle.target_count(1e-9, 1000) == 1
+
+
+# ------------------------------------------------------------------------------------------ P2
+def test_p2_zero_growth_leaves_exactly_the_seeds():
+    o = oracle.Oracle(40, 36, 28, False)
+    o.set_growth(0.0, 0.0, 0.0, 0)
+    n = o.seed(0.01, 0, 3)
+    g0 = o.grid()
+    N = 40 * 36 * 28
+    cand = np.array([oracle.seed_draw(3, v) < oracle.prob_to_threshold(0.01) for v in range(N)])
+    assert (g0.ravel() == cand).all() and n == cand.sum()
+    assert abs(n - 0.01 * N) <= 5 * math.sqrt(N * 0.01 * 0.99)            # binomial bound
+    for use_list in (True, False):
+        o.step(use_list)
+        assert (o.grid() == g0).all() and o.n_solid == n
+    rc, steps = o.generate(0.5, 7, True)
+    assert rc == oracle.MAX_STEPS and steps == 7 and (o.grid() == g0).all()
+
+
+# ------------------------------------------------------------------------------------- P3, P4
+def _ball_volumes():
+    return {int(a): int(b) for a, b in (l.split() for l in open(os.path.join(GOLDEN, "l1_ball_volumes.txt")) if l[0] != "#")}
+
+
+@pytest.mark.parametrize("use_list", [True, False])
+@pytest.mark.parametrize("periodic", [False, True])
+def test_p3_face_growth_prob_one_gives_l1_balls(use_list, periodic):
+    nx, ny, nz = 23, 19, 21
+    vol = _ball_volumes()
+    o = oracle.Oracle(nx, ny, nz, periodic)
+    o.set_growth(1.0, 0.0, 0.0, 0)
+    centre = (11, 9, 10)
+    o.seed_explicit([centre[0] + nx * (centre[1] + ny * centre[2])])
+    x, y, z = coords((nz, ny, nx))
+    for k in range(1, 13):
+        o.step(use_list)
+        dist = axis_d(x, centre[0], nx, periodic) + axis_d(y, centre[1], ny, periodic) + axis_d(z, centre[2], nz, periodic)
+        assert (o.grid() == (dist <= k)).all(), k
+        if k <= 9:                                    # ball still clear of walls / of its own images
+            assert o.n_solid == vol[k]
+    # several seeds, one against a wall / across the seam: union of balls
+    seeds = [(0, 0, 0), (22, 18, 20), (5, 17, 3)]
+    o.seed_explicit([sx + nx * (sy + ny * sz) for sx, sy, sz in seeds])
+    for k in range(1, 6):
+        o.step(use_list)
+        d = np.min([axis_d(x, sx, nx, periodic) + axis_d(y, sy, ny, periodic) + axis_d(z, sz, nz, periodic)
+                    for sx, sy, sz in seeds], axis=0)
+        assert (o.grid() == (d <= k)).all()
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+def test_p4_all_directions_prob_one_gives_chebyshev_cubes(periodic):
+    nx, ny, nz = 17, 15, 16
+    x, y, z = coords((nz, ny, nx))
+    c = (3, 7, 12)
+    ax, ay, az = axis_d(x, c[0], nx, periodic), axis_d(y, c[1], ny, periodic), axis_d(z, c[2], nz, periodic)
+    o = oracle.Oracle(nx, ny, nz, periodic)
+    o.set_growth(1.0, 1.0, 1.0, 0)
+    o.seed_explicit([c[0] + nx * (c[1] + ny * c[2])])
+    for k in range(1, 6):
+        o.step(True)
+        assert (o.grid() == (np.maximum(np.maximum(ax, ay), az) <= k)).all()
+    if not periodic:
+        o.seed_explicit([8 + nx * (7 + ny * 8)])
+        o.step(True); o.step(True)
+        assert o.n_solid == 5 ** 3
+    # face + edge at probability 1: {max|D| <= k and sum|D| <= 2k}
+    o.set_growth(1.0, 1.0, 0.0, 0)
+    o.seed_explicit([c[0] + nx * (c[1] + ny * c[2])])
+    for k in range(1, 5):
+        o.step(False)
+        expect = (np.maximum(np.maximum(ax, ay), az) <= k) & (ax + ay + az <= 2 * k)
+        assert (o.grid() == expect).all()
+    # corner only: parity-preserving diagonal moves -> after k steps {|Dx|,|Dy|,|Dz| <= k, all same parity as k ... }
+    if not periodic:
+        o.set_growth(0.0, 0.0, 1.0, 0)
+        o.seed_explicit([8 + nx * (7 + ny * 8)])
+        o.step(True)
+        assert o.n_solid == 1 + 8
+
+
+# ------------------------------------------------------------------------------------------ P5
+def _dilation_greedy(shape, periodic, cand_idx, s):
+    """The paper's spacing as literally described: keep a 'blocked' mask that is
+    the accepted set dilated s-1 times with the 6-neighbour kernel; accept a candidate iff not blocked."""
+    nz, ny, nx = shape
+    blocked = np.zeros(shape, bool)
+    accepted = []
+    for v in cand_idx:
+        x, y, z = v % nx, (v // nx) % ny, v // (nx * ny)
+        if blocked[z, y, x]:
+            continue
+        accepted.append(v)
+        m = np.zeros(shape, bool)
+        m[z, y, x] = True
+        for _ in range(max(s - 1, 0)):
+            n = m.copy()
+            for ax in range(3):
+                for sh in (1, -1):
+                    r = np.roll(m, sh, axis=ax)
+                    if not periodic:
+                        sl = [slice(None)] * 3
+                        sl[ax] = 0 if sh == 1 else -1
+                        r[tuple(sl)] = False
+                    n |= r
+            m = n
+        blocked |= m
+    return accepted
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("s", [0, 1, 2, 3, 5, 8])
+def test_p5_spacing_equals_dilation_greedy(periodic, s):
+    nx, ny, nz = 20, 17, 14
+    N = nx * ny * nz
+    seed, c = 9 + s, 0.02
+    Tc = oracle.prob_to_threshold(c)
+    cand = [v for v in range(N) if oracle.seed_draw(seed, v) < Tc]
+    expect = _dilation_greedy((nz, ny, nx), periodic, cand, s)
+    o = oracle.Oracle(nx, ny, nz, periodic)
+    n = o.seed(c, s, seed)
+    got = np.flatnonzero(o.grid().ravel())
+    assert n == len(expect) and (got == np.array(expect)).all()
+    # pairwise distance >= s and maximality (every rejected candidate has an accepted seed with a
+    # lower index at L1 < s)
+    pts = np.array([(v % nx, (v // nx) % ny, v // (nx * ny)) for v in got])
+    dims = np.array([nx, ny, nz])
+
+    def dist(a, b):
+        d = np.abs(a - b)
+        if periodic:
+            d = np.minimum(d, dims - d)
+        return d.sum(axis=-1)
+    if s > 1 and len(pts) > 1:
+        D = dist(pts[:, None, :], pts[None, :, :]) + np.eye(len(pts), dtype=int) * 10**6
+        assert D.min() >= s
+        for v in set(cand) - set(got.tolist()):
+            p = np.array((v % nx, (v // nx) % ny, v // (nx * ny)))
+            lower = pts[got < v]
+            assert (dist(lower, p) < s).any()
+    else:
+        assert list(got) == cand
+
+
+def test_p5_single_seed_dilation_has_closed_form_volume():
+    vol = _ball_volumes()
+    for s in (2, 4, 6):
+        acc = _dilation_greedy((21, 21, 21), False, [10 + 21 * (10 + 21 * 10)], s)
+        assert acc == [10 + 21 * (10 + 21 * 10)]
+    # the blocked region of one seed is the L1 ball of radius s-1: every point at L1 < s is rejected
+    o = oracle.Oracle(21, 21, 21, False)
+    x, y, z = coords((21, 21, 21))
+    d = np.abs(x - 10) + np.abs(y - 10) + np.abs(z - 10)
+    for s in (2, 4, 6):
+        assert int((d <= s - 1).sum()) == vol[s - 1]
+
+
+# ------------------------------------------------------------------------------------- P6, P7
+@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("dims", [(32, 32, 32), (45, 31, 38), (5, 4, 3), (1, 9, 2)])
+def test_p6_list_algorithm_equals_full_field_definition(periodic, dims):
+    nx, ny, nz = dims
+    a, b = oracle.Oracle(nx, ny, nz, periodic), oracle.Oracle(nx, ny, nz, periodic)
+    for o in (a, b):
+        o.set_growth(0.05, 0.02, 0.01, 1)
+        o.set_target(0.6)
+        o.seed(0.01 if nx * ny * nz > 1000 else 0.2, 3, 77)
+    assert (a.grid() == b.grid()).all()
+    for t in range(12):
+        a.step(True); b.step(False)
+        assert (a.grid() == b.grid()).all(), t
+        assert a.n_solid == b.n_solid == int(a.grid().sum())
+        assert a.n_front_exact == b.n_front_exact
+    ra, sa = a.generate(0.6, 1000, True)
+    rb, sb = b.generate(0.6, 1000, False)
+    assert (ra, sa) == (rb, sb) and (a.grid() == b.grid()).all()
+
+
+def test_p7_front_order_does_not_matter():
+    ref = None
+    for how in (0, 1, 2):
+        o = oracle.Oracle(36, 36, 36, False)
+        o.set_growth(0.04, 0.01, 0.002, 1)
+        o.set_target(0.5)
+        o.seed(0.004, 4, 21)
+        for t in range(10):
+            if how:
+                o.permute_front(how, 1000 + t)
+            o.step(True)
+        ref = o.grid() if ref is None else ref
+        assert (o.grid() == ref).all()
+
+
+# ------------------------------------------------------------------------------------------ P9
+def test_p9_per_direction_acceptance_rates():
+    o = oracle.Oracle(48, 48, 48, False)
+    gf, ge, gc = 0.20, 0.10, 0.05
+    o.set_growth(gf, ge, gc, 0)
+    o.seed(0.02, 0, 5)
+    for _ in range(3):
+        o.step(False)
+    att, suc = o.rates()
+    for d in range(26):
+        p = {1: gf, 2: ge, 3: gc}[oracle.direction(d)[3]]
+        n, k = int(att[d]), int(suc[d])
+        assert n > 3000
+        assert abs(k - n * p) <= 5 * math.sqrt(n * p * (1 - p)), (d, n, k)
+
+
+def test_p9_one_step_claim_probability_counts_once():
+    # a void cell with m_f/m_e/m_c solid face/edge/corner neighbours is claimed with
+    # probability 1 - (1-G_f)^m_f (1-G_e)^m_e (1-G_c)^m_c.  Fixed grid, many rng seeds.
+    nx = ny = nz = 7
+    solid = [(3, 3, 3), (4, 3, 3), (3, 4, 3), (2, 2, 4)]
+    idx = [x + nx * (y + ny * z) for x, y, z in solid]
+    gf, ge, gc = 0.3, 0.2, 0.1
+    trials = 4000
+    hits = np.zeros((nz, ny, nx))
+    o = oracle.Oracle(nx, ny, nz, False)
+    o.set_growth(gf, ge, gc, 0)
+    for s in range(trials):
+        o.seed_explicit(idx, rng_seed=1000 + s)
+        o.step(s % 2 == 0)
+        hits += o.grid()
+    g0 = np.zeros((nz, ny, nx), bool)
+    for x, y, z in solid:
+        g0[z, y, x] = True
+    for z, y, x in itertools.product(range(nz), range(ny), range(nx)):
+        if g0[z, y, x]:
+            assert hits[z, y, x] == trials
+            continue
+        m = {1: 0, 2: 0, 3: 0}
+        for sx, sy, sz in solid:
+            dd = (abs(sx - x), abs(sy - y), abs(sz - z))
+            if max(dd) == 1:
+                m[sum(dd)] += 1
+        p = 1 - (1 - gf) ** m[1] * (1 - ge) ** m[2] * (1 - gc) ** m[3]
+        k = hits[z, y, x]
+        assert abs(k - trials * p) <= 5 * math.sqrt(trials * p * (1 - p)) + 1e-9, ((x, y, z), m, k)
+
+
+# ------------------------------------------------------------------------------------ P10, P11
+def test_p10_p11_monotone_growth_and_stop_rule():
+    cfg = dict(dims=(40, 40, 40), c=0.005, s=0, g=(0.02, 0.005, 0.0005), phi=0.30, seed=1)
+    o = oracle.Oracle(*cfg["dims"], False)
+    o.set_growth(*cfg["g"], 1)
+    o.set_target(cfg["phi"])
+    o.seed(cfg["c"], cfg["s"], cfg["seed"])
+    prev, prev_n, history = o.grid(), o.n_solid, []
+    while o.n_solid < o.n_target:
+        o.step(True)
+        g = o.grid()
+        assert (g >= prev).all() and o.n_solid >= prev_n and o.n_solid == int(g.sum())
+        history.append(o.n_solid)
+        prev, prev_n = g, o.n_solid
+    steps_by_hand = len(history)
+    assert history[-1] >= o.n_target and (steps_by_hand == 1 or history[-2] < o.n_target)
+    # generate == repeated step, bit for bit
+    o2 = oracle.Oracle(*cfg["dims"], False)
+    o2.set_growth(*cfg["g"], 1)
+    o2.seed(cfg["c"], cfg["s"], cfg["seed"])
+    rc, steps = o2.generate(cfg["phi"], 10**6, True)
+    assert rc == oracle.OK and steps == steps_by_hand and (o2.grid() == prev).all()
+    # target already met: no step runs (R15)
+    rc, steps = o2.generate(cfg["phi"], 10**6, True)
+    assert (rc, steps) == (oracle.OK, 0)
+    # resuming with a higher target continues the same stream: t keeps counting
+    rc, more = o2.generate(0.5, 10**6, True)
+    assert rc == oracle.OK and o2.step_index == steps_by_hand + more and o2.n_solid >= o2.n_target
+    # max_steps (R14) and empty front
+    o3 = oracle.Oracle(6, 6, 6, False)
+    o3.set_growth(1.0, 1.0, 1.0, 0)
+    o3.seed_explicit([0])
+    rc, steps = o3.generate(1.0, 2, True)
+    assert (rc, steps) == (oracle.MAX_STEPS, 2)
+    rc, steps = o3.generate(1.0, 100, True)
+    assert rc == oracle.OK and o3.n_solid == 216 and o3.n_front_exact == 0
+    o4 = oracle.Oracle(6, 6, 6, False)
+    o4.set_growth(0.5, 0.5, 0.5, 0)
+    o4.seed(0.0, 0, 1)
+    assert o4.generate(0.5, 10, True) == (oracle.FRONT_EMPTY, 0)
+
+
+def test_solid_fraction_reaches_config1_target():
+    # BASELINE.json configs[0]; ceil(0.30 * 64^3) = 78644
+    o = oracle.Oracle(64, 64, 64, False)
+    o.set_growth(0.02, 0.005, 0.0005, 1)
+    n_seeds = o.seed(0.005, 0, 1)
+    assert abs(n_seeds - 0.005 * 64**3) <= 5 * math.sqrt(64**3 * 0.005)
+    rc, steps = o.generate(0.30, 1000, True)
+    assert rc == oracle.OK and o.n_target == 78644 and o.n_solid >= 78644 and 2 <= steps <= 20
+
+
+# ----------------------------------------------------------------------------------------- P12
+@pytest.mark.parametrize("periodic", [False, True])
+def test_p12_two_point_correlation(periodic):
+    rng = np.random.default_rng(3)
+    g = (rng.random((16, 14, 12)) < 0.4).astype(np.uint8)          # (nz, ny, nx)
+    void = g == 0
+    for axis, npax in ((0, 2), (1, 1), (2, 0)):                    # oracle axis 0 = x = numpy axis 2
+        pairs, valid = oracle.s2(g, periodic, axis, 6)
+        assert pairs[0] == void.sum() and valid[0] == g.size
+        for r in range(7):
+            if periodic:
+                b = np.roll(void, -r, axis=npax)
+                exp_pairs, exp_valid = int((void & b).sum()), g.size
+            else:
+                n = g.shape[npax]
+                a = np.take(void, range(0, n - r), axis=npax)
+                b = np.take(void, range(r, n), axis=npax)
+                exp_pairs, exp_valid = int((a & b).sum()), a.size
+            assert (int(pairs[r]), int(valid[r])) == (exp_pairs, exp_valid)
+    big = (np.random.default_rng(4).random((40, 40, 40)) < 0.3).astype(np.uint8)
+    pairs, valid = oracle.s2(big, True, 0, 5)
+    phi = pairs[0] / valid[0]
+    for r in range(1, 6):
+        assert abs(pairs[r] / valid[r] - phi**2) < 0.01
