@@ -1,0 +1,118 @@
+/*
+ * liets.h -- C ABI of libliets.so: the B200-native (sm_100a CUDA) hot path of the list-indexed
+ * explicit time-stepping (LIETS) QSGS generator of arxiv/paper_2602_11734.
+ *
+ * The calls follow the paper's statement of the problem (PAPER.md:38-39 seeding and growth,
+ * :110-116 / Algorithm 3 :133-169 the list-indexed step, :122 seed spacing, Eq. (1) :126 the
+ * volume-fraction dependent growth probability, :140 the stopping rule).  Readings of points
+ * where the paper is silent are listed in DESIGN.md ("Readings", R1..R17).
+ *
+ * Conventions
+ *   - Every call returns >= 0 (a status) or < 0 (an error); nothing throws or aborts across the
+ *     ABI.  After an error, liets_last_error(ctx) holds a message (owned by ctx).
+ *   - The library owns the ctx and, unless the caller passes one, the device workspace.  The
+ *     caller owns every dst / *_out pointer.  Pointers are HOST pointers unless marked DEVICE.
+ *   - All device work is enqueued on the CUDA stream given at create (a cudaStream_t passed as
+ *     void*, NULL = the legacy default stream).  Calls that return a value to the host
+ *     (*_out arguments, liets_grid with a host dst) synchronise that stream; the others do not.
+ *   - Voxel (x, y, z) has linear index idx = x + nx*(y + ny*z); N = nx*ny*nz <= 2^32.
+ *   - There is no CPU fallback: without a CUDA device every call fails with LIETS_E_CUDA.
+ */
+#ifndef LIETS_H
+#define LIETS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct liets_ctx liets_ctx;            /* opaque; owned by the library */
+
+enum {
+    LIETS_OK = 0,            /* success; for liets_generate: target solid fraction reached       */
+    LIETS_FRONT_EMPTY = 1,   /* generate stopped: no solid voxel has a void neighbour (:140)      */
+    LIETS_MAX_STEPS = 2,     /* generate stopped: max_steps steps done (R14)                      */
+    LIETS_E_ARG = -1,        /* bad argument (dims < 1, N > 2^32, probability outside [0,1], ...) */
+    LIETS_E_STATE = -2,      /* call order: step/generate before seed; Eq.(1) law without target  */
+    LIETS_E_CAPACITY = -3,   /* caller's workspace / dst buffer too small                         */
+    LIETS_E_CUDA = -4        /* CUDA runtime error or no device                                   */
+};
+
+enum { LIETS_BOUNDARY_WALL = 0, LIETS_BOUNDARY_PERIODIC = 1 };        /* R5 */
+enum { LIETS_STORAGE_U8 = 0,      /* uint8 grid + explicit list of front VOXELS (uint32 indices)  */
+       LIETS_STORAGE_BRICK = 1 }; /* bit-packed 8x8x8 bricks + explicit list of front BRICKS      */
+enum { LIETS_LAW_CONSTANT = 0, LIETS_LAW_EQ1 = 1 };
+enum { LIETS_FORMAT_U8 = 0,       /* one byte per voxel in {0,1}, x fastest, N bytes              */
+       LIETS_FORMAT_BITS = 1 };   /* bit idx%8 (LSB first) of byte idx/8, ceil(N/8) bytes         */
+
+/* Bytes of DEVICE workspace liets_create needs for this grid and storage (0 if arguments bad). */
+size_t liets_workspace_bytes(int nx, int ny, int nz, int storage);
+
+/* Create a generator for an nx*ny*nz grid ("solid-void map").
+ *   boundary   LIETS_BOUNDARY_*: neighbours outside the domain are dropped (:53, :145) or wrapped
+ *              per coordinate (:76 "roll").
+ *   storage    LIETS_STORAGE_*: internal layout of grid and front in HBM; results are identical.
+ *   workspace  DEVICE pointer to >= liets_workspace_bytes() bytes, 256-byte aligned, owned by the
+ *              caller and kept alive until liets_destroy; or NULL: the library allocates.
+ *   cuda_stream cudaStream_t (as void*) all work is enqueued on.
+ * Errors: E_ARG, E_CAPACITY (workspace_bytes too small), E_CUDA. */
+int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int storage,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Reference directional growth probabilities G_ref of the 6 face, 12 edge and 8 corner
+ * directions ("directional growth probability"; R1) and the law that turns them into
+ * the per-step probability: LIETS_LAW_CONSTANT (G = G_ref) or LIETS_LAW_EQ1 (Eq. (1), :126:
+ * G = G_ref (phi_s - 0.95 phi_a) / (0.05 phi_s), evaluated once per step from the solid count at
+ * the start of the step, as exact integer thresholds; R6, R8).  Default: all 0, Eq. (1). */
+int liets_set_growth(liets_ctx* ctx, double g_face, double g_edge, double g_corner, int law);
+
+/* Seeding: voxel v is a candidate core iff its keyed draw < core_prob; then seed
+ * spacing (:122, :131 diamond dilation): candidates are scanned in ascending index and accepted
+ * iff no accepted seed lies at L1 distance < spacing_s (torus metric if periodic; spacing_s <= 1
+ * accepts all; R11, R12) -- reproduced exactly by parallel rounds.  Resets the grid, the front
+ * (A_0 = seeds) and the step counter t = 0.  *n_seeds_out (may be NULL) = number of seeds. */
+int liets_seed(liets_ctx* ctx, double core_prob, int spacing_s, uint64_t rng_seed,
+               uint64_t* n_seeds_out);
+
+/* Same reset, but the seeds are the n given voxel indices (HOST array, duplicates allowed). */
+int liets_seed_explicit(liets_ctx* ctx, const uint64_t* idx, uint64_t n, uint64_t rng_seed);
+
+/* Target solid volume fraction phi_s in (0,1]: n_t = ceil(phi_s*N) (R7). Used by Eq. (1) and by
+ * the stopping rule. */
+int liets_set_target(liets_ctx* ctx, double target_solid_fraction);
+
+/* Exactly one growth step t -> t+1 (Algorithm 3 lines 4-15), regardless of the
+ * target: every front voxel p tries each of its 26 neighbours q = p + e_d that is void at the
+ * start of the step; q becomes solid iff draw(rng_seed, t, p, d) < T_class(d).  Outputs (may be
+ * NULL): solid count after the step; *n_front_out = size of the front the library holds, normative
+ * only as zero (no solid voxel has a void neighbour) / non-zero.  Errors: E_STATE. */
+int liets_step(liets_ctx* ctx, uint64_t* n_solid_out, uint64_t* n_front_out);
+
+/* set_target + "while phi_a < phi_s and A not empty" + at most max_steps steps,
+ * the loop running on the device with no host synchronisation per step.  Bit-exactly equal to
+ * repeated liets_step.  The fraction is tested between whole steps only.  Returns LIETS_OK /
+ * LIETS_FRONT_EMPTY / LIETS_MAX_STEPS; *steps_out = steps done by this call. */
+int liets_generate(liets_ctx* ctx, double target_solid_fraction, uint32_t max_steps,
+                   uint32_t* steps_out, uint64_t* n_solid_out);
+
+/* Copy the phase array out: dst (HOST, or DEVICE if dst_is_device) in LIETS_FORMAT_*. */
+int liets_grid(liets_ctx* ctx, void* dst, size_t dst_bytes, int format, int dst_is_device);
+
+/* Per-step counters of the steps done since the last seed (HOST arrays of capacity cap, may be
+ * NULL): front size at the start of step i (voxels for STORAGE_U8, bricks for STORAGE_BRICK) and
+ * solid count after it.  Returns the number of steps recorded (<= 4096 kept). */
+int liets_step_log(liets_ctx* ctx, uint64_t* front_in, uint64_t* solid_after, uint32_t cap);
+
+/* Device time in milliseconds of the last liets_seed and the last liets_generate (CUDA events on
+ * the ctx stream). */
+int liets_timings(liets_ctx* ctx, float* seed_ms, float* generate_ms);
+
+void liets_destroy(liets_ctx* ctx);
+const char* liets_last_error(const liets_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,10 @@
+"""B200-native LIETS-QSGS growth path (arxiv/paper_2602_11734): thin Python binding of libliets.so.
+
+Everything the method computes runs in the hand-written sm_100a kernels behind the C ABI of
+``include/liets.h``; this package only marshals arguments.  PyTorch supplies device memory
+(the workspace and output buffers) and the CUDA stream.  There is no CPU fallback: loading fails
+loudly if the library has not been built, and every call fails without a CUDA device.
+"""
+from .liets import (Liets, LietsError, lib, library_path, OK, FRONT_EMPTY, MAX_STEPS,  # noqa: F401
+                    BOUNDARY_WALL, BOUNDARY_PERIODIC, STORAGE_U8, STORAGE_BRICK, LAW_CONSTANT, LAW_EQ1,
+                    FORMAT_U8, FORMAT_BITS, EXPORTS)

@@ -1,0 +1,144 @@
+// grow_u8.cu -- STORAGE_U8 growth step: uint8 grid + explicit list of front voxel indices.
+//
+// This is the list-indexed step of Algorithm 3 with one thread per front
+// voxel p: gather the 26 neighbours (line 5-6), draw lazily per Philox block for the void ones
+// (line 8; R9), claim with atomicOr on the 32-bit word holding the target byte (line 9; the thread
+// that flips 0 -> 1 owns q, so A_new holds q once -- the paper's "duplicates removed", :113),
+// and emit A_{t+1} = survivors(A_t) U A_new with one CTA-wide prefix sum per 256 voxels.
+// Retirement is lazy ("cells that no longer have any void neighbors are discarded"):
+// p is dropped when this step's gather finds no void neighbour; the grid only grows, so that is
+// final.  Reading neighbours that other threads are claiming in the same step is harmless: a
+// target seen solid is solid at the end of the step anyway, and draws are keyed, not sequential.
+#include "liets_host.h"
+
+namespace liets {
+
+namespace {
+
+struct GridDims { int nx, ny, nz; };
+
+template <bool PERIODIC>
+__device__ __forceinline__ bool neighbour(int d, uint32_t p, int x, int y, int z, const GridDims& g,
+                                          uint32_t* q) {
+    const int dx = dir_dx(d), dy = dir_dy(d), dz = dir_dz(d);
+    int X = x + dx, Y = y + dy, Z = z + dz;
+    if (PERIODIC) {
+        if (dx < 0 && X < 0) X = g.nx - 1;
+        if (dx > 0 && X >= g.nx) X = 0;
+        if (dy < 0 && Y < 0) Y = g.ny - 1;
+        if (dy > 0 && Y >= g.ny) Y = 0;
+        if (dz < 0 && Z < 0) Z = g.nz - 1;
+        if (dz > 0 && Z >= g.nz) Z = 0;
+        *q = (uint32_t)X + (uint32_t)g.nx * ((uint32_t)Y + (uint32_t)g.ny * (uint32_t)Z);
+        return true;
+    } else {
+        if ((dx < 0 && X < 0) || (dx > 0 && X >= g.nx) || (dy < 0 && Y < 0) || (dy > 0 && Y >= g.ny) ||
+            (dz < 0 && Z < 0) || (dz > 0 && Z >= g.nz))
+            return false;
+        *q = (uint32_t)((long long)p + dx + (long long)g.nx * (dy + (long long)g.ny * dz));
+        return true;
+    }
+}
+
+template <bool PERIODIC>
+__global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint8_t* grid,
+                                                  uint32_t* list0, uint32_t* list1, GridDims dims,
+                                                  PhiloxKey key) {
+    if (!ctl->active) return;
+    __shared__ uint32_t s_scan[33];
+    __shared__ uint32_t s_base;
+    const uint32_t cur = ctl->cur;
+    const uint32_t n = ctl->count[cur];
+    const uint32_t* __restrict__ in = cur ? list1 : list0;
+    uint32_t* __restrict__ out = cur ? list0 : list1;
+    uint32_t* out_count = &ctl->count[cur ^ 1u];
+    const uint32_t t = ctl->step;
+    const uint32_t T0 = ctl->T[0], T1 = ctl->T[1], T2 = ctl->T[2];
+    const bool A0 = ctl->always[0], A1 = ctl->always[1], A2 = ctl->always[2];
+    uint32_t my_claims = 0;
+
+    for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t i = base + threadIdx.x;
+        const bool live = i < n;
+        uint32_t p = 0, mask = 0, won = 0;
+        int x = 0, y = 0, z = 0;
+        if (live) {
+            p = in[i];
+            x = (int)(p % (uint32_t)dims.nx);
+            const uint32_t rest = p / (uint32_t)dims.nx;
+            y = (int)(rest % (uint32_t)dims.ny);
+            z = (int)(rest / (uint32_t)dims.ny);
+#pragma unroll
+            for (int d = 0; d < 26; ++d) {                 // N_d, C_d (Algorithm 3 lines 5-6)
+                uint32_t q;
+                if (neighbour<PERIODIC>(d, p, x, y, z, dims, &q) && grid[q] == 0) mask |= 1u << d;
+            }
+#pragma unroll
+            for (int b = 0; b < 7; ++b) {                  // one Philox block = 4 directions (R9)
+                const uint32_t bm = (b < 6 ? 0xFu : 0x3u) << (4 * b);
+                if (mask & bm) {
+                    const uint4 r = philox4x32_10(p, 0u, t, (uint32_t)b, key);
+                    const uint32_t w[4] = { r.x, r.y, r.z, r.w };
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const int d = 4 * b + k;
+                        if (d >= 26) break;
+                        if (!((mask >> d) & 1u)) continue;
+                        const int cls = dir_class(d);
+                        const uint32_t T = cls == 0 ? T0 : (cls == 1 ? T1 : T2);
+                        const bool always = cls == 0 ? A0 : (cls == 1 ? A1 : A2);
+                        if (always || w[k] < T) {          // line 8: rand_num < G_d
+                            uint32_t q;
+                            neighbour<PERIODIC>(d, p, x, y, z, dims, &q);
+                            const uint32_t sh = (q & 3u) * 8u;
+                            const uint32_t old = atomicOr(reinterpret_cast<uint32_t*>(grid) + (q >> 2), 1u << sh);
+                            if (((old >> sh) & 0xFFu) == 0) won |= 1u << d;   // line 9-10: owner of q
+                        }
+                    }
+                }
+            }
+        }
+        // A_{t+1}: p survives iff it still saw a void neighbour; plus the voxels this thread claimed
+        const uint32_t keep = mask != 0 ? 1u : 0u;
+        const uint32_t cnt = keep + __popc(won);
+        my_claims += __popc(won);
+        uint32_t total;
+        uint32_t off = block_exclusive_scan(cnt, s_scan, &total);
+        if (threadIdx.x == 0) s_base = total ? atomicAdd(out_count, total) : 0u;
+        __syncthreads();
+        off += s_base;
+        if (keep) out[off++] = p;
+        while (won) {
+            const int d = __ffs(won) - 1;
+            won &= won - 1;
+            // recompute q for direction d (runtime d): offsets from the lexicographic code
+            const int raw = d + (d >= 13 ? 1 : 0);
+            int X = x + raw % 3 - 1, Y = y + (raw / 3) % 3 - 1, Z = z + raw / 9 - 1;
+            if (PERIODIC) {
+                X = X < 0 ? dims.nx - 1 : (X >= dims.nx ? 0 : X);
+                Y = Y < 0 ? dims.ny - 1 : (Y >= dims.ny ? 0 : Y);
+                Z = Z < 0 ? dims.nz - 1 : (Z >= dims.nz ? 0 : Z);
+            }
+            out[off++] = (uint32_t)X + (uint32_t)dims.nx * ((uint32_t)Y + (uint32_t)dims.ny * (uint32_t)Z);
+        }
+    }
+    // solid count: one atomic per warp at the end of the kernel
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) my_claims += __shfl_xor_sync(0xffffffffu, my_claims, o);
+    if ((threadIdx.x & 31u) == 0 && my_claims) atomicAdd(&ctl->claims, my_claims);
+}
+
+}  // namespace
+
+cudaError_t launch_grow_u8(liets_ctx* c) {
+    const GridDims dims{ c->nx, c->ny, c->nz };
+    const PhiloxKey key = philox_make_key(c->rng_seed);
+    const int grid = c->sm_count * 8;
+    if (c->boundary)
+        k_grow_u8<true><<<grid, 256, 0, c->stream>>>(c->ctl, c->grid_u8, c->list[0], c->list[1], dims, key);
+    else
+        k_grow_u8<false><<<grid, 256, 0, c->stream>>>(c->ctl, c->grid_u8, c->list[0], c->list[1], dims, key);
+    return cudaGetLastError();
+}
+
+}  // namespace liets

@@ -1,0 +1,283 @@
+// liets_api.cu -- the C ABI of libliets.so (include/liets.h).  Argument checking, workspace
+// layout, launch sequencing and read-back only: every step of the path runs in the kernels.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/liets.h"
+#include "liets_host.h"
+
+using namespace liets;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {
+    size_t ctl, grid, list0, list1, status2, total;
+};
+
+bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
+    if (nx < 1 || ny < 1 || nz < 1) return false;
+    const unsigned long long N = (unsigned long long)nx * (unsigned long long)ny * (unsigned long long)nz;
+    if (N >= (1ull << 32)) return false;
+    if (storage != LIETS_STORAGE_U8) return false;
+    size_t off = 0;
+    L->ctl = off;     off += align_up(sizeof(Control));
+    L->grid = off;    off += align_up((size_t)N + 4);
+    L->list0 = off;   off += align_up((size_t)N * 4);
+    L->list1 = off;   off += align_up((size_t)N * 4 < 64 ? 64 : (size_t)N * 4);
+    L->status2 = off; off += align_up(((size_t)N + 15) / 16 * 4);
+    L->total = off;
+    return true;
+}
+
+int fail(liets_ctx* c, int code, const char* msg) {
+    if (c) snprintf(c->err, sizeof(c->err), "%s", msg);
+    return code;
+}
+
+// prob in [0,1] -> floor(p 2^32 + 0.5) in [0, 2^32] (R8)
+uint64_t prob_to_threshold(double p) {
+    if (p <= 0.0) return 0;
+    if (p >= 1.0) return 1ull << 32;
+    return (uint64_t)std::floor(p * 4294967296.0 + 0.5);
+}
+
+int readback(liets_ctx* c) {
+    LIETS_CUDA_TRY(c, cudaMemcpyAsync(c->pinned, c->ctl, kControlScalarBytes, cudaMemcpyDeviceToHost, c->stream));
+    LIETS_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return 0;
+}
+
+int launch_step_kernel(liets_ctx* c) {
+    LIETS_CUDA_TRY(c, launch_grow_u8(c));
+    return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t liets_workspace_bytes(int nx, int ny, int nz, int storage) {
+    Layout L;
+    return make_layout(nx, ny, nz, storage, &L) ? L.total : 0;
+}
+
+int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int storage, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream) {
+    if (!out) return LIETS_E_ARG;
+    *out = nullptr;
+    Layout L;
+    if (!make_layout(nx, ny, nz, storage, &L)) return LIETS_E_ARG;
+    if (boundary != LIETS_BOUNDARY_WALL && boundary != LIETS_BOUNDARY_PERIODIC) return LIETS_E_ARG;
+    if (workspace && workspace_bytes < L.total) return LIETS_E_CAPACITY;
+    if (workspace && (reinterpret_cast<uintptr_t>(workspace) % kAlign)) return LIETS_E_ARG;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) return LIETS_E_CUDA;   // no CPU fallback
+
+    liets_ctx* c = new (std::nothrow) liets_ctx();
+    if (!c) return LIETS_E_CUDA;
+    memset(c, 0, sizeof(*c));
+    c->nx = nx; c->ny = ny; c->nz = nz; c->boundary = boundary; c->storage = storage;
+    c->N = (uint64_t)nx * (uint64_t)ny * (uint64_t)nz;
+    c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    c->law = LIETS_LAW_EQ1;
+    int dev = 0;
+    bool ok = cudaGetDevice(&dev) == cudaSuccess &&
+              cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess;
+    if (ok && !workspace) {
+        ok = cudaMalloc(&c->ws, L.total) == cudaSuccess;
+        c->owns_ws = ok;
+    } else {
+        c->ws = workspace;
+    }
+    c->ws_bytes = L.total;
+    ok = ok && cudaMallocHost(reinterpret_cast<void**>(&c->pinned), sizeof(Control)) == cudaSuccess;
+    ok = ok && cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
+    if (ok) {
+        char* base = static_cast<char*>(c->ws);
+        c->ctl = reinterpret_cast<Control*>(base + L.ctl);
+        c->grid_u8 = reinterpret_cast<uint8_t*>(base + L.grid);
+        c->list[0] = reinterpret_cast<uint32_t*>(base + L.list0);
+        c->list[1] = reinterpret_cast<uint32_t*>(base + L.list1);
+        c->status2 = reinterpret_cast<uint32_t*>(base + L.status2);
+        c->explicit_idx = reinterpret_cast<uint64_t*>(base + L.list1);
+        ok = cudaMemsetAsync(c->ctl, 0, sizeof(Control), c->stream) == cudaSuccess &&
+             launch_set_params(c) == cudaSuccess;
+    }
+    if (!ok) {
+        cudaGetLastError();
+        liets_destroy(c);
+        return LIETS_E_CUDA;
+    }
+    *out = c;
+    return LIETS_OK;
+}
+
+void liets_destroy(liets_ctx* c) {
+    if (!c) return;
+    if (c->stream || c->ws) cudaStreamSynchronize(c->stream);
+    if (c->owns_ws && c->ws) cudaFree(c->ws);
+    if (c->pinned) cudaFreeHost(c->pinned);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    delete c;
+}
+
+const char* liets_last_error(const liets_ctx* c) { return c ? c->err : "null ctx"; }
+
+int liets_set_growth(liets_ctx* c, double g_face, double g_edge, double g_corner, int law) {
+    if (!c) return LIETS_E_ARG;
+    const double g[3] = { g_face, g_edge, g_corner };
+    for (double v : g)
+        if (!(v >= 0.0 && v <= 1.0)) return fail(c, LIETS_E_ARG, "growth probability outside [0,1]");
+    if (law != LIETS_LAW_CONSTANT && law != LIETS_LAW_EQ1) return fail(c, LIETS_E_ARG, "unknown law");
+    for (int k = 0; k < 3; ++k) c->R[k] = prob_to_threshold(g[k]);
+    c->law = law;
+    c->growth_set = true;
+    LIETS_CUDA_TRY(c, launch_set_params(c));
+    return LIETS_OK;
+}
+
+int liets_set_target(liets_ctx* c, double phi) {
+    if (!c) return LIETS_E_ARG;
+    if (!(phi > 0.0 && phi <= 1.0)) return fail(c, LIETS_E_ARG, "target solid fraction outside (0,1]");
+    double x = std::ceil(phi * (double)c->N);               // R7: one IEEE multiply, then ceil
+    uint64_t n_t = x < 1.0 ? 1 : (x > (double)c->N ? c->N : (uint64_t)x);
+    c->n_t = n_t;
+    c->has_target = true;
+    LIETS_CUDA_TRY(c, launch_set_params(c));
+    return LIETS_OK;
+}
+
+int liets_seed(liets_ctx* c, double core_prob, int spacing_s, uint64_t rng_seed, uint64_t* n_seeds_out) {
+    if (!c) return LIETS_E_ARG;
+    if (!(core_prob >= 0.0 && core_prob <= 1.0)) return fail(c, LIETS_E_ARG, "core probability outside [0,1]");
+    if (spacing_s < 0) return fail(c, LIETS_E_ARG, "negative seed spacing");
+    c->rng_seed = rng_seed;
+    LIETS_CUDA_TRY(c, cudaEventRecord(c->ev0, c->stream));
+    LIETS_CUDA_TRY(c, launch_seed_reset(c));
+    const int accept_all = spacing_s <= 1;
+    LIETS_CUDA_TRY(c, launch_seed_candidates(c, prob_to_threshold(core_prob), accept_all));
+    if (!accept_all) {
+        for (;;) {                                          // rounds until no candidate is pending
+            for (int k = 0; k < 8; ++k) LIETS_CUDA_TRY(c, launch_spacing_round(c, spacing_s));
+            if (int rc = readback(c)) return rc;
+            if (c->pinned->n_unresolved == 0) break;
+        }
+    }
+    LIETS_CUDA_TRY(c, launch_seed_finalize(c));
+    LIETS_CUDA_TRY(c, cudaEventRecord(c->ev1, c->stream));
+    if (int rc = readback(c)) return rc;
+    LIETS_CUDA_TRY(c, cudaEventElapsedTime(&c->seed_ms, c->ev0, c->ev1));
+    c->seeded = true;
+    if (n_seeds_out) *n_seeds_out = c->pinned->n_solid;
+    return LIETS_OK;
+}
+
+int liets_seed_explicit(liets_ctx* c, const uint64_t* idx, uint64_t n, uint64_t rng_seed) {
+    if (!c || (n && !idx)) return LIETS_E_ARG;
+    if (n * 8 > c->N * 4) return fail(c, LIETS_E_CAPACITY, "too many explicit seeds for the staging buffer");
+    for (uint64_t i = 0; i < n; ++i)
+        if (idx[i] >= c->N) return fail(c, LIETS_E_ARG, "seed index outside the grid");
+    c->rng_seed = rng_seed;
+    LIETS_CUDA_TRY(c, launch_seed_reset(c));
+    if (n) LIETS_CUDA_TRY(c, cudaMemcpyAsync(c->explicit_idx, idx, n * 8, cudaMemcpyHostToDevice, c->stream));
+    LIETS_CUDA_TRY(c, launch_seed_explicit(c, n));
+    LIETS_CUDA_TRY(c, cudaStreamSynchronize(c->stream));    // idx may be pageable: do not outlive the call
+    c->seeded = true;
+    return LIETS_OK;
+}
+
+int liets_step(liets_ctx* c, uint64_t* n_solid_out, uint64_t* n_front_out) {
+    if (!c) return LIETS_E_ARG;
+    if (!c->seeded) return fail(c, LIETS_E_STATE, "liets_step before liets_seed");
+    if (c->law == LIETS_LAW_EQ1 && !c->has_target) return fail(c, LIETS_E_STATE, "Eq. (1) law needs a target");
+    LIETS_CUDA_TRY(c, launch_begin(c, 0, 0));
+    LIETS_CUDA_TRY(c, launch_control(c, kCtlPrepare | kCtlForce));
+    if (int rc = launch_step_kernel(c)) return rc;
+    LIETS_CUDA_TRY(c, launch_control(c, kCtlFinish));
+    if (n_solid_out || n_front_out) {
+        if (int rc = readback(c)) return rc;
+        const uint64_t ns = c->pinned->n_solid;
+        if (n_solid_out) *n_solid_out = ns;
+        if (n_front_out) *n_front_out = (ns == 0 || ns == c->N) ? 0 : c->pinned->count[c->pinned->cur];
+    }
+    return LIETS_OK;
+}
+
+int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps_out, uint64_t* n_solid_out) {
+    if (!c) return LIETS_E_ARG;
+    if (int rc = liets_set_target(c, phi)) return rc;
+    if (!c->seeded) return fail(c, LIETS_E_STATE, "liets_generate before liets_seed");
+    LIETS_CUDA_TRY(c, cudaEventRecord(c->ev0, c->stream));
+    LIETS_CUDA_TRY(c, launch_begin(c, 1, max_steps));
+    uint32_t enqueued = 0;
+    for (;;) {
+        // a batch of steps back to back; steps after the stop rule fired are no-ops on the device
+        uint32_t batch = 16;
+        if (max_steps - enqueued < batch) batch = max_steps - enqueued;
+        for (uint32_t k = 0; k < batch; ++k) {
+            LIETS_CUDA_TRY(c, launch_control(c, k == 0 ? kCtlPrepare : (kCtlFinish | kCtlPrepare)));
+            if (int rc = launch_step_kernel(c)) return rc;
+        }
+        enqueued += batch;
+        LIETS_CUDA_TRY(c, launch_control(c, kCtlFinish | kCtlEval));
+        if (int rc = readback(c)) return rc;
+        if (c->pinned->status != kStatusRunning) break;
+    }
+    LIETS_CUDA_TRY(c, cudaEventRecord(c->ev1, c->stream));
+    LIETS_CUDA_TRY(c, cudaEventSynchronize(c->ev1));
+    LIETS_CUDA_TRY(c, cudaEventElapsedTime(&c->gen_ms, c->ev0, c->ev1));
+    if (steps_out) *steps_out = c->pinned->steps_done;
+    if (n_solid_out) *n_solid_out = c->pinned->n_solid;
+    return c->pinned->status;
+}
+
+int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is_device) {
+    if (!c || !dst) return LIETS_E_ARG;
+    const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (format == LIETS_FORMAT_U8) {
+        if (dst_bytes < c->N) return fail(c, LIETS_E_CAPACITY, "dst smaller than N bytes");
+        LIETS_CUDA_TRY(c, cudaMemcpyAsync(dst, c->grid_u8, c->N, kind, c->stream));
+    } else if (format == LIETS_FORMAT_BITS) {
+        const size_t nb = (size_t)((c->N + 7) / 8);
+        if (dst_bytes < nb) return fail(c, LIETS_E_CAPACITY, "dst smaller than ceil(N/8) bytes");
+        if (dst_is_device) {
+            LIETS_CUDA_TRY(c, launch_pack_bits_u8(c, static_cast<uint8_t*>(dst)));
+        } else {                                            // pack into the (idle) seeding scratch, then copy
+            LIETS_CUDA_TRY(c, launch_pack_bits_u8(c, reinterpret_cast<uint8_t*>(c->status2)));
+            LIETS_CUDA_TRY(c, cudaMemcpyAsync(dst, c->status2, nb, kind, c->stream));
+        }
+    } else {
+        return fail(c, LIETS_E_ARG, "unknown grid format");
+    }
+    if (!dst_is_device) LIETS_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return LIETS_OK;
+}
+
+int liets_step_log(liets_ctx* c, uint64_t* front_in, uint64_t* solid_after, uint32_t cap) {
+    if (!c) return LIETS_E_ARG;
+    if (int rc = readback(c)) return rc;
+    uint32_t n = c->pinned->step;
+    if (n > kLogCap) n = kLogCap;
+    if (n > cap) n = cap;
+    if (n && front_in)
+        LIETS_CUDA_TRY(c, cudaMemcpyAsync(front_in, c->ctl->log_front, n * 8ull, cudaMemcpyDeviceToHost, c->stream));
+    if (n && solid_after)
+        LIETS_CUDA_TRY(c, cudaMemcpyAsync(solid_after, c->ctl->log_solid, n * 8ull, cudaMemcpyDeviceToHost, c->stream));
+    LIETS_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return (int)n;
+}
+
+int liets_timings(liets_ctx* c, float* seed_ms, float* generate_ms) {
+    if (!c) return LIETS_E_ARG;
+    if (seed_ms) *seed_ms = c->seed_ms;
+    if (generate_ms) *generate_ms = c->gen_ms;
+    return LIETS_OK;
+}
+
+}  // extern "C"

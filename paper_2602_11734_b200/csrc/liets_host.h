@@ -1,0 +1,67 @@
+// liets_host.h -- host-side context of libliets.so and the launchers each .cu file exports.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cstdio>
+#include <cuda_runtime.h>
+
+#include "liets_device.cuh"
+
+struct HostReadback {                 // pinned; filled by cudaMemcpyAsync from the Control block
+    liets::Control head;              // (only the leading scalar part is copied)
+};
+
+struct liets_ctx {
+    int nx, ny, nz, boundary, storage;
+    uint64_t N;
+    cudaStream_t stream;
+    void* ws;
+    size_t ws_bytes;
+    bool owns_ws;
+    int sm_count;
+    // device pointers into ws
+    liets::Control* ctl;
+    uint8_t* grid_u8;                 // STORAGE_U8: N bytes (padded to 4)
+    uint32_t* list[2];                // front lists (voxel indices / brick ids), capacity N each
+    uint32_t* status2;                // seeding: 2 bits per voxel (00 none/rejected, 01 pending, 11 accepted)
+    uint64_t* explicit_idx;           // staging for liets_seed_explicit (aliases list[1])
+    // host state
+    liets::Control* pinned;           // pinned host copy of the scalar part of Control
+    cudaEvent_t ev0, ev1;
+    bool seeded, has_target, growth_set;
+    uint64_t rng_seed;
+    uint64_t R[3];
+    int law;
+    uint64_t n_t;
+    float seed_ms, gen_ms;
+    char err[256];
+};
+
+#define LIETS_CUDA_TRY(ctx, expr)                                                                 \
+    do {                                                                                          \
+        cudaError_t e__ = (expr);                                                                 \
+        if (e__ != cudaSuccess) {                                                                 \
+            snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d: %s: %s", __FILE__, __LINE__, #expr,   \
+                     cudaGetErrorString(e__));                                                    \
+            return -4;                                                                            \
+        }                                                                                         \
+    } while (0)
+
+namespace liets {
+constexpr size_t kControlScalarBytes = offsetof(Control, log_front);
+
+// control.cu
+cudaError_t launch_control(liets_ctx* c, uint32_t flags);
+cudaError_t launch_begin(liets_ctx* c, int generate, uint32_t max_steps);
+cudaError_t launch_set_params(liets_ctx* c);
+// grow_u8.cu
+cudaError_t launch_grow_u8(liets_ctx* c);
+// seed.cu
+cudaError_t launch_seed_reset(liets_ctx* c);
+cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all);
+cudaError_t launch_spacing_round(liets_ctx* c, int s);
+cudaError_t launch_seed_finalize(liets_ctx* c);
+cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n);
+// export.cu
+cudaError_t launch_pack_bits_u8(liets_ctx* c, uint8_t* dst_bits);
+}  // namespace liets

@@ -1,0 +1,244 @@
+// seed.cu -- seeding and seed spacing by the L1 "diamond".
+//
+// Candidates: voxel v is a candidate core iff philox(seed; v>>2)[v&3] < T_core (R9).
+// Spacing (R11, R12): the sequential rule "scan candidates in ascending index, accept iff no
+// accepted seed within L1 < s" is reproduced exactly by parallel rounds over a 2-bit-per-voxel
+// status map (00 = no candidate / rejected, 01 = pending, 11 = accepted):
+//   a pending candidate v looks at every LOWER-index voxel within L1 < s (its diamond);
+//   - any accepted one  -> v is rejected (final: that seed is accepted in the sequential scan too);
+//   - else any pending  -> v waits (its fate depends on them);
+//   - else              -> v is accepted (all lower-index candidates in range are rejected).
+// Each state change is one atomic on one word, states only move 01 -> {00, 11}, so reading
+// neighbours that change during a round is safe, and the fixed point is the sequential result.
+#include "liets_host.h"
+
+namespace liets {
+
+namespace {
+
+__device__ __forceinline__ uint32_t ld_cg(const uint32_t* p) {
+    return __ldcg(p);
+}
+
+// --- reset: grid, status map, counters ---------------------------------------------------------
+__global__ void k_seed_reset(Control* c) {
+    c->n_solid = 0; c->step = 0; c->steps_done = 0; c->active = 0; c->status = 0; c->cur = 0;
+    c->count[0] = 0; c->count[1] = 0; c->claims = 0; c->n_cand = 0; c->n_unresolved = 0;
+    c->round_pending = 0;
+}
+
+// --- candidates: one thread per status word = 16 voxels = 4 Philox blocks -----------------------
+__global__ void __launch_bounds__(256) k_seed_candidates(Control* ctl, uint32_t* status2, uint32_t* cand,
+                                                          unsigned long long N, uint32_t T_core,
+                                                          uint32_t always, uint32_t accept_all,
+                                                          PhiloxKey key) {
+    __shared__ uint32_t s_scan[33];
+    __shared__ uint32_t s_base;
+    const unsigned long long n_words = (N + 15ull) / 16ull;
+    for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < n_words;
+         base += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long w = base + threadIdx.x;
+        uint32_t bits = 0;                                  // bit k: voxel 16w+k is a candidate
+        if (w < n_words) {
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const unsigned long long blk = 4ull * w + b;          // = v >> 2
+                if (blk * 4ull >= N) break;
+                const uint4 r = philox4x32_10((uint32_t)blk, (uint32_t)(blk >> 32), 0u, 0xFFFFFFFFu, key);
+                const uint32_t d[4] = { r.x, r.y, r.z, r.w };
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (blk * 4ull + k < N && (always || d[k] < T_core)) bits |= 1u << (4 * b + k);
+            }
+            uint32_t word = 0;                              // spread: bit k -> field 2k
+            for (uint32_t m = bits; m; m &= m - 1) {
+                const int k = __ffs(m) - 1;
+                word |= (accept_all ? 3u : 1u) << (2 * k);
+            }
+            status2[w] = word;
+        }
+        uint32_t total;
+        uint32_t off = block_exclusive_scan(__popc(bits), s_scan, &total);
+        if (threadIdx.x == 0) s_base = total ? atomicAdd(&ctl->n_cand, total) : 0u;
+        __syncthreads();
+        off += s_base;
+        for (uint32_t m = bits; m; m &= m - 1) cand[off++] = (uint32_t)(16ull * w + (__ffs(m) - 1));
+    }
+}
+
+// --- one spacing round: one warp per candidate, lanes over the rows of its diamond --------------
+struct Dims { int nx, ny, nz, periodic; };
+
+// scan the voxels [i0, i1] (linear indices, same row) of the status map; only those with linear
+// index < limit count.  Sets accepted / pending flags.
+__device__ __forceinline__ void scan_segment(const uint32_t* status2, unsigned long long i0,
+                                             unsigned long long i1, unsigned long long limit,
+                                             bool* accepted, bool* pending) {
+    if (i0 >= limit) return;
+    if (i1 >= limit) i1 = limit - 1;
+    for (unsigned long long w = i0 >> 4; w <= (i1 >> 4); ++w) {
+        uint32_t word = ld_cg(status2 + w);
+        if (!word) continue;
+        const unsigned long long lo = w << 4;
+        uint32_t field = 0xFFFFFFFFu;                       // keep fields of voxels in [i0, i1]
+        if (i0 > lo) field &= 0xFFFFFFFFu << (2 * (uint32_t)(i0 - lo));
+        if (i1 < lo + 15) field &= 0xFFFFFFFFu >> (2 * (uint32_t)(lo + 15 - i1));
+        word &= field;
+        const uint32_t b0 = word & 0x55555555u, b1 = (word >> 1) & 0x55555555u;
+        if (b0 & b1) *accepted = true;
+        if (b0 & ~b1) *pending = true;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_spacing_round(Control* ctl, uint32_t* status2,
+                                                        const uint32_t* cand, Dims g, int s) {
+    if (ctl->n_unresolved == 0) return;                     // fixed point reached: later rounds are no-ops
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t warp_global = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t n_cand = ctl->n_cand;
+    const int r = s - 1;                                    // diamond radius: L1 <= s-1  <=>  L1 < s
+    const int side = 2 * r + 1;
+    uint32_t still = 0;
+    for (uint32_t i = warp_global; i < n_cand; i += n_warps) {
+        const uint32_t v = cand[i];
+        const uint32_t st = (ld_cg(status2 + (v >> 4)) >> (2 * (v & 15u))) & 3u;
+        if (st != 1u) continue;                             // already resolved
+        const int x = (int)(v % (uint32_t)g.nx);
+        const uint32_t rest = v / (uint32_t)g.nx;
+        const int y = (int)(rest % (uint32_t)g.ny), z = (int)(rest / (uint32_t)g.ny);
+        bool accepted = false, pending = false;
+        for (int j = (int)lane; j < side * side; j += 32) {
+            const int dz = j / side - r, dy = j % side - r;
+            const int rem = r - abs(dz) - abs(dy);
+            if (rem < 0) continue;
+            int Y = y + dy, Z = z + dz;
+            if (g.periodic) {
+                Y %= g.ny; if (Y < 0) Y += g.ny;
+                Z %= g.nz; if (Z < 0) Z += g.nz;
+            } else if (Y < 0 || Y >= g.ny || Z < 0 || Z >= g.nz) {
+                continue;
+            }
+            const unsigned long long row = ((unsigned long long)Z * g.ny + Y) * (unsigned long long)g.nx;
+            int xa = x - rem, xb = x + rem;
+            if (g.periodic && 2 * rem + 1 >= g.nx) {        // the range covers the whole row
+                scan_segment(status2, row, row + g.nx - 1, v, &accepted, &pending);
+            } else if (!g.periodic) {                       // clipped at the walls
+                xa = xa < 0 ? 0 : xa;
+                xb = xb >= g.nx ? g.nx - 1 : xb;
+                scan_segment(status2, row + xa, row + xb, v, &accepted, &pending);
+            } else {                                        // wrapped range, at most two segments
+                if (xa < 0) {
+                    scan_segment(status2, row + (xa + g.nx), row + g.nx - 1, v, &accepted, &pending);
+                    xa = 0;
+                }
+                if (xb >= g.nx) {
+                    scan_segment(status2, row, row + (xb - g.nx), v, &accepted, &pending);
+                    xb = g.nx - 1;
+                }
+                scan_segment(status2, row + xa, row + xb, v, &accepted, &pending);
+            }
+        }
+        accepted = __any_sync(0xffffffffu, accepted);
+        pending = __any_sync(0xffffffffu, pending);
+        if (lane == 0) {
+            if (accepted) atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u))));        // 01 -> 00
+            else if (!pending) atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u)));       // 01 -> 11
+            else still++;
+        }
+    }
+    if (lane == 0 && still) atomicAdd(&ctl->round_pending, still);
+}
+
+// between rounds: n_unresolved <- number of candidates the round just done left pending
+__global__ void k_spacing_roll(Control* c, int first) {
+    c->n_unresolved = first ? c->n_cand : c->round_pending;
+    c->round_pending = 0;
+}
+
+// --- finalize: accepted candidates -> grid + initial front A_0 = seeds (R3) ---------------------
+__global__ void __launch_bounds__(256) k_seed_finalize_u8(Control* ctl, const uint32_t* status2,
+                                                           const uint32_t* cand, uint8_t* grid,
+                                                           uint32_t* front) {
+    __shared__ uint32_t s_scan[33];
+    __shared__ uint32_t s_base;
+    const uint32_t n = ctl->n_cand;
+    for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t i = base + threadIdx.x;
+        uint32_t v = 0, acc = 0;
+        if (i < n) {
+            v = cand[i];
+            acc = ((status2[v >> 4] >> (2 * (v & 15u))) & 3u) == 3u;
+        }
+        uint32_t total;
+        uint32_t off = block_exclusive_scan(acc, s_scan, &total);
+        if (threadIdx.x == 0) s_base = total ? atomicAdd(&ctl->count[0], total) : 0u;
+        __syncthreads();
+        if (acc) { front[s_base + off] = v; grid[v] = 1; }
+    }
+}
+
+__global__ void k_seed_close(Control* c) { c->n_solid = c->count[0]; c->cur = 0; }
+
+// --- explicit seeds: dedupe with the 0 -> 1 transition of the grid byte -------------------------
+__global__ void k_seed_explicit_u8(Control* ctl, const unsigned long long* idx, unsigned long long n,
+                                   uint8_t* grid, uint32_t* front) {
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t v = (uint32_t)idx[i];
+        const uint32_t sh = (v & 3u) * 8u;
+        const uint32_t old = atomicOr(reinterpret_cast<uint32_t*>(grid) + (v >> 2), 1u << sh);
+        if (((old >> sh) & 0xFFu) == 0) front[atomicAdd(&ctl->count[0], 1u)] = v;
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_seed_reset(liets_ctx* c) {
+    cudaError_t e = cudaMemsetAsync(c->grid_u8, 0, (c->N + 3) & ~3ull, c->stream);
+    if (e != cudaSuccess) return e;
+    k_seed_reset<<<1, 1, 0, c->stream>>>(c->ctl);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all) {
+    const PhiloxKey key = philox_make_key(c->rng_seed);
+    const uint32_t always = t_core >= (1ull << 32);
+    const uint32_t T = always ? 0xFFFFFFFFu : (uint32_t)t_core;
+    k_seed_candidates<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->status2, c->list[1], c->N, T, always,
+                                                              (uint32_t)accept_all, key);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    k_spacing_roll<<<1, 1, 0, c->stream>>>(c->ctl, 1);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_spacing_round(liets_ctx* c, int s) {
+    const Dims g{ c->nx, c->ny, c->nz, c->boundary };
+    k_spacing_round<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->list[1], g, s);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    k_spacing_roll<<<1, 1, 0, c->stream>>>(c->ctl, 0);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_seed_finalize(liets_ctx* c) {
+    k_seed_finalize_u8<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->list[1], c->grid_u8, c->list[0]);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    k_seed_close<<<1, 1, 0, c->stream>>>(c->ctl);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n) {
+    if (n) {
+        k_seed_explicit_u8<<<c->sm_count * 2, 256, 0, c->stream>>>(c->ctl, (const unsigned long long*)c->explicit_idx, n,
+                                                                  c->grid_u8, c->list[0]);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    k_seed_close<<<1, 1, 0, c->stream>>>(c->ctl);
+    return cudaGetLastError();
+}
+
+}  // namespace liets

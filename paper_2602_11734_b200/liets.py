@@ -1,0 +1,172 @@
+"""ctypes binding of libliets.so -- same names as include/liets.h, argument marshalling only."""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libliets.so")
+
+OK, FRONT_EMPTY, MAX_STEPS = 0, 1, 2
+E_ARG, E_STATE, E_CAPACITY, E_CUDA = -1, -2, -3, -4
+BOUNDARY_WALL, BOUNDARY_PERIODIC = 0, 1
+STORAGE_U8, STORAGE_BRICK = 0, 1
+LAW_CONSTANT, LAW_EQ1 = 0, 1
+FORMAT_U8, FORMAT_BITS = 0, 1
+
+# every symbol include/liets.h declares
+EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
+           "liets_set_target", "liets_step", "liets_generate", "liets_grid", "liets_step_log", "liets_timings",
+           "liets_destroy", "liets_last_error")
+
+
+class LietsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("liets error %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def library_path():
+    return _LIB_PATH
+
+
+def lib():
+    """Load libliets.so (built by ``python -m paper_2602_11734_b200.build``). No fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError("libliets.so is not built: run `python -m paper_2602_11734_b200.build` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(_LIB_PATH)
+    vp, ci, dbl, u32, u64, sz = (ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_uint32,
+                                 ctypes.c_uint64, ctypes.c_size_t)
+    P = ctypes.POINTER
+    L.liets_workspace_bytes.argtypes = [ci, ci, ci, ci]
+    L.liets_workspace_bytes.restype = sz
+    L.liets_create.argtypes = [P(vp), ci, ci, ci, ci, ci, vp, sz, vp]
+    L.liets_create.restype = ci
+    L.liets_set_growth.argtypes = [vp, dbl, dbl, dbl, ci]
+    L.liets_set_growth.restype = ci
+    L.liets_seed.argtypes = [vp, dbl, ci, u64, P(u64)]
+    L.liets_seed.restype = ci
+    L.liets_seed_explicit.argtypes = [vp, P(u64), u64, u64]
+    L.liets_seed_explicit.restype = ci
+    L.liets_set_target.argtypes = [vp, dbl]
+    L.liets_set_target.restype = ci
+    L.liets_step.argtypes = [vp, P(u64), P(u64)]
+    L.liets_step.restype = ci
+    L.liets_generate.argtypes = [vp, dbl, u32, P(u32), P(u64)]
+    L.liets_generate.restype = ci
+    L.liets_grid.argtypes = [vp, vp, sz, ci, ci]
+    L.liets_grid.restype = ci
+    L.liets_step_log.argtypes = [vp, P(u64), P(u64), u32]
+    L.liets_step_log.restype = ci
+    L.liets_timings.argtypes = [vp, P(ctypes.c_float), P(ctypes.c_float)]
+    L.liets_timings.restype = ci
+    L.liets_destroy.argtypes = [vp]
+    L.liets_destroy.restype = None
+    L.liets_last_error.argtypes = [vp]
+    L.liets_last_error.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+class Liets:
+    """One generator context.  Mirrors the C ABI: create -> set_growth -> seed -> step / generate -> grid."""
+
+    def __init__(self, nx, ny, nz, boundary=BOUNDARY_WALL, storage=STORAGE_U8, device="cuda:0", stream=None):
+        import torch  # device memory and streams only
+        self._L = lib()
+        self._torch = torch
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.N = self.nx * self.ny * self.nz
+        self.boundary, self.storage = int(boundary), int(storage)
+        if not torch.cuda.is_available():
+            raise LietsError(E_CUDA, "no CUDA device (there is no CPU fallback)")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        nbytes = self._L.liets_workspace_bytes(self.nx, self.ny, self.nz, self.storage)
+        if nbytes == 0:
+            raise LietsError(E_ARG, "bad grid dimensions or storage")
+        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self._ws.data_ptr() + 255) // 256 * 256
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = ctypes.c_void_p()
+        rc = self._L.liets_create(ctypes.byref(h), self.nx, self.ny, self.nz, self.boundary, self.storage,
+                                  ctypes.c_void_p(base), nbytes, ctypes.c_void_p(self._stream.cuda_stream))
+        if rc < 0:
+            raise LietsError(rc, "liets_create failed")
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.liets_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        self.close()
+
+    def _check(self, rc):
+        if rc < 0:
+            raise LietsError(rc, self._L.liets_last_error(self._h).decode())
+        return rc
+
+    def set_growth(self, g_face, g_edge, g_corner, law=LAW_EQ1):
+        self._check(self._L.liets_set_growth(self._h, g_face, g_edge, g_corner, law))
+
+    def seed(self, core_prob, spacing_s, rng_seed):
+        n = ctypes.c_uint64(0)
+        self._check(self._L.liets_seed(self._h, core_prob, spacing_s, rng_seed, ctypes.byref(n)))
+        return int(n.value)
+
+    def seed_explicit(self, idx, rng_seed=0):
+        a = np.ascontiguousarray(idx, dtype=np.uint64)
+        self._check(self._L.liets_seed_explicit(self._h, a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)),
+                                                a.size, rng_seed))
+
+    def set_target(self, phi):
+        self._check(self._L.liets_set_target(self._h, phi))
+
+    def step(self):
+        ns, nf = ctypes.c_uint64(0), ctypes.c_uint64(0)
+        self._check(self._L.liets_step(self._h, ctypes.byref(ns), ctypes.byref(nf)))
+        return int(ns.value), int(nf.value)
+
+    def generate(self, phi, max_steps=100000):
+        steps, ns = ctypes.c_uint32(0), ctypes.c_uint64(0)
+        rc = self._check(self._L.liets_generate(self._h, phi, max_steps, ctypes.byref(steps), ctypes.byref(ns)))
+        return rc, int(steps.value), int(ns.value)
+
+    def grid(self, format=FORMAT_U8):
+        """Phase array on the host: uint8 (nz, ny, nx) for FORMAT_U8, flat packed bytes for FORMAT_BITS."""
+        n = self.N if format == FORMAT_U8 else (self.N + 7) // 8
+        out = np.empty(n, dtype=np.uint8)
+        self._check(self._L.liets_grid(self._h, out.ctypes.data, n, format, 0))
+        return out.reshape(self.nz, self.ny, self.nx) if format == FORMAT_U8 else out
+
+    def grid_into(self, host_ptr, nbytes, format=FORMAT_U8):
+        """Copy the phase array into a caller-owned HOST buffer (e.g. pinned memory)."""
+        self._check(self._L.liets_grid(self._h, ctypes.c_void_p(host_ptr), nbytes, format, 0))
+
+    def grid_device(self, format=FORMAT_U8):
+        n = self.N if format == FORMAT_U8 else (self.N + 7) // 8
+        out = self._torch.empty(n, dtype=self._torch.uint8, device=self.device)
+        self._check(self._L.liets_grid(self._h, ctypes.c_void_p(out.data_ptr()), n, format, 1))
+        return out
+
+    def step_log(self, cap=4096):
+        f = np.zeros(cap, dtype=np.uint64)
+        s = np.zeros(cap, dtype=np.uint64)
+        P64 = ctypes.POINTER(ctypes.c_uint64)
+        n = self._check(self._L.liets_step_log(self._h, f.ctypes.data_as(P64), s.ctypes.data_as(P64), cap))
+        return f[:n].copy(), s[:n].copy()
+
+    def timings(self):
+        a, b = ctypes.c_float(0), ctypes.c_float(0)
+        self._check(self._L.liets_timings(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return float(a.value), float(b.value)

@@ -1,0 +1,160 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, bit for bit."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import CONFIGS
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def liets():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    import paper_2602_11734_b200 as m
+    m.lib()
+    return m
+
+
+STORAGES = [0]
+
+
+def run_both(liets, dims, periodic, core, s, seed, g, law, target, storage, max_steps=100000):
+    nx, ny, nz = dims
+    o = oracle.Oracle(nx, ny, nz, periodic)
+    o.set_growth(*g, law)
+    n_o = o.seed(core, s, seed)
+    L = liets.Liets(nx, ny, nz, int(periodic), storage)
+    L.set_growth(*g, law)
+    n_g = L.seed(core, s, seed)
+    assert n_g == n_o
+    assert (L.grid() == o.grid()).all(), "seeds differ"
+    rc_o, st_o = o.generate(target, max_steps, True)
+    rc_g, st_g, ns_g = L.generate(target, max_steps)
+    assert (rc_g, st_g, ns_g) == (rc_o, st_o, o.n_solid)
+    assert (L.grid() == o.grid()).all(), "grids differ"
+    return o, L
+
+
+@pytest.mark.parametrize("storage", STORAGES)
+def test_config1_bit_exact(liets, storage):
+    c = CONFIGS["cfg1_64"]
+    o, L = run_both(liets, c["dims"], c["periodic"], c["core"], c["s"], c["seeds"][0], c["g"], 1, c["targets"][0], storage)
+    # porosity matches exactly; bits format agrees with u8
+    assert int(L.grid().sum()) == o.n_solid
+    bits = np.unpackbits(L.grid(liets.FORMAT_BITS), bitorder="little")[: L.N]
+    assert (bits == o.grid().ravel()).all()
+    assert (L.grid_device().cpu().numpy() == o.grid().ravel()).all()
+    f, s = L.step_log()
+    assert len(f) == o.step_index and int(s[-1]) == o.n_solid
+
+
+@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("dims,core,s", [((37, 29, 41), 0.01, 4), ((70, 45, 33), 0.004, 7), ((5, 4, 3), 0.2, 2),
+                                          ((1, 9, 2), 0.3, 0), ((96, 96, 96), 0.003, 9), ((17, 130, 9), 0.02, 3)])
+def test_ragged_shapes_bit_exact(liets, storage, periodic, dims, core, s):
+    run_both(liets, dims, periodic, core, s, 5, (0.05, 0.02, 0.01), 1, 0.55, storage)
+
+
+@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("periodic", [False, True])
+def test_step_by_step_equals_generate(liets, storage, periodic):
+    dims, g = (48, 40, 52), (0.03, 0.01, 0.002)
+    o = oracle.Oracle(*dims, periodic)
+    o.set_growth(*g, 1); o.set_target(0.5); o.seed(0.004, 5, 9)
+    A = liets.Liets(*dims, int(periodic), storage)
+    A.set_growth(*g, 1); A.set_target(0.5); A.seed(0.004, 5, 9)
+    while o.n_solid < o.n_target:
+        o.step(True)
+        ns, nf = A.step()
+        assert ns == o.n_solid and (nf == 0) == (o.n_front_exact == 0)
+        assert (A.grid() == o.grid()).all(), o.step_index
+    B = liets.Liets(*dims, int(periodic), storage)
+    B.set_growth(*g, 1); B.seed(0.004, 5, 9)
+    rc, steps, ns = B.generate(0.5)
+    assert rc == liets.OK and steps == o.step_index and (B.grid() == A.grid()).all()
+    # resume with a higher target continues the same stream (P11)
+    rc_o, more_o = o.generate(0.7, 10**6, True)
+    rc, more, ns = B.generate(0.7)
+    assert (rc, more, ns) == (rc_o, more_o, o.n_solid) and (B.grid() == o.grid()).all()
+    # target already met: zero steps (R15)
+    assert B.generate(0.7)[:2] == (liets.OK, 0)
+
+
+@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("periodic", [False, True])
+def test_closed_forms_on_gpu(liets, storage, periodic):
+    nx, ny, nz = 23, 19, 21
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+
+    def ad(a, b, n):
+        d = np.abs(a - b)
+        return np.minimum(d, n - d) if periodic else d
+    seeds = [(0, 0, 0), (22, 18, 20), (11, 9, 10)]
+    idx = [sx + nx * (sy + ny * sz) for sx, sy, sz in seeds]
+    L = liets.Liets(nx, ny, nz, int(periodic), storage)
+    L.set_growth(1.0, 0.0, 0.0, liets.LAW_CONSTANT)          # faces only, p = 1: union of L1 balls (P3)
+    L.seed_explicit(idx + idx[:1])
+    for k in range(1, 6):
+        L.step()
+        d = np.min([ad(x, sx, nx) + ad(y, sy, ny) + ad(z, sz, nz) for sx, sy, sz in seeds], axis=0)
+        assert (L.grid() == (d <= k)).all()
+    L.set_growth(1.0, 1.0, 1.0, liets.LAW_CONSTANT)          # all 26, p = 1: Chebyshev cubes (P4)
+    L.seed_explicit(idx)
+    for k in range(1, 5):
+        L.step()
+        d = np.min([np.maximum(np.maximum(ad(x, sx, nx), ad(y, sy, ny)), ad(z, sz, nz)) for sx, sy, sz in seeds], axis=0)
+        assert (L.grid() == (d <= k)).all()
+    L.set_growth(0.0, 0.0, 0.0, liets.LAW_CONSTANT)          # all G = 0: exactly the seeds (P2)
+    L.seed(0.01, 0, 3)
+    g0 = L.grid()
+    rc, steps, ns = L.generate(0.5, 6)
+    assert (rc, steps) == (liets.MAX_STEPS, 6) and (L.grid() == g0).all() and ns == g0.sum()
+
+
+@pytest.mark.parametrize("storage", STORAGES)
+def test_degenerate_cases(liets, storage):
+    L = liets.Liets(6, 6, 6, 0, storage)
+    L.set_growth(0.5, 0.5, 0.5, liets.LAW_CONSTANT)
+    assert L.seed(0.0, 0, 1) == 0                             # no seeds: empty front
+    assert L.generate(0.5, 10)[:2] == (liets.FRONT_EMPTY, 0)
+    L.set_growth(1.0, 1.0, 1.0, liets.LAW_CONSTANT)
+    L.seed_explicit([0])
+    assert L.generate(1.0, 2)[:2] == (liets.MAX_STEPS, 2)
+    rc, steps, ns = L.generate(1.0, 100)
+    assert rc == liets.OK and ns == 216
+    assert L.step() == (216, 0)                               # full grid: front is empty
+    assert L.seed(1.0, 0, 1) == 216                           # every voxel a core
+    M = liets.Liets(12, 12, 12, 1, storage)
+    assert M.seed(1.0, 3, 1) == oracle_seed_count(12, True, 1.0, 3, 1)
+    with pytest.raises(liets.LietsError):
+        liets.Liets(0, 4, 4)
+    N = liets.Liets(4, 4, 4, 0, storage)
+    with pytest.raises(liets.LietsError):
+        N.step()                                              # before seed
+    with pytest.raises(liets.LietsError):
+        N.set_growth(1.5, 0, 0)
+    N.seed(0.5, 0, 1)
+    with pytest.raises(liets.LietsError):
+        N.step()                                              # Eq. (1) without target
+
+
+def oracle_seed_count(n, periodic, core, s, seed):
+    o = oracle.Oracle(n, n, n, periodic)
+    return o.seed(core, s, seed)
+
+
+@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("seed", CONFIGS["cfg2_200"]["seeds"][:2])
+def test_config2_bit_exact(liets, storage, seed):
+    c = CONFIGS["cfg2_200"]
+    o, L = run_both(liets, c["dims"], c["periodic"], c["core"], c["s"], seed, c["g"], 1, c["targets"][0], storage)
+    # two-point correlation of the GPU grid, computed with the oracle, equals that of the oracle grid
+    for axis in range(3):
+        pg, vg = oracle.s2(L.grid(), False, axis, 16)
+        po, vo = oracle.s2(o.grid(), False, axis, 16)
+        assert (pg == po).all() and (vg == vo).all()
+        assert pg[0] == L.N - o.n_solid
