@@ -1,0 +1,302 @@
+#!/usr/bin/env python
+"""bench.py -- whole-generation throughput of the LIETS growth path on B200 (one JSON line).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--storage 0|1]
+
+A "step" is one pass of the whole hot path over one synthetic workload: liets_seed (keyed seeding +
+L1 seed spacing) followed by liets_generate (device-resident growth loop to the target fraction)
+on BASELINE.json's 400^3 timing configuration (workloads.BENCH).  `value` = voxel nodes/s =
+N_voxels * n_gpus / device time, timed with CUDA events on the launching stream; `e2e` = the same
+through the C ABI with a HOST output buffer (device->host copy of the phase array inside the
+timed region).  Multi-GPU = independent replicas (one realisation per rank, no collective on the
+data path), timing = max over ranks.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML while the timed regions run."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def algorithmic_bytes(storage, N, front, solid_after, n_seeds):
+    """bytes the list-indexed step itself must move, per step.
+
+    STORAGE_U8 (front = voxels):  4|A_t| + min(27|A_t|, N) + c_t + 4|A_{t+1}|
+    STORAGE_BRICK (front = 8^3 bricks of 64 B): 4|B_t| + min(125|B_t|, N/8) + 64|B_t| + 4|B_{t+1}|
+      (read the brick list; each needed grid byte once -- a brick plus its one-voxel halo is 10^3
+      bits = 125 B; write the brick into the next buffer; write the next list)."""
+    out, prev = [], n_seeds
+    for t in range(len(front)):
+        a_t = int(front[t])
+        a_n = int(front[t + 1]) if t + 1 < len(front) else a_t
+        c_t = int(solid_after[t]) - prev
+        prev = int(solid_after[t])
+        if storage == 0:
+            out.append(4 * a_t + min(27 * a_t, N) + c_t + 4 * a_n)
+        else:
+            out.append(4 * a_t + min(125 * a_t, N // 8) + 64 * a_t + 4 * a_n)
+    return out
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    w = workloads.BENCH_CPU_SAMPLE
+    nx, ny, nz = w["dims"]
+    N = nx * ny * nz
+
+    def one():
+        o = oracle.Oracle(nx, ny, nz, w["periodic"])
+        o.set_growth(*w["g"], 1)
+        t0 = time.perf_counter()
+        o.seed(w["core"], w["s"], w["seed"])
+        o.generate(w["target"], 10**6, True)
+        dt = time.perf_counter() - t0
+        o.close()
+        return dt
+    for _ in range(args.warmup):
+        one()
+    total = sum(one() for _ in range(args.steps))
+    value = N * args.steps / total
+    sample = "%s: %dx%dx%d sub-volume of %s, same parameters, serial C oracle" % (w["name"], nx, ny, nz, workloads.BENCH["name"])
+    print(json.dumps({
+        "impl": "reference", "metric": "voxel nodes/s (whole generation: seeding + growth to target)",
+        "value": value, "unit": "nodes/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32", "data": "synthetic",
+        "config": {"workload": workloads.BENCH["name"], "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "nodes/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "nodes/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import paper_2602_11734_b200 as liets
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    w = workloads.BENCH
+    nx, ny, nz = w["dims"]
+    N = nx * ny * nz
+    storage = args.storage if args.storage is not None else DEFAULT_STORAGE
+    gen = liets.Liets(nx, ny, nz, int(w["periodic"]), storage, device="cuda:%d" % local)
+    gen.set_growth(*w["g"], liets.LAW_EQ1)
+    rng_seed = w["seed"] + rank                      # replicas: one realisation per rank
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    host_out = torch.empty(N, dtype=torch.uint8, pin_memory=True)        # e2e destination (pinned host)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one(e2e):
+        flush.zero_()                                # L2 flush between iterations (outside the events)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        n_seeds = gen.seed(w["core"], w["s"], rng_seed)
+        rc, steps, n_solid = gen.generate(w["target"])
+        if e2e:
+            gen.grid_into(host_out.data_ptr(), N, liets.FORMAT_U8)
+        ev1.record()
+        ev1.synchronize()
+        assert rc == liets.OK
+        return ev0.elapsed_time(ev1), n_seeds, steps, n_solid
+
+    for _ in range(args.warmup):
+        one(False)
+    sampler = ClockSampler(local)
+    sampler.start()
+    # --- device-resident leg -------------------------------------------------------------------
+    barrier()
+    launches0 = gen.launch_count
+    t_dev, seed_ms, gen_ms = 0.0, [], []
+    for _ in range(args.steps):
+        ms, n_seeds, n_steps, n_solid = one(False)
+        t_dev += ms
+        a, b = gen.timings()
+        seed_ms.append(a)
+        gen_ms.append(b)
+    launches = gen.launch_count - launches0
+    barrier()
+    # --- end-to-end leg: host output buffer, D2H copy inside the timed region ---------------------
+    one(True)
+    barrier()
+    t_e2e = 0.0
+    for _ in range(args.steps):
+        t_e2e += one(True)[0]
+    barrier()
+    clocks = sampler.stop()
+    if dist is not None:
+        tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_dev, t_e2e = float(tt[0]), float(tt[1])
+
+    # --- roofline of the dominant kernel (the growth kernel), timed live with CUDA events ---------
+    gen.set_profiling(True)
+    gen.seed(w["core"], w["s"], rng_seed)
+    gen.generate(w["target"])
+    step_ms = gen.step_times()[:n_steps]
+    gen.set_profiling(False)
+    front, solid_after = gen.step_log()
+    b_alg = algorithmic_bytes(storage, N, front[:n_steps], solid_after[:n_steps], n_seeds)
+    peaks, peaks_kind = load_peaks()
+    grow_ms = float(np.sum(step_ms))
+    achieved = sum(b_alg) / (grow_ms * 1e-3) / 1e9 if grow_ms > 0 else 0.0
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                "kernel": KERNEL_NAMES[storage], "peak_kind": "%s (MEASURED_PEAKS.json hbm_gbs, burst copy)" % peaks_kind,
+                "launches": int(n_steps), "algorithmic_bytes_per_launch": sum(b_alg) / max(n_steps, 1),
+                "avg_launch_ms": grow_ms / max(n_steps, 1),
+                "growth_kernel_share_of_generate": grow_ms / max(float(np.median(gen_ms)), 1e-9),
+                "front_voxel_updates_per_s": (float(np.sum(front[:n_steps])) / (grow_ms * 1e-3)) if storage == 0 else None}
+
+    out = None
+    if rank == 0:
+        value = N * world * args.steps / (t_dev * 1e-3)
+        e2e_value = N * world * args.steps / (t_e2e * 1e-3)
+        out = {
+            "metric": "voxel nodes/s (whole generation: seeding + growth to target)",
+            "value": value, "unit": "nodes/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u32", "data": "synthetic",
+            "config": {"workload": w["name"], "grid": [nx, ny, nz], "core_prob": w["core"], "spacing_s": w["s"],
+                       "g_face_edge_corner": list(w["g"]), "target_solid_fraction": w["target"], "rng_seed": w["seed"],
+                       "storage": ["u8+voxel-list", "bit-brick+brick-list"][storage], "parallelism": "replicas" if world > 1 else "1gpu",
+                       "l2": "flushed between iterations (256 MiB memset outside the timed events)",
+                       "growth_steps": int(n_steps), "seeds": int(n_seeds), "final_solid": int(n_solid)},
+            "seconds_per_generation": t_dev / args.steps * 1e-3,
+            "seed_ms": float(np.median(seed_ms)), "generate_ms": float(np.median(gen_ms)),
+            "e2e": {"value": e2e_value, "unit": "nodes/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": N,
+                    "ms_per_step": t_e2e / args.steps, "note": "inputs are parameters only; output = uint8 phase array to pinned host"},
+            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
+        }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline()
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def cpu_baseline():
+    """The oracle as it stands, on the box's host cores, on a bounded sample (one serial run)."""
+    import oracle
+    oracle.build()
+    w = workloads.BENCH_CPU_SAMPLE
+    nx, ny, nz = w["dims"]
+    o = oracle.Oracle(nx, ny, nz, w["periodic"])
+    o.set_growth(*w["g"], 1)
+    t0 = time.perf_counter()
+    o.seed(w["core"], w["s"], w["seed"])
+    o.generate(w["target"], 10**6, True)
+    dt = time.perf_counter() - t0
+    return {"value": nx * ny * nz / dt, "unit": "nodes/s", "cores": 1, "kind": "oracle", "seconds": dt,
+            "sample": "%s: %dx%dx%d sub-volume of %s with the same parameters (densities, spacing, target), "
+                      "one serial run of oracle/liets_oracle.c (gcc -O2)" % (w["name"], nx, ny, nz, workloads.BENCH["name"])}
+
+
+DEFAULT_STORAGE = 0
+KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_brick"}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
+# `ncu --set full` capture (profiles/); None until a capture exists for the current kernel.
+TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--storage", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = args.steps or 2
+        args.warmup = 0 if args.warmup is None else min(args.warmup, 1)
+        return run_reference(args)
+    args.steps = args.steps or 20
+    args.warmup = 3 if args.warmup is None else max(args.warmup, 3)
+    run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -15,7 +15,7 @@
  *   - All device work is enqueued on the CUDA stream given at create (a cudaStream_t passed as
  *     void*, NULL = the legacy default stream).  Calls that return a value to the host
  *     (*_out arguments, liets_grid with a host dst) synchronise that stream; the others do not.
- *   - Voxel (x, y, z) has linear index idx = x + nx*(y + ny*z); N = nx*ny*nz <= 2^32.
+ *   - Voxel (x, y, z) has linear index idx = x + nx*(y + ny*z); N = nx*ny*nz < 2^32.
  *   - There is no CPU fallback: without a CUDA device every call fails with LIETS_E_CUDA.
  */
 #ifndef LIETS_H
@@ -34,7 +34,7 @@ enum {
     LIETS_OK = 0,            /* success; for liets_generate: target solid fraction reached       */
     LIETS_FRONT_EMPTY = 1,   /* generate stopped: no solid voxel has a void neighbour (:140)      */
     LIETS_MAX_STEPS = 2,     /* generate stopped: max_steps steps done (R14)                      */
-    LIETS_E_ARG = -1,        /* bad argument (dims < 1, N > 2^32, probability outside [0,1], ...) */
+    LIETS_E_ARG = -1,        /* bad argument (dims < 1, N >= 2^32, probability outside [0,1], ..) */
     LIETS_E_STATE = -2,      /* call order: step/generate before seed; Eq.(1) law without target  */
     LIETS_E_CAPACITY = -3,   /* caller's workspace / dst buffer too small                         */
     LIETS_E_CUDA = -4        /* CUDA runtime error or no device                                   */
@@ -108,6 +108,15 @@ int liets_step_log(liets_ctx* ctx, uint64_t* front_in, uint64_t* solid_after, ui
 /* Device time in milliseconds of the last liets_seed and the last liets_generate (CUDA events on
  * the ctx stream). */
 int liets_timings(liets_ctx* ctx, float* seed_ms, float* generate_ms);
+
+/* Profiling aid for the roofline report: when on, liets_generate / liets_step bracket every
+ * growth-kernel launch with a CUDA event pair (at most 4096 kept per call). */
+int liets_set_profiling(liets_ctx* ctx, int on);
+/* Device time in milliseconds of each growth-kernel launch of the last liets_generate / liets_step
+ * made with profiling on (HOST array of capacity cap). Returns the number of launches recorded. */
+int liets_step_times(liets_ctx* ctx, float* ms, uint32_t cap);
+/* Number of kernels this ctx has launched since liets_create (memsets and copies not counted). */
+uint64_t liets_launch_count(const liets_ctx* ctx);
 
 void liets_destroy(liets_ctx* ctx);
 const char* liets_last_error(const liets_ctx* ctx);

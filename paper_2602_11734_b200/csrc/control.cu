@@ -70,17 +70,20 @@ __global__ void k_set_params(Control* c, unsigned long long R0, unsigned long lo
 
 cudaError_t launch_control(liets_ctx* c, uint32_t flags) {
     k_control<<<1, 32, 0, c->stream>>>(c->ctl, flags);
+    c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_begin(liets_ctx* c, int generate, uint32_t max_steps) {
     k_begin<<<1, 1, 0, c->stream>>>(c->ctl, generate, max_steps);
+    c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_set_params(liets_ctx* c) {
     k_set_params<<<1, 1, 0, c->stream>>>(c->ctl, c->R[0], c->R[1], c->R[2], (uint32_t)c->law, c->n_t,
                                          c->has_target ? 1u : 0u, c->N);
+    c->launches++;
     return cudaGetLastError();
 }
 

@@ -23,6 +23,7 @@ __global__ void __launch_bounds__(256) k_pack_bits_u8(const uint8_t* __restrict_
 
 cudaError_t launch_pack_bits_u8(liets_ctx* c, uint8_t* dst_bits) {
     k_pack_bits_u8<<<c->sm_count * 8, 256, 0, c->stream>>>(c->grid_u8, dst_bits, c->N);
+    c->launches++;
     return cudaGetLastError();
 }
 

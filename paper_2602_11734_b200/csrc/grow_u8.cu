@@ -138,6 +138,7 @@ cudaError_t launch_grow_u8(liets_ctx* c) {
         k_grow_u8<true><<<grid, 256, 0, c->stream>>>(c->ctl, c->grid_u8, c->list[0], c->list[1], dims, key);
     else
         k_grow_u8<false><<<grid, 256, 0, c->stream>>>(c->ctl, c->grid_u8, c->list[0], c->list[1], dims, key);
+    c->launches++;
     return cudaGetLastError();
 }
 

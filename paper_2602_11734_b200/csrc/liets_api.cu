@@ -53,7 +53,21 @@ int readback(liets_ctx* c) {
 }
 
 int launch_step_kernel(liets_ctx* c) {
+    const bool prof = c->profiling && c->prof_n < kProfCap;
+    if (prof) {
+        if (!c->prof_ev) {
+            c->prof_ev = static_cast<cudaEvent_t*>(calloc(2 * kProfCap, sizeof(cudaEvent_t)));
+            if (!c->prof_ev) return fail(c, LIETS_E_CUDA, "out of host memory");
+        }
+        for (int k = 0; k < 2; ++k)
+            if (!c->prof_ev[2 * c->prof_n + k]) LIETS_CUDA_TRY(c, cudaEventCreate(&c->prof_ev[2 * c->prof_n + k]));
+        LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream));
+    }
     LIETS_CUDA_TRY(c, launch_grow_u8(c));
+    if (prof) {
+        LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream));
+        c->prof_n++;
+    }
     return 0;
 }
 
@@ -124,6 +138,11 @@ void liets_destroy(liets_ctx* c) {
     if (c->pinned) cudaFreeHost(c->pinned);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->prof_ev) {
+        for (uint32_t k = 0; k < 2 * kProfCap; ++k)
+            if (c->prof_ev[k]) cudaEventDestroy(c->prof_ev[k]);
+        free(c->prof_ev);
+    }
     delete c;
 }
 
@@ -196,6 +215,7 @@ int liets_step(liets_ctx* c, uint64_t* n_solid_out, uint64_t* n_front_out) {
     if (!c) return LIETS_E_ARG;
     if (!c->seeded) return fail(c, LIETS_E_STATE, "liets_step before liets_seed");
     if (c->law == LIETS_LAW_EQ1 && !c->has_target) return fail(c, LIETS_E_STATE, "Eq. (1) law needs a target");
+    c->prof_n = 0;
     LIETS_CUDA_TRY(c, launch_begin(c, 0, 0));
     LIETS_CUDA_TRY(c, launch_control(c, kCtlPrepare | kCtlForce));
     if (int rc = launch_step_kernel(c)) return rc;
@@ -215,6 +235,7 @@ int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps
     if (!c->seeded) return fail(c, LIETS_E_STATE, "liets_generate before liets_seed");
     LIETS_CUDA_TRY(c, cudaEventRecord(c->ev0, c->stream));
     LIETS_CUDA_TRY(c, launch_begin(c, 1, max_steps));
+    c->prof_n = 0;
     uint32_t enqueued = 0;
     for (;;) {
         // a batch of steps back to back; steps after the stop rule fired are no-ops on the device
@@ -279,5 +300,22 @@ int liets_timings(liets_ctx* c, float* seed_ms, float* generate_ms) {
     if (generate_ms) *generate_ms = c->gen_ms;
     return LIETS_OK;
 }
+
+int liets_set_profiling(liets_ctx* c, int on) {
+    if (!c) return LIETS_E_ARG;
+    c->profiling = on != 0;
+    return LIETS_OK;
+}
+
+int liets_step_times(liets_ctx* c, float* ms, uint32_t cap) {
+    if (!c || (cap && !ms)) return LIETS_E_ARG;
+    LIETS_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    uint32_t n = c->prof_n < cap ? c->prof_n : cap;
+    for (uint32_t k = 0; k < n; ++k)
+        LIETS_CUDA_TRY(c, cudaEventElapsedTime(&ms[k], c->prof_ev[2 * k], c->prof_ev[2 * k + 1]));
+    return (int)n;
+}
+
+uint64_t liets_launch_count(const liets_ctx* c) { return c ? c->launches : 0; }
 
 }  // extern "C"

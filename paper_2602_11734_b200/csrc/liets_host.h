@@ -34,6 +34,10 @@ struct liets_ctx {
     int law;
     uint64_t n_t;
     float seed_ms, gen_ms;
+    uint64_t launches;                // kernels launched by this ctx
+    bool profiling;
+    cudaEvent_t* prof_ev;             // 2 * kProfCap events, created on first use
+    uint32_t prof_n;                  // growth launches bracketed by the last call
     char err[256];
 };
 
@@ -48,6 +52,7 @@ struct liets_ctx {
     } while (0)
 
 namespace liets {
+constexpr uint32_t kProfCap = 4096;
 constexpr size_t kControlScalarBytes = offsetof(Control, log_front);
 
 // control.cu

@@ -198,6 +198,7 @@ cudaError_t launch_seed_reset(liets_ctx* c) {
     cudaError_t e = cudaMemsetAsync(c->grid_u8, 0, (c->N + 3) & ~3ull, c->stream);
     if (e != cudaSuccess) return e;
     k_seed_reset<<<1, 1, 0, c->stream>>>(c->ctl);
+    c->launches++;
     return cudaGetLastError();
 }
 
@@ -207,26 +208,32 @@ cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all
     const uint32_t T = always ? 0xFFFFFFFFu : (uint32_t)t_core;
     k_seed_candidates<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->status2, c->list[1], c->N, T, always,
                                                               (uint32_t)accept_all, key);
+    c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     k_spacing_roll<<<1, 1, 0, c->stream>>>(c->ctl, 1);
+    c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_spacing_round(liets_ctx* c, int s) {
     const Dims g{ c->nx, c->ny, c->nz, c->boundary };
     k_spacing_round<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->list[1], g, s);
+    c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     k_spacing_roll<<<1, 1, 0, c->stream>>>(c->ctl, 0);
+    c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_seed_finalize(liets_ctx* c) {
     k_seed_finalize_u8<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->list[1], c->grid_u8, c->list[0]);
+    c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     k_seed_close<<<1, 1, 0, c->stream>>>(c->ctl);
+    c->launches++;
     return cudaGetLastError();
 }
 
@@ -234,10 +241,12 @@ cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n) {
     if (n) {
         k_seed_explicit_u8<<<c->sm_count * 2, 256, 0, c->stream>>>(c->ctl, (const unsigned long long*)c->explicit_idx, n,
                                                                   c->grid_u8, c->list[0]);
+        c->launches++;
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     k_seed_close<<<1, 1, 0, c->stream>>>(c->ctl);
+    c->launches++;
     return cudaGetLastError();
 }
 

@@ -17,7 +17,7 @@ FORMAT_U8, FORMAT_BITS = 0, 1
 # every symbol include/liets.h declares
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
            "liets_set_target", "liets_step", "liets_generate", "liets_grid", "liets_step_log", "liets_timings",
-           "liets_destroy", "liets_last_error")
+           "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_destroy", "liets_last_error")
 
 
 class LietsError(RuntimeError):
@@ -67,6 +67,12 @@ def lib():
     L.liets_step_log.restype = ci
     L.liets_timings.argtypes = [vp, P(ctypes.c_float), P(ctypes.c_float)]
     L.liets_timings.restype = ci
+    L.liets_set_profiling.argtypes = [vp, ci]
+    L.liets_set_profiling.restype = ci
+    L.liets_step_times.argtypes = [vp, P(ctypes.c_float), u32]
+    L.liets_step_times.restype = ci
+    L.liets_launch_count.argtypes = [vp]
+    L.liets_launch_count.restype = u64
     L.liets_destroy.argtypes = [vp]
     L.liets_destroy.restype = None
     L.liets_last_error.argtypes = [vp]
@@ -170,3 +176,15 @@ class Liets:
         a, b = ctypes.c_float(0), ctypes.c_float(0)
         self._check(self._L.liets_timings(self._h, ctypes.byref(a), ctypes.byref(b)))
         return float(a.value), float(b.value)
+
+    def set_profiling(self, on):
+        self._check(self._L.liets_set_profiling(self._h, int(on)))
+
+    def step_times(self, cap=4096):
+        ms = (ctypes.c_float * cap)()
+        n = self._check(self._L.liets_step_times(self._h, ms, cap))
+        return np.array(ms[:n], dtype=np.float64)
+
+    @property
+    def launch_count(self):
+        return int(self._L.liets_launch_count(self._h))
