@@ -1,0 +1,319 @@
+// grow_brick.cu -- STORAGE_BRICK growth step: bit-packed 8x8x8 bricks + explicit list of front BRICKS.
+//
+// Layout in HBM.  The grid is cut into 8x8x8 bricks of 64 bytes: eight 64-bit words, word z holds
+// z-slice z of the brick, bit (x + 8y).  Two copies G[0], G[1] are kept: step t reads G[t&1]
+// (immutable during the step, so the update is synchronous by construction) and ORs
+// into G[(t+1)&1].  The active set A is kept as a list of bricks that hold at least
+// one front voxel; which voxels of a brick are front voxels is recomputed from the bits, so the
+// list costs 4 bytes per 512 voxels instead of 4 bytes per front voxel.
+//
+// One warp owns one brick at a time:
+//   A  gather: the brick and the needed words of its 26 neighbour bricks -> shared memory, then the
+//      10x10x10 neighbourhood as 100 rows of 10 bits ("not void" = solid, outside the domain, or padding)
+//   B  masks: per interior row, the 26 void-target masks (Algorithm 3 lines 5-6) as bit operations;
+//      every (voxel, Philox block) pair with a void target becomes one 16-bit work item in a
+//      warp-wide list (prefix sum), so the Philox work is spread evenly over the 32 lanes
+//   C  draw + test: one Philox4x32-10 block per item, <= 4 directions tested against the integer
+//      thresholds (line 8); hits set bits in a shared-memory claim volume
+//   D  claim + compact: own slices are OR-ed into G[next] together with the carried state, halo hits
+//      go to the neighbour bricks with atomicOr; the returned old word tells who flipped the bit
+//      (line 9-10, "counted once" PAPER.md:77) for the solid count; a per-brick step stamp
+//      (atomicMax) makes every brick enter the next list exactly once; bricks without front voxels
+//      are not re-emitted (lazy retirement).
+#include "liets_host.h"
+
+namespace liets {
+
+namespace {
+
+constexpr int kWarpsPerCta = 8;
+constexpr int kItemCap = 2048;              // work items per pass (16 bit each)
+constexpr uint32_t kHole = 0xFFFFFFFFu;     // unused slot of a warp's list chunk
+constexpr int kChunk = 8;                   // list slots a warp reserves at a time
+
+struct WarpSmem {
+    unsigned long long nbw[27][8];          // words of the 27 bricks (own = index 13)
+    uint32_t rows[100];                     // 10 bits per row: bit (x'+1), rows (z'+1)*10 + (y'+1)
+    uint32_t claims[100];                   // same geometry: cells claimed in this step
+    uint32_t rowbase[64];                   // linear voxel index of (x=0, y, z) of the interior rows
+    uint16_t items[kItemCap];
+};
+
+// region index i in [-1, 8] along one axis of brick b -> brick index (or -1: no such cell) and local coordinate
+__device__ __forceinline__ void axis_map(int i, int b, int nb, int n, int periodic, int* ob, int* l) {
+    const int wc = min(8, n - 8 * b);
+    if (i < 0) {
+        if (b > 0) { *ob = b - 1; *l = 7; }
+        else if (periodic) { *ob = nb - 1; *l = n - 8 * (nb - 1) - 1; }
+        else { *ob = -1; *l = 0; }
+    } else if (i < wc) {
+        *ob = b; *l = i;
+    } else if (i == wc) {
+        if (b < nb - 1) { *ob = b + 1; *l = 0; }
+        else if (periodic) { *ob = 0; *l = 0; }
+        else { *ob = -1; *l = 0; }
+    } else {
+        *ob = -1; *l = 0;
+    }
+}
+
+struct StepParams {
+    uint32_t T[3];
+    uint32_t always[3];
+    uint32_t t;
+};
+
+__global__ void __launch_bounds__(kWarpsPerCta * 32) k_grow_brick(Control* __restrict__ ctl, BrickGeom g,
+                                                                    unsigned long long* G0, unsigned long long* G1,
+                                                                    uint32_t* stamp, uint32_t* list0, uint32_t* list1,
+                                                                    PhiloxKey key) {
+    if (!ctl->active) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ uint32_t s_T[28];            // threshold of direction d (R8), by class
+    __shared__ uint32_t s_always[28];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
+
+    const uint32_t cur = ctl->cur;
+    const uint32_t n_list = ctl->count[cur];
+    const uint32_t* __restrict__ in = cur ? list1 : list0;
+    uint32_t* __restrict__ out = cur ? list0 : list1;
+    uint32_t* out_count = &ctl->count[cur ^ 1u];
+    const uint32_t t = ctl->step;
+    const unsigned long long* __restrict__ Gc = (t & 1u) ? G1 : G0;     // g_t (read only)
+    unsigned long long* Gn = (t & 1u) ? G0 : G1;                        // g_{t+1} (OR target)
+    if (threadIdx.x < 28) {
+        const int d = threadIdx.x < 26 ? (int)threadIdx.x : 25;
+        const int raw = d + (d >= 13 ? 1 : 0);
+        const int cls = (raw % 3 != 1) + ((raw / 3) % 3 != 1) + (raw / 9 != 1) - 1;
+        s_T[threadIdx.x] = threadIdx.x < 26 ? ctl->T[cls] : 0u;
+        s_always[threadIdx.x] = threadIdx.x < 26 ? ctl->always[cls] : 0u;
+    }
+    __syncthreads();
+    const bool any_always = ctl->always[0] | ctl->always[1] | ctl->always[2];
+
+    uint32_t new_solid = 0;                 // per lane: bits this lane flipped 0 -> 1
+    uint32_t chunk_pos = 0, chunk_end = 0;  // lane 0: reserved slots of the next list
+
+    const uint32_t warp_global = blockIdx.x * kWarpsPerCta + warp;
+    const uint32_t n_warps = gridDim.x * kWarpsPerCta;
+    for (uint32_t li = warp_global; li < n_list; li += n_warps) {
+        const uint32_t id = in[li];
+        if (id == kHole) continue;
+        const int bxi = (int)(id % (uint32_t)g.bx), byi = (int)((id / (uint32_t)g.bx) % (uint32_t)g.by),
+                  bzi = (int)(id / ((uint32_t)g.bx * (uint32_t)g.by));
+        const int wcx = min(8, g.nx - 8 * bxi), wcy = min(8, g.ny - 8 * byi), wcz = min(8, g.nz - 8 * bzi);
+
+        // ---- A: gather ------------------------------------------------------------------------
+        if (lane < 27) {
+            const int ox = (int)lane % 3 - 1, oy = ((int)lane / 3) % 3 - 1, oz = (int)lane / 9 - 1;
+            int obx, oby, obz, lx, ly, lz;
+            axis_map(ox < 0 ? -1 : (ox == 0 ? 0 : wcx), bxi, g.bx, g.nx, g.periodic, &obx, &lx);
+            axis_map(oy < 0 ? -1 : (oy == 0 ? 0 : wcy), byi, g.by, g.ny, g.periodic, &oby, &ly);
+            axis_map(oz < 0 ? -1 : (oz == 0 ? 0 : wcz), bzi, g.bz, g.nz, g.periodic, &obz, &lz);
+            if (obx < 0 || oby < 0 || obz < 0) {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) S.nbw[lane][k] = ~0ull;      // outside the domain: never void
+            } else {
+                const unsigned long long* src = Gc + 8ull * ((unsigned long long)obx +
+                                                             (unsigned long long)g.bx * ((unsigned long long)oby + (unsigned long long)g.by * (unsigned long long)obz));
+                if (oz == 0) {
+                    const ulonglong2* s2 = reinterpret_cast<const ulonglong2*>(src);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const ulonglong2 v = __ldcg(s2 + k);
+                        S.nbw[lane][2 * k] = v.x; S.nbw[lane][2 * k + 1] = v.y;
+                    }
+                } else {
+                    S.nbw[lane][lz] = __ldcg(src + lz);                  // only the touching slice
+                }
+            }
+        }
+        __syncwarp();
+        // local coordinates of the cells just outside the brick on the low side
+        const int lxl = bxi > 0 ? 7 : g.nx - 8 * (g.bx - 1) - 1;
+        const int lyl = byi > 0 ? 7 : g.ny - 8 * (g.by - 1) - 1;
+        const int lzl = bzi > 0 ? 7 : g.nz - 8 * (g.bz - 1) - 1;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int r = (int)lane + 32 * k;
+            if (r < 100) {
+                const int zp = r / 10 - 1, yp = r % 10 - 1;
+                uint32_t row = 0x3FFu;
+                if (zp <= wcz && yp <= wcy) {
+                    const int ozi = zp < 0 ? 0 : (zp < wcz ? 1 : 2), lz = zp < 0 ? lzl : (zp < wcz ? zp : 0);
+                    const int oyi = yp < 0 ? 0 : (yp < wcy ? 1 : 2), ly = yp < 0 ? lyl : (yp < wcy ? yp : 0);
+                    const int jc = 1 + 3 * oyi + 9 * ozi;
+                    const uint32_t c = (uint32_t)(S.nbw[jc][lz] >> (8 * ly)) & 0xFFu;
+                    const uint32_t left = (uint32_t)(S.nbw[jc - 1][lz] >> (8 * ly + lxl)) & 1u;
+                    const uint32_t right = (uint32_t)(S.nbw[jc + 1][lz] >> (8 * ly)) & 1u;
+                    row = left | ((c & ((1u << wcx) - 1u)) << 1) | (right << (wcx + 1)) | ((0x3FFu << (wcx + 2)) & 0x3FFu);
+                }
+                S.rows[r] = row;
+                S.claims[r] = 0u;
+            }
+        }
+        __syncwarp();
+
+        // ---- B: masks and work items ------------------------------------------------------------
+        uint32_t V[2][7];                   // per owned row, per Philox block: 4 void-target masks of 8 bits
+        uint32_t cnt_lo = 0, cnt_hi = 0;    // items of blocks 0..3 / 4..6
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int r2 = (int)lane + 32 * h, y = r2 & 7, z = r2 >> 3;
+            uint32_t src = 0;
+            if (y < wcy && z < wcz) src = (S.rows[(z + 1) * 10 + (y + 1)] >> 1) & ((1u << wcx) - 1u);
+            uint32_t M[26];
+#pragma unroll
+            for (int d = 0; d < 26; ++d) {
+                const uint32_t voidrow = ~S.rows[(z + dir_dz(d) + 1) * 10 + (y + dir_dy(d) + 1)];
+                M[d] = src & (voidrow >> (dir_dx(d) + 1)) & 0xFFu;
+            }
+#pragma unroll
+            for (int b = 0; b < 7; ++b) {
+                uint32_t v = M[4 * b];
+                if (4 * b + 1 < 26) v |= M[4 * b + 1] << 8;
+                if (4 * b + 2 < 26) v |= M[4 * b + 2] << 16;
+                if (4 * b + 3 < 26) v |= M[4 * b + 3] << 24;
+                V[h][b] = v;
+                const uint32_t u = (v | (v >> 8) | (v >> 16) | (v >> 24)) & 0xFFu;
+                if (b < 4) cnt_lo += __popc(u); else cnt_hi += __popc(u);
+            }
+            S.rowbase[r2] = (uint32_t)(8 * bxi) + (uint32_t)g.nx * ((uint32_t)(8 * byi + y) + (uint32_t)g.ny * (uint32_t)(8 * bzi + z));
+        }
+        uint32_t tot_lo, tot_hi;
+        const uint32_t off_lo = warp_exclusive_scan(cnt_lo, lane, &tot_lo);
+        const uint32_t off_hi = warp_exclusive_scan(cnt_hi, lane, &tot_hi);
+        const uint32_t total = tot_lo + tot_hi;
+        const int n_pass = total > (uint32_t)kItemCap ? 2 : 1;      // each half is <= 4*512 items
+
+        for (int pass = 0; pass < n_pass; ++pass) {
+            const int b_lo = (n_pass == 2 && pass == 1) ? 4 : 0;
+            const int b_hi = (n_pass == 2 && pass == 0) ? 4 : 7;
+            uint32_t off = b_lo == 0 ? off_lo : off_hi;
+            if (n_pass == 1) off = off_lo + off_hi;                // one list: this lane's lo items then its hi items
+            const uint32_t n_items = n_pass == 1 ? total : (pass == 0 ? tot_lo : tot_hi);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const uint32_t r2 = lane + 32u * h;
+#pragma unroll
+                for (int b = 0; b < 7; ++b) {
+                    if (b < b_lo || b >= b_hi) continue;
+                    const uint32_t v = V[h][b];
+                    uint32_t u = (v | (v >> 8) | (v >> 16) | (v >> 24)) & 0xFFu;
+                    while (u) {
+                        const uint32_t x = __ffs(u) - 1;
+                        u &= u - 1;
+                        const uint32_t vm = (((v >> x) & 0x01010101u) * 0x10204080u) >> 28;
+                        S.items[off++] = (uint16_t)(r2 | (x << 6) | ((uint32_t)b << 9) | (vm << 12));
+                    }
+                }
+            }
+            __syncwarp();
+
+            // ---- C: draw + test -----------------------------------------------------------------
+            for (uint32_t k = lane; k < n_items; k += 32) {
+                const uint32_t it = S.items[k];
+                const uint32_t r2 = it & 63u, x = (it >> 6) & 7u, b = (it >> 9) & 7u, vm = it >> 12;
+                const uint32_t p = S.rowbase[r2] + x;
+                const uint4 rnd = philox4x32_10(p, 0u, t, b, key);
+                const uint32_t w[4] = { rnd.x, rnd.y, rnd.z, rnd.w };
+                uint32_t fire = 0;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    bool f = w[j] < s_T[4 * b + j];
+                    if (any_always) f = f || s_always[4 * b + j];
+                    if (f) fire |= 1u << j;
+                }
+                fire &= vm;
+                while (fire) {                                      // rare: a draw fell below the threshold
+                    const int j = __ffs(fire) - 1;
+                    fire &= fire - 1;
+                    const int d = 4 * (int)b + j, raw = d + (d >= 13 ? 1 : 0);
+                    const int dx = raw % 3 - 1, dy = (raw / 3) % 3 - 1, dz = raw / 9 - 1;
+                    const int y = (int)(r2 & 7u), z = (int)(r2 >> 3);
+                    atomicOr(&S.claims[(z + dz + 1) * 10 + (y + dy + 1)], 1u << ((int)x + dx + 1));
+                }
+            }
+            __syncwarp();
+        }
+
+        // ---- D: claim + compact ---------------------------------------------------------------------
+        const unsigned long long own_base = 8ull * id;
+        if ((int)lane < wcz) {                                      // own slices: carry g_t and add the hits
+            const int z = (int)lane;
+            unsigned long long cw = 0;
+#pragma unroll
+            for (int y = 0; y < 8; ++y)
+                if (y < wcy)
+                    cw |= (unsigned long long)((S.claims[(z + 1) * 10 + (y + 1)] >> 1) & ((1u << wcx) - 1u)) << (8 * y);
+            const unsigned long long val = S.nbw[13][z] | cw;
+            if (cw) {
+                const unsigned long long old = atomicOr(Gn + own_base + z, val);
+                new_solid += __popcll(cw & ~old);
+            } else if (val) {
+                atomicOr(Gn + own_base + z, val);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {                               // hits outside the brick
+            const int r = (int)lane + 32 * k;
+            if (r >= 100) continue;
+            const int zp = r / 10 - 1, yp = r % 10 - 1;
+            uint32_t hb = S.claims[r];
+            const bool halo_row = zp < 0 || zp == wcz || yp < 0 || yp == wcy;
+            if (!halo_row) hb &= 1u | (1u << (wcx + 1));
+            while (hb) {
+                const int i = __ffs(hb) - 1;
+                hb &= hb - 1;
+                int qbx, qby, qbz, qx, qy, qz;
+                axis_map(i - 1, bxi, g.bx, g.nx, g.periodic, &qbx, &qx);
+                axis_map(yp, byi, g.by, g.ny, g.periodic, &qby, &qy);
+                axis_map(zp, bzi, g.bz, g.nz, g.periodic, &qbz, &qz);
+                const uint32_t nb = (uint32_t)qbx + (uint32_t)g.bx * ((uint32_t)qby + (uint32_t)g.by * (uint32_t)qbz);
+                const unsigned long long bit = 1ull << (qx + 8 * qy);
+                const unsigned long long old = atomicOr(Gn + 8ull * nb + qz, bit);
+                if (!(old & bit)) new_solid++;
+                if (atomicMax(&stamp[nb], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = nb;   // newly active brick
+            }
+        }
+        if (lane == 0 && total > 0) {                               // this brick still has front voxels
+            if (atomicMax(&stamp[id], t + 2u) < t + 2u) {
+                if (chunk_pos == chunk_end) {
+                    chunk_pos = atomicAdd(out_count, (uint32_t)kChunk);
+                    chunk_end = chunk_pos + kChunk;
+                }
+                out[chunk_pos++] = id;
+            }
+        }
+        __syncwarp();
+    }
+    if (lane == 0)
+        for (; chunk_pos < chunk_end; ++chunk_pos) out[chunk_pos] = kHole;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) new_solid += __shfl_xor_sync(0xffffffffu, new_solid, o);
+    if (lane == 0 && new_solid) atomicAdd(&ctl->claims, new_solid);
+}
+
+}  // namespace
+
+size_t grow_brick_smem_bytes() { return sizeof(WarpSmem) * kWarpsPerCta; }
+int grow_brick_warps_per_cta() { return kWarpsPerCta; }
+int grow_brick_chunk() { return kChunk; }
+
+cudaError_t launch_grow_brick(liets_ctx* c) {
+    static bool attr_set = false;
+    const size_t smem = grow_brick_smem_bytes();
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_grow_brick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const PhiloxKey key = philox_make_key(c->rng_seed);
+    k_grow_brick<<<c->brick_grid, kWarpsPerCta * 32, smem, c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->stamp,
+                                                                       c->list[0], c->list[1], key);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace liets

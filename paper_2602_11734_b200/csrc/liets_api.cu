@@ -16,20 +16,39 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t ctl, grid, list0, list1, status2, total;
+    size_t ctl, grid, list0, list1, status2, cand, total;
+    size_t g0, g1, stamp;          // STORAGE_BRICK (contiguous: G0 | G1 | stamp)
+    size_t n_bricks, list_cap;
+    int brick_grid;
 };
+
+constexpr int kBrickCtasPerSm = 4;
+constexpr int kMaxSms = 256;       // list slack is sized for the largest grid we would ever launch
 
 bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
     if (nx < 1 || ny < 1 || nz < 1) return false;
     const unsigned long long N = (unsigned long long)nx * (unsigned long long)ny * (unsigned long long)nz;
     if (N >= (1ull << 32)) return false;
-    if (storage != LIETS_STORAGE_U8) return false;
+    if (storage != LIETS_STORAGE_U8 && storage != LIETS_STORAGE_BRICK) return false;
+    memset(L, 0, sizeof(*L));
     size_t off = 0;
     L->ctl = off;     off += align_up(sizeof(Control));
-    L->grid = off;    off += align_up((size_t)N + 4);
-    L->list0 = off;   off += align_up((size_t)N * 4);
-    L->list1 = off;   off += align_up((size_t)N * 4 < 64 ? 64 : (size_t)N * 4);
+    if (storage == LIETS_STORAGE_U8) {
+        L->grid = off;    off += align_up((size_t)N + 4);
+        L->list_cap = (size_t)N;
+    } else {
+        const size_t bx = ((size_t)nx + 7) / 8, by = ((size_t)ny + 7) / 8, bz = ((size_t)nz + 7) / 8;
+        L->n_bricks = bx * by * bz;
+        L->g0 = off;      off += L->n_bricks * 64;
+        L->g1 = off;      off += L->n_bricks * 64;
+        L->stamp = off;   off += align_up(L->n_bricks * 4);
+        // every brick at most once per list, plus the unused tail of each warp's last chunk
+        L->list_cap = L->n_bricks + (size_t)kMaxSms * kBrickCtasPerSm * grow_brick_warps_per_cta() * grow_brick_chunk() + 64;
+    }
+    L->list0 = off;   off += align_up(L->list_cap * 4);
+    L->list1 = off;   off += align_up(L->list_cap * 4);
     L->status2 = off; off += align_up(((size_t)N + 15) / 16 * 4);
+    L->cand = off;    off += align_up((size_t)N * 4 < 64 ? 64 : (size_t)N * 4);
     L->total = off;
     return true;
 }
@@ -63,7 +82,7 @@ int launch_step_kernel(liets_ctx* c) {
             if (!c->prof_ev[2 * c->prof_n + k]) LIETS_CUDA_TRY(c, cudaEventCreate(&c->prof_ev[2 * c->prof_n + k]));
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream));
     }
-    LIETS_CUDA_TRY(c, launch_grow_u8(c));
+    LIETS_CUDA_TRY(c, c->storage == LIETS_STORAGE_U8 ? launch_grow_u8(c) : launch_grow_brick(c));
     if (prof) {
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream));
         c->prof_n++;
@@ -118,7 +137,20 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
         c->list[0] = reinterpret_cast<uint32_t*>(base + L.list0);
         c->list[1] = reinterpret_cast<uint32_t*>(base + L.list1);
         c->status2 = reinterpret_cast<uint32_t*>(base + L.status2);
-        c->explicit_idx = reinterpret_cast<uint64_t*>(base + L.list1);
+        c->cand = reinterpret_cast<uint32_t*>(base + L.cand);
+        c->explicit_idx = reinterpret_cast<uint64_t*>(base + L.cand);
+        c->scratch_u8 = reinterpret_cast<uint8_t*>(base + L.cand);
+        c->list_cap = L.list_cap;
+        if (storage == LIETS_STORAGE_BRICK) {
+            c->geom = BrickGeom{ nx, ny, nz, (nx + 7) / 8, (ny + 7) / 8, (nz + 7) / 8, boundary };
+            c->n_bricks = L.n_bricks;
+            c->G[0] = reinterpret_cast<unsigned long long*>(base + L.g0);
+            c->G[1] = reinterpret_cast<unsigned long long*>(base + L.g1);
+            c->stamp = reinterpret_cast<uint32_t*>(base + L.stamp);
+            c->grid_u8 = nullptr;
+            const int sms = c->sm_count < kMaxSms ? c->sm_count : kMaxSms;
+            c->brick_grid = sms * kBrickCtasPerSm;
+        }
         ok = cudaMemsetAsync(c->ctl, 0, sizeof(Control), c->stream) == cudaSuccess &&
              launch_set_params(c) == cudaSuccess;
     }
@@ -199,7 +231,7 @@ int liets_seed(liets_ctx* c, double core_prob, int spacing_s, uint64_t rng_seed,
 
 int liets_seed_explicit(liets_ctx* c, const uint64_t* idx, uint64_t n, uint64_t rng_seed) {
     if (!c || (n && !idx)) return LIETS_E_ARG;
-    if (n * 8 > c->N * 4) return fail(c, LIETS_E_CAPACITY, "too many explicit seeds for the staging buffer");
+    if (n * 8 > (c->N * 4 < 64 ? 64 : c->N * 4)) return fail(c, LIETS_E_CAPACITY, "too many explicit seeds for the staging buffer");
     for (uint64_t i = 0; i < n; ++i)
         if (idx[i] >= c->N) return fail(c, LIETS_E_ARG, "seed index outside the grid");
     c->rng_seed = rng_seed;
@@ -261,16 +293,24 @@ int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps
 int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is_device) {
     if (!c || !dst) return LIETS_E_ARG;
     const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (format != LIETS_FORMAT_U8 && format != LIETS_FORMAT_BITS) return fail(c, LIETS_E_ARG, "unknown grid format");
+    const size_t nb = format == LIETS_FORMAT_U8 ? (size_t)c->N : (size_t)((c->N + 7) / 8);
+    if (dst_bytes < nb) return fail(c, LIETS_E_CAPACITY, "dst buffer too small for the requested format");
+    const uint8_t* u8 = c->grid_u8;
+    if (c->storage == LIETS_STORAGE_BRICK) {                // bricks -> linear uint8 (seeding scratch is idle)
+        if (int rc = readback(c)) return rc;                // which grid copy is current
+        c->host_step = c->pinned->step;
+        uint8_t* lin = (format == LIETS_FORMAT_U8 && dst_is_device) ? static_cast<uint8_t*>(dst) : c->scratch_u8;
+        LIETS_CUDA_TRY(c, launch_unpack_bricks_u8(c, lin));
+        u8 = lin;
+    }
     if (format == LIETS_FORMAT_U8) {
-        if (dst_bytes < c->N) return fail(c, LIETS_E_CAPACITY, "dst smaller than N bytes");
-        LIETS_CUDA_TRY(c, cudaMemcpyAsync(dst, c->grid_u8, c->N, kind, c->stream));
+        if (u8 != dst) LIETS_CUDA_TRY(c, cudaMemcpyAsync(dst, u8, c->N, kind, c->stream));
     } else if (format == LIETS_FORMAT_BITS) {
-        const size_t nb = (size_t)((c->N + 7) / 8);
-        if (dst_bytes < nb) return fail(c, LIETS_E_CAPACITY, "dst smaller than ceil(N/8) bytes");
         if (dst_is_device) {
-            LIETS_CUDA_TRY(c, launch_pack_bits_u8(c, static_cast<uint8_t*>(dst)));
+            LIETS_CUDA_TRY(c, launch_pack_bits_u8(c, u8, static_cast<uint8_t*>(dst)));
         } else {                                            // pack into the (idle) seeding scratch, then copy
-            LIETS_CUDA_TRY(c, launch_pack_bits_u8(c, reinterpret_cast<uint8_t*>(c->status2)));
+            LIETS_CUDA_TRY(c, launch_pack_bits_u8(c, u8, reinterpret_cast<uint8_t*>(c->status2)));
             LIETS_CUDA_TRY(c, cudaMemcpyAsync(dst, c->status2, nb, kind, c->stream));
         }
     } else {

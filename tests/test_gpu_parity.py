@@ -18,7 +18,7 @@ def liets():
     return m
 
 
-STORAGES = [0]
+STORAGES = [0, 1]
 
 
 def run_both(liets, dims, periodic, core, s, seed, g, law, target, storage, max_steps=100000):
