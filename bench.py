@@ -273,7 +273,7 @@ def cpu_baseline():
                       "one serial run of oracle/liets_oracle.c (gcc -O2)" % (w["name"], nx, ny, nz, workloads.BENCH["name"])}
 
 
-DEFAULT_STORAGE = 0
+DEFAULT_STORAGE = 1
 KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_brick"}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for the current kernel.

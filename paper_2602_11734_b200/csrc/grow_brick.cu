@@ -11,8 +11,9 @@
 //   A  gather: the brick and the needed words of its 26 neighbour bricks -> shared memory, then the
 //      10x10x10 neighbourhood as 100 rows of 10 bits ("not void" = solid, outside the domain, or padding)
 //   B  masks: per interior row, the 26 void-target masks (Algorithm 3 lines 5-6) as bit operations;
-//      every (voxel, Philox block) pair with a void target becomes one 16-bit work item in a
-//      warp-wide list (prefix sum), so the Philox work is spread evenly over the 32 lanes
+//      every (voxel, Philox block) pair with a void target is one set bit of a flat 3584-bit map in
+//      shared memory; the lanes split that map by RANK (lane l takes set bits [l n/32, (l+1) n/32)),
+//      so the Philox work is spread evenly over the 32 lanes whatever the shape of the front
 //   C  draw + test: one Philox4x32-10 block per item, <= 4 directions tested against the integer
 //      thresholds (line 8); hits set bits in a shared-memory claim volume
 //   D  claim + compact: own slices are OR-ed into G[next] together with the carried state, halo hits
@@ -27,16 +28,16 @@ namespace liets {
 namespace {
 
 constexpr int kWarpsPerCta = 8;
-constexpr int kItemCap = 2048;              // work items per pass (16 bit each)
 constexpr uint32_t kHole = 0xFFFFFFFFu;     // unused slot of a warp's list chunk
 constexpr int kChunk = 8;                   // list slots a warp reserves at a time
 
-struct WarpSmem {
+struct __align__(16) WarpSmem {
     unsigned long long nbw[27][8];          // words of the 27 bricks (own = index 13)
+    uint32_t V[7 * 64];                     // [block b][row]: the 4 void-target masks (8 bits each) of block b
+    uint32_t U[7 * 64 / 4];                 // [block b][row] bytes: OR of the 4 masks = voxels needing block b
     uint32_t rows[100];                     // 10 bits per row: bit (x'+1), rows (z'+1)*10 + (y'+1)
     uint32_t claims[100];                   // same geometry: cells claimed in this step
     uint32_t rowbase[64];                   // linear voxel index of (x=0, y, z) of the interior rows
-    uint16_t items[kItemCap];
 };
 
 // region index i in [-1, 8] along one axis of brick b -> brick index (or -1: no such cell) and local coordinate
@@ -63,14 +64,14 @@ struct StepParams {
     uint32_t t;
 };
 
-__global__ void __launch_bounds__(kWarpsPerCta * 32) k_grow_brick(Control* __restrict__ ctl, BrickGeom g,
+__global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __restrict__ ctl, BrickGeom g,
                                                                     unsigned long long* G0, unsigned long long* G1,
                                                                     uint32_t* stamp, uint32_t* list0, uint32_t* list1,
                                                                     PhiloxKey key) {
     if (!ctl->active) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ uint32_t s_T[28];            // threshold of direction d (R8), by class
-    __shared__ uint32_t s_always[28];
+    __shared__ uint4 s_T4[7];               // per Philox block: T-1 of its 4 directions (fire iff draw <= T-1)
+    __shared__ uint32_t s_dir[28];          // direction d: (row delta + 11) | (dx + 1) << 8 in the 10x10x10 geometry
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
 
@@ -85,12 +86,18 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) k_grow_brick(Control* __res
     if (threadIdx.x < 28) {
         const int d = threadIdx.x < 26 ? (int)threadIdx.x : 25;
         const int raw = d + (d >= 13 ? 1 : 0);
-        const int cls = (raw % 3 != 1) + ((raw / 3) % 3 != 1) + (raw / 9 != 1) - 1;
-        s_T[threadIdx.x] = threadIdx.x < 26 ? ctl->T[cls] : 0u;
-        s_always[threadIdx.x] = threadIdx.x < 26 ? ctl->always[cls] : 0u;
+        const int dx = raw % 3 - 1, dy = (raw / 3) % 3 - 1, dz = raw / 9 - 1;
+        const int cls = (dx != 0) + (dy != 0) + (dz != 0) - 1;
+        // T in [0, 2^32]: "draw < T" == "draw <= T-1" for T >= 1; directions with T = 0 are disabled in phase B
+        const uint32_t tm1 = ctl->always[cls] ? 0xFFFFFFFFu : ctl->T[cls] - 1u;
+        reinterpret_cast<uint32_t*>(s_T4)[threadIdx.x] = tm1;
+        s_dir[threadIdx.x] = (uint32_t)(dz * 10 + dy + 11) | ((uint32_t)(dx + 1) << 8);
     }
     __syncthreads();
-    const bool any_always = ctl->always[0] | ctl->always[1] | ctl->always[2];
+    // a class whose threshold is 0 never fires: its directions produce no work
+    const uint32_t en0 = (ctl->T[0] | ctl->always[0]) ? 0xFFu : 0u;
+    const uint32_t en1 = (ctl->T[1] | ctl->always[1]) ? 0xFFu : 0u;
+    const uint32_t en2 = (ctl->T[2] | ctl->always[2]) ? 0xFFu : 0u;
 
     uint32_t new_solid = 0;                 // per lane: bits this lane flipped 0 -> 1
     uint32_t chunk_pos = 0, chunk_end = 0;  // lane 0: reserved slots of the next list
@@ -155,88 +162,88 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) k_grow_brick(Control* __res
         }
         __syncwarp();
 
-        // ---- B: masks and work items ------------------------------------------------------------
-        uint32_t V[2][7];                   // per owned row, per Philox block: 4 void-target masks of 8 bits
-        uint32_t cnt_lo = 0, cnt_hi = 0;    // items of blocks 0..3 / 4..6
+        // ---- B: masks and the flat work map ---------------------------------------------------------
+        uint32_t front_bits = 0;            // sources of this lane's rows that have a void neighbour (R13)
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const int r2 = (int)lane + 32 * h, y = r2 & 7, z = r2 >> 3;
             uint32_t src = 0;
             if (y < wcy && z < wcz) src = (S.rows[(z + 1) * 10 + (y + 1)] >> 1) & ((1u << wcx) - 1u);
-            uint32_t M[26];
+            const uint32_t src_c[3] = { src & en0, src & en1, src & en2 };
+            uint32_t M[28];
+            M[26] = 0; M[27] = 0;
+            uint32_t anyvoid = 0;
 #pragma unroll
             for (int d = 0; d < 26; ++d) {
                 const uint32_t voidrow = ~S.rows[(z + dir_dz(d) + 1) * 10 + (y + dir_dy(d) + 1)];
-                M[d] = src & (voidrow >> (dir_dx(d) + 1)) & 0xFFu;
+                M[d] = src_c[dir_class(d)] & (voidrow >> (dir_dx(d) + 1));
+                if (dir_dx(d) == 0 || d == 12) anyvoid |= voidrow;          // each of the 9 rows once
             }
+            front_bits |= src & (anyvoid | (anyvoid >> 1) | (anyvoid >> 2));
 #pragma unroll
             for (int b = 0; b < 7; ++b) {
-                uint32_t v = M[4 * b];
-                if (4 * b + 1 < 26) v |= M[4 * b + 1] << 8;
-                if (4 * b + 2 < 26) v |= M[4 * b + 2] << 16;
-                if (4 * b + 3 < 26) v |= M[4 * b + 3] << 24;
-                V[h][b] = v;
-                const uint32_t u = (v | (v >> 8) | (v >> 16) | (v >> 24)) & 0xFFu;
-                if (b < 4) cnt_lo += __popc(u); else cnt_hi += __popc(u);
+                const uint32_t v = M[4 * b] | (M[4 * b + 1] << 8) | (M[4 * b + 2] << 16) | (M[4 * b + 3] << 24);
+                const uint32_t u = M[4 * b] | M[4 * b + 1] | M[4 * b + 2] | M[4 * b + 3];
+                S.V[b * 64 + r2] = v;
+                reinterpret_cast<uint8_t*>(S.U)[b * 64 + r2] = (uint8_t)u;
             }
             S.rowbase[r2] = (uint32_t)(8 * bxi) + (uint32_t)g.nx * ((uint32_t)(8 * byi + y) + (uint32_t)g.ny * (uint32_t)(8 * bzi + z));
         }
-        uint32_t tot_lo, tot_hi;
-        const uint32_t off_lo = warp_exclusive_scan(cnt_lo, lane, &tot_lo);
-        const uint32_t off_hi = warp_exclusive_scan(cnt_hi, lane, &tot_hi);
-        const uint32_t total = tot_lo + tot_hi;
-        const int n_pass = total > (uint32_t)kItemCap ? 2 : 1;      // each half is <= 4*512 items
+        __syncwarp();
+        // rank partition: lanes 0..27 count 4 words each, scan, every lane takes an equal share of set bits
+        uint32_t cnt = 0;
+        if (lane < 28) {
+            const uint4 u4 = reinterpret_cast<const uint4*>(S.U)[lane];
+            cnt = __popc(u4.x) + __popc(u4.y) + __popc(u4.z) + __popc(u4.w);
+        }
+        uint32_t total;
+        const uint32_t excl = warp_exclusive_scan(cnt, lane, &total);
 
-        for (int pass = 0; pass < n_pass; ++pass) {
-            const int b_lo = (n_pass == 2 && pass == 1) ? 4 : 0;
-            const int b_hi = (n_pass == 2 && pass == 0) ? 4 : 7;
-            uint32_t off = b_lo == 0 ? off_lo : off_hi;
-            if (n_pass == 1) off = off_lo + off_hi;                // one list: this lane's lo items then its hi items
-            const uint32_t n_items = n_pass == 1 ? total : (pass == 0 ? tot_lo : tot_hi);
+        // ---- C: draw + test ---------------------------------------------------------------------------
+        if (total) {
+            const uint32_t first = (lane * total) >> 5, last = ((lane + 1u) * total) >> 5;
+            // the lane whose 4 words hold item number `first`: largest o with excl[o] <= first
+            uint32_t lo = 0, hi = 27;
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const uint32_t r2 = lane + 32u * h;
-#pragma unroll
-                for (int b = 0; b < 7; ++b) {
-                    if (b < b_lo || b >= b_hi) continue;
-                    const uint32_t v = V[h][b];
-                    uint32_t u = (v | (v >> 8) | (v >> 16) | (v >> 24)) & 0xFFu;
-                    while (u) {
-                        const uint32_t x = __ffs(u) - 1;
-                        u &= u - 1;
-                        const uint32_t vm = (((v >> x) & 0x01010101u) * 0x10204080u) >> 28;
-                        S.items[off++] = (uint16_t)(r2 | (x << 6) | ((uint32_t)b << 9) | (vm << 12));
-                    }
-                }
+            for (int it = 0; it < 5; ++it) {
+                const uint32_t mid = (lo + hi + 1u) >> 1;
+                const uint32_t e = __shfl_sync(0xffffffffu, excl, mid);
+                if (e <= first) lo = mid; else hi = mid - 1u;
             }
-            __syncwarp();
-
-            // ---- C: draw + test -----------------------------------------------------------------
-            for (uint32_t k = lane; k < n_items; k += 32) {
-                const uint32_t it = S.items[k];
-                const uint32_t r2 = it & 63u, x = (it >> 6) & 7u, b = (it >> 9) & 7u, vm = it >> 12;
+            uint32_t rem = first - __shfl_sync(0xffffffffu, excl, lo);
+            uint32_t wi = 4u * lo;
+            uint32_t cur = S.U[wi];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const uint32_t pc = __popc(cur);
+                if (rem >= pc && wi < 111u) { rem -= pc; ++wi; cur = S.U[wi]; }
+            }
+            for (; rem; --rem) cur &= cur - 1u;                     // skip the set bits that belong to lower lanes
+            for (uint32_t n = last - first; n; --n) {
+                while (cur == 0u) cur = S.U[++wi];
+                const uint32_t bit = __ffs(cur) - 1u;
+                cur &= cur - 1u;
+                const uint32_t e = 4u * wi + (bit >> 3), x = bit & 7u;      // e = b*64 + row
+                const uint32_t b = e >> 6, r2 = e & 63u;
+                const uint32_t vm = (((S.V[e] >> x) & 0x01010101u) * 0x10204080u) >> 28;
                 const uint32_t p = S.rowbase[r2] + x;
                 const uint4 rnd = philox4x32_10(p, 0u, t, b, key);
-                const uint32_t w[4] = { rnd.x, rnd.y, rnd.z, rnd.w };
-                uint32_t fire = 0;
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    bool f = w[j] < s_T[4 * b + j];
-                    if (any_always) f = f || s_always[4 * b + j];
-                    if (f) fire |= 1u << j;
-                }
+                const uint4 T4 = s_T4[b];
+                uint32_t fire = (rnd.x <= T4.x ? 1u : 0u) | (rnd.y <= T4.y ? 2u : 0u) | (rnd.z <= T4.z ? 4u : 0u) |
+                                (rnd.w <= T4.w ? 8u : 0u);
                 fire &= vm;
-                while (fire) {                                      // rare: a draw fell below the threshold
-                    const int j = __ffs(fire) - 1;
-                    fire &= fire - 1;
-                    const int d = 4 * (int)b + j, raw = d + (d >= 13 ? 1 : 0);
-                    const int dx = raw % 3 - 1, dy = (raw / 3) % 3 - 1, dz = raw / 9 - 1;
-                    const int y = (int)(r2 & 7u), z = (int)(r2 >> 3);
-                    atomicOr(&S.claims[(z + dz + 1) * 10 + (y + dy + 1)], 1u << ((int)x + dx + 1));
+                if (fire) {                                         // a draw fell below its threshold: claim the target
+                    const uint32_t rowidx = ((r2 >> 3) + 1u) * 10u + (r2 & 7u) + 1u;
+                    do {
+                        const uint32_t j = __ffs(fire) - 1u;
+                        fire &= fire - 1u;
+                        const uint32_t lut = s_dir[4u * b + j];
+                        atomicOr(&S.claims[rowidx + (lut & 0xFFu) - 11u], 1u << (x + (lut >> 8)));
+                    } while (fire);
                 }
             }
-            __syncwarp();
         }
+        __syncwarp();
 
         // ---- D: claim + compact ---------------------------------------------------------------------
         const unsigned long long own_base = 8ull * id;
@@ -277,7 +284,8 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) k_grow_brick(Control* __res
                 if (atomicMax(&stamp[nb], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = nb;   // newly active brick
             }
         }
-        if (lane == 0 && total > 0) {                               // this brick still has front voxels
+        const bool has_front = __any_sync(0xffffffffu, front_bits != 0u);
+        if (lane == 0 && has_front) {                               // this brick still has front voxels
             if (atomicMax(&stamp[id], t + 2u) < t + 2u) {
                 if (chunk_pos == chunk_end) {
                     chunk_pos = atomicAdd(out_count, (uint32_t)kChunk);
