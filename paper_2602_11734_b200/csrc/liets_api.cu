@@ -213,13 +213,7 @@ int liets_seed(liets_ctx* c, double core_prob, int spacing_s, uint64_t rng_seed,
     LIETS_CUDA_TRY(c, launch_seed_reset(c));
     const int accept_all = spacing_s <= 1;
     LIETS_CUDA_TRY(c, launch_seed_candidates(c, prob_to_threshold(core_prob), accept_all));
-    if (!accept_all) {
-        for (;;) {                                          // rounds until no candidate is pending
-            for (int k = 0; k < 8; ++k) LIETS_CUDA_TRY(c, launch_spacing_round(c, spacing_s));
-            if (int rc = readback(c)) return rc;
-            if (c->pinned->n_unresolved == 0) break;
-        }
-    }
+    if (!accept_all) LIETS_CUDA_TRY(c, launch_spacing(c, spacing_s));
     LIETS_CUDA_TRY(c, launch_seed_finalize(c));
     LIETS_CUDA_TRY(c, cudaEventRecord(c->ev1, c->stream));
     if (int rc = readback(c)) return rc;

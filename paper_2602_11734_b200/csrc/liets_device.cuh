@@ -70,9 +70,10 @@ struct Control {
     uint32_t count[2];               // entries in each front list
     uint32_t claims;                 // voxels claimed by the live step (added to n_solid at finish)
     uint32_t n_cand;                 // seeding: candidates
-    uint32_t n_unresolved;           // seeding: candidates still pending after the last round
-    uint32_t round_pending;              // seeding: pending count accumulated by the running round
-    uint32_t pad[2];
+    uint32_t pool_head;              // seeding: used entries of the adjacency pool
+    uint32_t n_rescan;               // seeding: candidates whose adjacency was not stored
+    uint32_t pend3[3];               // seeding: pending candidates after round r, at index r % 3
+    uint32_t pad[1];
     unsigned long long log_front[kLogCap];
     unsigned long long log_solid[kLogCap];
 };

@@ -37,6 +37,7 @@ struct liets_ctx {
     uint32_t* stamp;                  // per brick: t+1 of the last step whose list holds it
     uint8_t* scratch_u8;              // N bytes for format conversion (aliases the candidate buffer)
     uint32_t host_step;               // step counter as of the last read-back (selects the current grid copy)
+    int resolve_grid;                 // CTAs of the cooperative spacing kernel (0 = not sized yet)
     int brick_grid;                   // CTAs of the brick growth kernel
     uint64_t list_cap;                // slots per front list
     // host state
@@ -83,7 +84,7 @@ int grow_brick_chunk();
 // seed.cu
 cudaError_t launch_seed_reset(liets_ctx* c);
 cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all);
-cudaError_t launch_spacing_round(liets_ctx* c, int s);
+cudaError_t launch_spacing(liets_ctx* c, int s);
 cudaError_t launch_seed_finalize(liets_ctx* c);
 cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n);
 // export.cu

@@ -10,7 +10,11 @@
 //   - else              -> v is accepted (all lower-index candidates in range are rejected).
 // Each state change is one atomic on one word, states only move 01 -> {00, 11}, so reading
 // neighbours that change during a round is safe, and the fixed point is the sequential result.
+#include <cooperative_groups.h>
+
 #include "liets_host.h"
+
+namespace cg = cooperative_groups;
 
 namespace liets {
 
@@ -23,8 +27,8 @@ __device__ __forceinline__ uint32_t ld_cg(const uint32_t* p) {
 // --- reset: grid, status map, counters ---------------------------------------------------------
 __global__ void k_seed_reset(Control* c) {
     c->n_solid = 0; c->step = 0; c->steps_done = 0; c->active = 0; c->status = 0; c->cur = 0;
-    c->count[0] = 0; c->count[1] = 0; c->claims = 0; c->n_cand = 0; c->n_unresolved = 0;
-    c->round_pending = 0;
+    c->count[0] = 0; c->count[1] = 0; c->claims = 0; c->n_cand = 0;
+    c->pool_head = 0; c->n_rescan = 0; c->pend3[0] = 0; c->pend3[1] = 0; c->pend3[2] = 0;
 }
 
 // --- candidates: one thread per status word = 16 voxels = 4 Philox blocks -----------------------
@@ -66,14 +70,18 @@ __global__ void __launch_bounds__(256) k_seed_candidates(Control* ctl, uint32_t*
     }
 }
 
-// --- one spacing round: one warp per candidate, lanes over the rows of its diamond --------------
+// --- seed spacing -------------------------------------------------------------------------------
 struct Dims { int nx, ny, nz, periodic; };
 
-// scan the voxels [i0, i1] (linear indices, same row) of the status map; only those with linear
-// index < limit count.  Sets accepted / pending flags.
+constexpr uint32_t kRescan = 0xFFFFFFFFu;       // adjacency of this candidate not stored: rescan its diamond
+constexpr int kAdjBuf = 96;                     // neighbours a warp can buffer per candidate
+
+// Warp-cooperative walk over the status words of the LOWER-index voxels within L1 < s of voxel v
+// (the candidate's diamond).  on_word(word, lo) gets each status word with the fields
+// of out-of-range voxels cleared; lo = linear index of the word's first voxel.
+template <class F>
 __device__ __forceinline__ void scan_segment(const uint32_t* status2, unsigned long long i0,
-                                             unsigned long long i1, unsigned long long limit,
-                                             bool* accepted, bool* pending) {
+                                             unsigned long long i1, unsigned long long limit, F& on_word) {
     if (i0 >= limit) return;
     if (i1 >= limit) i1 = limit - 1;
     for (unsigned long long w = i0 >> 4; w <= (i1 >> 4); ++w) {
@@ -84,76 +92,170 @@ __device__ __forceinline__ void scan_segment(const uint32_t* status2, unsigned l
         if (i0 > lo) field &= 0xFFFFFFFFu << (2 * (uint32_t)(i0 - lo));
         if (i1 < lo + 15) field &= 0xFFFFFFFFu >> (2 * (uint32_t)(lo + 15 - i1));
         word &= field;
-        const uint32_t b0 = word & 0x55555555u, b1 = (word >> 1) & 0x55555555u;
-        if (b0 & b1) *accepted = true;
-        if (b0 & ~b1) *pending = true;
+        if (word) on_word(word, lo);
     }
 }
 
-__global__ void __launch_bounds__(256) k_spacing_round(Control* ctl, uint32_t* status2,
-                                                        const uint32_t* cand, Dims g, int s) {
-    if (ctl->n_unresolved == 0) return;                     // fixed point reached: later rounds are no-ops
-    const uint32_t lane = threadIdx.x & 31u;
-    const uint32_t warp_global = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
-    const uint32_t n_cand = ctl->n_cand;
+template <class F>
+__device__ __forceinline__ void scan_diamond(const uint32_t* status2, uint32_t v, const Dims& g, int s,
+                                             uint32_t lane, F& on_word) {
+    const int x = (int)(v % (uint32_t)g.nx);
+    const uint32_t rest = v / (uint32_t)g.nx;
+    const int y = (int)(rest % (uint32_t)g.ny), z = (int)(rest / (uint32_t)g.ny);
     const int r = s - 1;                                    // diamond radius: L1 <= s-1  <=>  L1 < s
     const int side = 2 * r + 1;
-    uint32_t still = 0;
-    for (uint32_t i = warp_global; i < n_cand; i += n_warps) {
-        const uint32_t v = cand[i];
-        const uint32_t st = (ld_cg(status2 + (v >> 4)) >> (2 * (v & 15u))) & 3u;
-        if (st != 1u) continue;                             // already resolved
-        const int x = (int)(v % (uint32_t)g.nx);
-        const uint32_t rest = v / (uint32_t)g.nx;
-        const int y = (int)(rest % (uint32_t)g.ny), z = (int)(rest / (uint32_t)g.ny);
-        bool accepted = false, pending = false;
-        for (int j = (int)lane; j < side * side; j += 32) {
-            const int dz = j / side - r, dy = j % side - r;
-            const int rem = r - abs(dz) - abs(dy);
-            if (rem < 0) continue;
-            int Y = y + dy, Z = z + dz;
-            if (g.periodic) {
-                Y %= g.ny; if (Y < 0) Y += g.ny;
-                Z %= g.nz; if (Z < 0) Z += g.nz;
-            } else if (Y < 0 || Y >= g.ny || Z < 0 || Z >= g.nz) {
-                continue;
-            }
-            const unsigned long long row = ((unsigned long long)Z * g.ny + Y) * (unsigned long long)g.nx;
-            int xa = x - rem, xb = x + rem;
-            if (g.periodic && 2 * rem + 1 >= g.nx) {        // the range covers the whole row
-                scan_segment(status2, row, row + g.nx - 1, v, &accepted, &pending);
-            } else if (!g.periodic) {                       // clipped at the walls
-                xa = xa < 0 ? 0 : xa;
-                xb = xb >= g.nx ? g.nx - 1 : xb;
-                scan_segment(status2, row + xa, row + xb, v, &accepted, &pending);
-            } else {                                        // wrapped range, at most two segments
-                if (xa < 0) {
-                    scan_segment(status2, row + (xa + g.nx), row + g.nx - 1, v, &accepted, &pending);
-                    xa = 0;
-                }
-                if (xb >= g.nx) {
-                    scan_segment(status2, row, row + (xb - g.nx), v, &accepted, &pending);
-                    xb = g.nx - 1;
-                }
-                scan_segment(status2, row + xa, row + xb, v, &accepted, &pending);
-            }
+    // without wrap-around, lower-index voxels have dz < 0, or dz = 0 and dy <= 0
+    const int n_rows = g.periodic ? side * side : (r + 1) * side;
+    for (int j = (int)lane; j < n_rows; j += 32) {
+        const int dz = j / side - r, dy = j % side - r;
+        const int rem = r - abs(dz) - abs(dy);
+        if (rem < 0) continue;
+        int Y = y + dy, Z = z + dz;
+        if (g.periodic) {
+            Y %= g.ny; if (Y < 0) Y += g.ny;
+            Z %= g.nz; if (Z < 0) Z += g.nz;
+        } else if (Y < 0 || Y >= g.ny || Z < 0 || Z >= g.nz || (dz == 0 && dy > 0)) {
+            continue;
         }
-        accepted = __any_sync(0xffffffffu, accepted);
-        pending = __any_sync(0xffffffffu, pending);
-        if (lane == 0) {
-            if (accepted) atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u))));        // 01 -> 00
-            else if (!pending) atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u)));       // 01 -> 11
-            else still++;
+        const unsigned long long row = ((unsigned long long)Z * g.ny + Y) * (unsigned long long)g.nx;
+        int xa = x - rem, xb = x + rem;
+        if (g.periodic && 2 * rem + 1 >= g.nx) {            // the range covers the whole row
+            scan_segment(status2, row, row + g.nx - 1, v, on_word);
+        } else if (!g.periodic) {                           // clipped at the walls
+            xa = xa < 0 ? 0 : xa;
+            xb = xb >= g.nx ? g.nx - 1 : xb;
+            scan_segment(status2, row + xa, row + xb, v, on_word);
+        } else {                                            // wrapped range, at most two segments
+            if (xa < 0) {
+                scan_segment(status2, row + (xa + g.nx), row + g.nx - 1, v, on_word);
+                xa = 0;
+            }
+            if (xb >= g.nx) {
+                scan_segment(status2, row, row + (xb - g.nx), v, on_word);
+                xb = g.nx - 1;
+            }
+            scan_segment(status2, row + xa, row + xb, v, on_word);
         }
     }
-    if (lane == 0 && still) atomicAdd(&ctl->round_pending, still);
 }
 
-// between rounds: n_unresolved <- number of candidates the round just done left pending
-__global__ void k_spacing_roll(Control* c, int first) {
-    c->n_unresolved = first ? c->n_cand : c->round_pending;
-    c->round_pending = 0;
+// layout of the candidate buffer (capacity N words): cand[n] | off[n] | cnt[n] | rescan[n] | pool[N-4n]
+struct AdjView {
+    bool ok;
+    uint32_t *off, *cnt, *rescan, *pool;
+    unsigned long long pool_cap;
+};
+__device__ __forceinline__ AdjView adj_view(uint32_t* cand, uint32_t n, unsigned long long N) {
+    AdjView a;
+    a.ok = 4ull * n <= N;
+    a.off = cand + n; a.cnt = cand + 2ull * n; a.rescan = cand + 3ull * n; a.pool = cand + 4ull * n;
+    a.pool_cap = a.ok ? N - 4ull * n : 0ull;
+    return a;
+}
+
+// Pass 1: one warp per candidate lists the lower-index candidates inside its diamond, once.
+__global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const uint32_t* status2, uint32_t* cand,
+                                                            Dims g, int s, unsigned long long N) {
+    __shared__ uint32_t s_buf[8][kAdjBuf];
+    __shared__ uint32_t s_cnt[8];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t warp_global = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t n = ctl->n_cand;
+    const AdjView a = adj_view(cand, n, N);
+    if (!a.ok) return;
+    for (uint32_t i = warp_global; i < n; i += n_warps) {
+        const uint32_t v = cand[i];
+        if (lane == 0) s_cnt[warp] = 0;
+        __syncwarp();
+        auto collect = [&](uint32_t word, unsigned long long lo) {
+            for (uint32_t m = word & 0x55555555u; m; m &= m - 1) {          // every candidate in the word
+                const uint32_t slot = atomicAdd(&s_cnt[warp], 1u);
+                if (slot < (uint32_t)kAdjBuf) s_buf[warp][slot] = (uint32_t)lo + ((__ffs(m) - 1) >> 1);
+            }
+        };
+        scan_diamond(status2, v, g, s, lane, collect);
+        __syncwarp();
+        const uint32_t k = s_cnt[warp];
+        uint32_t base = 0;
+        bool stored = k <= (uint32_t)kAdjBuf;
+        if (stored && k) {
+            if (lane == 0) base = atomicAdd(&ctl->pool_head, k);
+            base = __shfl_sync(0xffffffffu, base, 0);
+            stored = (unsigned long long)base + k <= a.pool_cap;
+        }
+        if (stored) {
+            for (uint32_t e = lane; e < k; e += 32) a.pool[base + e] = s_buf[warp][e];
+            if (lane == 0) { a.off[i] = base; a.cnt[i] = k; }
+        } else if (lane == 0) {
+            a.cnt[i] = kRescan;
+            a.rescan[atomicAdd(&ctl->n_rescan, 1u)] = i;
+        }
+        __syncwarp();
+    }
+}
+
+__device__ __forceinline__ uint32_t status_of(const uint32_t* status2, uint32_t v) {
+    return (ld_cg(status2 + (v >> 4)) >> (2 * (v & 15u))) & 3u;
+}
+
+// Pass 2: all rounds in one cooperative launch.  A pending candidate is rejected as soon as a
+// lower-index neighbour is accepted, accepted once none of them is pending, else it waits.
+__global__ void __launch_bounds__(512) k_spacing_resolve(Control* ctl, uint32_t* status2, uint32_t* cand,
+                                                          Dims g, int s, unsigned long long N) {
+    cg::grid_group grid = cg::this_grid();
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, n_threads = gridDim.x * blockDim.x;
+    const uint32_t n = ctl->n_cand;
+    const AdjView a = adj_view(cand, n, N);
+    const uint32_t n_rescan = a.ok ? ld_cg(&ctl->n_rescan) : n;
+    for (uint32_t round = 0;; ++round) {
+        uint32_t still = 0;
+        if (a.ok) {
+            for (uint32_t i = tid; i < n; i += n_threads) {             // one thread per candidate
+                const uint32_t k = a.cnt[i];
+                if (k == kRescan) continue;
+                const uint32_t v = cand[i];
+                if (status_of(status2, v) != 1u) continue;
+                bool accepted = false, pending = false;
+                const uint32_t* nb = a.pool + a.off[i];
+                for (uint32_t e = 0; e < k && !accepted; ++e) {
+                    const uint32_t st = status_of(status2, nb[e]);
+                    accepted = st == 3u;
+                    pending = pending || st == 1u;
+                }
+                if (accepted) atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u))));        // 01 -> 00
+                else if (!pending) atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u)));       // 01 -> 11
+                else still++;
+            }
+        }
+        for (uint32_t q = tid >> 5; q < n_rescan; q += n_threads >> 5) { // one warp per candidate: rescan
+            const uint32_t i = a.ok ? a.rescan[q] : q;
+            const uint32_t v = cand[i];
+            if (status_of(status2, v) != 1u) continue;
+            bool accepted = false, pending = false;
+            auto look = [&](uint32_t word, unsigned long long) {
+                const uint32_t b0 = word & 0x55555555u, b1 = (word >> 1) & 0x55555555u;
+                if (b0 & b1) accepted = true;
+                if (b0 & ~b1) pending = true;
+            };
+            scan_diamond(status2, v, g, s, lane, look);
+            accepted = __any_sync(0xffffffffu, accepted);
+            pending = __any_sync(0xffffffffu, pending);
+            if (lane == 0) {
+                if (accepted) atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u))));
+                else if (!pending) atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u)));
+                else still++;
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) still += __shfl_xor_sync(0xffffffffu, still, o);
+        if (lane == 0 && still) atomicAdd(&ctl->pend3[round % 3u], still);
+        grid.sync();
+        const uint32_t left = ld_cg(&ctl->pend3[round % 3u]);
+        if (tid == 0) ctl->pend3[(round + 2u) % 3u] = 0;               // next used in round+2, after another sync
+        if (left == 0) break;
+    }
 }
 
 // --- finalize: accepted candidates -> grid + initial front A_0 = seeds (R3) ---------------------
@@ -247,22 +349,29 @@ cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all
     k_seed_candidates<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->N, T, always,
                                                               (uint32_t)accept_all, key);
     c->launches++;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    k_spacing_roll<<<1, 1, 0, c->stream>>>(c->ctl, 1);
-    c->launches++;
     return cudaGetLastError();
 }
 
-cudaError_t launch_spacing_round(liets_ctx* c, int s) {
-    const Dims g{ c->nx, c->ny, c->nz, c->boundary };
-    k_spacing_round<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, g, s);
+// exact parallel reproduction of the ascending-index greedy (R12): adjacency once, then all rounds
+// inside one cooperative kernel (grid-wide syncs on the device, no host round trip)
+cudaError_t launch_spacing(liets_ctx* c, int s) {
+    Dims g{ c->nx, c->ny, c->nz, c->boundary };
+    unsigned long long N = c->N;
+    k_spacing_adjacency<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, g, s, N);
     c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    k_spacing_roll<<<1, 1, 0, c->stream>>>(c->ctl, 0);
+    if (c->resolve_grid == 0) {
+        int per_sm = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spacing_resolve, 512, 0);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+        c->resolve_grid = c->sm_count * (per_sm > 2 ? 2 : per_sm);
+    }
+    void* args[] = { &c->ctl, &c->status2, &c->cand, &g, &s, &N };
+    e = cudaLaunchCooperativeKernel((const void*)k_spacing_resolve, dim3(c->resolve_grid), dim3(512), args, 0, c->stream);
     c->launches++;
-    return cudaGetLastError();
+    return e;
 }
 
 cudaError_t launch_seed_finalize(liets_ctx* c) {
