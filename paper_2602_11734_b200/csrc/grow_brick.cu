@@ -32,12 +32,18 @@ constexpr uint32_t kHole = 0xFFFFFFFFu;     // unused slot of a warp's list chun
 constexpr int kChunk = 8;                   // list slots a warp reserves at a time
 
 struct __align__(16) WarpSmem {
-    unsigned long long nbw[27][8];          // words of the 27 bricks (own = index 13)
+    union {
+        unsigned long long nbw[27][8];      // phase A: words of the 27 bricks (own = index 13)
+        uint2 nz[7 * 64 / 4 + 4];           // phases B-C: the non-zero words of U, in order: (word, word index)
+    };
+    unsigned long long own[8];              // this brick's words (carried into the next grid copy)
     uint32_t V[7 * 64];                     // [block b][row]: the 4 void-target masks (8 bits each) of block b
     uint32_t U[7 * 64 / 4];                 // [block b][row] bytes: OR of the 4 masks = voxels needing block b
     uint32_t rows[100];                     // 10 bits per row: bit (x'+1), rows (z'+1)*10 + (y'+1)
     uint32_t claims[100];                   // same geometry: cells claimed in this step
     uint32_t rowbase[64];                   // linear voxel index of (x=0, y, z) of the interior rows
+    uint4 T4[7];                            // per Philox block: T-1 of its 4 directions (fire iff draw <= T-1)
+    uint32_t dir[28];                       // direction d: (row delta + 11) | (dx + 1) << 8 in the 10x10x10 geometry
 };
 
 // region index i in [-1, 8] along one axis of brick b -> brick index (or -1: no such cell) and local coordinate
@@ -69,11 +75,9 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
                                                                     uint32_t* stamp, uint32_t* list0, uint32_t* list1,
                                                                     PhiloxKey key) {
     if (!ctl->active) return;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ uint4 s_T4[7];               // per Philox block: T-1 of its 4 directions (fire iff draw <= T-1)
-    __shared__ uint32_t s_dir[28];          // direction d: (row delta + 11) | (dx + 1) << 8 in the 10x10x10 geometry
+    __shared__ WarpSmem s_ws[kWarpsPerCta];  // static: addresses are compile-time constants + warp offset
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
+    WarpSmem& S = s_ws[warp];
 
     const uint32_t cur = ctl->cur;
     const uint32_t n_list = ctl->count[cur];
@@ -83,17 +87,17 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
     const uint32_t t = ctl->step;
     const unsigned long long* __restrict__ Gc = (t & 1u) ? G1 : G0;     // g_t (read only)
     unsigned long long* Gn = (t & 1u) ? G0 : G1;                        // g_{t+1} (OR target)
-    if (threadIdx.x < 28) {
-        const int d = threadIdx.x < 26 ? (int)threadIdx.x : 25;
+    if (lane < 28) {                        // every warp keeps its own copy: one base register serves all tables
+        const int d = lane < 26 ? (int)lane : 25;
         const int raw = d + (d >= 13 ? 1 : 0);
         const int dx = raw % 3 - 1, dy = (raw / 3) % 3 - 1, dz = raw / 9 - 1;
         const int cls = (dx != 0) + (dy != 0) + (dz != 0) - 1;
         // T in [0, 2^32]: "draw < T" == "draw <= T-1" for T >= 1; directions with T = 0 are disabled in phase B
         const uint32_t tm1 = ctl->always[cls] ? 0xFFFFFFFFu : ctl->T[cls] - 1u;
-        reinterpret_cast<uint32_t*>(s_T4)[threadIdx.x] = tm1;
-        s_dir[threadIdx.x] = (uint32_t)(dz * 10 + dy + 11) | ((uint32_t)(dx + 1) << 8);
+        reinterpret_cast<uint32_t*>(S.T4)[lane] = tm1;
+        S.dir[lane] = (uint32_t)(dz * 10 + dy + 11) | ((uint32_t)(dx + 1) << 8);
     }
-    __syncthreads();
+    __syncwarp();
     // a class whose threshold is 0 never fires: its directions produce no work
     const uint32_t en0 = (ctl->T[0] | ctl->always[0]) ? 0xFFu : 0u;
     const uint32_t en1 = (ctl->T[1] | ctl->always[1]) ? 0xFFu : 0u;
@@ -137,6 +141,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
             }
         }
         __syncwarp();
+        if (lane < 8) S.own[lane] = S.nbw[13][lane];
         // local coordinates of the cells just outside the brick on the low side
         const int lxl = bxi > 0 ? 7 : g.nx - 8 * (g.bx - 1) - 1;
         const int lyl = byi > 0 ? 7 : g.ny - 8 * (g.by - 1) - 1;
@@ -190,14 +195,27 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
             S.rowbase[r2] = (uint32_t)(8 * bxi) + (uint32_t)g.nx * ((uint32_t)(8 * byi + y) + (uint32_t)g.ny * (uint32_t)(8 * bzi + z));
         }
         __syncwarp();
-        // rank partition: lanes 0..27 count 4 words each, scan, every lane takes an equal share of set bits
-        uint32_t cnt = 0;
+        // rank partition: lanes 0..27 count 4 words each, scan, every lane takes an equal share of set bits;
+        // the non-zero words are also copied to a dense list so that moving to the next word is one load
+        uint32_t cnt = 0, nzc = 0;
+        uint4 u4 = make_uint4(0u, 0u, 0u, 0u);
         if (lane < 28) {
-            const uint4 u4 = reinterpret_cast<const uint4*>(S.U)[lane];
+            u4 = reinterpret_cast<const uint4*>(S.U)[lane];
             cnt = __popc(u4.x) + __popc(u4.y) + __popc(u4.z) + __popc(u4.w);
+            nzc = (u4.x != 0u) + (u4.y != 0u) + (u4.z != 0u) + (u4.w != 0u);
         }
-        uint32_t total;
+        uint32_t total, nz_total;
         const uint32_t excl = warp_exclusive_scan(cnt, lane, &total);
+        const uint32_t nz_excl = warp_exclusive_scan(nzc, lane, &nz_total);
+        {
+            uint32_t k = nz_excl;
+            if (u4.x) S.nz[k++] = make_uint2(u4.x, 4u * lane);
+            if (u4.y) S.nz[k++] = make_uint2(u4.y, 4u * lane + 1u);
+            if (u4.z) S.nz[k++] = make_uint2(u4.z, 4u * lane + 2u);
+            if (u4.w) S.nz[k++] = make_uint2(u4.w, 4u * lane + 3u);
+            if (lane == 31) S.nz[nz_total] = make_uint2(0xFFFFFFFFu, 0u);      // sentinel: never dereferenced as an item
+        }
+        __syncwarp();
 
         // ---- C: draw + test ---------------------------------------------------------------------------
         if (total) {
@@ -211,35 +229,36 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
                 if (e <= first) lo = mid; else hi = mid - 1u;
             }
             uint32_t rem = first - __shfl_sync(0xffffffffu, excl, lo);
-            uint32_t wi = 4u * lo;
-            uint32_t cur = S.U[wi];
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const uint32_t pc = __popc(cur);
-                if (rem >= pc && wi < 111u) { rem -= pc; ++wi; cur = S.U[wi]; }
+            uint32_t k = __shfl_sync(0xffffffffu, nz_excl, lo);     // position in the non-zero list
+            uint2 w = S.nz[k];
+            if (last > first) {                                     // walk to the word that holds item `first`
+                uint32_t pc = __popc(w.x);
+                while (rem >= pc) { rem -= pc; w = S.nz[++k]; pc = __popc(w.x); }
             }
+            uint32_t cur = w.x, wi = w.y;
             for (; rem; --rem) cur &= cur - 1u;                     // skip the set bits that belong to lower lanes
-            for (uint32_t n = last - first; n; --n) {
-                while (cur == 0u) cur = S.U[++wi];
+            // flat loop, one item per lane per iteration: the lanes stay in lockstep
+            for (uint32_t n_left = last - first; n_left; --n_left) {
+                if (cur == 0u) { w = S.nz[++k]; cur = w.x; wi = w.y; }
                 const uint32_t bit = __ffs(cur) - 1u;
                 cur &= cur - 1u;
-                const uint32_t e = 4u * wi + (bit >> 3), x = bit & 7u;      // e = b*64 + row
+                const uint32_t e = (wi << 2) + (bit >> 3), x = bit & 7u;    // e = b*64 + row
                 const uint32_t b = e >> 6, r2 = e & 63u;
-                const uint32_t vm = (((S.V[e] >> x) & 0x01010101u) * 0x10204080u) >> 28;
                 const uint32_t p = S.rowbase[r2] + x;
                 const uint4 rnd = philox4x32_10(p, 0u, t, b, key);
-                const uint4 T4 = s_T4[b];
-                uint32_t fire = (rnd.x <= T4.x ? 1u : 0u) | (rnd.y <= T4.y ? 2u : 0u) | (rnd.z <= T4.z ? 4u : 0u) |
-                                (rnd.w <= T4.w ? 8u : 0u);
-                fire &= vm;
-                if (fire) {                                         // a draw fell below its threshold: claim the target
-                    const uint32_t rowidx = ((r2 >> 3) + 1u) * 10u + (r2 & 7u) + 1u;
-                    do {
+                const uint4 T4 = S.T4[b];
+                if (rnd.x <= T4.x || rnd.y <= T4.y || rnd.z <= T4.z || rnd.w <= T4.w) {
+                    // a draw fell below its threshold: claim the target if that direction was a void one
+                    uint32_t fire = (rnd.x <= T4.x ? 1u : 0u) | (rnd.y <= T4.y ? 2u : 0u) | (rnd.z <= T4.z ? 4u : 0u) |
+                                    (rnd.w <= T4.w ? 8u : 0u);
+                    fire &= (((S.V[e] >> x) & 0x01010101u) * 0x10204080u) >> 28;
+                    const uint32_t zy = 10u * (r2 >> 3) + (r2 & 7u);
+                    while (fire) {
                         const uint32_t j = __ffs(fire) - 1u;
                         fire &= fire - 1u;
-                        const uint32_t lut = s_dir[4u * b + j];
-                        atomicOr(&S.claims[rowidx + (lut & 0xFFu) - 11u], 1u << (x + (lut >> 8)));
-                    } while (fire);
+                        const uint32_t lut = S.dir[4u * b + j];
+                        atomicOr(&S.claims[zy + (lut & 0xFFu)], 1u << (x + (lut >> 8)));
+                    }
                 }
             }
         }
@@ -254,7 +273,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
             for (int y = 0; y < 8; ++y)
                 if (y < wcy)
                     cw |= (unsigned long long)((S.claims[(z + 1) * 10 + (y + 1)] >> 1) & ((1u << wcx) - 1u)) << (8 * y);
-            const unsigned long long val = S.nbw[13][z] | cw;
+            const unsigned long long val = S.own[z] | cw;
             if (cw) {
                 const unsigned long long old = atomicOr(Gn + own_base + z, val);
                 new_solid += __popcll(cw & ~old);
@@ -305,18 +324,19 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
 
 }  // namespace
 
-size_t grow_brick_smem_bytes() { return sizeof(WarpSmem) * kWarpsPerCta; }
+size_t grow_brick_smem_bytes() { return 0; }   // static shared memory only
 int grow_brick_warps_per_cta() { return kWarpsPerCta; }
 int grow_brick_chunk() { return kChunk; }
 
 cudaError_t launch_grow_brick(liets_ctx* c) {
     static bool attr_set = false;
-    const size_t smem = grow_brick_smem_bytes();
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_grow_brick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (!attr_set) {                                        // 4 CTAs x 40 KB of static shared memory per SM
+        cudaError_t e = cudaFuncSetAttribute(k_grow_brick, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                             (int)cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
+    const size_t smem = 0;
     const PhiloxKey key = philox_make_key(c->rng_seed);
     k_grow_brick<<<c->brick_grid, kWarpsPerCta * 32, smem, c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->stamp,
                                                                        c->list[0], c->list[1], key);

@@ -199,34 +199,57 @@ __device__ __forceinline__ uint32_t status_of(const uint32_t* status2, uint32_t 
     return (ld_cg(status2 + (v >> 4)) >> (2 * (v & 15u))) & 3u;
 }
 
+// one look at the stored lower-index neighbours of pending candidate v:
+// 0 = still waiting, 1 = resolved now (v's status word updated)
+__device__ __forceinline__ uint32_t try_resolve(uint32_t* status2, uint32_t v, const uint32_t* nb, uint32_t k) {
+    bool accepted = false, pending = false;
+    for (uint32_t e = 0; e < k; ++e) {
+        const uint32_t st = status_of(status2, nb[e]);
+        accepted = accepted || st == 3u;
+        pending = pending || st == 1u;
+    }
+    if (accepted) { atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u)))); return 1u; }     // 01 -> 00
+    if (!pending) { atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u))); return 1u; }         // 01 -> 11
+    return 0u;
+}
+
+constexpr int kPolls = 24;      // looks per round before falling back to a grid-wide sync
+
 // Pass 2: all rounds in one cooperative launch.  A pending candidate is rejected as soon as a
-// lower-index neighbour is accepted, accepted once none of them is pending, else it waits.
-__global__ void __launch_bounds__(512) k_spacing_resolve(Control* ctl, uint32_t* status2, uint32_t* cand,
-                                                          Dims g, int s, unsigned long long N) {
+// lower-index neighbour is accepted, accepted once none of them is pending, else it waits.  Every
+// thread keeps its first candidate in registers and polls its neighbours' status words (L2) a
+// bounded number of times per round, so a dependency chain of length L needs about L / kPolls
+// grid-wide syncs instead of L.
+__global__ void __launch_bounds__(1024) k_spacing_resolve(Control* ctl, uint32_t* status2, uint32_t* cand,
+                                                           Dims g, int s, unsigned long long N) {
     cg::grid_group grid = cg::this_grid();
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, n_threads = gridDim.x * blockDim.x;
     const uint32_t n = ctl->n_cand;
     const AdjView a = adj_view(cand, n, N);
     const uint32_t n_rescan = a.ok ? ld_cg(&ctl->n_rescan) : n;
+    // this thread's own candidate (i = tid), cached
+    uint32_t v0 = 0, k0 = 0;
+    const uint32_t* nb0 = nullptr;
+    bool open0 = false;
+    if (a.ok && tid < n) {
+        k0 = a.cnt[tid];
+        if (k0 != kRescan) { v0 = cand[tid]; nb0 = a.pool + a.off[tid]; open0 = status_of(status2, v0) == 1u; }
+    }
     for (uint32_t round = 0;; ++round) {
         uint32_t still = 0;
+        for (int poll = 0; poll < kPolls; ++poll) {
+            if (!__any_sync(0xffffffffu, open0)) break;
+            if (open0 && try_resolve(status2, v0, nb0, k0)) open0 = false;
+        }
+        if (open0) still++;
         if (a.ok) {
-            for (uint32_t i = tid; i < n; i += n_threads) {             // one thread per candidate
+            for (uint32_t i = tid + n_threads; i < n; i += n_threads) {     // more candidates than threads
                 const uint32_t k = a.cnt[i];
                 if (k == kRescan) continue;
                 const uint32_t v = cand[i];
                 if (status_of(status2, v) != 1u) continue;
-                bool accepted = false, pending = false;
-                const uint32_t* nb = a.pool + a.off[i];
-                for (uint32_t e = 0; e < k && !accepted; ++e) {
-                    const uint32_t st = status_of(status2, nb[e]);
-                    accepted = st == 3u;
-                    pending = pending || st == 1u;
-                }
-                if (accepted) atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u))));        // 01 -> 00
-                else if (!pending) atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u)));       // 01 -> 11
-                else still++;
+                if (!try_resolve(status2, v, a.pool + a.off[i], k)) still++;
             }
         }
         for (uint32_t q = tid >> 5; q < n_rescan; q += n_threads >> 5) { // one warp per candidate: rescan
@@ -363,13 +386,13 @@ cudaError_t launch_spacing(liets_ctx* c, int s) {
     if (e != cudaSuccess) return e;
     if (c->resolve_grid == 0) {
         int per_sm = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spacing_resolve, 512, 0);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spacing_resolve, 1024, 0);
         if (e != cudaSuccess) return e;
         if (per_sm < 1) return cudaErrorLaunchOutOfResources;
-        c->resolve_grid = c->sm_count * (per_sm > 2 ? 2 : per_sm);
+        c->resolve_grid = c->sm_count;
     }
     void* args[] = { &c->ctl, &c->status2, &c->cand, &g, &s, &N };
-    e = cudaLaunchCooperativeKernel((const void*)k_spacing_resolve, dim3(c->resolve_grid), dim3(512), args, 0, c->stream);
+    e = cudaLaunchCooperativeKernel((const void*)k_spacing_resolve, dim3(c->resolve_grid), dim3(1024), args, 0, c->stream);
     c->launches++;
     return e;
 }
