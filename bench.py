@@ -100,6 +100,21 @@ def algorithmic_bytes(storage, N, front, solid_after, n_seeds):
     return out
 
 
+def max_over_ranks(values, dist, device):
+    """Replicas only: the one exchange of a multi-GPU run is the max of the device times."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    tt = torch.tensor(values, dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return [float(v) for v in tt]
+
+
+def whole_job_throughput(n_voxels, world, steps, total_ms):
+    """nodes/s of the whole job: every rank generates `steps` grids of n_voxels in total_ms (max over ranks)."""
+    return n_voxels * world * steps / (total_ms * 1e-3)
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on a bounded sample of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -204,10 +219,7 @@ def run_ours(args):
         t_e2e += one(True)[0]
     barrier()
     clocks = sampler.stop()
-    if dist is not None:
-        tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_dev, t_e2e = float(tt[0]), float(tt[1])
+    t_dev, t_e2e = max_over_ranks([t_dev, t_e2e], dist, "cuda")
 
     # --- roofline of the dominant kernel (the growth kernel), timed live with CUDA events ---------
     gen.set_profiling(True)
@@ -215,23 +227,37 @@ def run_ours(args):
     gen.generate(w["target"])
     step_ms = gen.step_times()[:n_steps]
     gen.set_profiling(False)
-    front, solid_after = gen.step_log()
+    front, solid_after, philox_blocks = gen.step_log()
     b_alg = algorithmic_bytes(storage, N, front[:n_steps], solid_after[:n_steps], n_seeds)
     peaks, peaks_kind = load_peaks()
     grow_ms = float(np.sum(step_ms))
-    achieved = sum(b_alg) / (grow_ms * 1e-3) / 1e9 if grow_ms > 0 else 0.0
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / peaks["hbm_gbs"], "traffic": TRAFFIC_BYTES_PER_LAUNCH,
-                "kernel": KERNEL_NAMES[storage], "peak_kind": "%s (MEASURED_PEAKS.json hbm_gbs, burst copy)" % peaks_kind,
-                "launches": int(n_steps), "algorithmic_bytes_per_launch": sum(b_alg) / max(n_steps, 1),
-                "avg_launch_ms": grow_ms / max(n_steps, 1),
+    n_blocks = float(np.sum(philox_blocks[:n_steps]))
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    # the path is bound by integer issue, not by bytes.  Algorithmic work of a launch =
+    # Philox4x32-10 blocks the keyed draws need (one per (front voxel, block of 4 directions) with a void
+    # target) x 40 integer instructions (20 32x32->64 multiplies + 20 three-input XORs).  Peak = SMs x 4
+    # schedulers x 32 lanes x 1 instruction/clock x the maximum SM clock.
+    alu_peak = sm_count * 4 * 32 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    alu_achieved = n_blocks * PHILOX_INT_OPS / (grow_ms * 1e-3) / 1e12 if grow_ms > 0 else 0.0
+    hbm_achieved = sum(b_alg) / (grow_ms * 1e-3) / 1e9 if grow_ms > 0 else 0.0
+    roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Tiop/s (thread-level integer instructions)",
+                "frac": alu_achieved / alu_peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                "kernel": KERNEL_NAMES[storage],
+                "peak_kind": "derived: %d SMs x 4 schedulers x 32 lanes x %.0f MHz (sm_max_mhz, %s)" % (
+                    sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peaks_kind),
+                "launches": int(n_steps), "philox_blocks_per_launch": n_blocks / max(n_steps, 1),
+                "int_ops_per_philox_block": PHILOX_INT_OPS, "avg_launch_ms": grow_ms / max(n_steps, 1),
                 "growth_kernel_share_of_generate": grow_ms / max(float(np.median(gen_ms)), 1e-9),
-                "front_voxel_updates_per_s": (float(np.sum(front[:n_steps])) / (grow_ms * 1e-3)) if storage == 0 else None}
+                "hbm": {"bound": "hbm", "achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                        "frac": hbm_achieved / peaks["hbm_gbs"],
+                        "peak_kind": "%s (MEASURED_PEAKS.json hbm_gbs, burst copy)" % peaks_kind,
+                        "algorithmic_bytes_per_launch": sum(b_alg) / max(n_steps, 1),
+                        "note": "SURVEY.md 8(d) byte model; the grid (2 x %.1f MB) is L2 resident" % (N / 8e6)}}
 
     out = None
     if rank == 0:
-        value = N * world * args.steps / (t_dev * 1e-3)
-        e2e_value = N * world * args.steps / (t_e2e * 1e-3)
+        value = whole_job_throughput(N, world, args.steps, t_dev)
+        e2e_value = whole_job_throughput(N, world, args.steps, t_e2e)
         out = {
             "metric": "voxel nodes/s (whole generation: seeding + growth to target)",
             "value": value, "unit": "nodes/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -274,6 +300,7 @@ def cpu_baseline():
 
 
 DEFAULT_STORAGE = 1
+PHILOX_INT_OPS = 40
 KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_brick"}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for the current kernel.

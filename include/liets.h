@@ -101,9 +101,12 @@ int liets_generate(liets_ctx* ctx, double target_solid_fraction, uint32_t max_st
 int liets_grid(liets_ctx* ctx, void* dst, size_t dst_bytes, int format, int dst_is_device);
 
 /* Per-step counters of the steps done since the last seed (HOST arrays of capacity cap, may be
- * NULL): front size at the start of step i (voxels for STORAGE_U8, bricks for STORAGE_BRICK) and
- * solid count after it.  Returns the number of steps recorded (<= 4096 kept). */
-int liets_step_log(liets_ctx* ctx, uint64_t* front_in, uint64_t* solid_after, uint32_t cap);
+ * NULL): front size at the start of step i (list entries: voxels for STORAGE_U8, brick slots for
+ * STORAGE_BRICK), solid count after it, and the number of Philox4x32-10 blocks the step evaluated
+ * (one per (front voxel, block of 4 directions) with at least one void target).
+ * Returns the number of steps recorded (<= 4096 kept). */
+int liets_step_log(liets_ctx* ctx, uint64_t* front_in, uint64_t* solid_after, uint64_t* philox_blocks,
+                   uint32_t cap);
 
 /* Device time in milliseconds of the last liets_seed and the last liets_generate (CUDA events on
  * the ctx stream). */

@@ -27,7 +27,7 @@ __global__ void k_control(Control* c, uint32_t flags) {
     if ((flags & kCtlFinish) && c->active) {             // close the step that just ran
         c->n_solid += c->claims;                         // phi_a update
         c->claims = 0;
-        if (c->step < kLogCap) c->log_solid[c->step] = c->n_solid;
+        if (c->step < kLogCap) { c->log_solid[c->step] = c->n_solid; c->log_items[c->step] = c->items; }
         c->cur ^= 1u;                                    // A <- prune(A U A_new) (R4)
         c->step += 1;
         c->steps_done += 1;
@@ -49,6 +49,7 @@ __global__ void k_control(Control* c, uint32_t flags) {
         }
         c->count[c->cur ^ 1u] = 0;
         c->claims = 0;
+        c->items = 0;
         if (c->step < kLogCap) c->log_front[c->step] = c->count[c->cur];
         c->active = 1;
     }

@@ -104,6 +104,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
     const uint32_t en2 = (ctl->T[2] | ctl->always[2]) ? 0xFFu : 0u;
 
     uint32_t new_solid = 0;                 // per lane: bits this lane flipped 0 -> 1
+    uint32_t n_items = 0;                   // lane 0: Philox blocks this warp evaluated
     uint32_t chunk_pos = 0, chunk_end = 0;  // lane 0: reserved slots of the next list
 
     const uint32_t warp_global = blockIdx.x * kWarpsPerCta + warp;
@@ -218,6 +219,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
         __syncwarp();
 
         // ---- C: draw + test ---------------------------------------------------------------------------
+        n_items += total;
         if (total) {
             const uint32_t first = (lane * total) >> 5, last = ((lane + 1u) * total) >> 5;
             // the lane whose 4 words hold item number `first`: largest o with excl[o] <= first
@@ -320,6 +322,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) k_grow_brick(Control* __
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) new_solid += __shfl_xor_sync(0xffffffffu, new_solid, o);
     if (lane == 0 && new_solid) atomicAdd(&ctl->claims, new_solid);
+    if (lane == 0 && n_items) atomicAdd(&ctl->items, n_items);
 }
 
 }  // namespace

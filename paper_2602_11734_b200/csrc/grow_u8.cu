@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
     const uint32_t t = ctl->step;
     const uint32_t T0 = ctl->T[0], T1 = ctl->T[1], T2 = ctl->T[2];
     const bool A0 = ctl->always[0], A1 = ctl->always[1], A2 = ctl->always[2];
-    uint32_t my_claims = 0;
+    uint32_t my_claims = 0, my_items = 0;
 
     for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
         const uint64_t i = base + threadIdx.x;
@@ -77,6 +77,7 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
             for (int b = 0; b < 7; ++b) {                  // one Philox block = 4 directions (R9)
                 const uint32_t bm = (b < 6 ? 0xFu : 0x3u) << (4 * b);
                 if (mask & bm) {
+                    ++my_items;
                     const uint4 r = philox4x32_10(p, 0u, t, (uint32_t)b, key);
                     const uint32_t w[4] = { r.x, r.y, r.z, r.w };
 #pragma unroll
@@ -126,6 +127,9 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) my_claims += __shfl_xor_sync(0xffffffffu, my_claims, o);
     if ((threadIdx.x & 31u) == 0 && my_claims) atomicAdd(&ctl->claims, my_claims);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) my_items += __shfl_xor_sync(0xffffffffu, my_items, o);
+    if ((threadIdx.x & 31u) == 0 && my_items) atomicAdd(&ctl->items, my_items);
 }
 
 }  // namespace

@@ -265,7 +265,7 @@ int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps
     uint32_t enqueued = 0;
     for (;;) {
         // a batch of steps back to back; steps after the stop rule fired are no-ops on the device
-        uint32_t batch = 16;
+        uint32_t batch = 32;
         if (max_steps - enqueued < batch) batch = max_steps - enqueued;
         for (uint32_t k = 0; k < batch; ++k) {
             LIETS_CUDA_TRY(c, launch_control(c, k == 0 ? kCtlPrepare : (kCtlFinish | kCtlPrepare)));
@@ -314,7 +314,7 @@ int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is
     return LIETS_OK;
 }
 
-int liets_step_log(liets_ctx* c, uint64_t* front_in, uint64_t* solid_after, uint32_t cap) {
+int liets_step_log(liets_ctx* c, uint64_t* front_in, uint64_t* solid_after, uint64_t* philox_blocks, uint32_t cap) {
     if (!c) return LIETS_E_ARG;
     if (int rc = readback(c)) return rc;
     uint32_t n = c->pinned->step;
@@ -324,6 +324,8 @@ int liets_step_log(liets_ctx* c, uint64_t* front_in, uint64_t* solid_after, uint
         LIETS_CUDA_TRY(c, cudaMemcpyAsync(front_in, c->ctl->log_front, n * 8ull, cudaMemcpyDeviceToHost, c->stream));
     if (n && solid_after)
         LIETS_CUDA_TRY(c, cudaMemcpyAsync(solid_after, c->ctl->log_solid, n * 8ull, cudaMemcpyDeviceToHost, c->stream));
+    if (n && philox_blocks)
+        LIETS_CUDA_TRY(c, cudaMemcpyAsync(philox_blocks, c->ctl->log_items, n * 8ull, cudaMemcpyDeviceToHost, c->stream));
     LIETS_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return (int)n;
 }

@@ -73,9 +73,10 @@ struct Control {
     uint32_t pool_head;              // seeding: used entries of the adjacency pool
     uint32_t n_rescan;               // seeding: candidates whose adjacency was not stored
     uint32_t pend3[3];               // seeding: pending candidates after round r, at index r % 3
-    uint32_t pad[1];
+    uint32_t items;                  // Philox blocks evaluated by the live step (profiling counter)
     unsigned long long log_front[kLogCap];
     unsigned long long log_solid[kLogCap];
+    unsigned long long log_items[kLogCap];
 };
 
 // control-kernel flags

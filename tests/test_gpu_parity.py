@@ -47,7 +47,7 @@ def test_config1_bit_exact(liets, storage):
     bits = np.unpackbits(L.grid(liets.FORMAT_BITS), bitorder="little")[: L.N]
     assert (bits == o.grid().ravel()).all()
     assert (L.grid_device().cpu().numpy() == o.grid().ravel()).all()
-    f, s = L.step_log()
+    f, s, blocks = L.step_log()
     assert len(f) == o.step_index and int(s[-1]) == o.n_solid
 
 

@@ -24,6 +24,6 @@ CONFIGS = {
 # the configuration BASELINE.json's metric is quoted on ("seconds per full 400^3 generation"), porosity 0.20
 BENCH = dict(name="cfg3_400", dims=(400, 400, 400), periodic=False, core=0.001, s=20, seed=7,
              g=(0.01, 0.0025, 0.00025), target=0.80)
-# bounded CPU-baseline sample: a 120^3 sub-volume of the same workload (same densities, same
-# probabilities, same spacing, same target) -- intensive quantities match, ~15-25 s of oracle time
-BENCH_CPU_SAMPLE = dict(BENCH, name="cfg3_400/sample120", dims=(120, 120, 120))
+# bounded CPU-baseline sample: a 160^3 sub-volume of the same workload (same densities, same
+# probabilities, same spacing, same target) -- intensive quantities match, ~15-25 s of oracle time on the GPU box host
+BENCH_CPU_SAMPLE = dict(BENCH, name="cfg3_400/sample160", dims=(160, 160, 160))
