@@ -84,9 +84,9 @@ def algorithmic_bytes(storage, N, front, solid_after, n_seeds):
     """bytes the list-indexed step itself must move, per step.
 
     STORAGE_U8 (front = voxels):  4|A_t| + min(27|A_t|, N) + c_t + 4|A_{t+1}|
-    STORAGE_BRICK (front = 8^3 bricks of 64 B): 4|B_t| + min(125|B_t|, N/8) + 64|B_t| + 4|B_{t+1}|
-      (read the brick list; each needed grid byte once -- a brick plus its one-voxel halo is 10^3
-      bits = 125 B; write the brick into the next buffer; write the next list)."""
+    STORAGE_TILE (front = 256x8x8 tiles of 2 KiB): 4|L_t| + min(3225|L_t|, N/8) + 2048|L_t| + 4|L_{t+1}|
+      (read the tile list; each needed grid byte once -- a tile plus its one-voxel halo is 258x10x10
+      bits = 3225 B; write the tile's rows into the next buffer; write the next list)."""
     out, prev = [], n_seeds
     for t in range(len(front)):
         a_t = int(front[t])
@@ -96,7 +96,7 @@ def algorithmic_bytes(storage, N, front, solid_after, n_seeds):
         if storage == 0:
             out.append(4 * a_t + min(27 * a_t, N) + c_t + 4 * a_n)
         else:
-            out.append(4 * a_t + min(125 * a_t, N // 8) + 64 * a_t + 4 * a_n)
+            out.append(4 * a_t + min(3225 * a_t, N // 8) + 2048 * a_t + 4 * a_n)
     return out
 
 
@@ -265,7 +265,7 @@ def run_ours(args):
             "dtype": "u32", "data": "synthetic",
             "config": {"workload": w["name"], "grid": [nx, ny, nz], "core_prob": w["core"], "spacing_s": w["s"],
                        "g_face_edge_corner": list(w["g"]), "target_solid_fraction": w["target"], "rng_seed": w["seed"],
-                       "storage": ["u8+voxel-list", "bit-brick+brick-list"][storage], "parallelism": "replicas" if world > 1 else "1gpu",
+                       "storage": ["u8+voxel-list", "bit-rows+tile-list"][storage], "parallelism": "replicas" if world > 1 else "1gpu",
                        "l2": "flushed between iterations (256 MiB memset outside the timed events)",
                        "growth_steps": int(n_steps), "seeds": int(n_seeds), "final_solid": int(n_solid)},
             "seconds_per_generation": t_dev / args.steps * 1e-3,
@@ -301,7 +301,7 @@ def cpu_baseline():
 
 DEFAULT_STORAGE = 1
 PHILOX_INT_OPS = 40
-KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_brick"}
+KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_tile"}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for the current kernel.
 TRAFFIC_BYTES_PER_LAUNCH = None

@@ -42,7 +42,8 @@ enum {
 
 enum { LIETS_BOUNDARY_WALL = 0, LIETS_BOUNDARY_PERIODIC = 1 };        /* R5 */
 enum { LIETS_STORAGE_U8 = 0,      /* uint8 grid + explicit list of front VOXELS (uint32 indices)  */
-       LIETS_STORAGE_BRICK = 1 }; /* bit-packed 8x8x8 bricks + explicit list of front BRICKS      */
+       LIETS_STORAGE_TILE = 1 };  /* bit-packed x-rows + explicit list of active 256x8x8 TILES; the
+                                     front voxels of a tile are re-listed in shared memory each step */
 enum { LIETS_LAW_CONSTANT = 0, LIETS_LAW_EQ1 = 1 };
 enum { LIETS_FORMAT_U8 = 0,       /* one byte per voxel in {0,1}, x fastest, N bytes              */
        LIETS_FORMAT_BITS = 1 };   /* bit idx%8 (LSB first) of byte idx/8, ceil(N/8) bytes         */
@@ -101,9 +102,9 @@ int liets_generate(liets_ctx* ctx, double target_solid_fraction, uint32_t max_st
 int liets_grid(liets_ctx* ctx, void* dst, size_t dst_bytes, int format, int dst_is_device);
 
 /* Per-step counters of the steps done since the last seed (HOST arrays of capacity cap, may be
- * NULL): front size at the start of step i (list entries: voxels for STORAGE_U8, brick slots for
- * STORAGE_BRICK), solid count after it, and the number of Philox4x32-10 blocks the step evaluated
- * (one per (front voxel, block of 4 directions) with at least one void target).
+ * NULL): front size at the start of step i (list entries: voxels for STORAGE_U8, tiles for
+ * STORAGE_TILE), solid count after it, and the number of Philox4x32-10 blocks the step evaluated
+ * (one per front voxel with a void target, plus one per further nibble level of its tied directions).
  * Returns the number of steps recorded (<= 4096 kept). */
 int liets_step_log(liets_ctx* ctx, uint64_t* front_in, uint64_t* solid_after, uint64_t* philox_blocks,
                    uint32_t cap);

@@ -32,18 +32,27 @@ void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* R9: growth draw.  key = (seed lo, seed hi); counter = (p lo, p hi, step t, d / 4);
- * the draw of direction d is output word d % 4. */
+/* R9: growth draw.  The 32-bit draw of (voxel p, step t, direction d) is written nibble by nibble,
+ * most significant first, from eight Philox blocks of the voxel -- block k holds nibble k of the
+ * draws of all 26 directions:
+ *   key = (seed lo, seed hi);   B_k = philox(counter = (p lo, p hi, step t, k)),  k = 0..7;
+ *   nibble k of draw(d) = bits [4 (d / 4), 4 (d / 4) + 4) of word d % 4 of B_k;
+ *   draw(d) = sum_k  nibble_k << (28 - 4 k). */
 uint32_t oracle_growth_draw(uint64_t rng_seed, uint32_t t, uint64_t p, int d) {
     uint32_t key[2] = { (uint32_t)(rng_seed & 0xFFFFFFFFu), (uint32_t)(rng_seed >> 32) };
-    uint32_t ctr[4] = { (uint32_t)(p & 0xFFFFFFFFu), (uint32_t)(p >> 32), t, (uint32_t)(d / 4) };
-    uint32_t out[4];
-    oracle_philox4x32_10(ctr, key, out);
-    return out[d % 4];
+    uint32_t draw = 0;
+    for (uint32_t k = 0; k < 8; ++k) {
+        uint32_t ctr[4] = { (uint32_t)(p & 0xFFFFFFFFu), (uint32_t)(p >> 32), t, k };
+        uint32_t B[4];
+        oracle_philox4x32_10(ctr, key, B);
+        uint32_t nibble = (B[d % 4] >> (4 * (d / 4))) & 0xFu;
+        draw |= nibble << (28 - 4 * k);
+    }
+    return draw;
 }
 
 /* R9: seeding draw.  counter = ((v/4) lo, (v/4) hi, 0, 0xFFFFFFFF); draw of voxel v is word v % 4.
- * (c3 = 0xFFFFFFFF never collides with a growth counter, whose c3 is 0..6.) */
+ * (c3 = 0xFFFFFFFF never collides with a growth counter, whose c3 is 0..7.) */
 uint32_t oracle_seed_draw(uint64_t rng_seed, uint64_t v) {
     uint32_t key[2] = { (uint32_t)(rng_seed & 0xFFFFFFFFu), (uint32_t)(rng_seed >> 32) };
     uint64_t blk = v / 4;

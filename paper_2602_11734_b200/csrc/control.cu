@@ -44,9 +44,23 @@ __global__ void k_control(Control* c, uint32_t flags) {
         if (!(flags & kCtlPrepare)) return;
         for (int k = 0; k < 3; ++k) {
             unsigned long long T = c->law ? eq1_threshold(c->R[k], c->n_t, c->n_solid) : c->R[k];
-            c->always[k] = T >= (1ull << 32);
-            c->T[k] = T >= (1ull << 32) ? 0xFFFFFFFFu : (uint32_t)T;
+            c->en[k] = T >= 1ull;                                            // T in [0, 2^32]
+            c->U[k] = T >= 1ull ? (uint32_t)(T - 1ull) : 0u;                 // draw < T  <=>  draw <= T - 1
         }
+        // the thresholds nibble by nibble, laid out like the draws (direction d: nibble d>>2 of word d&3)
+        uint32_t en26 = 0, h0_any = 0;
+        for (int lv = 0; lv < 8; ++lv)
+            for (int w = 0; w < 4; ++w) c->hpat[lv][w] = 0;
+        for (int d = 0; d < 26; ++d) {
+            const int cls = dir_class(d);
+            if (c->en[cls]) en26 |= 1u << d;
+            for (int lv = 0; lv < 8; ++lv)
+                c->hpat[lv][d & 3] |= ((c->U[cls] >> (28 - 4 * lv)) & 15u) << (4 * (d >> 2));
+            if (c->en[cls] && (c->U[cls] >> 28)) h0_any = 1;
+        }
+        c->en26 = en26;
+        c->h0_any = h0_any;
+        c->tile_cursor = 0;
         c->count[c->cur ^ 1u] = 0;
         c->claims = 0;
         c->items = 0;

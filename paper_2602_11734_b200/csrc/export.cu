@@ -19,22 +19,18 @@ __global__ void __launch_bounds__(256) k_pack_bits_u8(const uint8_t* __restrict_
         dst[b] = (uint8_t)out;
     }
 }
-// bit bricks -> uint8 {0,1} per voxel, x fastest: one thread per brick row (8 voxels)
-__global__ void __launch_bounds__(256) k_unpack_bricks_u8(const unsigned long long* __restrict__ G, uint8_t* __restrict__ dst,
-                                                           BrickGeom g, unsigned long long n_rows) {
-    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_rows;
+// bit rows -> uint8 {0,1} per voxel, x fastest: one thread per 8 voxels of a row
+__global__ void __launch_bounds__(256) k_unpack_rows_u8(const unsigned long long* __restrict__ G, uint8_t* __restrict__ dst,
+                                                         TileGeom g, unsigned long long n_rows) {
+    const unsigned long long per_row = ((unsigned long long)g.nx + 7ull) / 8ull;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_rows * per_row;
          i += (unsigned long long)gridDim.x * blockDim.x) {
-        const unsigned long long b = i >> 6;
-        const uint32_t ly = (uint32_t)i & 7u, lz = ((uint32_t)i >> 3) & 7u;
-        const uint32_t bxi = (uint32_t)(b % (unsigned long long)g.bx);
-        const uint32_t byi = (uint32_t)((b / (unsigned long long)g.bx) % (unsigned long long)g.by);
-        const uint32_t bzi = (uint32_t)(b / ((unsigned long long)g.bx * (unsigned long long)g.by));
-        const uint32_t y = 8u * byi + ly, z = 8u * bzi + lz, x0 = 8u * bxi;
-        if (y >= (uint32_t)g.ny || z >= (uint32_t)g.nz) continue;
-        const uint32_t bits = (uint32_t)(G[8ull * b + lz] >> (8u * ly)) & 0xFFu;
-        const unsigned long long base = (unsigned long long)x0 + (unsigned long long)g.nx * ((unsigned long long)y + (unsigned long long)g.ny * z);
+        const unsigned long long row = i / per_row;
+        const uint32_t b = (uint32_t)(i - row * per_row), x0 = 8u * b;
+        const uint32_t bits = (uint32_t)(G[row * (unsigned long long)g.Wp + (b >> 3)] >> (8u * (b & 7u))) & 0xFFu;
+        const unsigned long long base = row * (unsigned long long)g.nx + x0;
         const uint32_t w = min(8u, (uint32_t)g.nx - x0);
-        if (w == 8u && (base & 7ull) == 0) {                 // aligned full row: one 8-byte store
+        if (w == 8u && (base & 7ull) == 0) {                 // aligned full group: one 8-byte store
             unsigned long long v = 0;
 #pragma unroll
             for (int k = 0; k < 8; ++k) v |= (unsigned long long)((bits >> k) & 1u) << (8 * k);
@@ -52,8 +48,9 @@ cudaError_t launch_pack_bits_u8(liets_ctx* c, const uint8_t* src_u8, uint8_t* ds
     return cudaGetLastError();
 }
 
-cudaError_t launch_unpack_bricks_u8(liets_ctx* c, uint8_t* dst_u8) {
-    k_unpack_bricks_u8<<<c->sm_count * 8, 256, 0, c->stream>>>(c->G[c->host_step & 1u], dst_u8, c->geom, c->n_bricks * 64ull);
+cudaError_t launch_unpack_rows_u8(liets_ctx* c, uint8_t* dst_u8) {
+    k_unpack_rows_u8<<<c->sm_count * 8, 256, 0, c->stream>>>(c->G[c->host_step & 1u], dst_u8, c->geom,
+                                                             (unsigned long long)c->ny * (unsigned long long)c->nz);
     c->launches++;
     return cudaGetLastError();
 }

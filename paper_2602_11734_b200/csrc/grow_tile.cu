@@ -1,0 +1,339 @@
+// grow_tile.cu -- STORAGE_TILE growth step: bit-packed x-rows + explicit list of active TILES.
+//
+// Layout in HBM.  The phase array is stored one bit per voxel in x-rows of Wp = ceil(nx/64) 64-bit
+// words (bit i of word w of row (y, z) = voxel x = 64 w + i; bits with x >= nx stay 0).  Two copies
+// G[0], G[1] are kept: step t reads G[t&1] (immutable during the step, so the update is synchronous
+// by construction) and ORs into G[(t+1)&1].  The active set A is kept
+// at two levels: in HBM a list of active TILES of kTileW words x 8 x 8 rows (256 x 8 x 8 voxels)
+// that hold at least one front voxel, 4 bytes per 16384 voxels; and, per tile and step, the explicit
+// list of its front VOXELS, rebuilt from the bits in shared memory.
+//
+// One CTA owns one tile at a time (tiles are handed out through an atomic cursor):
+//   A  gather: the 10 x 10 rows of the tile's one-voxel neighbourhood, kTileW + 2 words each, as "not void"
+//      bits (solid, outside the domain, or padding), plus a copy in overlapping 32-bit windows so that
+//      any three x-adjacent bits come from one word
+//   B  front voxels: solid cells with a void neighbour, 64 cells per bit operation;
+//      their ids are compacted into a shared-memory list (popc + CTA-wide prefix sum)
+//   C  one thread per front voxel: its 26 void-target bits (Algorithm 3 lines 5-6) from nine window
+//      loads, ONE Philox4x32-10 block = the leading nibble of all 26 draws (R9), one carry-free
+//      per-nibble compare = the directions that fire or tie with the threshold (line 8); voxels with ties go
+//      to a per-warp queue
+//   D  one lane per queued voxel: the next blocks until no direction ties
+//      hits of C and D set bits in a shared-memory claim volume (atomicOr)
+//   E  claim + compact: own rows are OR-ed into G[next] together with the carried state, halo hits
+//      go to the neighbour tiles' rows with atomicOr; the returned old word tells who flipped the bit
+//      (line 9-10, "counted once" PAPER.md:77) for the solid count; a per-tile step stamp
+//      (atomicMax) makes every tile enter the next list exactly once; tiles without front voxels
+//      are not re-emitted (lazy retirement).
+#include "liets_host.h"
+
+namespace liets {
+
+namespace {
+
+constexpr int kTileW = 4;                       // 64-bit words per tile row
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
+constexpr int kWin = (64 * kTileW + 1) / 30 + 1;   // 32-bit windows per row; window k starts at tile bit 30 k - 1
+constexpr int kQueueCap = 128;                  // voxels with ties per warp queue
+constexpr int kMaxFront = 64 * 64 * kTileW;     // every cell of the tile
+
+struct Smem {
+    unsigned long long nv[100][kRowWords];      // not-void bits, row (z'+1)*10 + (y'+1)
+    uint32_t win[100][kWin];                    // the same rows as overlapping windows
+    uint32_t claims[100][2 * kRowWords];        // cells claimed in this step, same geometry as nv (32-bit view)
+    uint32_t queue[kWarps][2 * kQueueCap];      // (voxel id, tied directions)
+    uint32_t hpat[8][4];
+    uint32_t dir[28];                           // direction d: (row delta + 11) | (dx + 1) << 8
+    uint32_t scan[33];
+    uint32_t tile, base, n_front;
+    uint16_t flist[kMaxFront];                  // x | (y | z << 3) << 8 of the tile's front voxels (x relative to the tile)
+};
+
+struct TileCoord {
+    int w0, y0, z0;                             // first word / row / slice of the tile
+    int wcy, wcz;                               // valid rows / slices (< 8 on the high border)
+};
+
+// "not void" word of global row (y, z), global word index wg in [-1, Wp]: data inside the domain, the wrap or
+// wall value at x = -1 and x = nx, ones beyond.  yz_ok = the row exists (after wrapping).
+__device__ __forceinline__ unsigned long long not_void_word(const unsigned long long* __restrict__ G, const TileGeom& g,
+                                                            bool yz_ok, unsigned long long row_base, int wg) {
+    if (!yz_ok) return ~0ull;
+    if (wg < 0) {                               // only bit 63 (x = -1) is ever looked at
+        if (!g.periodic) return ~0ull;
+        const int xl = g.nx - 1;
+        return ((__ldcg(G + row_base + (xl >> 6)) >> (xl & 63)) & 1ull) << 63;
+    }
+    const int xbase = 64 * wg;
+    if (xbase > g.nx) return ~0ull;
+    unsigned long long v = xbase < g.nx ? __ldcg(G + row_base + wg) : 0ull;
+    if (xbase + 64 > g.nx) {                    // the row ends inside this word: halo bit at x = nx, ones above
+        const int nvalid = g.nx - xbase;        // 0..63
+        const unsigned long long halo = g.periodic ? (__ldcg(G + row_base) & 1ull) : 1ull;
+        v |= (~0ull << nvalid);
+        if (!halo) v &= ~(1ull << nvalid);
+    }
+    return v;
+}
+
+// local row coordinate i in [-1, 8] of a tile that starts at c0 and has wc valid rows -> global coordinate, or -1
+__device__ __forceinline__ int row_coord(int i, int c0, int wc, int n, int periodic) {
+    if (i > wc) return -1;
+    int c = c0 + i;
+    if (c < 0) return periodic ? n - 1 : -1;
+    if (c >= n) return periodic ? 0 : -1;
+    return c;
+}
+
+__global__ void __launch_bounds__(kThreads, 4) k_grow_tile(Control* __restrict__ ctl, TileGeom g,
+                                                           unsigned long long* G0, unsigned long long* G1,
+                                                           uint32_t* stamp, uint32_t* list0, uint32_t* list1,
+                                                           PhiloxKey key) {
+    if (!ctl->active) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Smem& S = *reinterpret_cast<Smem*>(smem_raw);
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+
+    const uint32_t cur = ctl->cur;
+    const uint32_t n_list = ctl->count[cur];
+    const uint32_t* __restrict__ in = cur ? list1 : list0;
+    uint32_t* __restrict__ out = cur ? list0 : list1;
+    uint32_t* out_count = &ctl->count[cur ^ 1u];
+    const uint32_t t = ctl->step;
+    const unsigned long long* __restrict__ Gc = (t & 1u) ? G1 : G0;     // g_t (read only)
+    unsigned long long* Gn = (t & 1u) ? G0 : G1;                        // g_{t+1} (OR target)
+    if (tid < 32) S.hpat[tid >> 2][tid & 3] = ctl->hpat[tid >> 2][tid & 3];
+    if (tid < 28) {
+        const int d = tid < 26 ? (int)tid : 25;
+        const int raw = d + (d >= 13 ? 1 : 0);
+        const int dx = raw % 3 - 1, dy = (raw / 3) % 3 - 1, dz = raw / 9 - 1;
+        S.dir[tid] = (uint32_t)(dz * 10 + dy + 11) | ((uint32_t)(dx + 1) << 8);
+    }
+    const uint32_t en26 = ctl->en26;
+    const bool h0_any = ctl->h0_any != 0u;
+    uint32_t new_solid = 0;                 // per thread: bits this thread flipped 0 -> 1
+    uint32_t n_items = 0;                   // per thread: Philox blocks evaluated
+    uint32_t* const my_queue = S.queue[warp];
+
+    for (;;) {
+        __syncthreads();                    // the previous tile's shared memory is no longer read
+        if (tid == 0) S.tile = atomicAdd(&ctl->tile_cursor, 1u);
+        __syncthreads();
+        const uint32_t li = S.tile;
+        if (li >= n_list) break;
+        const uint32_t id = in[li];
+        TileCoord tc;
+        {
+            const uint32_t tx = id % (uint32_t)g.ntx, rest = id / (uint32_t)g.ntx;
+            tc.w0 = (int)tx * kTileW;
+            tc.y0 = 8 * (int)(rest % (uint32_t)g.nty);
+            tc.z0 = 8 * (int)(rest / (uint32_t)g.nty);
+            tc.wcy = min(8, g.ny - tc.y0);
+            tc.wcz = min(8, g.nz - tc.z0);
+        }
+
+        // ---- A: gather ------------------------------------------------------------------------
+        for (int task = (int)tid; task < 100 * kRowWords; task += kThreads) {
+            const int r = task / kRowWords, c = task - r * kRowWords;
+            const int zg = row_coord(r / 10 - 1, tc.z0, tc.wcz, g.nz, g.periodic);
+            const int yg = row_coord(r % 10 - 1, tc.y0, tc.wcy, g.ny, g.periodic);
+            const bool ok = zg >= 0 && yg >= 0;
+            const unsigned long long row_base = ok ? (unsigned long long)g.Wp * ((unsigned long long)yg + (unsigned long long)g.ny * (unsigned long long)zg) : 0ull;
+            S.nv[r][c] = not_void_word(Gc, g, ok, row_base, tc.w0 + c - 1);
+            S.claims[r][2 * c] = 0u;
+            S.claims[r][2 * c + 1] = 0u;
+        }
+        __syncthreads();
+        for (int task = (int)tid; task < 100 * kWin; task += kThreads) {
+            const int r = task / kWin, k = task - r * kWin;
+            const int pos = 63 + 30 * k;                            // bit of the row that holds tile x = 30 k - 1
+            const int wd = pos >> 6, sh = pos & 63;
+            unsigned long long v = S.nv[r][wd] >> sh;
+            if (sh > 32 && wd + 1 < kRowWords) v |= S.nv[r][wd + 1] << (64 - sh);
+            S.win[r][k] = (uint32_t)v;
+        }
+
+        // ---- B: front voxels of the tile ------------------------------------------------------------
+        uint32_t n_front = 0;
+        {
+            unsigned long long F[(64 * kTileW + kThreads - 1) / kThreads];
+            uint32_t cnt = 0;
+#pragma unroll
+            for (int u = 0; u < (64 * kTileW + kThreads - 1) / kThreads; ++u) {
+                const int task = (int)tid + u * kThreads;
+                F[u] = 0ull;
+                if (task < 64 * kTileW) {
+                    const int row = task / kTileW, j = task - row * kTileW, y = row & 7, z = row >> 3;
+                    const int xbase = 64 * (tc.w0 + j);
+                    if (y < tc.wcy && z < tc.wcz && xbase < g.nx) {
+                        unsigned long long anyvoid = 0ull;
+#pragma unroll
+                        for (int k = 0; k < 9; ++k) {
+                            const int rr = (z + k / 3) * 10 + (y + k % 3);
+                            const unsigned long long v = ~S.nv[rr][1 + j];
+                            const unsigned long long l = ~S.nv[rr][j] >> 63, rgt = ~S.nv[rr][2 + j] << 63;
+                            anyvoid |= v | (v << 1) | l | (v >> 1) | rgt;
+                        }
+                        unsigned long long src = S.nv[(z + 1) * 10 + (y + 1)][1 + j];
+                        if (xbase + 64 > g.nx) src &= ~(~0ull << (g.nx - xbase));       // padding is not a source
+                        F[u] = src & anyvoid;                                           // R13
+                    }
+                    cnt += __popcll(F[u]);
+                }
+            }
+            uint32_t off = block_exclusive_scan(cnt, S.scan, &n_front);
+#pragma unroll
+            for (int u = 0; u < (64 * kTileW + kThreads - 1) / kThreads; ++u) {
+                const int task = (int)tid + u * kThreads;
+                const int row = task / kTileW, j = task - row * kTileW;
+                const uint32_t hi = ((uint32_t)row << 8) | (uint32_t)(64 * j);
+                for (unsigned long long m = F[u]; m; m &= m - 1ull)
+                    S.flist[off++] = (uint16_t)(hi | (uint32_t)(__ffsll((long long)m) - 1));
+            }
+        }
+        const uint32_t p0 = (uint32_t)(64 * tc.w0) + (uint32_t)g.nx * ((uint32_t)tc.y0 + (uint32_t)g.ny * (uint32_t)tc.z0);
+        __syncthreads();                    // flist, win complete
+
+        // ---- C + D -----------------------------------------------------------------------------------
+        auto claim = [&](uint32_t fire, uint32_t x, uint32_t zy) {
+            while (fire) {
+                const uint32_t d = __ffs(fire) - 1u;
+                fire &= fire - 1u;
+                const uint32_t lut = S.dir[d];
+                const uint32_t xb = x + 63u + (lut >> 8);           // bit of the row: 64 + x + dx
+                atomicOr(&S.claims[zy + (lut & 0xFFu)][xb >> 5], 1u << (xb & 31u));
+            }
+        };
+        uint32_t qn = 0;                    // queue fill (warp-uniform)
+        auto drain = [&]() {                // D: one lane per queued voxel
+            __syncwarp();
+            for (uint32_t j = lane; j < qn; j += 32u) {
+                const uint32_t v = my_queue[2 * j], tie = my_queue[2 * j + 1];
+                const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = v >> 11;
+                const uint32_t p = p0 + x + (uint32_t)g.nx * (y + (uint32_t)g.ny * z);
+                claim(resolve_ties(p, t, tie, S.hpat, key, &n_items), x, 10u * z + y);
+            }
+            __syncwarp();
+            qn = 0;
+        };
+        for (uint32_t i0 = 0; i0 < n_front; i0 += kThreads) {      // C: one thread per front voxel
+            const uint32_t i = i0 + tid;
+            uint32_t tie = 0, v = 0;
+            if (i < n_front) {
+                v = S.flist[i];
+                const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = v >> 11;
+                const uint32_t k = (x * 2185u) >> 16, s = x - 30u * k;     // window k holds tile bits 30k-1 .. 30k+30
+                uint32_t nb27 = 0;          // bit 9(dz+1) + 3(dy+1) + (dx+1): that neighbour is not void
+#pragma unroll
+                for (int e = 0; e < 9; ++e)
+                    nb27 |= ((S.win[(z + e / 3) * 10u + (y + e % 3)][k] >> s) & 7u) << (3 * e);
+                const uint32_t void27 = ~nb27;
+                const uint32_t void26 = ((void27 & 0x1FFFu) | ((void27 >> 14) << 13)) & en26;
+                if (void26) {
+                    const uint32_t p = p0 + x + (uint32_t)g.nx * (y + (uint32_t)g.ny * z);
+                    const uint4 B0 = philox4x32_10(p, 0u, t, 0u, key);
+                    ++n_items;
+                    if (h0_any) {           // some leading threshold nibble is non-zero: a draw can fire at level 0
+                        uint32_t le;
+                        level_compare(B0, S.hpat[0], void26, &le, &tie);
+                        claim(le & ~tie, x, 10u * z + y);
+                    } else {                // all leading nibbles are 0: "<=" and "==" coincide
+                        tie = level_le(B0, S.hpat[0], void26);
+                    }
+                }
+            }
+            const uint32_t have = __ballot_sync(0xffffffffu, tie != 0u);
+            if (have) {
+                if (qn + 32u > (uint32_t)kQueueCap) drain();
+                if (tie) {
+                    const uint32_t slot = qn + __popc(have & ((1u << lane) - 1u));
+                    my_queue[2 * slot] = v;
+                    my_queue[2 * slot + 1] = tie;
+                }
+                qn += __popc(have);
+            }
+        }
+        if (qn) drain();
+        __syncthreads();                    // all claims are in shared memory
+
+        // ---- E: claim + compact ---------------------------------------------------------------------
+        for (int task = (int)tid; task < 100 * kRowWords; task += kThreads) {
+            const int r = task / kRowWords, c = task - r * kRowWords;
+            const unsigned long long cw = (unsigned long long)S.claims[r][2 * c] | ((unsigned long long)S.claims[r][2 * c + 1] << 32);
+            const int zl = r / 10 - 1, yl = r % 10 - 1;
+            const bool own_row = zl >= 0 && zl < tc.wcz && yl >= 0 && yl < tc.wcy;
+            const int wg = tc.w0 + c - 1;
+            const bool own_word = own_row && c >= 1 && c <= kTileW && 64 * wg < g.nx;
+            if (!own_word && cw == 0ull) continue;
+            const int zg = row_coord(zl, tc.z0, tc.wcz, g.nz, g.periodic);
+            const int yg = row_coord(yl, tc.y0, tc.wcy, g.ny, g.periodic);
+            const unsigned long long row_base = (unsigned long long)g.Wp * ((unsigned long long)yg + (unsigned long long)g.ny * (unsigned long long)zg);
+            // bits of this word that lie in the row itself (x < nx) and the one bit that may lie at x = nx or x = -1
+            unsigned long long in_row = 0ull, wrap = 0ull;
+            int x_wrap = 0;
+            if (c == 0) { wrap = cw >> 63; x_wrap = wg >= 0 ? 64 * wg + 63 : g.nx - 1; }
+            else if (64 * wg + 64 <= g.nx) in_row = cw;
+            else if (64 * wg <= g.nx) {
+                const int nvalid = g.nx - 64 * wg;                  // 0..63
+                in_row = cw & ~(~0ull << nvalid);
+                wrap = (cw >> nvalid) & 1ull;                       // periodic only: the cell at x = nx is x = 0
+                x_wrap = 0;
+            }
+            if (own_word) {                                         // carry g_t and add the hits
+                unsigned long long curw = S.nv[r][c];
+                if (64 * wg + 64 > g.nx) curw &= ~(~0ull << (g.nx - 64 * wg));
+                const unsigned long long val = curw | in_row;
+                if (in_row) {
+                    const unsigned long long old = atomicOr(Gn + row_base + wg, val);
+                    new_solid += __popcll(in_row & ~old);
+                } else if (val) {
+                    atomicOr(Gn + row_base + wg, val);
+                }
+            } else if (in_row) {                                    // hits in a neighbour tile's rows
+                const unsigned long long old = atomicOr(Gn + row_base + wg, in_row);
+                new_solid += __popcll(in_row & ~old);
+                const uint32_t nb = (uint32_t)(wg / kTileW) + (uint32_t)g.ntx * ((uint32_t)(yg >> 3) + (uint32_t)g.nty * (uint32_t)(zg >> 3));
+                if (atomicMax(&stamp[nb], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = nb;   // newly active tile
+            }
+            if (wrap) {                                             // one cell across the tile's x border
+                const unsigned long long bit = 1ull << (x_wrap & 63);
+                const unsigned long long old = atomicOr(Gn + row_base + (x_wrap >> 6), bit);
+                if (!(old & bit)) new_solid++;
+                const uint32_t nb = (uint32_t)((x_wrap >> 6) / kTileW) + (uint32_t)g.ntx * ((uint32_t)(yg >> 3) + (uint32_t)g.nty * (uint32_t)(zg >> 3));
+                if (nb != id && atomicMax(&stamp[nb], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = nb;
+            }
+        }
+        if (tid == 0 && n_front) {                                  // this tile still has front voxels
+            if (atomicMax(&stamp[id], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = id;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        new_solid += __shfl_xor_sync(0xffffffffu, new_solid, o);
+        n_items += __shfl_xor_sync(0xffffffffu, n_items, o);
+    }
+    if (lane == 0 && new_solid) atomicAdd(&ctl->claims, new_solid);
+    if (lane == 0 && n_items) atomicAdd(&ctl->items, n_items);
+}
+
+}  // namespace
+
+int grow_tile_words() { return kTileW; }
+
+cudaError_t launch_grow_tile(liets_ctx* c) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_grow_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const PhiloxKey key = philox_make_key(c->rng_seed);
+    k_grow_tile<<<c->tile_grid, kThreads, sizeof(Smem), c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->stamp,
+                                                                      c->list[0], c->list[1], key);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace liets

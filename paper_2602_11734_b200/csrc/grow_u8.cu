@@ -1,8 +1,8 @@
 // grow_u8.cu -- STORAGE_U8 growth step: uint8 grid + explicit list of front voxel indices.
 //
 // This is the list-indexed step of Algorithm 3 with one thread per front
-// voxel p: gather the 26 neighbours (line 5-6), draw lazily per Philox block for the void ones
-// (line 8; R9), claim with atomicOr on the 32-bit word holding the target byte (line 9; the thread
+// voxel p: gather the 26 neighbours (line 5-6), draw for the void ones (line 8; nibble-wise draw, R9),
+// claim with atomicOr on the 32-bit word holding the target byte (line 9; the thread
 // that flips 0 -> 1 owns q, so A_new holds q once -- the paper's "duplicates removed", :113),
 // and emit A_{t+1} = survivors(A_t) U A_new with one CTA-wide prefix sum per 256 voxels.
 // Retirement is lazy ("cells that no longer have any void neighbors are discarded"):
@@ -53,8 +53,10 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
     uint32_t* __restrict__ out = cur ? list0 : list1;
     uint32_t* out_count = &ctl->count[cur ^ 1u];
     const uint32_t t = ctl->step;
-    const uint32_t T0 = ctl->T[0], T1 = ctl->T[1], T2 = ctl->T[2];
-    const bool A0 = ctl->always[0], A1 = ctl->always[1], A2 = ctl->always[2];
+    __shared__ uint32_t s_hpat[8][4];
+    if (threadIdx.x < 32) s_hpat[threadIdx.x >> 2][threadIdx.x & 3] = ctl->hpat[threadIdx.x >> 2][threadIdx.x & 3];
+    const uint32_t en26 = ctl->en26;
+    __syncthreads();
     uint32_t my_claims = 0, my_items = 0;
 
     for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
@@ -73,29 +75,29 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
                 uint32_t q;
                 if (neighbour<PERIODIC>(d, p, x, y, z, dims, &q) && grid[q] == 0) mask |= 1u << d;
             }
-#pragma unroll
-            for (int b = 0; b < 7; ++b) {                  // one Philox block = 4 directions (R9)
-                const uint32_t bm = (b < 6 ? 0xFu : 0x3u) << (4 * b);
-                if (mask & bm) {
-                    ++my_items;
-                    const uint4 r = philox4x32_10(p, 0u, t, (uint32_t)b, key);
-                    const uint32_t w[4] = { r.x, r.y, r.z, r.w };
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const int d = 4 * b + k;
-                        if (d >= 26) break;
-                        if (!((mask >> d) & 1u)) continue;
-                        const int cls = dir_class(d);
-                        const uint32_t T = cls == 0 ? T0 : (cls == 1 ? T1 : T2);
-                        const bool always = cls == 0 ? A0 : (cls == 1 ? A1 : A2);
-                        if (always || w[k] < T) {          // line 8: rand_num < G_d
-                            uint32_t q;
-                            neighbour<PERIODIC>(d, p, x, y, z, dims, &q);
-                            const uint32_t sh = (q & 3u) * 8u;
-                            const uint32_t old = atomicOr(reinterpret_cast<uint32_t*>(grid) + (q >> 2), 1u << sh);
-                            if (((old >> sh) & 0xFFu) == 0) won |= 1u << d;   // line 9-10: owner of q
-                        }
+            if (mask & en26) {
+                // line 8 (rand_num < G_d) with the nibble-wise draw (R9): block 0 for all directions at once, the
+                // next blocks only for the directions that still tie with the threshold
+                ++my_items;
+                const uint4 B0 = philox4x32_10(p, 0u, t, 0u, key);
+                uint32_t le, eq;
+                level_compare(B0, s_hpat[0], mask & en26, &le, &eq);
+                uint32_t fire = le & ~eq;
+                if (eq) fire |= resolve_ties(p, t, eq, s_hpat, key, &my_items);
+                while (fire) {
+                    const uint32_t d = __ffs(fire) - 1u;
+                    fire &= fire - 1u;
+                    const uint32_t raw = d + (d >= 13u ? 1u : 0u);
+                    int X = x + (int)(raw % 3u) - 1, Y = y + (int)((raw / 3u) % 3u) - 1, Z = z + (int)(raw / 9u) - 1;
+                    if (PERIODIC) {
+                        X = X < 0 ? dims.nx - 1 : (X >= dims.nx ? 0 : X);
+                        Y = Y < 0 ? dims.ny - 1 : (Y >= dims.ny ? 0 : Y);
+                        Z = Z < 0 ? dims.nz - 1 : (Z >= dims.nz ? 0 : Z);
                     }
+                    const uint32_t q = (uint32_t)X + (uint32_t)dims.nx * ((uint32_t)Y + (uint32_t)dims.ny * (uint32_t)Z);
+                    const uint32_t sh = (q & 3u) * 8u;
+                    const uint32_t old = atomicOr(reinterpret_cast<uint32_t*>(grid) + (q >> 2), 1u << sh);
+                    if (((old >> sh) & 0xFFu) == 0) won |= 1u << d;       // line 9-10: owner of q
                 }
             }
         }

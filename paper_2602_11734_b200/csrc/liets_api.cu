@@ -17,19 +17,18 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t ctl, grid, list0, list1, status2, cand, total;
-    size_t g0, g1, stamp;          // STORAGE_BRICK (contiguous: G0 | G1 | stamp)
-    size_t n_bricks, list_cap;
-    int brick_grid;
+    size_t g0, g1, stamp;          // STORAGE_TILE (contiguous: G0 | G1 | stamp)
+    size_t n_tiles, grid_words, list_cap;
+    int Wp, ntx, nty, ntz;
 };
 
-constexpr int kBrickCtasPerSm = 4;
-constexpr int kMaxSms = 256;       // list slack is sized for the largest grid we would ever launch
+constexpr int kTileCtasPerSm = 4;
 
 bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
     if (nx < 1 || ny < 1 || nz < 1) return false;
     const unsigned long long N = (unsigned long long)nx * (unsigned long long)ny * (unsigned long long)nz;
     if (N >= (1ull << 32)) return false;
-    if (storage != LIETS_STORAGE_U8 && storage != LIETS_STORAGE_BRICK) return false;
+    if (storage != LIETS_STORAGE_U8 && storage != LIETS_STORAGE_TILE) return false;
     memset(L, 0, sizeof(*L));
     size_t off = 0;
     L->ctl = off;     off += align_up(sizeof(Control));
@@ -37,13 +36,16 @@ bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
         L->grid = off;    off += align_up((size_t)N + 4);
         L->list_cap = (size_t)N;
     } else {
-        const size_t bx = ((size_t)nx + 7) / 8, by = ((size_t)ny + 7) / 8, bz = ((size_t)nz + 7) / 8;
-        L->n_bricks = bx * by * bz;
-        L->g0 = off;      off += L->n_bricks * 64;
-        L->g1 = off;      off += L->n_bricks * 64;
-        L->stamp = off;   off += align_up(L->n_bricks * 4);
-        // every brick at most once per list, plus the unused tail of each warp's last chunk
-        L->list_cap = L->n_bricks + (size_t)kMaxSms * kBrickCtasPerSm * grow_brick_warps_per_cta() * grow_brick_chunk() + 64;
+        L->Wp = (nx + 63) / 64;
+        L->ntx = (L->Wp + grow_tile_words() - 1) / grow_tile_words();
+        L->nty = (ny + 7) / 8;
+        L->ntz = (nz + 7) / 8;
+        L->n_tiles = (size_t)L->ntx * L->nty * L->ntz;
+        L->grid_words = (size_t)L->Wp * ny * nz;
+        L->g0 = off;      off += L->grid_words * 8;
+        L->g1 = off;      off += L->grid_words * 8;
+        L->stamp = off;   off += align_up(L->n_tiles * 4);
+        L->list_cap = L->n_tiles;                           // the step stamp admits every tile at most once per list
     }
     L->list0 = off;   off += align_up(L->list_cap * 4);
     L->list1 = off;   off += align_up(L->list_cap * 4);
@@ -82,7 +84,7 @@ int launch_step_kernel(liets_ctx* c) {
             if (!c->prof_ev[2 * c->prof_n + k]) LIETS_CUDA_TRY(c, cudaEventCreate(&c->prof_ev[2 * c->prof_n + k]));
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream));
     }
-    LIETS_CUDA_TRY(c, c->storage == LIETS_STORAGE_U8 ? launch_grow_u8(c) : launch_grow_brick(c));
+    LIETS_CUDA_TRY(c, c->storage == LIETS_STORAGE_U8 ? launch_grow_u8(c) : launch_grow_tile(c));
     if (prof) {
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream));
         c->prof_n++;
@@ -141,15 +143,15 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
         c->explicit_idx = reinterpret_cast<uint64_t*>(base + L.cand);
         c->scratch_u8 = reinterpret_cast<uint8_t*>(base + L.cand);
         c->list_cap = L.list_cap;
-        if (storage == LIETS_STORAGE_BRICK) {
-            c->geom = BrickGeom{ nx, ny, nz, (nx + 7) / 8, (ny + 7) / 8, (nz + 7) / 8, boundary };
-            c->n_bricks = L.n_bricks;
+        if (storage == LIETS_STORAGE_TILE) {
+            c->geom = TileGeom{ nx, ny, nz, L.Wp, L.ntx, L.nty, L.ntz, boundary };
+            c->n_tiles = L.n_tiles;
+            c->grid_words = L.grid_words;
             c->G[0] = reinterpret_cast<unsigned long long*>(base + L.g0);
             c->G[1] = reinterpret_cast<unsigned long long*>(base + L.g1);
             c->stamp = reinterpret_cast<uint32_t*>(base + L.stamp);
             c->grid_u8 = nullptr;
-            const int sms = c->sm_count < kMaxSms ? c->sm_count : kMaxSms;
-            c->brick_grid = sms * kBrickCtasPerSm;
+            c->tile_grid = c->sm_count * kTileCtasPerSm;
         }
         ok = cudaMemsetAsync(c->ctl, 0, sizeof(Control), c->stream) == cudaSuccess &&
              launch_set_params(c) == cudaSuccess;
@@ -291,11 +293,11 @@ int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is
     const size_t nb = format == LIETS_FORMAT_U8 ? (size_t)c->N : (size_t)((c->N + 7) / 8);
     if (dst_bytes < nb) return fail(c, LIETS_E_CAPACITY, "dst buffer too small for the requested format");
     const uint8_t* u8 = c->grid_u8;
-    if (c->storage == LIETS_STORAGE_BRICK) {                // bricks -> linear uint8 (seeding scratch is idle)
+    if (c->storage == LIETS_STORAGE_TILE) {                 // bit rows -> linear uint8 (seeding scratch is idle)
         if (int rc = readback(c)) return rc;                // which grid copy is current
         c->host_step = c->pinned->step;
         uint8_t* lin = (format == LIETS_FORMAT_U8 && dst_is_device) ? static_cast<uint8_t*>(dst) : c->scratch_u8;
-        LIETS_CUDA_TRY(c, launch_unpack_bricks_u8(c, lin));
+        LIETS_CUDA_TRY(c, launch_unpack_rows_u8(c, lin));
         u8 = lin;
     }
     if (format == LIETS_FORMAT_U8) {

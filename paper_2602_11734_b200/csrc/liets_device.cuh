@@ -9,7 +9,11 @@ namespace liets {
 // ---------------------------------------------------------------------------------------------
 // Philox4x32-10 (Salmon et al., SC'11) -- the counter-based stream of DESIGN.md reading R9
 // ("an independent random number in (0,1) is drawn").
-//   growth:  key = (rng_seed lo, hi), counter = (p lo, p hi, step t, d>>2), draw of direction d = word d&3
+//   growth:  key = (rng_seed lo, hi); the 32-bit draw of (voxel p, step t, direction d) is written nibble by
+//            nibble, most significant first, from the voxel's eight blocks B_k = philox(p lo, p hi, t, k):
+//            nibble k of draw(d) = nibble d>>2 of word d&3 of B_k.  Block 0 alone decides, for all 26 directions
+//            at once, which draws can still fall below the threshold; block k+1 is evaluated only for the
+//            directions whose nibbles 0..k all tie with the threshold's
 //   seeding: counter = ((v>>2) lo, (v>>2) hi, 0, 0xFFFFFFFF), draw of voxel v = word v&3
 // ---------------------------------------------------------------------------------------------
 constexpr uint32_t kPhiloxM0 = 0xD2511F53u;
@@ -57,8 +61,13 @@ struct Control {
     unsigned long long n_t;          // target count ceil(phi_s N) (R7)
     unsigned long long R[3];         // reference thresholds floor(G_ref 2^32 + .5): face, edge, corner (R8)
     unsigned long long N;
-    uint32_t T[3];                   // thresholds of the current step (Eq. (1))
-    uint32_t always[3];              // T == 2^32: fire regardless of the draw
+    uint32_t U[3];                   // T - 1 of the current step's thresholds T in [1, 2^32] (Eq. (1)):
+                                     // a draw fires iff draw <= U
+    uint32_t en[3];                  // T >= 1; a class with T == 0 never fires
+    uint32_t hpat[8][4];             // [k][w]: nibble k (most significant first) of U of the class of each nibble's direction
+    uint32_t en26;                   // directions whose class can fire at all
+    uint32_t h0_any;                 // some class has a non-zero leading nibble: level 0 can fire without a tie
+    uint32_t tile_cursor;            // STORAGE_TILE: next list entry to hand out (dynamic tile scheduling)
     uint32_t law;
     uint32_t has_target;
     uint32_t step;                   // t, continues across step / generate calls
@@ -124,6 +133,66 @@ __host__ __device__ constexpr int dir_dy(int d) { return (dir_raw(d) / 3) % 3 - 
 __host__ __device__ constexpr int dir_dz(int d) { return dir_raw(d) / 9 - 1; }
 __host__ __device__ constexpr int dir_class(int d) {       // 0 face, 1 edge, 2 corner
     return (dir_dx(d) != 0) + (dir_dy(d) != 0) + (dir_dz(d) != 0) - 1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// The per-step thresholds in the form the two-level draw needs (all warp-uniform).
+//   U = T - 1, H = U >> 28 (top nibble), L = U & 0x0FFFFFFF.  draw <= U  <=>  nib < H, or nib == H and low28 <= L.
+// Direction d owns nibble d>>2 of word d&3.  A mask that holds one flag per nibble of word w at bit 3 of the
+// nibble, shifted right by 3 - w, has the flag of direction d at bit d: the four words interleave into a
+// mask in direction order without any bit permutation.
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ constexpr uint32_t class_nibble_ones(int w, int cls) {      // 0x1 in every nibble n of word w whose direction 4n+w is of class cls
+    uint32_t m = 0;
+    for (int n = 0; n < 7; ++n)
+        if (4 * n + w < 26 && dir_class(4 * n + w) == cls) m |= 1u << (4 * n);
+    return m;
+}
+__host__ __device__ constexpr uint32_t class_dir_mask(int cls) {                // bit d set iff direction d is of class cls
+    uint32_t m = 0;
+    for (int d = 0; d < 26; ++d)
+        if (dir_class(d) == cls) m |= 1u << d;
+    return m;
+}
+
+// Per-nibble compares of a Philox word a with a pattern word h, carry-free: the result has bit 3 of nibble n set
+// iff the relation holds for nibble n.
+__device__ __forceinline__ uint32_t nib_le(uint32_t a, uint32_t h) {            // a <= h
+    const uint32_t dd = (h | 0x88888888u) - (a & 0x77777777u);                  // bit 3: low 3 bits of h >= those of a
+    return ((h & ~a) | (~(h ^ a) & dd)) & 0x88888888u;
+}
+__device__ __forceinline__ uint32_t nib_eq(uint32_t a, uint32_t h) {            // a == h
+    const uint32_t z = a ^ h;
+    return ~(((z & 0x77777777u) + 0x77777777u) | z | 0x77777777u);
+}
+// four per-word masks (flag of nibble n at bit 4n+3) -> one mask in direction order (flag of direction d at bit d)
+__device__ __forceinline__ uint32_t interleave_dirs(uint32_t m0, uint32_t m1, uint32_t m2, uint32_t m3) {
+    return (m0 >> 3) | (m1 >> 2) | (m2 >> 1) | m3;
+}
+// For the directions in `mask`: le = nibble of block B <= the threshold's nibble, eq = they tie.
+__device__ __forceinline__ void level_compare(const uint4& B, const uint32_t* h, uint32_t mask, uint32_t* le, uint32_t* eq) {
+    const uint32_t l0 = nib_le(B.x, h[0]), l1 = nib_le(B.y, h[1]), l2 = nib_le(B.z, h[2]), l3 = nib_le(B.w, h[3]);
+    const uint32_t e0 = nib_eq(B.x, h[0]), e1 = nib_eq(B.y, h[1]), e2 = nib_eq(B.z, h[2]), e3 = nib_eq(B.w, h[3]);
+    *le = interleave_dirs(l0, l1, l2, l3) & mask;
+    *eq = interleave_dirs(e0, e1, e2, e3) & mask;
+}
+__device__ __forceinline__ uint32_t level_le(const uint4& B, const uint32_t* h, uint32_t mask) {
+    return interleave_dirs(nib_le(B.x, h[0]), nib_le(B.y, h[1]), nib_le(B.z, h[2]), nib_le(B.w, h[3])) & mask;
+}
+
+// Levels 1..7 for the directions of voxel p that tied at level 0: returns the directions that fire.
+__device__ __forceinline__ uint32_t resolve_ties(uint32_t p, uint32_t t, uint32_t tie, const uint32_t (*hpat)[4],
+                                                 const PhiloxKey& key, uint32_t* n_blocks) {
+    uint32_t fire = 0;
+    for (uint32_t k = 1; k < 8u && tie; ++k) {
+        const uint4 B = philox4x32_10(p, 0u, t, k, key);
+        uint32_t le, eq;
+        level_compare(B, hpat[k], tie, &le, &eq);
+        ++*n_blocks;
+        if (k < 7u) { fire |= le & ~eq; tie = eq; }
+        else fire |= le;                                                        // last nibble: draw <= U
+    }
+    return fire;
 }
 
 }  // namespace liets

@@ -12,7 +12,7 @@ struct HostReadback {                 // pinned; filled by cudaMemcpyAsync from 
 };
 
 namespace liets {
-struct BrickGeom { int nx, ny, nz, bx, by, bz, periodic; };   // b* = number of 8-voxel bricks per axis
+struct TileGeom { int nx, ny, nz, Wp, ntx, nty, ntz, periodic; };   // Wp = 64-bit words per x-row; nt* = tiles per axis
 }
 
 struct liets_ctx {
@@ -26,19 +26,20 @@ struct liets_ctx {
     // device pointers into ws
     liets::Control* ctl;
     uint8_t* grid_u8;                 // STORAGE_U8: N bytes (padded to 4)
-    uint32_t* list[2];                // front lists (voxel indices / brick ids), capacity N each
+    uint32_t* list[2];                // front lists (voxel indices / tile ids)
     uint32_t* status2;                // seeding: 2 bits per voxel (00 none/rejected, 01 pending, 11 accepted)
     uint64_t* explicit_idx;           // staging for liets_seed_explicit (aliases the candidate buffer)
     uint32_t* cand;                   // seeding: candidate voxel indices (capacity N)
-    // STORAGE_BRICK
-    liets::BrickGeom geom;
-    uint64_t n_bricks;
-    unsigned long long* G[2];         // double-buffered bit grid, 8 words per brick
-    uint32_t* stamp;                  // per brick: t+1 of the last step whose list holds it
+    // STORAGE_TILE
+    liets::TileGeom geom;
+    uint64_t n_tiles;
+    uint64_t grid_words;              // 64-bit words per grid copy: Wp * ny * nz
+    unsigned long long* G[2];         // double-buffered bit grid, x-rows of Wp words
+    uint32_t* stamp;                  // per tile: t+1 of the last step whose list holds it
     uint8_t* scratch_u8;              // N bytes for format conversion (aliases the candidate buffer)
     uint32_t host_step;               // step counter as of the last read-back (selects the current grid copy)
     int resolve_grid;                 // CTAs of the cooperative spacing kernel (0 = not sized yet)
-    int brick_grid;                   // CTAs of the brick growth kernel
+    int tile_grid;                    // CTAs of the tile growth kernel
     uint64_t list_cap;                // slots per front list
     // host state
     liets::Control* pinned;           // pinned host copy of the scalar part of Control
@@ -76,11 +77,9 @@ cudaError_t launch_begin(liets_ctx* c, int generate, uint32_t max_steps);
 cudaError_t launch_set_params(liets_ctx* c);
 // grow_u8.cu
 cudaError_t launch_grow_u8(liets_ctx* c);
-// grow_brick.cu
-cudaError_t launch_grow_brick(liets_ctx* c);
-size_t grow_brick_smem_bytes();
-int grow_brick_warps_per_cta();
-int grow_brick_chunk();
+// grow_tile.cu
+cudaError_t launch_grow_tile(liets_ctx* c);
+int grow_tile_words();
 // seed.cu
 cudaError_t launch_seed_reset(liets_ctx* c);
 cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all);
@@ -89,5 +88,5 @@ cudaError_t launch_seed_finalize(liets_ctx* c);
 cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n);
 // export.cu
 cudaError_t launch_pack_bits_u8(liets_ctx* c, const uint8_t* src_u8, uint8_t* dst_bits);
-cudaError_t launch_unpack_bricks_u8(liets_ctx* c, uint8_t* dst_u8);
+cudaError_t launch_unpack_rows_u8(liets_ctx* c, uint8_t* dst_u8);
 }  // namespace liets

@@ -305,38 +305,39 @@ __global__ void __launch_bounds__(256) k_seed_finalize_u8(Control* ctl, const ui
 
 __global__ void k_seed_close(Control* c) { c->n_solid = c->count[0]; c->cur = 0; }
 
-// STORAGE_BRICK: set the seed's bit in both grid copies; the brick enters the list of step 0 once
+// STORAGE_TILE: set the seed's bit in both grid copies; the tile enters the list of step 0 once
 // (stamp = 1).  The 0 -> 1 transition of the bit in G0 dedupes explicit seeds and counts them.
-__device__ __forceinline__ void place_seed_brick(Control* ctl, uint32_t v, BrickGeom g, unsigned long long* G0,
-                                                 unsigned long long* G1, uint32_t* stamp, uint32_t* front) {
+__device__ __forceinline__ void place_seed_tile(Control* ctl, uint32_t v, TileGeom g, int tile_w, unsigned long long* G0,
+                                                unsigned long long* G1, uint32_t* stamp, uint32_t* front) {
     const uint32_t x = v % (uint32_t)g.nx, rest = v / (uint32_t)g.nx;
     const uint32_t y = rest % (uint32_t)g.ny, z = rest / (uint32_t)g.ny;
-    const uint32_t b = (x >> 3) + (uint32_t)g.bx * ((y >> 3) + (uint32_t)g.by * (z >> 3));
-    const unsigned long long bit = 1ull << ((x & 7u) + 8u * (y & 7u));
-    const unsigned long long old = atomicOr(G0 + 8ull * b + (z & 7u), bit);
-    atomicOr(G1 + 8ull * b + (z & 7u), bit);
+    const unsigned long long w = (unsigned long long)(x >> 6) + (unsigned long long)g.Wp * ((unsigned long long)y + (unsigned long long)g.ny * z);
+    const unsigned long long bit = 1ull << (x & 63u);
+    const unsigned long long old = atomicOr(G0 + w, bit);
+    atomicOr(G1 + w, bit);
     if (!(old & bit)) atomicAdd(&ctl->n_solid, 1ull);
-    if (atomicMax(&stamp[b], 1u) < 1u) front[atomicAdd(&ctl->count[0], 1u)] = b;
+    const uint32_t tile = (x >> 6) / (uint32_t)tile_w + (uint32_t)g.ntx * ((y >> 3) + (uint32_t)g.nty * (z >> 3));
+    if (atomicMax(&stamp[tile], 1u) < 1u) front[atomicAdd(&ctl->count[0], 1u)] = tile;
 }
 
-__global__ void __launch_bounds__(256) k_seed_finalize_brick(Control* ctl, const uint32_t* status2, const uint32_t* cand,
-                                                              BrickGeom g, unsigned long long* G0, unsigned long long* G1,
-                                                              uint32_t* stamp, uint32_t* front) {
+__global__ void __launch_bounds__(256) k_seed_finalize_tile(Control* ctl, const uint32_t* status2, const uint32_t* cand,
+                                                             TileGeom g, int tile_w, unsigned long long* G0, unsigned long long* G1,
+                                                             uint32_t* stamp, uint32_t* front) {
     const uint32_t n = ctl->n_cand;
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
         const uint32_t v = cand[i];
-        if (((status2[v >> 4] >> (2 * (v & 15u))) & 3u) == 3u) place_seed_brick(ctl, v, g, G0, G1, stamp, front);
+        if (((status2[v >> 4] >> (2 * (v & 15u))) & 3u) == 3u) place_seed_tile(ctl, v, g, tile_w, G0, G1, stamp, front);
     }
 }
 
-__global__ void k_seed_explicit_brick(Control* ctl, const unsigned long long* idx, unsigned long long n, BrickGeom g,
-                                      unsigned long long* G0, unsigned long long* G1, uint32_t* stamp, uint32_t* front) {
+__global__ void k_seed_explicit_tile(Control* ctl, const unsigned long long* idx, unsigned long long n, TileGeom g, int tile_w,
+                                     unsigned long long* G0, unsigned long long* G1, uint32_t* stamp, uint32_t* front) {
     for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (unsigned long long)gridDim.x * blockDim.x)
-        place_seed_brick(ctl, (uint32_t)idx[i], g, G0, G1, stamp, front);
+        place_seed_tile(ctl, (uint32_t)idx[i], g, tile_w, G0, G1, stamp, front);
 }
 
-__global__ void k_seed_close_brick(Control* c) { c->cur = 0; }
+__global__ void k_seed_close_tile(Control* c) { c->cur = 0; }
 
 // --- explicit seeds: dedupe with the 0 -> 1 transition of the grid byte -------------------------
 __global__ void k_seed_explicit_u8(Control* ctl, const unsigned long long* idx, unsigned long long n,
@@ -357,7 +358,7 @@ cudaError_t launch_seed_reset(liets_ctx* c) {
     if (c->storage == 0) {
         e = cudaMemsetAsync(c->grid_u8, 0, (c->N + 3) & ~3ull, c->stream);
     } else {                                                // G[0], G[1] and the stamps are contiguous
-        e = cudaMemsetAsync(c->G[0], 0, c->n_bricks * (64 + 64 + 4), c->stream);
+        e = cudaMemsetAsync(c->G[0], 0, c->grid_words * 16 + c->n_tiles * 4, c->stream);
     }
     if (e != cudaSuccess) return e;
     k_seed_reset<<<1, 1, 0, c->stream>>>(c->ctl);
@@ -401,13 +402,13 @@ cudaError_t launch_seed_finalize(liets_ctx* c) {
     if (c->storage == 0)
         k_seed_finalize_u8<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->grid_u8, c->list[0]);
     else
-        k_seed_finalize_brick<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->geom, c->G[0], c->G[1],
-                                                                     c->stamp, c->list[0]);
+        k_seed_finalize_tile<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->geom, grow_tile_words(),
+                                                                    c->G[0], c->G[1], c->stamp, c->list[0]);
     c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (c->storage == 0) k_seed_close<<<1, 1, 0, c->stream>>>(c->ctl);
-    else k_seed_close_brick<<<1, 1, 0, c->stream>>>(c->ctl);
+    else k_seed_close_tile<<<1, 1, 0, c->stream>>>(c->ctl);
     c->launches++;
     return cudaGetLastError();
 }
@@ -418,14 +419,14 @@ cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n) {
             k_seed_explicit_u8<<<c->sm_count * 2, 256, 0, c->stream>>>(c->ctl, (const unsigned long long*)c->explicit_idx, n,
                                                                       c->grid_u8, c->list[0]);
         else
-            k_seed_explicit_brick<<<c->sm_count * 2, 256, 0, c->stream>>>(c->ctl, (const unsigned long long*)c->explicit_idx, n,
-                                                                         c->geom, c->G[0], c->G[1], c->stamp, c->list[0]);
+            k_seed_explicit_tile<<<c->sm_count * 2, 256, 0, c->stream>>>(c->ctl, (const unsigned long long*)c->explicit_idx, n,
+                                                                        c->geom, grow_tile_words(), c->G[0], c->G[1], c->stamp, c->list[0]);
         c->launches++;
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     if (c->storage == 0) k_seed_close<<<1, 1, 0, c->stream>>>(c->ctl);
-    else k_seed_close_brick<<<1, 1, 0, c->stream>>>(c->ctl);
+    else k_seed_close_tile<<<1, 1, 0, c->stream>>>(c->ctl);
     c->launches++;
     return cudaGetLastError();
 }

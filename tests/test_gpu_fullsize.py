@@ -42,7 +42,7 @@ def liets():
 @pytest.mark.parametrize("rec", records(), ids=ident)
 def test_fullsize_matches_oracle_hash(liets, rec):
     nx, ny, nz = rec["dims"]
-    storages = (1,) if nx * ny * nz > 2 * 10**8 else (1, 0)      # the uint8 layout of 1024^3 needs ~11 GB: brick only
+    storages = (1,) if nx * ny * nz > 2 * 10**8 else (1, 0)      # the uint8 layout of 1024^3 needs ~11 GB: tile storage only
     for storage in storages:
         L = liets.Liets(nx, ny, nz, int(rec["periodic"]), storage)
         L.set_growth(*rec["g"], liets.LAW_EQ1)

@@ -44,7 +44,7 @@ def test_workspace_bytes_host_logic(liets):
         a = L.liets_workspace_bytes(64, 64, 64, storage)
         b = L.liets_workspace_bytes(128, 128, 128, storage)
         assert 0 < a < b and a % 256 == 0
-    # brick storage keeps the grid at 2 x N/8 bytes: far below the uint8 layout's grid + two voxel lists
+    # tile storage keeps the grid at about 2 x N/8 bytes: far below the uint8 layout's grid + two voxel lists
     n = 400 ** 3
     assert L.liets_workspace_bytes(400, 400, 400, 0) > 9 * n
     assert L.liets_workspace_bytes(400, 400, 400, 1) < 5 * n
@@ -120,5 +120,6 @@ def test_algorithmic_bytes_model():
     assert b == [4 * 10 + 270 + 15 + 4 * 30, 4 * 30 + 810 + 35 + 4 * 30]
     b = bench.algorithmic_bytes(0, 100, [10], [25], 10)
     assert b == [40 + 100 + 15 + 40]
-    # STORAGE_BRICK: 4|B_t| + min(125|B_t|, N/8) + 64|B_t| + 4|B_{t+1}|
-    assert bench.algorithmic_bytes(1, 8000, [2, 3], [0, 0], 0)[0] == 8 + 250 + 128 + 12
+    # STORAGE_TILE: 4|L_t| + min(3225|L_t|, N/8) + 2048|L_t| + 4|L_{t+1}|
+    assert bench.algorithmic_bytes(1, 10**6, [2, 3], [0, 0], 0)[0] == 8 + 6450 + 4096 + 12
+    assert bench.algorithmic_bytes(1, 8000, [2, 3], [0, 0], 0)[0] == 8 + 1000 + 4096 + 12

@@ -36,15 +36,34 @@ def test_p1_philox_known_answers():
 
 
 def test_p1_draw_layout_matches_philox_block():
-    # R9: growth counter = (p lo, p hi, t, d//4), word d%4; seeding counter = (v//4, 0, 0, ~0), word v%4
+    # R9: hex digit k (most significant first) of the growth draw of direction d = hex digit d//4 (least significant
+    # first) of word d%4 of block (p lo, p hi, t, k); seeding counter = (v//4, 0, 0, ~0), word v%4
     seed = 0x0123456789ABCDEF
     key = (seed & 0xFFFFFFFF, seed >> 32)
-    for p, t, d in [(0, 0, 0), (12345, 7, 13), (2**32 - 1, 40, 25), (2**31 + 5, 3, 22)]:
-        blk = oracle.philox4x32_10([p & 0xFFFFFFFF, p >> 32, t, d // 4], key)
-        assert oracle.growth_draw(seed, t, p, d) == blk[d % 4]
+    for p, t, d in [(0, 0, 0), (12345, 7, 13), (2**32 - 1, 40, 25), (2**31 + 5, 3, 22), (77, 1, 8), (77, 1, 15)]:
+        digits = ""
+        for k in range(8):
+            blk = oracle.philox4x32_10([p & 0xFFFFFFFF, p >> 32, t, k], key)
+            digits += ("%08x" % blk[d % 4])[7 - d // 4]
+        assert "%08x" % oracle.growth_draw(seed, t, p, d) == digits
     for v in [0, 1, 2, 3, 4, 1000003, 2**32 - 1]:
         blk = oracle.philox4x32_10([(v // 4) & 0xFFFFFFFF, (v // 4) >> 32, 0, 0xFFFFFFFF], key)
         assert oracle.seed_draw(seed, v) == blk[v % 4]
+
+
+def test_p1_growth_draws_are_uniform_and_independent_across_directions():
+    # the 26 draws of one (seed, t, p) must behave as independent uniforms: chi-square of
+    # the top byte per direction, and no correlation between the draws of direction pairs
+    seed, n = 99, 6000
+    draws = np.array([[oracle.growth_draw(seed, t, p, d) for d in range(26)]
+                      for t, p in zip(np.arange(n) % 7, np.arange(n) * 977 + 5)], dtype=np.float64) / 2**32
+    assert np.all(np.abs(draws.mean(axis=0) - 0.5) < 5 * math.sqrt(1 / 12 / n))
+    for d in range(26):
+        hist = np.bincount((draws[:, d] * 16).astype(int), minlength=16)
+        chi2 = ((hist - n / 16) ** 2 / (n / 16)).sum()
+        assert chi2 < 50, (d, chi2)                                # 15 dof: P(chi2 > 50) ~ 1e-5
+    c = np.corrcoef(draws.T)
+    assert np.abs(c - np.eye(26)).max() < 5 / math.sqrt(n)
 
 
 def test_direction_table_is_the_26_neighbourhood():
