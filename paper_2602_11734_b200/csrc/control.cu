@@ -47,17 +47,23 @@ __global__ void k_control(Control* c, uint32_t flags) {
             c->en[k] = T >= 1ull;                                            // T in [0, 2^32]
             c->U[k] = T >= 1ull ? (uint32_t)(T - 1ull) : 0u;                 // draw < T  <=>  draw <= T - 1
         }
-        // the thresholds nibble by nibble, laid out like the draws (direction d: nibble d>>2 of word d&3)
+        // the thresholds nibble by nibble, laid out like the draws (direction d: nibble d>>2 of word d&3);
+        // built in registers: class masks are compile-time constants
         uint32_t en26 = 0, h0_any = 0;
-        for (int lv = 0; lv < 8; ++lv)
-            for (int w = 0; w < 4; ++w) c->hpat[lv][w] = 0;
-        for (int d = 0; d < 26; ++d) {
-            const int cls = dir_class(d);
-            if (c->en[cls]) en26 |= 1u << d;
-            for (int lv = 0; lv < 8; ++lv)
-                c->hpat[lv][d & 3] |= ((c->U[cls] >> (28 - 4 * lv)) & 15u) << (4 * (d >> 2));
-            if (c->en[cls] && (c->U[cls] >> 28)) h0_any = 1;
+        uint32_t U[3], en[3];
+        for (int k = 0; k < 3; ++k) { U[k] = c->U[k]; en[k] = c->en[k]; }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            if (en[k]) en26 |= class_dir_mask(k);
+            if (en[k] && (U[k] >> 28)) h0_any = 1;
         }
+#pragma unroll
+        for (int lv = 0; lv < 8; ++lv)
+#pragma unroll
+            for (int w = 0; w < 4; ++w)
+                c->hpat[lv][w] = ((U[0] >> (28 - 4 * lv)) & 15u) * class_nibble_ones(w, 0) +
+                                 ((U[1] >> (28 - 4 * lv)) & 15u) * class_nibble_ones(w, 1) +
+                                 ((U[2] >> (28 - 4 * lv)) & 15u) * class_nibble_ones(w, 2);
         c->en26 = en26;
         c->h0_any = h0_any;
         c->tile_cursor = 0;

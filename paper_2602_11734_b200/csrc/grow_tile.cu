@@ -4,8 +4,8 @@
 // words (bit i of word w of row (y, z) = voxel x = 64 w + i; bits with x >= nx stay 0).  Two copies
 // G[0], G[1] are kept: step t reads G[t&1] (immutable during the step, so the update is synchronous
 // by construction) and ORs into G[(t+1)&1].  The active set A is kept
-// at two levels: in HBM a list of active TILES of kTileW words x 8 x 8 rows (256 x 8 x 8 voxels)
-// that hold at least one front voxel, 4 bytes per 16384 voxels; and, per tile and step, the explicit
+// at two levels: in HBM a list of active TILES of kTileW words x 8 x 8 rows (128 x 8 x 8 voxels)
+// that hold at least one front voxel, 4 bytes per 8192 voxels; and, per tile and step, the explicit
 // list of its front VOXELS, rebuilt from the bits in shared memory.
 //
 // One CTA owns one tile at a time (tiles are handed out through an atomic cursor):
@@ -31,24 +31,24 @@ namespace liets {
 
 namespace {
 
-constexpr int kTileW = 4;                       // 64-bit words per tile row
-constexpr int kThreads = 256;
+constexpr int kTileW = 2;                       // 64-bit words per tile row
+constexpr int kThreads = 128;
 constexpr int kWarps = kThreads / 32;
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
 constexpr int kWin = (64 * kTileW + 1) / 30 + 1;   // 32-bit windows per row; window k starts at tile bit 30 k - 1
 constexpr int kQueueCap = 128;                  // voxels with ties per warp queue
-constexpr int kMaxFront = 64 * 64 * kTileW;     // every cell of the tile
+constexpr int kFrontCap = 32 * 64 * kTileW;     // front voxels listed at a time (half the tile; more -> several passes)
 
 struct Smem {
     unsigned long long nv[100][kRowWords];      // not-void bits, row (z'+1)*10 + (y'+1)
     uint32_t win[100][kWin];                    // the same rows as overlapping windows
     uint32_t claims[100][2 * kRowWords];        // cells claimed in this step, same geometry as nv (32-bit view)
-    uint32_t queue[kWarps][2 * kQueueCap];      // (voxel id, tied directions)
+    uint32_t queue[kWarps][2 * kQueueCap];      // (voxel id | nibble level << 14, tied directions)
     uint32_t hpat[8][4];
     uint32_t dir[28];                           // direction d: (row delta + 11) | (dx + 1) << 8
     uint32_t scan[33];
-    uint32_t tile, base, n_front;
-    uint16_t flist[kMaxFront];                  // x | (y | z << 3) << 8 of the tile's front voxels (x relative to the tile)
+    uint32_t tile, tile_id;
+    uint16_t flist[kFrontCap];                  // x | (y | z << 3) << 8 of the tile's front voxels (x relative to the tile)
 };
 
 struct TileCoord {
@@ -78,6 +78,17 @@ __device__ __forceinline__ unsigned long long not_void_word(const unsigned long 
     return v;
 }
 
+__device__ __forceinline__ TileCoord tile_coord(uint32_t id, const TileGeom& g) {
+    TileCoord tc;
+    const uint32_t tx = id % (uint32_t)g.ntx, rest = id / (uint32_t)g.ntx;
+    tc.w0 = (int)tx * kTileW;
+    tc.y0 = 8 * (int)(rest % (uint32_t)g.nty);
+    tc.z0 = 8 * (int)(rest / (uint32_t)g.nty);
+    tc.wcy = min(8, g.ny - tc.y0);
+    tc.wcz = min(8, g.nz - tc.z0);
+    return tc;
+}
+
 // local row coordinate i in [-1, 8] of a tile that starts at c0 and has wc valid rows -> global coordinate, or -1
 __device__ __forceinline__ int row_coord(int i, int c0, int wc, int n, int periodic) {
     if (i > wc) return -1;
@@ -87,7 +98,7 @@ __device__ __forceinline__ int row_coord(int i, int c0, int wc, int n, int perio
     return c;
 }
 
-__global__ void __launch_bounds__(kThreads, 4) k_grow_tile(Control* __restrict__ ctl, TileGeom g,
+__global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__ ctl, TileGeom g,
                                                            unsigned long long* G0, unsigned long long* G1,
                                                            uint32_t* stamp, uint32_t* list0, uint32_t* list1,
                                                            PhiloxKey key) {
@@ -113,26 +124,29 @@ __global__ void __launch_bounds__(kThreads, 4) k_grow_tile(Control* __restrict__
     }
     const uint32_t en26 = ctl->en26;
     const bool h0_any = ctl->h0_any != 0u;
+    const uint32_t h0[4] = { ctl->hpat[0][0], ctl->hpat[0][1], ctl->hpat[0][2], ctl->hpat[0][3] };
     uint32_t new_solid = 0;                 // per thread: bits this thread flipped 0 -> 1
     uint32_t n_items = 0;                   // per thread: Philox blocks evaluated
     uint32_t* const my_queue = S.queue[warp];
 
+    uint32_t next_li = 0, next_id = 0;      // thread 0: the list entry fetched ahead
+    if (tid == 0) {
+        next_li = atomicAdd(&ctl->tile_cursor, 1u);
+        if (next_li < n_list) next_id = in[next_li];
+    }
+    unsigned long long own_new = 0ull, own_old = 0ull;      // the own word's atomicOr of the previous tile, looked at late
     for (;;) {
         __syncthreads();                    // the previous tile's shared memory is no longer read
-        if (tid == 0) S.tile = atomicAdd(&ctl->tile_cursor, 1u);
+        if (tid == 0) { S.tile = next_li; S.tile_id = next_id; }
         __syncthreads();
         const uint32_t li = S.tile;
         if (li >= n_list) break;
-        const uint32_t id = in[li];
-        TileCoord tc;
-        {
-            const uint32_t tx = id % (uint32_t)g.ntx, rest = id / (uint32_t)g.ntx;
-            tc.w0 = (int)tx * kTileW;
-            tc.y0 = 8 * (int)(rest % (uint32_t)g.nty);
-            tc.z0 = 8 * (int)(rest / (uint32_t)g.nty);
-            tc.wcy = min(8, g.ny - tc.y0);
-            tc.wcz = min(8, g.nz - tc.z0);
+        const uint32_t id = S.tile_id;
+        if (tid == 0) {                     // latency hidden behind this tile's work
+            next_li = atomicAdd(&ctl->tile_cursor, 1u);
+            if (next_li < n_list) next_id = in[next_li];
         }
+        const TileCoord tc = tile_coord(id, g);
 
         // ---- A: gather ------------------------------------------------------------------------
         for (int task = (int)tid; task < 100 * kRowWords; task += kThreads) {
@@ -156,45 +170,29 @@ __global__ void __launch_bounds__(kThreads, 4) k_grow_tile(Control* __restrict__
         }
 
         // ---- B: front voxels of the tile ------------------------------------------------------------
-        uint32_t n_front = 0;
+        uint32_t n_front = 0, off0 = 0;
+        unsigned long long F = 0ull;        // this thread's word (row tid / kTileW, word tid % kTileW): its front voxels
+        const int f_row = (int)tid / kTileW, f_j = (int)tid - f_row * kTileW;
         {
-            unsigned long long F[(64 * kTileW + kThreads - 1) / kThreads];
-            uint32_t cnt = 0;
+            static_assert(64 * kTileW == kThreads, "one tile word per thread");
+            const int y = f_row & 7, z = f_row >> 3;
+            const int xbase = 64 * (tc.w0 + f_j);
+            if (y < tc.wcy && z < tc.wcz && xbase < g.nx) {
+                unsigned long long anyvoid = 0ull;
 #pragma unroll
-            for (int u = 0; u < (64 * kTileW + kThreads - 1) / kThreads; ++u) {
-                const int task = (int)tid + u * kThreads;
-                F[u] = 0ull;
-                if (task < 64 * kTileW) {
-                    const int row = task / kTileW, j = task - row * kTileW, y = row & 7, z = row >> 3;
-                    const int xbase = 64 * (tc.w0 + j);
-                    if (y < tc.wcy && z < tc.wcz && xbase < g.nx) {
-                        unsigned long long anyvoid = 0ull;
-#pragma unroll
-                        for (int k = 0; k < 9; ++k) {
-                            const int rr = (z + k / 3) * 10 + (y + k % 3);
-                            const unsigned long long v = ~S.nv[rr][1 + j];
-                            const unsigned long long l = ~S.nv[rr][j] >> 63, rgt = ~S.nv[rr][2 + j] << 63;
-                            anyvoid |= v | (v << 1) | l | (v >> 1) | rgt;
-                        }
-                        unsigned long long src = S.nv[(z + 1) * 10 + (y + 1)][1 + j];
-                        if (xbase + 64 > g.nx) src &= ~(~0ull << (g.nx - xbase));       // padding is not a source
-                        F[u] = src & anyvoid;                                           // R13
-                    }
-                    cnt += __popcll(F[u]);
+                for (int k = 0; k < 9; ++k) {
+                    const int rr = (z + k / 3) * 10 + (y + k % 3);
+                    const unsigned long long v = ~S.nv[rr][1 + f_j];
+                    const unsigned long long l = ~S.nv[rr][f_j] >> 63, rgt = ~S.nv[rr][2 + f_j] << 63;
+                    anyvoid |= v | (v << 1) | l | (v >> 1) | rgt;
                 }
+                unsigned long long src = S.nv[(z + 1) * 10 + (y + 1)][1 + f_j];
+                if (xbase + 64 > g.nx) src &= ~(~0ull << (g.nx - xbase));               // padding is not a source
+                F = src & anyvoid;                                                      // R13
             }
-            uint32_t off = block_exclusive_scan(cnt, S.scan, &n_front);
-#pragma unroll
-            for (int u = 0; u < (64 * kTileW + kThreads - 1) / kThreads; ++u) {
-                const int task = (int)tid + u * kThreads;
-                const int row = task / kTileW, j = task - row * kTileW;
-                const uint32_t hi = ((uint32_t)row << 8) | (uint32_t)(64 * j);
-                for (unsigned long long m = F[u]; m; m &= m - 1ull)
-                    S.flist[off++] = (uint16_t)(hi | (uint32_t)(__ffsll((long long)m) - 1));
-            }
+            off0 = block_exclusive_scan(__popcll(F), S.scan, &n_front);
         }
         const uint32_t p0 = (uint32_t)(64 * tc.w0) + (uint32_t)g.nx * ((uint32_t)tc.y0 + (uint32_t)g.ny * (uint32_t)tc.z0);
-        __syncthreads();                    // flist, win complete
 
         // ---- C + D -----------------------------------------------------------------------------------
         auto claim = [&](uint32_t fire, uint32_t x, uint32_t zy) {
@@ -207,21 +205,57 @@ __global__ void __launch_bounds__(kThreads, 4) k_grow_tile(Control* __restrict__
             }
         };
         uint32_t qn = 0;                    // queue fill (warp-uniform)
-        auto drain = [&]() {                // D: one lane per queued voxel
+        auto drain = [&]() {                // D: one lane per queued voxel, one nibble level per visit
             __syncwarp();
-            for (uint32_t j = lane; j < qn; j += 32u) {
-                const uint32_t v = my_queue[2 * j], tie = my_queue[2 * j + 1];
-                const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = v >> 11;
-                const uint32_t p = p0 + x + (uint32_t)g.nx * (y + (uint32_t)g.ny * z);
-                claim(resolve_ties(p, t, tie, S.hpat, key, &n_items), x, 10u * z + y);
+            uint32_t wpos = 0;              // entries that still tie are queued again, one level deeper
+            for (uint32_t j0 = 0; j0 < qn; j0 += 32u) {
+                const uint32_t j = j0 + lane;
+                uint32_t v = 0, tie = 0, still = 0;
+                if (j < qn) { v = my_queue[2 * j]; tie = my_queue[2 * j + 1]; }
+                __syncwarp();               // this round's entries are read before any slot is written again
+                if (tie) {
+                    const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = (v >> 11) & 7u, k = v >> 14;
+                    const uint32_t p = p0 + x + (uint32_t)g.nx * (y + (uint32_t)g.ny * z);
+                    const uint4 B = philox4x32_10(p, 0u, t, k, key);
+                    ++n_items;
+                    uint32_t le, eq;
+                    level_compare(B, S.hpat[k], tie, &le, &eq);
+                    const uint32_t fire = k < 7u ? (le & ~eq) : le;        // last nibble: draw <= U
+                    still = k < 7u ? eq : 0u;
+                    claim(fire, x, 10u * z + y);
+                }
+                const uint32_t have = __ballot_sync(0xffffffffu, still != 0u);
+                if (still) {
+                    const uint32_t slot = wpos + __popc(have & ((1u << lane) - 1u));
+                    my_queue[2 * slot] = v + (1u << 14);
+                    my_queue[2 * slot + 1] = still;
+                }
+                wpos += __popc(have);
             }
             __syncwarp();
-            qn = 0;
+            qn = wpos;
         };
-        for (uint32_t i0 = 0; i0 < n_front; i0 += kThreads) {      // C: one thread per front voxel
+        for (uint32_t pass0 = 0; pass0 < n_front; pass0 += (uint32_t)kFrontCap) {   // almost always a single pass
+            if (pass0) __syncthreads();     // the previous pass no longer reads the list
+            {                               // list the front voxels pass0 .. pass0 + kFrontCap - 1
+                uint32_t off = off0;
+                const uint32_t hi = ((uint32_t)f_row << 8) | (uint32_t)(64 * f_j);
+#pragma unroll
+                for (int half = 1; half >= 0; --half) {             // highest bit first: one FLO per voxel
+                    const uint32_t hh = hi | (uint32_t)(32 * half);
+                    for (uint32_t m = (uint32_t)(F >> (32 * half)); m; ++off) {
+                        const uint32_t b = 31u - __clz(m);
+                        m ^= 1u << b;
+                        if (off - pass0 < (uint32_t)kFrontCap) S.flist[off - pass0] = (uint16_t)(hh | b);
+                    }
+                }
+            }
+            __syncthreads();                // flist (and win) complete
+            const uint32_t n_pass = min((uint32_t)kFrontCap, n_front - pass0);
+        for (uint32_t i0 = 0; i0 < n_pass; i0 += kThreads) {       // C: one thread per front voxel
             const uint32_t i = i0 + tid;
             uint32_t tie = 0, v = 0;
-            if (i < n_front) {
+            if (i < n_pass) {
                 v = S.flist[i];
                 const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = v >> 11;
                 const uint32_t k = (x * 2185u) >> 16, s = x - 30u * k;     // window k holds tile bits 30k-1 .. 30k+30
@@ -237,40 +271,37 @@ __global__ void __launch_bounds__(kThreads, 4) k_grow_tile(Control* __restrict__
                     ++n_items;
                     if (h0_any) {           // some leading threshold nibble is non-zero: a draw can fire at level 0
                         uint32_t le;
-                        level_compare(B0, S.hpat[0], void26, &le, &tie);
+                        level_compare(B0, h0, void26, &le, &tie);
                         claim(le & ~tie, x, 10u * z + y);
-                    } else {                // all leading nibbles are 0: "<=" and "==" coincide
-                        tie = level_le(B0, S.hpat[0], void26);
+                    } else {                // all leading nibbles are 0: "<=" and "==" coincide with "== 0"
+                        tie = level_zero(B0, void26);
                     }
                 }
             }
             const uint32_t have = __ballot_sync(0xffffffffu, tie != 0u);
             if (have) {
-                if (qn + 32u > (uint32_t)kQueueCap) drain();
+                while (qn + 32u > (uint32_t)kQueueCap) drain();
                 if (tie) {
                     const uint32_t slot = qn + __popc(have & ((1u << lane) - 1u));
-                    my_queue[2 * slot] = v;
+                    my_queue[2 * slot] = v | (1u << 14);   // next nibble level: 1
                     my_queue[2 * slot + 1] = tie;
                 }
                 qn += __popc(have);
             }
         }
-        if (qn) drain();
+        }
+        while (qn) drain();
         __syncthreads();                    // all claims are in shared memory
 
         // ---- E: claim + compact ---------------------------------------------------------------------
-        for (int task = (int)tid; task < 100 * kRowWords; task += kThreads) {
-            const int r = task / kRowWords, c = task - r * kRowWords;
-            const unsigned long long cw = (unsigned long long)S.claims[r][2 * c] | ((unsigned long long)S.claims[r][2 * c + 1] << 32);
+        // word (r, c) of the claim volume -> global row, the bits that lie in the row itself (x < nx) and the one
+        // bit that may lie across the x border (x = -1, or x = nx on a periodic grid)
+        auto halo_word = [&](int r, int c, unsigned long long cw) {
             const int zl = r / 10 - 1, yl = r % 10 - 1;
-            const bool own_row = zl >= 0 && zl < tc.wcz && yl >= 0 && yl < tc.wcy;
             const int wg = tc.w0 + c - 1;
-            const bool own_word = own_row && c >= 1 && c <= kTileW && 64 * wg < g.nx;
-            if (!own_word && cw == 0ull) continue;
             const int zg = row_coord(zl, tc.z0, tc.wcz, g.nz, g.periodic);
             const int yg = row_coord(yl, tc.y0, tc.wcy, g.ny, g.periodic);
             const unsigned long long row_base = (unsigned long long)g.Wp * ((unsigned long long)yg + (unsigned long long)g.ny * (unsigned long long)zg);
-            // bits of this word that lie in the row itself (x < nx) and the one bit that may lie at x = nx or x = -1
             unsigned long long in_row = 0ull, wrap = 0ull;
             int x_wrap = 0;
             if (c == 0) { wrap = cw >> 63; x_wrap = wg >= 0 ? 64 * wg + 63 : g.nx - 1; }
@@ -279,23 +310,12 @@ __global__ void __launch_bounds__(kThreads, 4) k_grow_tile(Control* __restrict__
                 const int nvalid = g.nx - 64 * wg;                  // 0..63
                 in_row = cw & ~(~0ull << nvalid);
                 wrap = (cw >> nvalid) & 1ull;                       // periodic only: the cell at x = nx is x = 0
-                x_wrap = 0;
             }
-            if (own_word) {                                         // carry g_t and add the hits
-                unsigned long long curw = S.nv[r][c];
-                if (64 * wg + 64 > g.nx) curw &= ~(~0ull << (g.nx - 64 * wg));
-                const unsigned long long val = curw | in_row;
-                if (in_row) {
-                    const unsigned long long old = atomicOr(Gn + row_base + wg, val);
-                    new_solid += __popcll(in_row & ~old);
-                } else if (val) {
-                    atomicOr(Gn + row_base + wg, val);
-                }
-            } else if (in_row) {                                    // hits in a neighbour tile's rows
+            if (in_row) {                                           // hits in a neighbour tile's rows
                 const unsigned long long old = atomicOr(Gn + row_base + wg, in_row);
                 new_solid += __popcll(in_row & ~old);
                 const uint32_t nb = (uint32_t)(wg / kTileW) + (uint32_t)g.ntx * ((uint32_t)(yg >> 3) + (uint32_t)g.nty * (uint32_t)(zg >> 3));
-                if (atomicMax(&stamp[nb], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = nb;   // newly active tile
+                if (nb != id && atomicMax(&stamp[nb], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = nb;   // newly active tile
             }
             if (wrap) {                                             // one cell across the tile's x border
                 const unsigned long long bit = 1ull << (x_wrap & 63);
@@ -304,11 +324,41 @@ __global__ void __launch_bounds__(kThreads, 4) k_grow_tile(Control* __restrict__
                 const uint32_t nb = (uint32_t)((x_wrap >> 6) / kTileW) + (uint32_t)g.ntx * ((uint32_t)(yg >> 3) + (uint32_t)g.nty * (uint32_t)(zg >> 3));
                 if (nb != id && atomicMax(&stamp[nb], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = nb;
             }
+        };
+        // own words first, one per thread: carry g_t and add the hits; the old word is looked at after the halo pass
+        new_solid += __popcll(own_new & ~own_old);                  // the previous tile's own word
+        own_new = 0ull;
+        {
+            static_assert(64 * kTileW == kThreads, "one own word per thread");
+            const int row = (int)tid / kTileW, j = (int)tid - row * kTileW, y = row & 7, z = row >> 3;
+            const int wg = tc.w0 + j, r = (z + 1) * 10 + (y + 1);
+            if (y < tc.wcy && z < tc.wcz && 64 * wg < g.nx) {
+                const unsigned long long cw = (unsigned long long)S.claims[r][2 * (j + 1)] | ((unsigned long long)S.claims[r][2 * (j + 1) + 1] << 32);
+                unsigned long long curw = S.nv[r][j + 1], in_row = cw;
+                if (64 * wg + 64 > g.nx) {                          // the row ends inside this word
+                    const unsigned long long valid = ~(~0ull << (g.nx - 64 * wg));
+                    curw &= valid;
+                    in_row &= valid;
+                    if (cw & ~valid) halo_word(r, j + 1, cw & ~valid);       // the cell at x = nx (periodic wrap)
+                }
+                unsigned long long* dst = Gn + (unsigned long long)g.Wp * ((unsigned long long)(tc.y0 + y) + (unsigned long long)g.ny * (unsigned long long)(tc.z0 + z)) + wg;
+                if (in_row) { own_old = atomicOr(dst, curw | in_row); own_new = in_row; }
+                else if (curw) atomicOr(dst, curw);
+            }
+        }
+        for (int task = (int)tid; task < 100 * kRowWords; task += kThreads) {   // halo words: rarely non-zero
+            const int r = task / kRowWords, c = task - r * kRowWords;
+            const unsigned long long cw = (unsigned long long)S.claims[r][2 * c] | ((unsigned long long)S.claims[r][2 * c + 1] << 32);
+            if (cw == 0ull) continue;
+            const int zl = r / 10 - 1, yl = r % 10 - 1;
+            const bool own_word = zl >= 0 && zl < tc.wcz && yl >= 0 && yl < tc.wcy && c >= 1 && c <= kTileW && 64 * (tc.w0 + c - 1) < g.nx;
+            if (!own_word) halo_word(r, c, cw);
         }
         if (tid == 0 && n_front) {                                  // this tile still has front voxels
             if (atomicMax(&stamp[id], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = id;
         }
     }
+    new_solid += __popcll(own_new & ~own_old);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         new_solid += __shfl_xor_sync(0xffffffffu, new_solid, o);

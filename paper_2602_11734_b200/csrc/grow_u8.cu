@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
     uint32_t* __restrict__ out = cur ? list0 : list1;
     uint32_t* out_count = &ctl->count[cur ^ 1u];
     const uint32_t t = ctl->step;
-    __shared__ uint32_t s_hpat[8][4];
+    __shared__ __align__(16) uint32_t s_hpat[8][4];
     if (threadIdx.x < 32) s_hpat[threadIdx.x >> 2][threadIdx.x & 3] = ctl->hpat[threadIdx.x >> 2][threadIdx.x & 3];
     const uint32_t en26 = ctl->en26;
     __syncthreads();

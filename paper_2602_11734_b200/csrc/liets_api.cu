@@ -22,7 +22,7 @@ struct Layout {
     int Wp, ntx, nty, ntz;
 };
 
-constexpr int kTileCtasPerSm = 4;
+constexpr int kTileCtasPerSm = 8;
 
 bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
     if (nx < 1 || ny < 1 || nz < 1) return false;

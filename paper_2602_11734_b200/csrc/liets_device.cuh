@@ -180,6 +180,14 @@ __device__ __forceinline__ uint32_t level_le(const uint4& B, const uint32_t* h, 
     return interleave_dirs(nib_le(B.x, h[0]), nib_le(B.y, h[1]), nib_le(B.z, h[2]), nib_le(B.w, h[3])) & mask;
 }
 
+// all-zero thresholds nibbles (every class has probability < 1/16): "<=" is "== 0"; flag at bit 3 of zero nibbles
+__device__ __forceinline__ uint32_t nib_is_zero(uint32_t a) {
+    return ~(((a & 0x77777777u) + 0x77777777u) | a | 0x77777777u);
+}
+__device__ __forceinline__ uint32_t level_zero(const uint4& B, uint32_t mask) {
+    return interleave_dirs(nib_is_zero(B.x), nib_is_zero(B.y), nib_is_zero(B.z), nib_is_zero(B.w)) & mask;
+}
+
 // Levels 1..7 for the directions of voxel p that tied at level 0: returns the directions that fire.
 __device__ __forceinline__ uint32_t resolve_ties(uint32_t p, uint32_t t, uint32_t tie, const uint32_t (*hpat)[4],
                                                  const PhiloxKey& key, uint32_t* n_blocks) {

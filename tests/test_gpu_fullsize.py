@@ -81,3 +81,66 @@ def test_fullsize_properties_hold_at_any_size(liets):
     n_t = oracle.target_count(0.80, nx * ny * nz)
     assert solid_after[-1] == n_solid >= n_t and solid_after[-2] < n_t
     assert (blocks > 0).all()
+
+
+def test_config5_1024_periodic_sampled_transitions_and_properties(liets):
+    """BASELINE.json config 5 (1024^3, periodic, bit-packed, 2 x 128 MiB > L2) at full size.  A whole-run oracle hash
+    needs about ten CPU-hours (tests/golden/make_fullsize_hashes.py cfg5_1024; tested above once recorded), so here:
+    (a) seeding properties with the oracle's draw, torus L1 spacing; (b) ONE growth step checked cell by cell on
+    sampled voxels with the oracle's draw and threshold functions: a cell is solid after the step iff it was solid
+    before or some solid neighbour's keyed draw fell below the threshold (SURVEY 8(c) plain definition);
+    (c) stop rule and monotone solid count of the whole run."""
+    c = CONFIGS["cfg5_1024"]
+    nx, ny, nz = c["dims"]
+    N, seed = nx * ny * nz, c["seeds"][0]
+    L = liets.Liets(nx, ny, nz, 1, 1)
+    L.set_growth(*c["g"], liets.LAW_EQ1)
+    n_seeds = L.seed(c["core"], c["s"], seed)
+    seeds = np.flatnonzero(L.grid().ravel())
+    assert len(seeds) == n_seeds
+    Tc = oracle.prob_to_threshold(c["core"])
+    rng = np.random.default_rng(1)
+    for v in rng.choice(seeds, 200, replace=False):
+        assert oracle.seed_draw(seed, int(v)) < Tc
+    pts = np.stack([seeds % nx, (seeds // nx) % ny, seeds // (nx * ny)], axis=1).astype(np.int64)
+    dims = np.array([nx, ny, nz])
+    for i in rng.choice(len(pts), 100, replace=False):
+        d = np.abs(pts - pts[i])
+        d = np.minimum(d, dims - d).sum(axis=1)
+        d[i] = 10**6
+        assert d.min() >= c["s"]
+    # (b) one step in the middle of the run
+    n_t = oracle.target_count(0.80, N)
+    rc, steps0, n0 = L.generate(0.25)
+    L.set_target(0.80)
+    g0 = L.grid()
+    t = steps0                                                     # step counter continues from generate
+    n1, _ = L.step()
+    g1 = L.grid()
+    assert int(g1.sum(dtype=np.uint64)) == n1 and n1 > n0 and (g1 >= g0).all()
+    R = [oracle.prob_to_threshold(p) for p in c["g"]]
+    T = {k + 1: oracle.step_threshold(R[k], 1, n_t, n0) for k in range(3)}
+    dirs = [oracle.direction(d) for d in range(26)]
+    changed = np.flatnonzero((g1 != g0).ravel())
+    void_after = np.flatnonzero((g1 == 0).ravel())
+    sample = np.concatenate([rng.choice(changed, 1500, replace=False), rng.choice(void_after, 1500, replace=False),
+                             rng.integers(0, N, 1000)])
+    for q in sample:
+        q = int(q)
+        x, y, z = q % nx, (q // nx) % ny, q // (nx * ny)
+        expect = int(g0[z, y, x])
+        if not expect:
+            for d, (dx, dy, dz, cls) in enumerate(dirs):           # source p = q - e_d tries direction d
+                px, py, pz = (x - dx) % nx, (y - dy) % ny, (z - dz) % nz
+                if g0[pz, py, px] and oracle.growth_draw(seed, t, px + nx * (py + ny * pz), d) < T[cls]:
+                    expect = 1
+                    break
+        assert int(g1[z, y, x]) == expect, (q, expect)
+    del g0, g1
+    # (c) the rest of the run
+    rc, steps1, n_solid = L.generate(0.80)
+    front, solid_after, blocks = L.step_log()
+    assert rc == liets.OK and len(solid_after) == steps0 + 1 + steps1
+    assert (np.diff(solid_after.astype(np.int64)) > 0).all()
+    assert solid_after[-1] == n_solid >= n_t and solid_after[-2] < n_t
+    L.close()
