@@ -84,9 +84,9 @@ def algorithmic_bytes(storage, N, front, solid_after, n_seeds):
     """bytes the list-indexed step itself must move, per step.
 
     STORAGE_U8 (front = voxels):  4|A_t| + min(27|A_t|, N) + c_t + 4|A_{t+1}|
-    STORAGE_TILE (front = 256x8x8 tiles of 2 KiB): 4|L_t| + min(3225|L_t|, N/8) + 2048|L_t| + 4|L_{t+1}|
-      (read the tile list; each needed grid byte once -- a tile plus its one-voxel halo is 258x10x10
-      bits = 3225 B; write the tile's rows into the next buffer; write the next list)."""
+    STORAGE_TILE (front = 128x8x8 tiles of 1 KiB): 4|L_t| + min(1625|L_t|, N/8) + 1024|L_t| + 4|L_{t+1}|
+      (read the tile list; each needed grid byte once -- a tile plus its one-voxel halo is 130x10x10
+      bits = 1625 B; write the tile's rows into the next buffer; write the next list)."""
     out, prev = [], n_seeds
     for t in range(len(front)):
         a_t = int(front[t])
@@ -96,7 +96,7 @@ def algorithmic_bytes(storage, N, front, solid_after, n_seeds):
         if storage == 0:
             out.append(4 * a_t + min(27 * a_t, N) + c_t + 4 * a_n)
         else:
-            out.append(4 * a_t + min(3225 * a_t, N // 8) + 2048 * a_t + 4 * a_n)
+            out.append(4 * a_t + min(1625 * a_t, N // 8) + 1024 * a_t + 4 * a_n)
     return out
 
 
@@ -232,21 +232,28 @@ def run_ours(args):
     peaks, peaks_kind = load_peaks()
     grow_ms = float(np.sum(step_ms))
     n_blocks = float(np.sum(philox_blocks[:n_steps]))
+    n_fvox = float(np.sum(gen.front_voxels[:n_steps]))
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
-    # DESIGN.md "Roofline": the path is bound by integer issue, not by bytes.  Algorithmic work of a launch =
-    # Philox4x32-10 blocks the keyed draws need (one per (front voxel, block of 4 directions) with a void
-    # target) x 40 integer instructions (20 32x32->64 multiplies + 20 three-input XORs).  Peak = SMs x 4
-    # schedulers x 32 lanes x 1 instruction/clock x the maximum SM clock.
+    # DESIGN.md section 5: the path is bound by integer issue, not by bytes.  Algorithmic work of a launch =
+    #   40 integer instructions per Philox4x32-10 block the keyed draws need (20 32x32->64 multiplies + 20
+    #   three-input XORs), plus 2 per (front voxel, direction): the void test of the target and the compare of the
+    #   draw with the threshold (Algorithm 3 lines 6 and 8), 52 per front voxel that makes attempts.
+    # Peak = SMs x 4 schedulers x 32 lanes x 1 instruction/clock x the maximum SM clock.
     alu_peak = sm_count * 4 * 32 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
-    alu_achieved = n_blocks * PHILOX_INT_OPS / (grow_ms * 1e-3) / 1e12 if grow_ms > 0 else 0.0
+    alg_ops = n_blocks * PHILOX_INT_OPS + n_fvox * PER_FRONT_VOXEL_OPS
+    alu_achieved = alg_ops / (grow_ms * 1e-3) / 1e12 if grow_ms > 0 else 0.0
+    philox_only = n_blocks * PHILOX_INT_OPS / (grow_ms * 1e-3) / 1e12 if grow_ms > 0 else 0.0
     hbm_achieved = sum(b_alg) / (grow_ms * 1e-3) / 1e9 if grow_ms > 0 else 0.0
     roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Tiop/s (thread-level integer instructions)",
-                "frac": alu_achieved / alu_peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                "frac": alu_achieved / alu_peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH[storage],
                 "kernel": KERNEL_NAMES[storage],
                 "peak_kind": "derived: %d SMs x 4 schedulers x 32 lanes x %.0f MHz (sm_max_mhz, %s)" % (
                     sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peaks_kind),
                 "launches": int(n_steps), "philox_blocks_per_launch": n_blocks / max(n_steps, 1),
-                "int_ops_per_philox_block": PHILOX_INT_OPS, "avg_launch_ms": grow_ms / max(n_steps, 1),
+                "front_voxels_per_launch": n_fvox / max(n_steps, 1),
+                "int_ops_per_philox_block": PHILOX_INT_OPS, "int_ops_per_front_voxel": PER_FRONT_VOXEL_OPS,
+                "frac_philox_only": philox_only / alu_peak,
+                "avg_launch_ms": grow_ms / max(n_steps, 1),
                 "growth_kernel_share_of_generate": grow_ms / max(float(np.median(gen_ms)), 1e-9),
                 "hbm": {"bound": "hbm", "achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": hbm_achieved / peaks["hbm_gbs"],
@@ -301,10 +308,11 @@ def cpu_baseline():
 
 DEFAULT_STORAGE = 1
 PHILOX_INT_OPS = 40
+PER_FRONT_VOXEL_OPS = 52
 KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_tile"}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for the current kernel.
-TRAFFIC_BYTES_PER_LAUNCH = None
+TRAFFIC_BYTES_PER_LAUNCH = {0: None, 1: 18.03e6}     # profiles/r1_k_grow_tile_ncu.md (k_grow_tile, steps 18-20)
 
 
 def main():

@@ -103,11 +103,12 @@ int liets_grid(liets_ctx* ctx, void* dst, size_t dst_bytes, int format, int dst_
 
 /* Per-step counters of the steps done since the last seed (HOST arrays of capacity cap, may be
  * NULL): front size at the start of step i (list entries: voxels for STORAGE_U8, tiles for
- * STORAGE_TILE), solid count after it, and the number of Philox4x32-10 blocks the step evaluated
- * (one per front voxel with a void target, plus one per further nibble level of its tied directions).
+ * STORAGE_TILE), solid count after it, the number of Philox4x32-10 blocks the step evaluated
+ * (one per front voxel with a void target, plus one per further nibble level of its tied directions),
+ * and the number of front voxels with a void target (the sources of Algorithm 3 that made attempts).
  * Returns the number of steps recorded (<= 4096 kept). */
 int liets_step_log(liets_ctx* ctx, uint64_t* front_in, uint64_t* solid_after, uint64_t* philox_blocks,
-                   uint32_t cap);
+                   uint64_t* front_voxels, uint32_t cap);
 
 /* Device time in milliseconds of the last liets_seed and the last liets_generate (CUDA events on
  * the ctx stream). */

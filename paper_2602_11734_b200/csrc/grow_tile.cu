@@ -11,7 +11,7 @@
 // One CTA owns one tile at a time (tiles are handed out through an atomic cursor):
 //   A  gather: the 10 x 10 rows of the tile's one-voxel neighbourhood, kTileW + 2 words each, as "not void"
 //      bits (solid, outside the domain, or padding), plus a copy in overlapping 32-bit windows so that
-//      any three x-adjacent bits come from one word
+//      any three x-adjacent bits come from one word (at a shift of 1..29, done as a multiply)
 //   B  front voxels: solid cells with a void neighbour, 64 cells per bit operation;
 //      their ids are compacted into a shared-memory list (popc + CTA-wide prefix sum)
 //   C  one thread per front voxel: its 26 void-target bits (Algorithm 3 lines 5-6) from nine window
@@ -35,7 +35,7 @@ constexpr int kTileW = 2;                       // 64-bit words per tile row
 constexpr int kThreads = 128;
 constexpr int kWarps = kThreads / 32;
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
-constexpr int kWin = (64 * kTileW + 1) / 30 + 1;   // 32-bit windows per row; window k starts at tile bit 30 k - 1
+constexpr int kWin = (64 * kTileW - 1) / 29 + 1;   // 32-bit windows per row; window k starts at tile bit 29 k - 2
 constexpr int kQueueCap = 128;                  // voxels with ties per warp queue
 constexpr int kFrontCap = 32 * 64 * kTileW;     // front voxels listed at a time (half the tile; more -> several passes)
 
@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
     const bool h0_any = ctl->h0_any != 0u;
     const uint32_t h0[4] = { ctl->hpat[0][0], ctl->hpat[0][1], ctl->hpat[0][2], ctl->hpat[0][3] };
     uint32_t new_solid = 0;                 // per thread: bits this thread flipped 0 -> 1
-    uint32_t n_items = 0;                   // per thread: Philox blocks evaluated
+    uint32_t n_items = 0, n_items0 = 0;     // per thread: Philox blocks evaluated, front voxels with a void target
     uint32_t* const my_queue = S.queue[warp];
 
     uint32_t next_li = 0, next_id = 0;      // thread 0: the list entry fetched ahead
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         __syncthreads();
         for (int task = (int)tid; task < 100 * kWin; task += kThreads) {
             const int r = task / kWin, k = task - r * kWin;
-            const int pos = 63 + 30 * k;                            // bit of the row that holds tile x = 30 k - 1
+            const int pos = 62 + 29 * k;                            // bit of the row that holds tile x = 29 k - 2
             const int wd = pos >> 6, sh = pos & 63;
             unsigned long long v = S.nv[r][wd] >> sh;
             if (sh > 32 && wd + 1 < kRowWords) v |= S.nv[r][wd + 1] << (64 - sh);
@@ -258,17 +258,18 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
             if (i < n_pass) {
                 v = S.flist[i];
                 const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = v >> 11;
-                const uint32_t k = (x * 2185u) >> 16, s = x - 30u * k;     // window k holds tile bits 30k-1 .. 30k+30
+                const uint32_t k = (x * 2260u) >> 16;                       // x / 29: window k holds tile bits 29k-2 .. 29k+29
+                const uint32_t shr = 1u << (31u + 29u * k - x);            // umulhi(w, shr) = w >> (x - 29k + 1): a shift on the FMA pipe
                 uint32_t nb27 = 0;          // bit 9(dz+1) + 3(dy+1) + (dx+1): that neighbour is not void
 #pragma unroll
                 for (int e = 0; e < 9; ++e)
-                    nb27 |= ((S.win[(z + e / 3) * 10u + (y + e % 3)][k] >> s) & 7u) << (3 * e);
+                    nb27 |= (__umulhi(S.win[(z + e / 3) * 10u + (y + e % 3)][k], shr) & 7u) << (3 * e);
                 const uint32_t void27 = ~nb27;
                 const uint32_t void26 = ((void27 & 0x1FFFu) | ((void27 >> 14) << 13)) & en26;
                 if (void26) {
                     const uint32_t p = p0 + x + (uint32_t)g.nx * (y + (uint32_t)g.ny * z);
                     const uint4 B0 = philox4x32_10(p, 0u, t, 0u, key);
-                    ++n_items;
+                    ++n_items0;
                     if (h0_any) {           // some leading threshold nibble is non-zero: a draw can fire at level 0
                         uint32_t le;
                         level_compare(B0, h0, void26, &le, &tie);
@@ -363,9 +364,10 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
     for (int o = 16; o > 0; o >>= 1) {
         new_solid += __shfl_xor_sync(0xffffffffu, new_solid, o);
         n_items += __shfl_xor_sync(0xffffffffu, n_items, o);
+        n_items0 += __shfl_xor_sync(0xffffffffu, n_items0, o);
     }
     if (lane == 0 && new_solid) atomicAdd(&ctl->claims, new_solid);
-    if (lane == 0 && n_items) atomicAdd(&ctl->items, n_items);
+    if (lane == 0 && n_items0) { atomicAdd(&ctl->items, n_items + n_items0); atomicAdd(&ctl->items0, n_items0); }
 }
 
 }  // namespace

@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
     if (threadIdx.x < 32) s_hpat[threadIdx.x >> 2][threadIdx.x & 3] = ctl->hpat[threadIdx.x >> 2][threadIdx.x & 3];
     const uint32_t en26 = ctl->en26;
     __syncthreads();
-    uint32_t my_claims = 0, my_items = 0;
+    uint32_t my_claims = 0, my_items = 0, my_items0 = 0;
 
     for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
         const uint64_t i = base + threadIdx.x;
@@ -79,6 +79,7 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
                 // line 8 (rand_num < G_d) with the nibble-wise draw (R9): block 0 for all directions at once, the
                 // next blocks only for the directions that still tie with the threshold
                 ++my_items;
+                ++my_items0;
                 const uint4 B0 = philox4x32_10(p, 0u, t, 0u, key);
                 uint32_t le, eq;
                 level_compare(B0, s_hpat[0], mask & en26, &le, &eq);
@@ -132,6 +133,9 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) my_items += __shfl_xor_sync(0xffffffffu, my_items, o);
     if ((threadIdx.x & 31u) == 0 && my_items) atomicAdd(&ctl->items, my_items);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) my_items0 += __shfl_xor_sync(0xffffffffu, my_items0, o);
+    if ((threadIdx.x & 31u) == 0 && my_items0) atomicAdd(&ctl->items0, my_items0);
 }
 
 }  // namespace

@@ -316,7 +316,8 @@ int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is
     return LIETS_OK;
 }
 
-int liets_step_log(liets_ctx* c, uint64_t* front_in, uint64_t* solid_after, uint64_t* philox_blocks, uint32_t cap) {
+int liets_step_log(liets_ctx* c, uint64_t* front_in, uint64_t* solid_after, uint64_t* philox_blocks,
+                   uint64_t* front_voxels, uint32_t cap) {
     if (!c) return LIETS_E_ARG;
     if (int rc = readback(c)) return rc;
     uint32_t n = c->pinned->step;
@@ -328,6 +329,8 @@ int liets_step_log(liets_ctx* c, uint64_t* front_in, uint64_t* solid_after, uint
         LIETS_CUDA_TRY(c, cudaMemcpyAsync(solid_after, c->ctl->log_solid, n * 8ull, cudaMemcpyDeviceToHost, c->stream));
     if (n && philox_blocks)
         LIETS_CUDA_TRY(c, cudaMemcpyAsync(philox_blocks, c->ctl->log_items, n * 8ull, cudaMemcpyDeviceToHost, c->stream));
+    if (n && front_voxels)
+        LIETS_CUDA_TRY(c, cudaMemcpyAsync(front_voxels, c->ctl->log_items0, n * 8ull, cudaMemcpyDeviceToHost, c->stream));
     LIETS_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return (int)n;
 }

@@ -83,9 +83,11 @@ struct Control {
     uint32_t n_rescan;               // seeding: candidates whose adjacency was not stored
     uint32_t pend3[3];               // seeding: pending candidates after round r, at index r % 3
     uint32_t items;                  // Philox blocks evaluated by the live step (profiling counter)
+    uint32_t items0;                 // front voxels with a void target in the live step (= level-0 blocks)
     unsigned long long log_front[kLogCap];
     unsigned long long log_solid[kLogCap];
     unsigned long long log_items[kLogCap];
+    unsigned long long log_items0[kLogCap];
 };
 
 // control-kernel flags
@@ -201,6 +203,84 @@ __device__ __forceinline__ uint32_t resolve_ties(uint32_t p, uint32_t t, uint32_
         else fire |= le;                                                        // last nibble: draw <= U
     }
     return fire;
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// The step loop's control logic (control.cu explains the protocol).
+// ---------------------------------------------------------------------------------------------
+// T = min(2^32, floor(R * max(0, 20 n_t - 19 n_solid) / n_t)) without 128-bit arithmetic:
+// a = 20 n_t - 19 n_solid = q n_t + r  =>  floor(R a / n_t) = R q + floor(R r / n_t),
+// with q <= 20, R <= 2^32, r < n_t <= 2^32, so every product fits 64 bits.
+__device__ __forceinline__ unsigned long long eq1_threshold(unsigned long long R, unsigned long long n_t,
+                                            unsigned long long n_solid) {
+    unsigned long long a = 20ull * n_t, b = 19ull * n_solid;
+    if (b >= a) return 0ull;
+    a -= b;
+    unsigned long long q = a / n_t, r = a % n_t;
+    unsigned long long T = R * q + (R * r) / n_t;
+    return T > (1ull << 32) ? (1ull << 32) : T;
+}
+
+// One call by ONE thread between two growth kernels.  All inputs are read up front in one batch of L2 loads (fields that other CTAs update with
+// atomics must not come from L1), the logic runs on registers, the results are stored at the end.
+static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
+    unsigned long long n_solid = __ldcg(&c->n_solid);
+    const unsigned long long n_t = __ldcg(&c->n_t), N = __ldcg(&c->N);
+    const unsigned long long R[3] = { __ldcg(&c->R[0]), __ldcg(&c->R[1]), __ldcg(&c->R[2]) };
+    const uint32_t claims = __ldcg(&c->claims), items = __ldcg(&c->items), items0 = __ldcg(&c->items0);
+    const uint32_t count[2] = { __ldcg(&c->count[0]), __ldcg(&c->count[1]) };
+    const uint32_t law = __ldcg(&c->law), max_steps = __ldcg(&c->max_steps);
+    uint32_t step = __ldcg(&c->step), steps_done = __ldcg(&c->steps_done), cur = __ldcg(&c->cur);
+    uint32_t active = __ldcg(&c->active);
+    int32_t status = __ldcg(&c->status);
+    if ((flags & kCtlFinish) && active) {                // close the step that just ran
+        n_solid += claims;                               // phi_a update
+        c->n_solid = n_solid;
+        if (step < kLogCap) { c->log_solid[step] = n_solid; c->log_items[step] = items; c->log_items0[step] = items0; }
+        cur ^= 1u;                                       // A <- prune(A U A_new) (R4)
+        step += 1;
+        steps_done += 1;
+        active = 0;
+        c->cur = cur; c->step = step; c->steps_done = steps_done; c->active = 0; c->claims = 0;
+    }
+    if (!(flags & (kCtlPrepare | kCtlEval))) return;
+    if (!(flags & kCtlForce)) {                          // stop rule, between whole steps only
+        if (status != kStatusRunning) return;
+        if (n_solid >= n_t) status = 0;                                      // LIETS_OK
+        else if (count[cur] == 0 || n_solid == N) status = 1;                // FRONT_EMPTY
+        else if (steps_done >= max_steps) status = 2;                        // MAX_STEPS
+        if (status != kStatusRunning) { c->status = status; return; }
+    }
+    if (!(flags & kCtlPrepare)) return;
+    uint32_t U[3], en[3], en26 = 0, h0_any = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const unsigned long long T = law ? eq1_threshold(R[k], n_t, n_solid) : R[k];
+        en[k] = T >= 1ull;                                                   // T in [0, 2^32]
+        U[k] = T >= 1ull ? (uint32_t)(T - 1ull) : 0u;                        // draw < T  <=>  draw <= T - 1
+        c->en[k] = en[k];
+        c->U[k] = U[k];
+        if (en[k]) en26 |= class_dir_mask(k);
+        if (en[k] && (U[k] >> 28)) h0_any = 1;
+    }
+    // the thresholds nibble by nibble, laid out like the draws (direction d: nibble d>>2 of word d&3)
+#pragma unroll
+    for (int lv = 0; lv < 8; ++lv)
+#pragma unroll
+        for (int w = 0; w < 4; ++w)
+            c->hpat[lv][w] = ((U[0] >> (28 - 4 * lv)) & 15u) * class_nibble_ones(w, 0) +
+                             ((U[1] >> (28 - 4 * lv)) & 15u) * class_nibble_ones(w, 1) +
+                             ((U[2] >> (28 - 4 * lv)) & 15u) * class_nibble_ones(w, 2);
+    c->en26 = en26;
+    c->h0_any = h0_any;
+    c->tile_cursor = 0;
+    c->count[cur ^ 1u] = 0;
+    c->claims = 0;
+    c->items = 0;
+    c->items0 = 0;
+    if (step < kLogCap) c->log_front[step] = count[cur];
+    c->active = 1;
 }
 
 }  // namespace liets

@@ -213,7 +213,25 @@ __device__ __forceinline__ uint32_t try_resolve(uint32_t* status2, uint32_t v, c
     return 0u;
 }
 
-constexpr int kPolls = 24;      // looks per round before falling back to a grid-wide sync
+// the same look with the neighbour indices in registers (k <= 8): the status loads are independent, so one look
+// costs one L2 round trip instead of k
+__device__ __forceinline__ uint32_t try_resolve_reg(uint32_t* status2, uint32_t v, const uint32_t (&nbr)[8], uint32_t k) {
+    uint32_t w[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) w[e] = (uint32_t)e < k ? ld_cg(status2 + (nbr[e] >> 4)) : 0u;
+    bool accepted = false, pending = false;
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+        const uint32_t st = (uint32_t)e < k ? (w[e] >> (2 * (nbr[e] & 15u))) & 3u : 0u;
+        accepted = accepted || st == 3u;
+        pending = pending || st == 1u;
+    }
+    if (accepted) { atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u)))); return 1u; }     // 01 -> 00
+    if (!pending) { atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u))); return 1u; }         // 01 -> 11
+    return 0u;
+}
+
+constexpr int kPolls = 64;      // looks per round before falling back to a grid-wide sync
 
 // Pass 2: all rounds in one cooperative launch.  A pending candidate is rejected as soon as a
 // lower-index neighbour is accepted, accepted once none of them is pending, else it waits.  Every
@@ -236,11 +254,18 @@ __global__ void __launch_bounds__(1024) k_spacing_resolve(Control* ctl, uint32_t
         k0 = a.cnt[tid];
         if (k0 != kRescan) { v0 = cand[tid]; nb0 = a.pool + a.off[tid]; open0 = status_of(status2, v0) == 1u; }
     }
+    uint32_t nbr[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
+    const bool in_regs = k0 <= 8u;
+    if (open0 && in_regs) {
+#pragma unroll
+        for (int e = 0; e < 8; ++e)
+            if ((uint32_t)e < k0) nbr[e] = nb0[e];
+    }
     for (uint32_t round = 0;; ++round) {
         uint32_t still = 0;
         for (int poll = 0; poll < kPolls; ++poll) {
             if (!__any_sync(0xffffffffu, open0)) break;
-            if (open0 && try_resolve(status2, v0, nb0, k0)) open0 = false;
+            if (open0 && (in_regs ? try_resolve_reg(status2, v0, nbr, k0) : try_resolve(status2, v0, nb0, k0))) open0 = false;
         }
         if (open0) still++;
         if (a.ok) {

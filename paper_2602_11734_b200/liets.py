@@ -63,7 +63,7 @@ def lib():
     L.liets_generate.restype = ci
     L.liets_grid.argtypes = [vp, vp, sz, ci, ci]
     L.liets_grid.restype = ci
-    L.liets_step_log.argtypes = [vp, P(u64), P(u64), P(u64), u32]
+    L.liets_step_log.argtypes = [vp, P(u64), P(u64), P(u64), P(u64), u32]
     L.liets_step_log.restype = ci
     L.liets_timings.argtypes = [vp, P(ctypes.c_float), P(ctypes.c_float)]
     L.liets_timings.restype = ci
@@ -169,9 +169,11 @@ class Liets:
         f = np.zeros(cap, dtype=np.uint64)
         s = np.zeros(cap, dtype=np.uint64)
         b = np.zeros(cap, dtype=np.uint64)
+        v = np.zeros(cap, dtype=np.uint64)
         P64 = ctypes.POINTER(ctypes.c_uint64)
         n = self._check(self._L.liets_step_log(self._h, f.ctypes.data_as(P64), s.ctypes.data_as(P64),
-                                               b.ctypes.data_as(P64), cap))
+                                               b.ctypes.data_as(P64), v.ctypes.data_as(P64), cap))
+        self.front_voxels = v[:n].copy()      # front voxels with a void target per step
         return f[:n].copy(), s[:n].copy(), b[:n].copy()
 
     def timings(self):

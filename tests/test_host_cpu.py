@@ -120,6 +120,6 @@ def test_algorithmic_bytes_model():
     assert b == [4 * 10 + 270 + 15 + 4 * 30, 4 * 30 + 810 + 35 + 4 * 30]
     b = bench.algorithmic_bytes(0, 100, [10], [25], 10)
     assert b == [40 + 100 + 15 + 40]
-    # STORAGE_TILE: 4|L_t| + min(3225|L_t|, N/8) + 2048|L_t| + 4|L_{t+1}|
-    assert bench.algorithmic_bytes(1, 10**6, [2, 3], [0, 0], 0)[0] == 8 + 6450 + 4096 + 12
-    assert bench.algorithmic_bytes(1, 8000, [2, 3], [0, 0], 0)[0] == 8 + 1000 + 4096 + 12
+    # STORAGE_TILE: 4|L_t| + min(1625|L_t|, N/8) + 1024|L_t| + 4|L_{t+1}|
+    assert bench.algorithmic_bytes(1, 10**6, [2, 3], [0, 0], 0)[0] == 8 + 3250 + 2048 + 12
+    assert bench.algorithmic_bytes(1, 8000, [2, 3], [0, 0], 0)[0] == 8 + 1000 + 2048 + 12
