@@ -16,7 +16,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t ctl, grid, list0, list1, status2, cand, total;
+    size_t ctl, grid, list0, list1, status2, coff, rowoff, cand, total;
     size_t g0, g1, stamp;          // STORAGE_TILE (contiguous: G0 | G1 | stamp)
     size_t n_tiles, grid_words, list_cap;
     int Wp, ntx, nty, ntz;
@@ -50,6 +50,8 @@ bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
     L->list0 = off;   off += align_up(L->list_cap * 4);
     L->list1 = off;   off += align_up(L->list_cap * 4);
     L->status2 = off; off += align_up(((size_t)N + 15) / 16 * 4);
+    L->coff = off;    off += align_up((((size_t)N + 15) / 16 + 31) / 32 * 32 / 8 * 4 + 64);
+    L->rowoff = off;  off += align_up(((size_t)ny * nz + 2) * 4);
     L->cand = off;    off += align_up((size_t)N * 4 < 64 ? 64 : (size_t)N * 4);
     L->total = off;
     return true;
@@ -140,6 +142,8 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
         c->list[1] = reinterpret_cast<uint32_t*>(base + L.list1);
         c->status2 = reinterpret_cast<uint32_t*>(base + L.status2);
         c->cand = reinterpret_cast<uint32_t*>(base + L.cand);
+        c->coff = reinterpret_cast<uint32_t*>(base + L.coff);
+        c->rowoff = reinterpret_cast<uint32_t*>(base + L.rowoff);
         c->explicit_idx = reinterpret_cast<uint64_t*>(base + L.cand);
         c->scratch_u8 = reinterpret_cast<uint8_t*>(base + L.cand);
         c->list_cap = L.list_cap;
@@ -216,7 +220,7 @@ int liets_seed(liets_ctx* c, double core_prob, int spacing_s, uint64_t rng_seed,
     const int accept_all = spacing_s <= 1;
     LIETS_CUDA_TRY(c, launch_seed_candidates(c, prob_to_threshold(core_prob), accept_all));
     if (!accept_all) LIETS_CUDA_TRY(c, launch_spacing(c, spacing_s));
-    LIETS_CUDA_TRY(c, launch_seed_finalize(c));
+    LIETS_CUDA_TRY(c, launch_seed_finalize(c, !accept_all));
     LIETS_CUDA_TRY(c, cudaEventRecord(c->ev1, c->stream));
     if (int rc = readback(c)) return rc;
     LIETS_CUDA_TRY(c, cudaEventElapsedTime(&c->seed_ms, c->ev0, c->ev1));

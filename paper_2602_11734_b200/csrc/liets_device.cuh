@@ -82,12 +82,14 @@ struct Control {
     uint32_t pool_head;              // seeding: used entries of the adjacency pool
     uint32_t n_rescan;               // seeding: candidates whose adjacency was not stored
     uint32_t pend3[3];               // seeding: pending candidates after round r, at index r % 3
+    uint32_t spacing_slow;           // seeding: the adjacency lists do not fit the fast resolve -> rescan rounds
     uint32_t items;                  // Philox blocks evaluated by the live step (profiling counter)
     uint32_t items0;                 // front voxels with a void target in the live step (= level-0 blocks)
     unsigned long long log_front[kLogCap];
     unsigned long long log_solid[kLogCap];
     unsigned long long log_items[kLogCap];
     unsigned long long log_items0[kLogCap];
+    uint32_t scan_sums[1024];        // seeding: per-CTA sums of the chunk-count prefix scan
 };
 
 // control-kernel flags

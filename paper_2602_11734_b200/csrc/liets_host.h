@@ -29,7 +29,9 @@ struct liets_ctx {
     uint32_t* list[2];                // front lists (voxel indices / tile ids)
     uint32_t* status2;                // seeding: 2 bits per voxel (00 none/rejected, 01 pending, 11 accepted)
     uint64_t* explicit_idx;           // staging for liets_seed_explicit (aliases the candidate buffer)
-    uint32_t* cand;                   // seeding: candidate voxel indices (capacity N)
+    uint32_t* cand;                   // seeding: candidate voxel indices in ascending order (capacity N) + adjacency
+    uint32_t* coff;                   // seeding: candidates before each chunk of 128 voxels
+    uint32_t* rowoff;                 // seeding: candidates before each x-row
     // STORAGE_TILE
     liets::TileGeom geom;
     uint64_t n_tiles;
@@ -84,7 +86,7 @@ int grow_tile_words();
 cudaError_t launch_seed_reset(liets_ctx* c);
 cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all);
 cudaError_t launch_spacing(liets_ctx* c, int s);
-cudaError_t launch_seed_finalize(liets_ctx* c);
+cudaError_t launch_seed_finalize(liets_ctx* c, int spaced);
 cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n);
 // export.cu
 cudaError_t launch_pack_bits_u8(liets_ctx* c, const uint8_t* src_u8, uint8_t* dst_bits);

@@ -28,20 +28,26 @@ __device__ __forceinline__ uint32_t ld_cg(const uint32_t* p) {
 __global__ void k_seed_reset(Control* c) {
     c->n_solid = 0; c->step = 0; c->steps_done = 0; c->active = 0; c->status = 0; c->cur = 0;
     c->count[0] = 0; c->count[1] = 0; c->claims = 0; c->n_cand = 0;
-    c->pool_head = 0; c->n_rescan = 0; c->pend3[0] = 0; c->pend3[1] = 0; c->pend3[2] = 0;
+    c->pool_head = 0; c->n_rescan = 0; c->pend3[0] = 0; c->pend3[1] = 0; c->pend3[2] = 0; c->spacing_slow = 0;
 }
 
 // --- candidates: one thread per status word = 16 voxels = 4 Philox blocks -----------------------
-__global__ void __launch_bounds__(256) k_seed_candidates(Control* ctl, uint32_t* status2, uint32_t* cand,
+// Also counts the candidates of every CHUNK of 8 status words (128 voxels): the prefix sum of these counts
+// (k_seed_scan) gives every candidate its rank in ascending index order without sorting.
+constexpr int kChunkWords = 8;
+
+__device__ __forceinline__ uint32_t candidate_fields(uint32_t status_word) {      // bit 2k: voxel k of the word is a candidate
+    return (status_word | (status_word >> 1)) & 0x55555555u;
+}
+
+__global__ void __launch_bounds__(256) k_seed_candidates(uint32_t* status2, uint32_t* ccount,
                                                           unsigned long long N, uint32_t T_core,
                                                           uint32_t always, uint32_t accept_all,
                                                           PhiloxKey key) {
-    __shared__ uint32_t s_scan[33];
-    __shared__ uint32_t s_base;
     const unsigned long long n_words = (N + 15ull) / 16ull;
-    for (unsigned long long base = (unsigned long long)blockIdx.x * blockDim.x; base < n_words;
-         base += (unsigned long long)gridDim.x * blockDim.x) {
-        const unsigned long long w = base + threadIdx.x;
+    const unsigned long long n_padded = (n_words + 31ull) / 32ull * 32ull;      // whole warps: the chunk shuffles need every lane
+    for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < n_padded;
+         w += (unsigned long long)gridDim.x * blockDim.x) {
         uint32_t bits = 0;                                  // bit k: voxel 16w+k is a candidate
         if (w < n_words) {
 #pragma unroll
@@ -61,19 +67,81 @@ __global__ void __launch_bounds__(256) k_seed_candidates(Control* ctl, uint32_t*
             }
             status2[w] = word;
         }
-        uint32_t total;
-        uint32_t off = block_exclusive_scan(__popc(bits), s_scan, &total);
-        if (threadIdx.x == 0) s_base = total ? atomicAdd(&ctl->n_cand, total) : 0u;
-        __syncthreads();
-        off += s_base;
-        for (uint32_t m = bits; m; m &= m - 1) cand[off++] = (uint32_t)(16ull * w + (__ffs(m) - 1));
+        uint32_t cnt = __popc(bits);                        // the 8 lanes of a chunk add up their counts
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, 1);
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, 2);
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, 4);
+        if ((threadIdx.x & (kChunkWords - 1)) == 0) ccount[w / kChunkWords] = cnt;
     }
+}
+
+// chunk counts -> exclusive prefix sums (in place), total -> ctl->n_cand.  One cooperative launch: per-CTA sums,
+// grid-wide sync, then every CTA scans its own contiguous segment tile by tile.
+__global__ void __launch_bounds__(1024) k_seed_scan(Control* ctl, uint32_t* ccount, uint32_t* block_sums,
+                                                     unsigned long long n_chunks) {
+    cg::grid_group grid = cg::this_grid();
+    __shared__ uint32_t s_scan[33];
+    const unsigned long long per_cta = (n_chunks + gridDim.x - 1) / gridDim.x;
+    const unsigned long long lo = min(n_chunks, per_cta * blockIdx.x), hi = min(n_chunks, lo + per_cta);
+    uint32_t sum = 0;
+    for (unsigned long long i = lo + threadIdx.x; i < hi; i += blockDim.x) sum += ccount[i];
+    uint32_t total;
+    block_exclusive_scan(sum, s_scan, &total);
+    if (threadIdx.x == 0) block_sums[blockIdx.x] = total;
+    grid.sync();
+    uint32_t before = 0, all = 0;                           // candidates in lower CTAs' segments / in all
+    for (uint32_t b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
+        const uint32_t v = ld_cg(block_sums + b);
+        all += v;
+        if (b < blockIdx.x) before += v;
+    }
+    uint32_t t0, t1;
+    block_exclusive_scan(before, s_scan, &t0);
+    block_exclusive_scan(all, s_scan, &t1);
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->n_cand = t1;
+    uint32_t base = t0;
+    for (unsigned long long i0 = lo; i0 < hi; i0 += blockDim.x) {
+        const unsigned long long i = i0 + threadIdx.x;
+        const uint32_t v = i < hi ? ccount[i] : 0u;
+        const uint32_t excl = block_exclusive_scan(v, s_scan, &total);
+        if (i < hi) ccount[i] = base + excl;
+        base += total;
+    }
+}
+
+// the candidates in ascending index order: cand[rank] = voxel index
+__global__ void __launch_bounds__(256) k_seed_list(const uint32_t* __restrict__ status2, const uint32_t* __restrict__ coff,
+                                                    uint32_t* __restrict__ cand, unsigned long long N) {
+    const unsigned long long n_words = (N + 15ull) / 16ull;
+    const unsigned long long n_padded = (n_words + 31ull) / 32ull * 32ull;      // whole warps: the chunk shuffles need every lane
+    for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < n_padded;
+         w += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t f = w < n_words ? candidate_fields(status2[w]) : 0u;
+        const uint32_t cnt = __popc(f);
+        uint32_t incl = cnt;                                // prefix over the 8 lanes of the chunk
+#pragma unroll
+        for (int o = 1; o < kChunkWords; o <<= 1) {
+            const uint32_t up = __shfl_up_sync(0xffffffffu, incl, o, kChunkWords);
+            if ((threadIdx.x & (kChunkWords - 1)) >= (uint32_t)o) incl += up;
+        }
+        if (cnt) {
+            uint32_t r = coff[w / kChunkWords] + incl - cnt;
+            for (uint32_t m = f; m; m &= m - 1) cand[r++] = (uint32_t)(16ull * w) + (uint32_t)((__ffs(m) - 1) >> 1);
+        }
+    }
+}
+
+// rank (in ascending index order) of candidate voxel w
+__device__ __forceinline__ uint32_t rank_of(const uint32_t* status2, const uint32_t* coff, uint32_t w) {
+    const uint32_t word = w >> 4, first = word & ~(uint32_t)(kChunkWords - 1);
+    uint32_t r = ld_cg(coff + (word / kChunkWords));
+    for (uint32_t k = first; k < word; ++k) r += __popc(candidate_fields(ld_cg(status2 + k)));
+    return r + __popc(candidate_fields(ld_cg(status2 + word)) & ((1u << (2 * (w & 15u))) - 1u));
 }
 
 // --- seed spacing -------------------------------------------------------------------------------
 struct Dims { int nx, ny, nz, periodic; };
 
-constexpr uint32_t kRescan = 0xFFFFFFFFu;       // adjacency of this candidate not stored: rescan its diamond
 constexpr int kAdjBuf = 96;                     // neighbours a warp can buffer per candidate
 
 // Warp-cooperative walk over the status words of the LOWER-index voxels within L1 < s of voxel v
@@ -139,22 +207,42 @@ __device__ __forceinline__ void scan_diamond(const uint32_t* status2, uint32_t v
     }
 }
 
-// layout of the candidate buffer (capacity N words): cand[n] | off[n] | cnt[n] | rescan[n] | pool[N-4n]
+// layout of the candidate buffer (capacity N words):
+//   cand[n] | off[n] | cnt[n] | st_rank[n] | first8[8][n] | pool[N-12n]
+// first8[e][i] = rank of the e-th listed neighbour of candidate i (struct of arrays: a warp's loads are coalesced);
+// pool holds every list in full (lists longer than 8 continue there)
 struct AdjView {
     bool ok;
-    uint32_t *off, *cnt, *rescan, *pool;
+    uint32_t *off, *cnt, *st_rank, *first8, *pool;
     unsigned long long pool_cap;
 };
 __device__ __forceinline__ AdjView adj_view(uint32_t* cand, uint32_t n, unsigned long long N) {
     AdjView a;
-    a.ok = 4ull * n <= N;
-    a.off = cand + n; a.cnt = cand + 2ull * n; a.rescan = cand + 3ull * n; a.pool = cand + 4ull * n;
-    a.pool_cap = a.ok ? N - 4ull * n : 0ull;
+    a.ok = 12ull * n <= N;
+    a.off = cand + n; a.cnt = cand + 2ull * n; a.st_rank = cand + 3ull * n; a.first8 = cand + 4ull * n; a.pool = cand + 12ull * n;
+    a.pool_cap = a.ok ? N - 12ull * n : 0ull;
     return a;
 }
 
-// Pass 1: one warp per candidate lists the lower-index candidates inside its diamond, once.
-__global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const uint32_t* status2, uint32_t* cand,
+// Ranks of the statuses kept in shared memory by k_spacing_resolve_cta: a ring of kRing candidates.  A candidate only
+// looks at candidates at most (candidates in s-1 slices) ranks below it; k_spacing_adjacency checks that this fits.
+constexpr uint32_t kRing = 1u << 19;
+
+// rowoff[rho] = number of candidates below row rho = y + ny z (rowoff[ny nz] = all): the candidates of any run of
+// consecutive rows are a run of consecutive ranks
+__global__ void __launch_bounds__(256) k_seed_rows(const Control* ctl, const uint32_t* status2, const uint32_t* coff,
+                                                    uint32_t* rowoff, Dims g) {
+    const unsigned long long n_rows = (unsigned long long)g.ny * g.nz;
+    for (unsigned long long rho = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; rho <= n_rows;
+         rho += (unsigned long long)gridDim.x * blockDim.x)
+        rowoff[rho] = rho < n_rows ? rank_of(status2, coff, (uint32_t)(rho * g.nx)) : ctl->n_cand;
+}
+
+// Pass 1: one warp per candidate (rank i, ascending index order) lists the RANKS of the lower-index candidates
+// within L1 < s, once: one lane per z-slice of the diamond, which walks the candidates of the slice's rows
+// (consecutive ranks) and keeps those in range.  Sets ctl->spacing_slow if a list does not fit or a neighbour is
+// too far back in rank for the ring of k_spacing_resolve_cta.
+__global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const uint32_t* __restrict__ rowoff, uint32_t* cand,
                                                             Dims g, int s, unsigned long long N) {
     __shared__ uint32_t s_buf[8][kAdjBuf];
     __shared__ uint32_t s_cnt[8];
@@ -163,18 +251,58 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
     const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
     const uint32_t n = ctl->n_cand;
     const AdjView a = adj_view(cand, n, N);
-    if (!a.ok) return;
+    if (!a.ok) { if (threadIdx.x == 0 && blockIdx.x == 0) ctl->spacing_slow = 1u; return; }
+    const int r = s - 1;                                    // diamond radius: L1 <= s-1  <=>  L1 < s
+    // slices to visit: dz = -r..0 between walls (lower index = lower z, or same z and lower row), all slices within r
+    // on the torus (each once)
+    const int n_slices = g.periodic ? min(2 * r + 1, g.nz) : r + 1;
     for (uint32_t i = warp_global; i < n; i += n_warps) {
         const uint32_t v = cand[i];
+        const int x = (int)(v % (uint32_t)g.nx);
+        const uint32_t rest = v / (uint32_t)g.nx;
+        const int y = (int)(rest % (uint32_t)g.ny), z = (int)(rest / (uint32_t)g.ny);
         if (lane == 0) s_cnt[warp] = 0;
         __syncwarp();
-        auto collect = [&](uint32_t word, unsigned long long lo) {
-            for (uint32_t m = word & 0x55555555u; m; m &= m - 1) {          // every candidate in the word
-                const uint32_t slot = atomicAdd(&s_cnt[warp], 1u);
-                if (slot < (uint32_t)kAdjBuf) s_buf[warp][slot] = (uint32_t)lo + ((__ffs(m) - 1) >> 1);
+        for (int t = (int)lane; t < n_slices; t += 32) {
+            int Z = z - r + t, dz;
+            if (g.periodic) {
+                if (n_slices == g.nz) Z = t;                // the diamond covers every slice
+                Z %= g.nz; if (Z < 0) Z += g.nz;
+                dz = abs(Z - z); dz = min(dz, g.nz - dz);
+            } else {
+                if (Z < 0) continue;
+                dz = z - Z;
             }
-        };
-        scan_diamond(status2, v, g, s, lane, collect);
+            const int rho = r - dz;                         // rows y - rho .. y + rho of slice Z can hold neighbours
+            if (rho < 0) continue;
+            int ya = y - rho, yb = y + rho;
+            int run_lo[2], run_hi[2], n_runs = 1;           // row runs [lo, hi] inside the slice
+            if (!g.periodic) {
+                run_lo[0] = max(ya, 0); run_hi[0] = min(yb, g.ny - 1);
+                if (Z == z) run_hi[0] = min(run_hi[0], y);  // same slice: only rows up to the candidate's own
+            } else if (2 * rho + 1 >= g.ny) {
+                run_lo[0] = 0; run_hi[0] = g.ny - 1;
+            } else {
+                ya = (ya % g.ny + g.ny) % g.ny; yb = (yb % g.ny + g.ny) % g.ny;
+                if (ya <= yb) { run_lo[0] = ya; run_hi[0] = yb; }
+                else { run_lo[0] = 0; run_hi[0] = yb; run_lo[1] = ya; run_hi[1] = g.ny - 1; n_runs = 2; }
+            }
+            for (int q = 0; q < n_runs; ++q) {
+                const uint32_t row0 = (uint32_t)Z * (uint32_t)g.ny;
+                const uint32_t r0 = rowoff[row0 + run_lo[q]], r1 = min(rowoff[row0 + run_hi[q] + 1], i);   // ranks below i only
+                for (uint32_t k = r0; k < r1; ++k) {
+                    const uint32_t w = cand[k];
+                    const int wx = (int)(w % (uint32_t)g.nx);
+                    const int wy = (int)((w / (uint32_t)g.nx) % (uint32_t)g.ny);
+                    int dx = abs(wx - x), dy = abs(wy - y);
+                    if (g.periodic) { dx = min(dx, g.nx - dx); dy = min(dy, g.ny - dy); }
+                    if (dx + dy + dz <= r) {
+                        const uint32_t slot = atomicAdd(&s_cnt[warp], 1u);
+                        if (slot < (uint32_t)kAdjBuf) s_buf[warp][slot] = k;
+                    }
+                }
+            }
+        }
         __syncwarp();
         const uint32_t k = s_cnt[warp];
         uint32_t base = 0;
@@ -185,11 +313,17 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
             stored = (unsigned long long)base + k <= a.pool_cap;
         }
         if (stored) {
-            for (uint32_t e = lane; e < k; e += 32) a.pool[base + e] = s_buf[warp][e];
+            bool far = false;
+            for (uint32_t e = lane; e < k; e += 32) {
+                const uint32_t rk = s_buf[warp][e];
+                a.pool[base + e] = rk;
+                if (e < 8u) a.first8[(unsigned long long)e * n + i] = rk;
+                far = far || i - rk >= kRing;
+            }
+            if (far) ctl->spacing_slow = 1u;
             if (lane == 0) { a.off[i] = base; a.cnt[i] = k; }
         } else if (lane == 0) {
-            a.cnt[i] = kRescan;
-            a.rescan[atomicAdd(&ctl->n_rescan, 1u)] = i;
+            ctl->spacing_slow = 1u;
         }
         __syncwarp();
     }
@@ -199,86 +333,82 @@ __device__ __forceinline__ uint32_t status_of(const uint32_t* status2, uint32_t 
     return (ld_cg(status2 + (v >> 4)) >> (2 * (v & 15u))) & 3u;
 }
 
-// one look at the stored lower-index neighbours of pending candidate v:
-// 0 = still waiting, 1 = resolved now (v's status word updated)
-__device__ __forceinline__ uint32_t try_resolve(uint32_t* status2, uint32_t v, const uint32_t* nb, uint32_t k) {
-    bool accepted = false, pending = false;
-    for (uint32_t e = 0; e < k; ++e) {
-        const uint32_t st = status_of(status2, nb[e]);
-        accepted = accepted || st == 3u;
-        pending = pending || st == 1u;
+// Pass 2: ONE CTA resolves all candidates in ascending rank, 1024 at a time, with the statuses (2 bits: 01 pending,
+// 11 accepted, 00 rejected) in shared memory, so a link of a dependency chain costs a shared-memory round trip
+// instead of an L2 one (the chains are long: ~140 links at 400^3, they sweep the whole grid in index order).
+// A pending candidate is rejected as soon as a lower-rank neighbour is accepted, accepted once none of them is
+// pending, else it waits; neighbours of lower passes are already final.  The adjacency of the next passes is loaded
+// while the current one is resolved.  The final statuses go to st_rank (2 bits per candidate, by rank) for finalize.
+__global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, uint32_t* cand, unsigned long long N) {
+    extern __shared__ uint32_t s_st[];                      // kRing / 16 words
+    if (ctl->spacing_slow) return;
+    const uint32_t n = ctl->n_cand;
+    const AdjView a = adj_view(cand, n, N);
+    uint32_t* const st_rank = a.st_rank;                    // n / 16 words of the n-word region
+    const uint32_t tid = threadIdx.x;
+    constexpr uint32_t kMask = kRing / 16u - 1u;
+    // the next pass's lists (count, offset, first 8 ranks: coalesced) are loaded while this pass is resolved
+    uint32_t kB = 0, offB = 0, nbrB[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
+    auto load = [&](uint32_t i) {
+        kB = 0; offB = 0;
+        if (i < n) {
+            kB = a.cnt[i]; offB = a.off[i];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) nbrB[e] = a.first8[(unsigned long long)e * n + i];
+        }
+    };
+    load(tid);
+    for (uint32_t i0 = 0; i0 < n; i0 += 1024u) {
+        const uint32_t i = i0 + tid;
+        const uint32_t k = kB, off = offB;
+        uint32_t widx[8], wsh[8];                           // ring word and bit position of each neighbour's status
+#pragma unroll
+        for (int e = 0; e < 8; ++e) { widx[e] = (nbrB[e] >> 4) & kMask; wsh[e] = 2u * (nbrB[e] & 15u); }
+        // this pass's slots of the ring: all pending (64 words = 1024 candidates)
+        if (tid < 64u) s_st[((i0 >> 4) + tid) & kMask] = 0x55555555u;
+        load(i + 1024u);                                    // in flight while this pass is resolved
+        __syncthreads();
+        bool open = i < n;
+        for (;;) {
+            if (open) {
+                uint32_t w[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) w[e] = s_st[widx[e]];          // independent loads (unused slots: any valid word)
+                bool accepted = false, pending = false;
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const uint32_t st = (uint32_t)e < k ? (w[e] >> wsh[e]) & 3u : 0u;
+                    accepted = accepted || st == 3u;
+                    pending = pending || st == 1u;
+                }
+                for (uint32_t e = 8; e < k; ++e) {          // long lists: the rest from the pool
+                    const uint32_t r = a.pool[off + e];
+                    const uint32_t st = (s_st[(r >> 4) & kMask] >> (2u * (r & 15u))) & 3u;
+                    accepted = accepted || st == 3u;
+                    pending = pending || st == 1u;
+                }
+                uint32_t* mine = &s_st[(i >> 4) & kMask];
+                if (accepted) { atomicAnd(mine, ~(1u << (2u * (i & 15u)))); open = false; }              // 01 -> 00
+                else if (!pending) { atomicOr(mine, 2u << (2u * (i & 15u))); open = false; }             // 01 -> 11
+            }
+            if (__syncthreads_and(!open)) break;                // (no global atomic in this loop: the barrier would wait for it)
+        }
+        if (tid < 64u) st_rank[(i0 >> 4) + tid] = s_st[((i0 >> 4) + tid) & kMask];     // final statuses by rank
     }
-    if (accepted) { atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u)))); return 1u; }     // 01 -> 00
-    if (!pending) { atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u))); return 1u; }         // 01 -> 11
-    return 0u;
 }
 
-// the same look with the neighbour indices in registers (k <= 8): the status loads are independent, so one look
-// costs one L2 round trip instead of k
-__device__ __forceinline__ uint32_t try_resolve_reg(uint32_t* status2, uint32_t v, const uint32_t (&nbr)[8], uint32_t k) {
-    uint32_t w[8];
-#pragma unroll
-    for (int e = 0; e < 8; ++e) w[e] = (uint32_t)e < k ? ld_cg(status2 + (nbr[e] >> 4)) : 0u;
-    bool accepted = false, pending = false;
-#pragma unroll
-    for (int e = 0; e < 8; ++e) {
-        const uint32_t st = (uint32_t)e < k ? (w[e] >> (2 * (nbr[e] & 15u))) & 3u : 0u;
-        accepted = accepted || st == 3u;
-        pending = pending || st == 1u;
-    }
-    if (accepted) { atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u)))); return 1u; }     // 01 -> 00
-    if (!pending) { atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u))); return 1u; }         // 01 -> 11
-    return 0u;
-}
-
-constexpr int kPolls = 64;      // looks per round before falling back to a grid-wide sync
-
-// Pass 2: all rounds in one cooperative launch.  A pending candidate is rejected as soon as a
-// lower-index neighbour is accepted, accepted once none of them is pending, else it waits.  Every
-// thread keeps its first candidate in registers and polls its neighbours' status words (L2) a
-// bounded number of times per round, so a dependency chain of length L needs about L / kPolls
-// grid-wide syncs instead of L.
+// Slow path (lists that do not fit, extreme densities): every pending candidate rescans its diamond in the global
+// status map each round; all rounds in one cooperative launch.  Does nothing unless ctl->spacing_slow is set.
 __global__ void __launch_bounds__(1024) k_spacing_resolve(Control* ctl, uint32_t* status2, uint32_t* cand,
                                                            Dims g, int s, unsigned long long N) {
     cg::grid_group grid = cg::this_grid();
+    if (!ctl->spacing_slow) return;
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, n_threads = gridDim.x * blockDim.x;
     const uint32_t n = ctl->n_cand;
-    const AdjView a = adj_view(cand, n, N);
-    const uint32_t n_rescan = a.ok ? ld_cg(&ctl->n_rescan) : n;
-    // this thread's own candidate (i = tid), cached
-    uint32_t v0 = 0, k0 = 0;
-    const uint32_t* nb0 = nullptr;
-    bool open0 = false;
-    if (a.ok && tid < n) {
-        k0 = a.cnt[tid];
-        if (k0 != kRescan) { v0 = cand[tid]; nb0 = a.pool + a.off[tid]; open0 = status_of(status2, v0) == 1u; }
-    }
-    uint32_t nbr[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
-    const bool in_regs = k0 <= 8u;
-    if (open0 && in_regs) {
-#pragma unroll
-        for (int e = 0; e < 8; ++e)
-            if ((uint32_t)e < k0) nbr[e] = nb0[e];
-    }
     for (uint32_t round = 0;; ++round) {
         uint32_t still = 0;
-        for (int poll = 0; poll < kPolls; ++poll) {
-            if (!__any_sync(0xffffffffu, open0)) break;
-            if (open0 && (in_regs ? try_resolve_reg(status2, v0, nbr, k0) : try_resolve(status2, v0, nb0, k0))) open0 = false;
-        }
-        if (open0) still++;
-        if (a.ok) {
-            for (uint32_t i = tid + n_threads; i < n; i += n_threads) {     // more candidates than threads
-                const uint32_t k = a.cnt[i];
-                if (k == kRescan) continue;
-                const uint32_t v = cand[i];
-                if (status_of(status2, v) != 1u) continue;
-                if (!try_resolve(status2, v, a.pool + a.off[i], k)) still++;
-            }
-        }
-        for (uint32_t q = tid >> 5; q < n_rescan; q += n_threads >> 5) { // one warp per candidate: rescan
-            const uint32_t i = a.ok ? a.rescan[q] : q;
+        for (uint32_t i = tid >> 5; i < n; i += n_threads >> 5) {      // one warp per candidate
             const uint32_t v = cand[i];
             if (status_of(status2, v) != 1u) continue;
             bool accepted = false, pending = false;
@@ -296,8 +426,6 @@ __global__ void __launch_bounds__(1024) k_spacing_resolve(Control* ctl, uint32_t
                 else still++;
             }
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) still += __shfl_xor_sync(0xffffffffu, still, o);
         if (lane == 0 && still) atomicAdd(&ctl->pend3[round % 3u], still);
         grid.sync();
         const uint32_t left = ld_cg(&ctl->pend3[round % 3u]);
@@ -307,9 +435,19 @@ __global__ void __launch_bounds__(1024) k_spacing_resolve(Control* ctl, uint32_t
 }
 
 // --- finalize: accepted candidates -> grid + initial front A_0 = seeds (R3) ---------------------
+// accepted = status 11: by rank in the spacing fast path's st_rank, else by voxel in the global status map
+__device__ __forceinline__ bool seed_accepted(const Control* ctl, const uint32_t* status2, const uint32_t* cand,
+                                              uint32_t n, unsigned long long N, uint32_t spaced, uint32_t i, uint32_t v) {
+    if (spaced && !ctl->spacing_slow) {
+        const uint32_t* st_rank = cand + 3ull * n;          // AdjView::st_rank
+        return ((st_rank[i >> 4] >> (2u * (i & 15u))) & 3u) == 3u;
+    }
+    return ((status2[v >> 4] >> (2u * (v & 15u))) & 3u) == 3u;
+}
+
 __global__ void __launch_bounds__(256) k_seed_finalize_u8(Control* ctl, const uint32_t* status2,
                                                            const uint32_t* cand, uint8_t* grid,
-                                                           uint32_t* front) {
+                                                           uint32_t* front, unsigned long long N, uint32_t spaced) {
     __shared__ uint32_t s_scan[33];
     __shared__ uint32_t s_base;
     const uint32_t n = ctl->n_cand;
@@ -318,7 +456,7 @@ __global__ void __launch_bounds__(256) k_seed_finalize_u8(Control* ctl, const ui
         uint32_t v = 0, acc = 0;
         if (i < n) {
             v = cand[i];
-            acc = ((status2[v >> 4] >> (2 * (v & 15u))) & 3u) == 3u;
+            acc = seed_accepted(ctl, status2, cand, n, N, spaced, (uint32_t)i, v);
         }
         uint32_t total;
         uint32_t off = block_exclusive_scan(acc, s_scan, &total);
@@ -347,11 +485,11 @@ __device__ __forceinline__ void place_seed_tile(Control* ctl, uint32_t v, TileGe
 
 __global__ void __launch_bounds__(256) k_seed_finalize_tile(Control* ctl, const uint32_t* status2, const uint32_t* cand,
                                                              TileGeom g, int tile_w, unsigned long long* G0, unsigned long long* G1,
-                                                             uint32_t* stamp, uint32_t* front) {
+                                                             uint32_t* stamp, uint32_t* front, unsigned long long N, uint32_t spaced) {
     const uint32_t n = ctl->n_cand;
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
         const uint32_t v = cand[i];
-        if (((status2[v >> 4] >> (2 * (v & 15u))) & 3u) == 3u) place_seed_tile(ctl, v, g, tile_w, G0, G1, stamp, front);
+        if (seed_accepted(ctl, status2, cand, n, N, spaced, (uint32_t)i, v)) place_seed_tile(ctl, v, g, tile_w, G0, G1, stamp, front);
     }
 }
 
@@ -395,20 +533,47 @@ cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all
     const PhiloxKey key = philox_make_key(c->rng_seed);
     const uint32_t always = t_core >= (1ull << 32);
     const uint32_t T = always ? 0xFFFFFFFFu : (uint32_t)t_core;
-    k_seed_candidates<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->N, T, always,
-                                                              (uint32_t)accept_all, key);
+    k_seed_candidates<<<c->sm_count * 8, 256, 0, c->stream>>>(c->status2, c->coff, c->N, T, always, (uint32_t)accept_all, key);
+    c->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    // ranks: prefix sums of the chunk counts, then the candidate list in ascending index order
+    Control* ctl = c->ctl;
+    uint32_t* coff = c->coff;
+    uint32_t* sums = c->ctl->scan_sums;
+    unsigned long long n_chunks = (((c->N + 15ull) / 16ull + 31ull) / 32ull * 32ull) / (unsigned long long)kChunkWords;
+    void* args[] = { &ctl, &coff, &sums, &n_chunks };
+    const int scan_grid = c->sm_count < 1024 ? c->sm_count : 1024;
+    e = cudaLaunchCooperativeKernel((const void*)k_seed_scan, dim3(scan_grid), dim3(1024), args, 0, c->stream);
+    c->launches++;
+    if (e != cudaSuccess) return e;
+    k_seed_list<<<c->sm_count * 8, 256, 0, c->stream>>>(c->status2, c->coff, c->cand, c->N);
     c->launches++;
     return cudaGetLastError();
 }
 
-// exact parallel reproduction of the ascending-index greedy (R12): adjacency once, then all rounds
-// inside one cooperative kernel (grid-wide syncs on the device, no host round trip)
+// exact parallel reproduction of the ascending-index greedy (R12): adjacency lists (ranks) once, then all
+// candidates resolved in rank order by one CTA with the statuses in shared memory; a cooperative rescan kernel
+// takes over only when the lists do not fit (it returns at once otherwise)
 cudaError_t launch_spacing(liets_ctx* c, int s) {
     Dims g{ c->nx, c->ny, c->nz, c->boundary };
     unsigned long long N = c->N;
-    k_spacing_adjacency<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, g, s, N);
+    k_seed_rows<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->coff, c->rowoff, g);
+    c->launches++;
+    k_spacing_adjacency<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->rowoff, c->cand, g, s, N);
     c->launches++;
     cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    static bool attr_set = false;
+    const int ring_bytes = (int)(kRing / 16u * 4u);
+    if (!attr_set) {
+        e = cudaFuncSetAttribute(k_spacing_resolve_cta, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_bytes);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    k_spacing_resolve_cta<<<1, 1024, ring_bytes, c->stream>>>(c->ctl, c->cand, N);
+    c->launches++;
+    e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (c->resolve_grid == 0) {
         int per_sm = 0;
@@ -423,12 +588,12 @@ cudaError_t launch_spacing(liets_ctx* c, int s) {
     return e;
 }
 
-cudaError_t launch_seed_finalize(liets_ctx* c) {
+cudaError_t launch_seed_finalize(liets_ctx* c, int spaced) {
     if (c->storage == 0)
-        k_seed_finalize_u8<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->grid_u8, c->list[0]);
+        k_seed_finalize_u8<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->grid_u8, c->list[0], c->N, (uint32_t)spaced);
     else
         k_seed_finalize_tile<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->geom, grow_tile_words(),
-                                                                    c->G[0], c->G[1], c->stamp, c->list[0]);
+                                                                    c->G[0], c->G[1], c->stamp, c->list[0], c->N, (uint32_t)spaced);
     c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;

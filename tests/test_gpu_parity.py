@@ -54,7 +54,8 @@ def test_config1_bit_exact(liets, storage):
 @pytest.mark.parametrize("storage", STORAGES)
 @pytest.mark.parametrize("periodic", [False, True])
 @pytest.mark.parametrize("dims,core,s", [((37, 29, 41), 0.01, 4), ((70, 45, 33), 0.004, 7), ((5, 4, 3), 0.2, 2),
-                                          ((1, 9, 2), 0.3, 0), ((96, 96, 96), 0.003, 9), ((17, 130, 9), 0.02, 3)])
+                                          ((1, 9, 2), 0.3, 0), ((96, 96, 96), 0.003, 9), ((17, 130, 9), 0.02, 3),
+                                          ((24, 20, 28), 0.5, 8)])    # > 96 lower neighbours per candidate: the rescan path of the spacing
 def test_ragged_shapes_bit_exact(liets, storage, periodic, dims, core, s):
     run_both(liets, dims, periodic, core, s, 5, (0.05, 0.02, 0.01), 1, 0.55, storage)
 
