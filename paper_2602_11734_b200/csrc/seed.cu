@@ -1,15 +1,20 @@
 // seed.cu -- seeding and seed spacing by the L1 "diamond".
 //
-// Candidates: voxel v is a candidate core iff philox(seed; v>>2)[v&3] < T_core (R9).
-// Spacing (R11, R12): the sequential rule "scan candidates in ascending index, accept iff no
-// accepted seed within L1 < s" is reproduced exactly by parallel rounds over a 2-bit-per-voxel
-// status map (00 = no candidate / rejected, 01 = pending, 11 = accepted):
-//   a pending candidate v looks at every LOWER-index voxel within L1 < s (its diamond);
-//   - any accepted one  -> v is rejected (final: that seed is accepted in the sequential scan too);
-//   - else any pending  -> v waits (its fate depends on them);
-//   - else              -> v is accepted (all lower-index candidates in range are rejected).
-// Each state change is one atomic on one word, states only move 01 -> {00, 11}, so reading
-// neighbours that change during a round is safe, and the fixed point is the sequential result.
+// Candidates: voxel v is a candidate core iff philox(seed; v>>2)[v&3] < T_core (R9).  They are marked in a
+// 2-bit-per-voxel status map (00 = no candidate / rejected, 01 = pending, 11 = accepted); prefix sums of the
+// per-chunk counts give every candidate its RANK in ascending index order, and the list cand[rank] = voxel.
+// Spacing (R11, R12): the sequential rule "scan candidates in ascending index, accept iff no accepted seed
+// within L1 < s" is reproduced exactly:
+//   a pending candidate looks at every LOWER-index candidate within L1 < s (its neighbours);
+//   - any accepted one  -> it is rejected (final: that seed is accepted in the sequential scan too);
+//   - else any pending  -> it waits (its fate depends on them);
+//   - else              -> it is accepted (all lower-index candidates in range are rejected).
+// States only move pending -> {rejected, accepted}, so reading neighbours that change meanwhile is safe, and the
+// fixed point is the sequential result.  The dependency chains are long (about 140 links at 400^3: they sweep the
+// grid in index order), so the fast path keeps the statuses in ONE CTA's shared memory (a link costs a
+// shared-memory round trip, not an L2 one): k_spacing_adjacency lists each candidate's neighbours by rank,
+// k_spacing_resolve_cta resolves 1024 ranks per pass.  Lists that do not fit fall back to rescan rounds over
+// the global status map (k_spacing_resolve).
 #include <cooperative_groups.h>
 
 #include "liets_host.h"
@@ -226,7 +231,10 @@ __device__ __forceinline__ AdjView adj_view(uint32_t* cand, uint32_t n, unsigned
 
 // Ranks of the statuses kept in shared memory by k_spacing_resolve_cta: a ring of kRing candidates.  A candidate only
 // looks at candidates at most (candidates in s-1 slices) ranks below it; k_spacing_adjacency checks that this fits.
-constexpr uint32_t kRing = 1u << 19;
+constexpr uint32_t kRing = 1u << 17;             // one status byte per candidate: plain byte stores, no shared-memory atomics
+// On a periodic grid the candidates of the last slices also look at those of the first slices (ranks near 0): the
+// statuses of the first kHead ranks are kept for the whole run, next to the ring.
+constexpr uint32_t kHead = 1u << 16;
 
 // rowoff[rho] = number of candidates below row rho = y + ny z (rowoff[ny nz] = all): the candidates of any run of
 // consecutive rows are a run of consecutive ranks
@@ -318,7 +326,7 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
                 const uint32_t rk = s_buf[warp][e];
                 a.pool[base + e] = rk;
                 if (e < 8u) a.first8[(unsigned long long)e * n + i] = rk;
-                far = far || i - rk >= kRing;
+                far = far || (i - rk >= kRing && rk >= kHead);
             }
             if (far) ctl->spacing_slow = 1u;
             if (lane == 0) { a.off[i] = base; a.cnt[i] = k; }
@@ -333,20 +341,20 @@ __device__ __forceinline__ uint32_t status_of(const uint32_t* status2, uint32_t 
     return (ld_cg(status2 + (v >> 4)) >> (2 * (v & 15u))) & 3u;
 }
 
-// Pass 2: ONE CTA resolves all candidates in ascending rank, 1024 at a time, with the statuses (2 bits: 01 pending,
-// 11 accepted, 00 rejected) in shared memory, so a link of a dependency chain costs a shared-memory round trip
+// Pass 2: ONE CTA resolves all candidates in ascending rank, 1024 at a time, with the statuses (one byte: 1 pending,
+// 3 accepted, 0 rejected) in shared memory, so a link of a dependency chain costs a shared-memory round trip
 // instead of an L2 one (the chains are long: ~140 links at 400^3, they sweep the whole grid in index order).
 // A pending candidate is rejected as soon as a lower-rank neighbour is accepted, accepted once none of them is
 // pending, else it waits; neighbours of lower passes are already final.  The adjacency of the next passes is loaded
 // while the current one is resolved.  The final statuses go to st_rank (2 bits per candidate, by rank) for finalize.
 __global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, uint32_t* cand, unsigned long long N) {
-    extern __shared__ uint32_t s_st[];                      // kRing / 16 words
+    extern __shared__ uint8_t s_st[];                       // kRing + kHead status bytes: 1 pending, 3 accepted, 0 rejected
     if (ctl->spacing_slow) return;
     const uint32_t n = ctl->n_cand;
     const AdjView a = adj_view(cand, n, N);
-    uint32_t* const st_rank = a.st_rank;                    // n / 16 words of the n-word region
+    uint8_t* const st_rank = reinterpret_cast<uint8_t*>(a.st_rank);    // n bytes of the n-word region
     const uint32_t tid = threadIdx.x;
-    constexpr uint32_t kMask = kRing / 16u - 1u;
+    constexpr uint32_t kMask = kRing - 1u;
     // the next pass's lists (count, offset, first 8 ranks: coalesced) are loaded while this pass is resolved
     uint32_t kB = 0, offB = 0, nbrB[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
     auto load = [&](uint32_t i) {
@@ -361,39 +369,41 @@ __global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, u
     for (uint32_t i0 = 0; i0 < n; i0 += 1024u) {
         const uint32_t i = i0 + tid;
         const uint32_t k = kB, off = offB;
-        uint32_t widx[8], wsh[8];                           // ring word and bit position of each neighbour's status
+        uint32_t slot[8];                                   // ring slot of each neighbour's status
 #pragma unroll
-        for (int e = 0; e < 8; ++e) { widx[e] = (nbrB[e] >> 4) & kMask; wsh[e] = 2u * (nbrB[e] & 15u); }
-        // this pass's slots of the ring: all pending (64 words = 1024 candidates)
-        if (tid < 64u) s_st[((i0 >> 4) + tid) & kMask] = 0x55555555u;
+        for (int e = 0; e < 8; ++e) slot[e] = nbrB[e] < kHead ? kRing + nbrB[e] : (nbrB[e] & kMask);
+        s_st[i & kMask] = 1u;                               // this pass's slots of the ring: all pending
+        if (i < kHead) s_st[kRing + i] = 1u;
         load(i + 1024u);                                    // in flight while this pass is resolved
         __syncthreads();
         bool open = i < n;
         for (;;) {
             if (open) {
-                uint32_t w[8];
+                uint32_t st[8];
 #pragma unroll
-                for (int e = 0; e < 8; ++e) w[e] = s_st[widx[e]];          // independent loads (unused slots: any valid word)
+                for (int e = 0; e < 8; ++e) st[e] = s_st[slot[e]];         // independent loads (unused slots: any valid byte)
                 bool accepted = false, pending = false;
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    const uint32_t st = (uint32_t)e < k ? (w[e] >> wsh[e]) & 3u : 0u;
-                    accepted = accepted || st == 3u;
-                    pending = pending || st == 1u;
+                    accepted = accepted || ((uint32_t)e < k && st[e] == 3u);
+                    pending = pending || ((uint32_t)e < k && st[e] == 1u);
                 }
                 for (uint32_t e = 8; e < k; ++e) {          // long lists: the rest from the pool
                     const uint32_t r = a.pool[off + e];
-                    const uint32_t st = (s_st[(r >> 4) & kMask] >> (2u * (r & 15u))) & 3u;
-                    accepted = accepted || st == 3u;
-                    pending = pending || st == 1u;
+                    const uint32_t sv = s_st[r < kHead ? kRing + r : (r & kMask)];
+                    accepted = accepted || sv == 3u;
+                    pending = pending || sv == 1u;
                 }
-                uint32_t* mine = &s_st[(i >> 4) & kMask];
-                if (accepted) { atomicAnd(mine, ~(1u << (2u * (i & 15u)))); open = false; }              // 01 -> 00
-                else if (!pending) { atomicOr(mine, 2u << (2u * (i & 15u))); open = false; }             // 01 -> 11
+                if (accepted || !pending) {                 // pending -> rejected (0) / accepted (3)
+                    const uint8_t fin = accepted ? 0u : 3u;
+                    s_st[i & kMask] = fin;
+                    if (i < kHead) s_st[kRing + i] = fin;
+                    open = false;
+                }
             }
             if (__syncthreads_and(!open)) break;                // (no global atomic in this loop: the barrier would wait for it)
         }
-        if (tid < 64u) st_rank[(i0 >> 4) + tid] = s_st[((i0 >> 4) + tid) & kMask];     // final statuses by rank
+        if (i < n) st_rank[i] = s_st[i & kMask];            // final statuses by rank
     }
 }
 
@@ -439,8 +449,8 @@ __global__ void __launch_bounds__(1024) k_spacing_resolve(Control* ctl, uint32_t
 __device__ __forceinline__ bool seed_accepted(const Control* ctl, const uint32_t* status2, const uint32_t* cand,
                                               uint32_t n, unsigned long long N, uint32_t spaced, uint32_t i, uint32_t v) {
     if (spaced && !ctl->spacing_slow) {
-        const uint32_t* st_rank = cand + 3ull * n;          // AdjView::st_rank
-        return ((st_rank[i >> 4] >> (2u * (i & 15u))) & 3u) == 3u;
+        const uint8_t* st_rank = reinterpret_cast<const uint8_t*>(cand + 3ull * n);     // AdjView::st_rank, one byte per rank
+        return st_rank[i] == 3u;
     }
     return ((status2[v >> 4] >> (2u * (v & 15u))) & 3u) == 3u;
 }
@@ -565,7 +575,7 @@ cudaError_t launch_spacing(liets_ctx* c, int s) {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     static bool attr_set = false;
-    const int ring_bytes = (int)(kRing / 16u * 4u);
+    const int ring_bytes = (int)(kRing + kHead);
     if (!attr_set) {
         e = cudaFuncSetAttribute(k_spacing_resolve_cta, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_bytes);
         if (e != cudaSuccess) return e;
