@@ -149,16 +149,20 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         const TileCoord tc = tile_coord(id, g);
 
         // ---- A: gather ------------------------------------------------------------------------
-        for (int task = (int)tid; task < 100 * kRowWords; task += kThreads) {
-            const int r = task / kRowWords, c = task - r * kRowWords;
+        if (tid < 100u) {                   // one thread per row: the row's address once, its words as independent loads
+            const int r = (int)tid;
             const int zg = row_coord(r / 10 - 1, tc.z0, tc.wcz, g.nz, g.periodic);
             const int yg = row_coord(r % 10 - 1, tc.y0, tc.wcy, g.ny, g.periodic);
             const bool ok = zg >= 0 && yg >= 0;
             const unsigned long long row_base = ok ? (unsigned long long)g.Wp * ((unsigned long long)yg + (unsigned long long)g.ny * (unsigned long long)zg) : 0ull;
-            S.nv[r][c] = not_void_word(Gc, g, ok, row_base, tc.w0 + c - 1);
-            S.claims[r][2 * c] = 0u;
-            S.claims[r][2 * c + 1] = 0u;
+            unsigned long long w[kRowWords];
+#pragma unroll
+            for (int c = 0; c < kRowWords; ++c) w[c] = not_void_word(Gc, g, ok, row_base, tc.w0 + c - 1);
+#pragma unroll
+            for (int c = 0; c < kRowWords; ++c) S.nv[r][c] = w[c];
         }
+        for (int q = (int)tid; q < 100 * 2 * kRowWords / 4; q += kThreads)
+            reinterpret_cast<uint4*>(&S.claims[0][0])[q] = make_uint4(0u, 0u, 0u, 0u);
         __syncthreads();
         for (int task = (int)tid; task < 100 * kWin; task += kThreads) {
             const int r = task / kWin, k = task - r * kWin;
@@ -178,17 +182,19 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
             const int y = f_row & 7, z = f_row >> 3;
             const int xbase = 64 * (tc.w0 + f_j);
             if (y < tc.wcy && z < tc.wcz && xbase < g.nx) {
-                unsigned long long anyvoid = 0ull;
-#pragma unroll
-                for (int k = 0; k < 9; ++k) {
-                    const int rr = (z + k / 3) * 10 + (y + k % 3);
-                    const unsigned long long v = ~S.nv[rr][1 + f_j];
-                    const unsigned long long l = ~S.nv[rr][f_j] >> 63, rgt = ~S.nv[rr][2 + f_j] << 63;
-                    anyvoid |= v | (v << 1) | l | (v >> 1) | rgt;
-                }
                 unsigned long long src = S.nv[(z + 1) * 10 + (y + 1)][1 + f_j];
                 if (xbase + 64 > g.nx) src &= ~(~0ull << (g.nx - xbase));               // padding is not a source
-                F = src & anyvoid;                                                      // R13
+                if (src) {                                                              // (sparse early steps: most words hold no solid)
+                    unsigned long long anyvoid = 0ull;
+#pragma unroll
+                    for (int k = 0; k < 9; ++k) {
+                        const int rr = (z + k / 3) * 10 + (y + k % 3);
+                        const unsigned long long v = ~S.nv[rr][1 + f_j];
+                        const unsigned long long l = ~S.nv[rr][f_j] >> 63, rgt = ~S.nv[rr][2 + f_j] << 63;
+                        anyvoid |= v | (v << 1) | l | (v >> 1) | rgt;
+                    }
+                    F = src & anyvoid;                                                  // R13
+                }
             }
             off0 = block_exclusive_scan(__popcll(F), S.scan, &n_front);
         }
@@ -347,13 +353,23 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                 else if (curw) atomicOr(dst, curw);
             }
         }
-        for (int task = (int)tid; task < 100 * kRowWords; task += kThreads) {   // halo words: rarely non-zero
-            const int r = task / kRowWords, c = task - r * kRowWords;
-            const unsigned long long cw = (unsigned long long)S.claims[r][2 * c] | ((unsigned long long)S.claims[r][2 * c + 1] << 32);
-            if (cw == 0ull) continue;
-            const int zl = r / 10 - 1, yl = r % 10 - 1;
-            const bool own_word = zl >= 0 && zl < tc.wcz && yl >= 0 && yl < tc.wcy && c >= 1 && c <= kTileW && 64 * (tc.w0 + c - 1) < g.nx;
-            if (!own_word) halo_word(r, c, cw);
+        if (tid < 100u) {                   // halo words, one thread per row: rarely non-zero
+            const int r = (int)tid;
+            unsigned long long cw[kRowWords], any = 0ull;
+#pragma unroll
+            for (int c = 0; c < kRowWords; ++c) {
+                cw[c] = (unsigned long long)S.claims[r][2 * c] | ((unsigned long long)S.claims[r][2 * c + 1] << 32);
+                any |= cw[c];
+            }
+            if (any) {
+                const int zl = r / 10 - 1, yl = r % 10 - 1;
+                const bool own_row = zl >= 0 && zl < tc.wcz && yl >= 0 && yl < tc.wcy;
+#pragma unroll
+                for (int c = 0; c < kRowWords; ++c) {
+                    const bool own_word = own_row && c >= 1 && c <= kTileW && 64 * (tc.w0 + c - 1) < g.nx;
+                    if (cw[c] && !own_word) halo_word(r, c, cw[c]);
+                }
+            }
         }
         if (tid == 0 && n_front) {                                  // this tile still has front voxels
             if (atomicMax(&stamp[id], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = id;
