@@ -47,7 +47,8 @@ struct Smem {
     uint32_t hpat[8][4];
     uint32_t dir[28];                           // direction d: (row delta + 11) | (dx + 1) << 8
     uint32_t scan[33];
-    uint32_t tile, tile_id;
+    uint32_t tile[2], tile_id[2];               // list entry handed to the CTA, double-buffered by tile parity
+    uint32_t wsum[2][kWarps];                   // per-warp front-voxel counts, double-buffered
     uint16_t flist[kFrontCap];                  // x | (y | z << 3) << 8 of the tile's front voxels (x relative to the tile)
 };
 
@@ -135,13 +136,12 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         if (next_li < n_list) next_id = in[next_li];
     }
     unsigned long long own_new = 0ull, own_old = 0ull;      // the own word's atomicOr of the previous tile, looked at late
-    for (;;) {
-        __syncthreads();                    // the previous tile's shared memory is no longer read
-        if (tid == 0) { S.tile = next_li; S.tile_id = next_id; }
-        __syncthreads();
-        const uint32_t li = S.tile;
+    if (tid == 0) { S.tile[0] = next_li; S.tile_id[0] = next_id; }
+    for (uint32_t kt = 0;; ++kt) {
+        __syncthreads();                    // the previous tile's shared memory is no longer read; this tile's slot is written
+        const uint32_t li = S.tile[kt & 1u];
         if (li >= n_list) break;
-        const uint32_t id = S.tile_id;
+        const uint32_t id = S.tile_id[kt & 1u];
         if (tid == 0) {                     // latency hidden behind this tile's work
             next_li = atomicAdd(&ctl->tile_cursor, 1u);
             if (next_li < n_list) next_id = in[next_li];
@@ -160,19 +160,18 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
             for (int c = 0; c < kRowWords; ++c) w[c] = not_void_word(Gc, g, ok, row_base, tc.w0 + c - 1);
 #pragma unroll
             for (int c = 0; c < kRowWords; ++c) S.nv[r][c] = w[c];
+#pragma unroll
+            for (int k = 0; k < kWin; ++k) {                        // window k: 32 row bits from tile x = 29 k - 2
+                constexpr int kFirst = 62;
+                const int pos = kFirst + 29 * k, wd = pos >> 6, sh = pos & 63;
+                unsigned long long v = w[wd] >> sh;
+                if (sh > 32 && wd + 1 < kRowWords) v |= w[wd + 1] << (64 - sh);
+                S.win[r][k] = (uint32_t)v;
+            }
         }
         for (int q = (int)tid; q < 100 * 2 * kRowWords / 4; q += kThreads)
             reinterpret_cast<uint4*>(&S.claims[0][0])[q] = make_uint4(0u, 0u, 0u, 0u);
         __syncthreads();
-        for (int task = (int)tid; task < 100 * kWin; task += kThreads) {
-            const int r = task / kWin, k = task - r * kWin;
-            const int pos = 62 + 29 * k;                            // bit of the row that holds tile x = 29 k - 2
-            const int wd = pos >> 6, sh = pos & 63;
-            unsigned long long v = S.nv[r][wd] >> sh;
-            if (sh > 32 && wd + 1 < kRowWords) v |= S.nv[r][wd + 1] << (64 - sh);
-            S.win[r][k] = (uint32_t)v;
-        }
-
         // ---- B: front voxels of the tile ------------------------------------------------------------
         uint32_t n_front = 0, off0 = 0;
         unsigned long long F = 0ull;        // this thread's word (row tid / kTileW, word tid % kTileW): its front voxels
@@ -196,7 +195,19 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                     F = src & anyvoid;                                                  // R13
                 }
             }
-            off0 = block_exclusive_scan(__popcll(F), S.scan, &n_front);
+            // CTA prefix sum with one barrier: warp scan, warp totals to shared memory (double-buffered per tile),
+            // every thread adds the totals of the warps below its own
+            uint32_t wtotal;
+            const uint32_t wexcl = warp_exclusive_scan((uint32_t)__popcll(F), lane, &wtotal);
+            if (lane == 0) S.wsum[kt & 1u][warp] = wtotal;
+            __syncthreads();
+            off0 = wexcl;
+#pragma unroll
+            for (int q = 0; q < kWarps; ++q) {
+                const uint32_t v = S.wsum[kt & 1u][q];
+                n_front += v;
+                if ((uint32_t)q < warp) off0 += v;
+            }
         }
         const uint32_t p0 = (uint32_t)(64 * tc.w0) + (uint32_t)g.nx * ((uint32_t)tc.y0 + (uint32_t)g.ny * (uint32_t)tc.z0);
 
@@ -298,6 +309,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         }
         }
         while (qn) drain();
+        if (tid == 0) { S.tile[(kt + 1u) & 1u] = next_li; S.tile_id[(kt + 1u) & 1u] = next_id; }   // read after the next barrier but one
         __syncthreads();                    // all claims are in shared memory
 
         // ---- E: claim + compact ---------------------------------------------------------------------
