@@ -42,6 +42,7 @@ constexpr int kFrontCap = 32 * 64 * kTileW;     // front voxels listed at a time
 struct Smem {
     unsigned long long nv[100][kRowWords];      // not-void bits, row (z'+1)*10 + (y'+1)
     uint32_t win[100][kWin];                    // the same rows as overlapping windows
+    unsigned long long vx[100][kTileW];         // per tile word: cells with a void cell at x-1, x or x+1 in the same row
     uint32_t claims[100][2 * kRowWords];        // cells claimed in this step, same geometry as nv (32-bit view)
     uint32_t queue[kWarps][2 * kQueueCap];      // (voxel id | nibble level << 14, tied directions)
     uint32_t hpat[8][4];
@@ -161,6 +162,11 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
 #pragma unroll
             for (int c = 0; c < kRowWords; ++c) S.nv[r][c] = w[c];
 #pragma unroll
+            for (int j = 0; j < kTileW; ++j) {                      // void at x-1, x or x+1 (the x part of the 3x3x3 dilation)
+                const unsigned long long v = ~w[1 + j];
+                S.vx[r][j] = v | (v << 1) | (~w[j] >> 63) | (v >> 1) | (~w[2 + j] << 63);
+            }
+#pragma unroll
             for (int k = 0; k < kWin; ++k) {                        // window k: 32 row bits from tile x = 29 k - 2
                 constexpr int kFirst = 62;
                 const int pos = kFirst + 29 * k, wd = pos >> 6, sh = pos & 63;
@@ -186,12 +192,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                 if (src) {                                                              // (sparse early steps: most words hold no solid)
                     unsigned long long anyvoid = 0ull;
 #pragma unroll
-                    for (int k = 0; k < 9; ++k) {
-                        const int rr = (z + k / 3) * 10 + (y + k % 3);
-                        const unsigned long long v = ~S.nv[rr][1 + f_j];
-                        const unsigned long long l = ~S.nv[rr][f_j] >> 63, rgt = ~S.nv[rr][2 + f_j] << 63;
-                        anyvoid |= v | (v << 1) | l | (v >> 1) | rgt;
-                    }
+                    for (int k = 0; k < 9; ++k) anyvoid |= S.vx[(z + k / 3) * 10 + (y + k % 3)][f_j];
                     F = src & anyvoid;                                                  // R13
                 }
             }
