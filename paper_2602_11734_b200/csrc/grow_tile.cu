@@ -37,6 +37,7 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
 constexpr int kWin = (64 * kTileW - 1) / 29 + 1;   // 32-bit windows per row; window k starts at tile bit 29 k - 2
 constexpr int kQueueCap = 128;                  // voxels with ties per warp queue
+constexpr int kHeavyFront = 64 * 64 * kTileW / 8;  // a tile with at least this many front voxels (1/8 of its cells) is "heavy"
 constexpr int kFrontCap = 32 * 64 * kTileW;     // front voxels listed at a time (half the tile; more -> several passes)
 
 struct Smem {
@@ -102,7 +103,7 @@ __device__ __forceinline__ int row_coord(int i, int c0, int wc, int n, int perio
 
 __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__ ctl, TileGeom g,
                                                            unsigned long long* G0, unsigned long long* G1,
-                                                           uint32_t* stamp, uint32_t* list0, uint32_t* list1,
+                                                           uint32_t* stamp, uint32_t* weight, uint32_t* list0, uint32_t* list1,
                                                            PhiloxKey key) {
     if (!ctl->active) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -110,10 +111,19 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
 
     const uint32_t cur = ctl->cur;
-    const uint32_t n_list = ctl->count[cur];
+    // the list of step t: heavy tiles in slots [0, n_head), light ones in the last n_back slots; heavy ones are handed
+    // out first, so the kernel's tail is made of short tiles
+    const uint32_t n_head = ctl->count[cur], n_back = ctl->count_back[cur], list_cap = ctl->list_cap;
+    const uint32_t n_list = n_head + n_back;
     const uint32_t* __restrict__ in = cur ? list1 : list0;
     uint32_t* __restrict__ out = cur ? list0 : list1;
     uint32_t* out_count = &ctl->count[cur ^ 1u];
+    uint32_t* out_count_back = &ctl->count_back[cur ^ 1u];
+    auto list_entry = [&](uint32_t li) { return in[li < n_head ? li : list_cap - 1u - (li - n_head)]; };
+    auto emit_tile = [&](uint32_t tile, uint32_t n_front_seen) {        // heavy tiles to the front of the next list, light to its back
+        if (n_front_seen >= (uint32_t)kHeavyFront) out[atomicAdd(out_count, 1u)] = tile;
+        else out[list_cap - 1u - atomicAdd(out_count_back, 1u)] = tile;
+    };
     const uint32_t t = ctl->step;
     const unsigned long long* __restrict__ Gc = (t & 1u) ? G1 : G0;     // g_t (read only)
     unsigned long long* Gn = (t & 1u) ? G0 : G1;                        // g_{t+1} (OR target)
@@ -134,7 +144,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
     uint32_t next_li = 0, next_id = 0;      // thread 0: the list entry fetched ahead
     if (tid == 0) {
         next_li = atomicAdd(&ctl->tile_cursor, 1u);
-        if (next_li < n_list) next_id = in[next_li];
+        if (next_li < n_list) next_id = list_entry(next_li);
     }
     unsigned long long own_new = 0ull, own_old = 0ull;      // the own word's atomicOr of the previous tile, looked at late
     if (tid == 0) { S.tile[0] = next_li; S.tile_id[0] = next_id; }
@@ -145,7 +155,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         const uint32_t id = S.tile_id[kt & 1u];
         if (tid == 0) {                     // latency hidden behind this tile's work
             next_li = atomicAdd(&ctl->tile_cursor, 1u);
-            if (next_li < n_list) next_id = in[next_li];
+            if (next_li < n_list) next_id = list_entry(next_li);
         }
         const TileCoord tc = tile_coord(id, g);
 
@@ -335,14 +345,14 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                 const unsigned long long old = atomicOr(Gn + row_base + wg, in_row);
                 new_solid += __popcll(in_row & ~old);
                 const uint32_t nb = (uint32_t)(wg / kTileW) + (uint32_t)g.ntx * ((uint32_t)(yg >> 3) + (uint32_t)g.nty * (uint32_t)(zg >> 3));
-                if (nb != id && atomicMax(&stamp[nb], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = nb;   // newly active tile
+                if (nb != id && atomicMax(&stamp[nb], t + 2u) < t + 2u) emit_tile(nb, weight[nb]);          // newly active tile
             }
             if (wrap) {                                             // one cell across the tile's x border
                 const unsigned long long bit = 1ull << (x_wrap & 63);
                 const unsigned long long old = atomicOr(Gn + row_base + (x_wrap >> 6), bit);
                 if (!(old & bit)) new_solid++;
                 const uint32_t nb = (uint32_t)((x_wrap >> 6) / kTileW) + (uint32_t)g.ntx * ((uint32_t)(yg >> 3) + (uint32_t)g.nty * (uint32_t)(zg >> 3));
-                if (nb != id && atomicMax(&stamp[nb], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = nb;
+                if (nb != id && atomicMax(&stamp[nb], t + 2u) < t + 2u) emit_tile(nb, weight[nb]);
             }
         };
         // own words first, one per thread: carry g_t and add the hits; the old word is looked at after the halo pass
@@ -385,7 +395,8 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
             }
         }
         if (tid == 0 && n_front) {                                  // this tile still has front voxels
-            if (atomicMax(&stamp[id], t + 2u) < t + 2u) out[atomicAdd(out_count, 1u)] = id;
+            weight[id] = n_front;                                   // whoever lists the tile for the next step sorts it by this
+            if (atomicMax(&stamp[id], t + 2u) < t + 2u) emit_tile(id, n_front);
         }
     }
     new_solid += __popcll(own_new & ~own_old);
@@ -411,7 +422,7 @@ cudaError_t launch_grow_tile(liets_ctx* c) {
         attr_set = true;
     }
     const PhiloxKey key = philox_make_key(c->rng_seed);
-    k_grow_tile<<<c->tile_grid, kThreads, sizeof(Smem), c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->stamp,
+    k_grow_tile<<<c->tile_grid, kThreads, sizeof(Smem), c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->stamp, c->weight,
                                                                       c->list[0], c->list[1], key);
     c->launches++;
     return cudaGetLastError();

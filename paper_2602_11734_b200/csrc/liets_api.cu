@@ -17,7 +17,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t ctl, grid, list0, list1, status2, coff, rowoff, cand, total;
-    size_t g0, g1, stamp;          // STORAGE_TILE (contiguous: G0 | G1 | stamp)
+    size_t g0, g1, stamp, weight;  // STORAGE_TILE (contiguous: G0 | G1 | stamp | weight)
     size_t n_tiles, grid_words, list_cap;
     int Wp, ntx, nty, ntz;
 };
@@ -44,7 +44,8 @@ bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
         L->grid_words = (size_t)L->Wp * ny * nz;
         L->g0 = off;      off += L->grid_words * 8;
         L->g1 = off;      off += L->grid_words * 8;
-        L->stamp = off;   off += align_up(L->n_tiles * 4);
+        L->stamp = off;   off += L->n_tiles * 4;                // (memset together with G0 | G1 and the weights)
+        L->weight = off;  off = align_up(off + L->n_tiles * 4);
         L->list_cap = L->n_tiles;                           // the step stamp admits every tile at most once per list
     }
     L->list0 = off;   off += align_up(L->list_cap * 4);
@@ -154,6 +155,7 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
             c->G[0] = reinterpret_cast<unsigned long long*>(base + L.g0);
             c->G[1] = reinterpret_cast<unsigned long long*>(base + L.g1);
             c->stamp = reinterpret_cast<uint32_t*>(base + L.stamp);
+            c->weight = reinterpret_cast<uint32_t*>(base + L.weight);
             c->grid_u8 = nullptr;
             c->tile_grid = c->sm_count * kTileCtasPerSm;
         }
@@ -256,7 +258,7 @@ int liets_step(liets_ctx* c, uint64_t* n_solid_out, uint64_t* n_front_out) {
         if (int rc = readback(c)) return rc;
         const uint64_t ns = c->pinned->n_solid;
         if (n_solid_out) *n_solid_out = ns;
-        if (n_front_out) *n_front_out = (ns == 0 || ns == c->N) ? 0 : c->pinned->count[c->pinned->cur];
+        if (n_front_out) *n_front_out = (ns == 0 || ns == c->N) ? 0 : c->pinned->count[c->pinned->cur] + c->pinned->count_back[c->pinned->cur];
     }
     return LIETS_OK;
 }

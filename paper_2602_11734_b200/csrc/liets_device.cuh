@@ -76,7 +76,9 @@ struct Control {
     uint32_t active;                 // the step between two control kernels is live
     int32_t  status;                 // kStatusRunning or a LIETS_* status
     uint32_t cur;                    // which of the two front lists is A_t
-    uint32_t count[2];               // entries in each front list
+    uint32_t count[2];               // entries in each front list (STORAGE_TILE: the heavy tiles, filled from the front)
+    uint32_t count_back[2];          // STORAGE_TILE: light tiles of each list, filled from the back of the array
+    uint32_t list_cap;               // STORAGE_TILE: slots per list
     uint32_t claims;                 // voxels claimed by the live step (added to n_solid at finish)
     uint32_t n_cand;                 // seeding: candidates
     uint32_t pool_head;              // seeding: used entries of the adjacency pool
@@ -231,7 +233,7 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     const unsigned long long n_t = __ldcg(&c->n_t), N = __ldcg(&c->N);
     const unsigned long long R[3] = { __ldcg(&c->R[0]), __ldcg(&c->R[1]), __ldcg(&c->R[2]) };
     const uint32_t claims = __ldcg(&c->claims), items = __ldcg(&c->items), items0 = __ldcg(&c->items0);
-    const uint32_t count[2] = { __ldcg(&c->count[0]), __ldcg(&c->count[1]) };
+    const uint32_t count[2] = { __ldcg(&c->count[0]) + __ldcg(&c->count_back[0]), __ldcg(&c->count[1]) + __ldcg(&c->count_back[1]) };
     const uint32_t law = __ldcg(&c->law), max_steps = __ldcg(&c->max_steps);
     uint32_t step = __ldcg(&c->step), steps_done = __ldcg(&c->steps_done), cur = __ldcg(&c->cur);
     uint32_t active = __ldcg(&c->active);
@@ -278,6 +280,7 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     c->h0_any = h0_any;
     c->tile_cursor = 0;
     c->count[cur ^ 1u] = 0;
+    c->count_back[cur ^ 1u] = 0;
     c->claims = 0;
     c->items = 0;
     c->items0 = 0;

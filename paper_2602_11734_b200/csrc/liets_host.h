@@ -38,6 +38,7 @@ struct liets_ctx {
     uint64_t grid_words;              // 64-bit words per grid copy: Wp * ny * nz
     unsigned long long* G[2];         // double-buffered bit grid, x-rows of Wp words
     uint32_t* stamp;                  // per tile: t+1 of the last step whose list holds it
+    uint32_t* weight;                 // per tile: front voxels it had when it last ran (orders the list: heavy first)
     uint8_t* scratch_u8;              // N bytes for format conversion (aliases the candidate buffer)
     uint32_t host_step;               // step counter as of the last read-back (selects the current grid copy)
     int resolve_grid;                 // CTAs of the cooperative spacing kernel (0 = not sized yet)

@@ -32,7 +32,7 @@ __device__ __forceinline__ uint32_t ld_cg(const uint32_t* p) {
 // --- reset: grid, status map, counters ---------------------------------------------------------
 __global__ void k_seed_reset(Control* c) {
     c->n_solid = 0; c->step = 0; c->steps_done = 0; c->active = 0; c->status = 0; c->cur = 0;
-    c->count[0] = 0; c->count[1] = 0; c->claims = 0; c->n_cand = 0;
+    c->count[0] = 0; c->count[1] = 0; c->count_back[0] = 0; c->count_back[1] = 0; c->claims = 0; c->n_cand = 0;
     c->pool_head = 0; c->n_rescan = 0; c->pend3[0] = 0; c->pend3[1] = 0; c->pend3[2] = 0; c->spacing_slow = 0;
 }
 
@@ -530,8 +530,8 @@ cudaError_t launch_seed_reset(liets_ctx* c) {
     cudaError_t e;
     if (c->storage == 0) {
         e = cudaMemsetAsync(c->grid_u8, 0, (c->N + 3) & ~3ull, c->stream);
-    } else {                                                // G[0], G[1] and the stamps are contiguous
-        e = cudaMemsetAsync(c->G[0], 0, c->grid_words * 16 + c->n_tiles * 4, c->stream);
+    } else {                                                // G[0], G[1], the stamps and the weights are contiguous
+        e = cudaMemsetAsync(c->G[0], 0, c->grid_words * 16 + c->n_tiles * 8, c->stream);
     }
     if (e != cudaSuccess) return e;
     k_seed_reset<<<1, 1, 0, c->stream>>>(c->ctl);
