@@ -62,6 +62,14 @@ def test_ragged_shapes_bit_exact(liets, storage, periodic, dims, core, s):
 
 @pytest.mark.parametrize("storage", STORAGES)
 @pytest.mark.parametrize("periodic", [False, True])
+def test_dense_front_bit_exact(liets, storage, periodic):
+    # 55 % of the cells are seeds, nearly all of them front voxels: more than 4096 front voxels in one 128x8x8 tile,
+    # i.e. several passes over the tile's shared-memory voxel list; every class fires at level 0 (large probabilities)
+    run_both(liets, (130, 16, 16), periodic, 0.55, 0, 3, (0.3, 0.1, 0.02), 0, 0.97, storage)
+
+
+@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("periodic", [False, True])
 def test_step_by_step_equals_generate(liets, storage, periodic):
     dims, g = (48, 40, 52), (0.03, 0.01, 0.002)
     o = oracle.Oracle(*dims, periodic)
