@@ -173,7 +173,8 @@ __device__ __forceinline__ uint32_t nib_eq(uint32_t a, uint32_t h) {            
 }
 // four per-word masks (flag of nibble n at bit 4n+3) -> one mask in direction order (flag of direction d at bit d)
 __device__ __forceinline__ uint32_t interleave_dirs(uint32_t m0, uint32_t m1, uint32_t m2, uint32_t m3) {
-    return (m0 >> 3) | (m1 >> 2) | (m2 >> 1) | m3;
+    // the flags do not overlap, so the left shifts and ORs can be multiply-adds (FMA pipe), one right shift at the end
+    return (m0 + 2u * m1 + 4u * m2 + 8u * m3) >> 3;
 }
 // For the directions in `mask`: le = nibble of block B <= the threshold's nibble, eq = they tie.
 __device__ __forceinline__ void level_compare(const uint4& B, const uint32_t* h, uint32_t mask, uint32_t* le, uint32_t* eq) {
