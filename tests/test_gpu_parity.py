@@ -167,3 +167,42 @@ def test_config2_bit_exact(liets, storage, seed):
         po, vo = oracle.s2(o.grid(), False, axis, 16)
         assert (pg == po).all() and (vg == vo).all()
         assert pg[0] == L.N - o.n_solid
+
+
+def test_boundary_library_workspace_stream_and_capacity_errors(liets):
+    """The C ABI directly: library-owned workspace (NULL), a non-default stream, device-side output, and the
+    capacity errors of liets_create / liets_grid."""
+    import ctypes
+    import torch
+    L = liets.lib()
+    dims = (40, 24, 33)
+    N = dims[0] * dims[1] * dims[2]
+    o = oracle.Oracle(*dims, True)
+    o.set_growth(0.04, 0.01, 0.002, 1)
+    n_o = o.seed(0.01, 4, 21)
+    rc_o, st_o = o.generate(0.4, 10**6, True)
+    stream = torch.cuda.Stream()
+    for storage in STORAGES:
+        h = ctypes.c_void_p()
+        need = L.liets_workspace_bytes(*dims, storage)
+        small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+        assert L.liets_create(ctypes.byref(h), *dims, 1, storage, ctypes.c_void_p(small.data_ptr()), 1024,
+                              ctypes.c_void_p(stream.cuda_stream)) == liets.E_CAPACITY and need > 1024
+        assert L.liets_create(ctypes.byref(h), *dims, 1, storage, None, 0, ctypes.c_void_p(stream.cuda_stream)) == liets.OK
+        assert L.liets_set_growth(h, 0.04, 0.01, 0.002, liets.LAW_EQ1) == liets.OK
+        n = ctypes.c_uint64(0)
+        assert L.liets_seed(h, 0.01, 4, 21, ctypes.byref(n)) == liets.OK and n.value == n_o
+        steps, ns = ctypes.c_uint32(0), ctypes.c_uint64(0)
+        assert L.liets_generate(h, 0.4, 10**6, ctypes.byref(steps), ctypes.byref(ns)) == rc_o
+        assert (steps.value, ns.value) == (st_o, o.n_solid)
+        out = torch.empty(N, dtype=torch.uint8, device="cuda")
+        assert L.liets_grid(h, ctypes.c_void_p(out.data_ptr()), N - 1, liets.FORMAT_U8, 1) == liets.E_CAPACITY
+        assert L.liets_grid(h, ctypes.c_void_p(out.data_ptr()), N, liets.FORMAT_U8, 1) == liets.OK
+        stream.synchronize()
+        assert (out.cpu().numpy() == o.grid().ravel()).all()
+        bits = torch.empty((N + 7) // 8, dtype=torch.uint8, device="cuda")
+        assert L.liets_grid(h, ctypes.c_void_p(bits.data_ptr()), (N + 7) // 8, liets.FORMAT_BITS, 1) == liets.OK
+        stream.synchronize()
+        assert (np.unpackbits(bits.cpu().numpy(), bitorder="little")[:N] == o.grid().ravel()).all()
+        assert L.liets_launch_count(h) > 0
+        L.liets_destroy(h)
