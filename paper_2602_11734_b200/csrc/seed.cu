@@ -348,7 +348,8 @@ __device__ __forceinline__ uint32_t status_of(const uint32_t* status2, uint32_t 
 // pending, else it waits; neighbours of lower passes are already final.  The adjacency of the next passes is loaded
 // while the current one is resolved.  The final statuses go to st_rank (2 bits per candidate, by rank) for finalize.
 __global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, uint32_t* cand, unsigned long long N) {
-    extern __shared__ uint8_t s_st[];                       // kRing + kHead status bytes: 1 pending, 3 accepted, 0 rejected
+    extern __shared__ uint8_t s_st_raw[];                   // kRing + kHead status bytes: 1 pending, 3 accepted, 0 rejected
+    volatile uint8_t* const s_st = s_st_raw;                // read afresh in every look: other warps write them meanwhile
     if (ctl->spacing_slow) return;
     const uint32_t n = ctl->n_cand;
     const AdjView a = adj_view(cand, n, N);
@@ -376,8 +377,10 @@ __global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, u
         if (i < kHead) s_st[kRing + i] = 1u;
         load(i + 1024u);                                    // in flight while this pass is resolved
         __syncthreads();
+        // every warp keeps looking until its 32 candidates are resolved -- no CTA barrier inside: a link of a chain costs
+        // one shared-memory round trip.  Progress: a candidate only waits for lower ranks, all of them resident here.
         bool open = i < n;
-        for (;;) {
+        while (__any_sync(0xffffffffu, open)) {
             if (open) {
                 uint32_t st[8];
 #pragma unroll
@@ -388,11 +391,13 @@ __global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, u
                     accepted = accepted || ((uint32_t)e < k && st[e] == 3u);
                     pending = pending || ((uint32_t)e < k && st[e] == 1u);
                 }
-                for (uint32_t e = 8; e < k; ++e) {          // long lists: the rest from the pool
-                    const uint32_t r = a.pool[off + e];
-                    const uint32_t sv = s_st[r < kHead ? kRing + r : (r & kMask)];
-                    accepted = accepted || sv == 3u;
-                    pending = pending || sv == 1u;
+                if (k > 8u && !accepted && !pending) {      // long lists: the rest from the pool (global memory), only once the
+                    for (uint32_t e = 8; e < k; ++e) {      // first 8 are all rejected -- a pending one makes the candidate wait anyway
+                        const uint32_t r = a.pool[off + e];
+                        const uint32_t sv = s_st[r < kHead ? kRing + r : (r & kMask)];
+                        accepted = accepted || sv == 3u;
+                        pending = pending || sv == 1u;
+                    }
                 }
                 if (accepted || !pending) {                 // pending -> rejected (0) / accepted (3)
                     const uint8_t fin = accepted ? 0u : 3u;
@@ -401,9 +406,9 @@ __global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, u
                     open = false;
                 }
             }
-            if (__syncthreads_and(!open)) break;                // (no global atomic in this loop: the barrier would wait for it)
         }
         if (i < n) st_rank[i] = s_st[i & kMask];            // final statuses by rank
+        __syncthreads();                                    // the pass is final before the next one starts
     }
 }
 
