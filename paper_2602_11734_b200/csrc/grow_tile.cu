@@ -160,8 +160,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         const TileCoord tc = tile_coord(id, g);
 
         // ---- A: gather ------------------------------------------------------------------------
-        if (tid < 100u) {                   // one thread per row: the row's address once, its words as independent loads
-            const int r = (int)tid;
+        for (int r = (int)tid; r < 100; r += kThreads) {    // one thread per row: the row's address once, its words as independent loads
             const int zg = row_coord(r / 10 - 1, tc.z0, tc.wcz, g.nz, g.periodic);
             const int yg = row_coord(r % 10 - 1, tc.y0, tc.wcy, g.ny, g.periodic);
             const bool ok = zg >= 0 && yg >= 0;
@@ -376,8 +375,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                 else if (curw) atomicOr(dst, curw);
             }
         }
-        if (tid < 100u) {                   // halo words, one thread per row: rarely non-zero
-            const int r = (int)tid;
+        for (int r = (int)tid; r < 100; r += kThreads) {    // halo words, one thread per row: rarely non-zero
             unsigned long long cw[kRowWords], any = 0ull;
 #pragma unroll
             for (int c = 0; c < kRowWords; ++c) {
