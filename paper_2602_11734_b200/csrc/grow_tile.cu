@@ -101,13 +101,30 @@ __device__ __forceinline__ int row_coord(int i, int c0, int wc, int n, int perio
     return c;
 }
 
+// Shared-memory accesses of the per-voxel loops by 32-bit shared-window address held in a register (see flist_addr).
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v) {
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void atoms_or_u32(uint32_t addr, uint32_t v) {
+    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t opaque_shared_addr(const void* p) {     // a register the compiler cannot rematerialise
+    uint32_t a;
+    asm volatile("mov.u32 %0, %1;" : "=r"(a) : "r"((uint32_t)__cvta_generic_to_shared(p)));
+    return a;
+}
+
 __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__ ctl, TileGeom g,
                                                            unsigned long long* G0, unsigned long long* G1,
                                                            uint32_t* stamp, uint32_t* weight, uint32_t* list0, uint32_t* list1,
                                                            PhiloxKey key) {
     if (!ctl->active) return;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    Smem& S = *reinterpret_cast<Smem*>(smem_raw);
+    __shared__ __align__(16) Smem S;        // static (< 48 KB): shared-memory addresses are immediates, not generic pointers
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
 
     const uint32_t cur = ctl->cur;
@@ -139,7 +156,11 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
     const uint32_t h0[4] = { ctl->hpat[0][0], ctl->hpat[0][1], ctl->hpat[0][2], ctl->hpat[0][3] };
     uint32_t new_solid = 0;                 // per thread: bits this thread flipped 0 -> 1
     uint32_t n_items = 0, n_items0 = 0;     // per thread: Philox blocks evaluated, front voxels with a void target
-    uint32_t* const my_queue = S.queue[warp];
+    // shared-window address of the voxel list, kept in a register: left to itself the compiler rebuilds it (S2R
+    // CgaCtaId, MOV, LEA) at every access inside the per-voxel loops
+    const uint32_t flist_addr = opaque_shared_addr(S.flist), win_addr = opaque_shared_addr(S.win);
+    const uint32_t claims_addr = opaque_shared_addr(S.claims), queue_addr = opaque_shared_addr(S.queue[warp]);
+    const uint32_t hpat_addr = opaque_shared_addr(S.hpat), dir_addr = opaque_shared_addr(S.dir);
 
     uint32_t next_li = 0, next_id = 0;      // thread 0: the list entry fetched ahead
     if (tid == 0) {
@@ -226,9 +247,9 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
             while (fire) {
                 const uint32_t d = __ffs(fire) - 1u;
                 fire &= fire - 1u;
-                const uint32_t lut = S.dir[d];
+                const uint32_t lut = lds_u32(dir_addr + 4u * d);
                 const uint32_t xb = x + 63u + (lut >> 8);           // bit of the row: 64 + x + dx
-                atomicOr(&S.claims[zy + (lut & 0xFFu)][xb >> 5], 1u << (xb & 31u));
+                atoms_or_u32(claims_addr + 4u * ((zy + (lut & 0xFFu)) * (2u * kRowWords) + (xb >> 5)), 1u << (xb & 31u));
             }
         };
         uint32_t qn = 0;                    // queue fill (warp-uniform)
@@ -238,7 +259,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
             for (uint32_t j0 = 0; j0 < qn; j0 += 32u) {
                 const uint32_t j = j0 + lane;
                 uint32_t v = 0, tie = 0, still = 0;
-                if (j < qn) { v = my_queue[2 * j]; tie = my_queue[2 * j + 1]; }
+                if (j < qn) { v = lds_u32(queue_addr + 8u * j); tie = lds_u32(queue_addr + 8u * j + 4u); }
                 __syncwarp();               // this round's entries are read before any slot is written again
                 if (tie) {
                     const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = (v >> 11) & 7u, k = v >> 14;
@@ -246,7 +267,9 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                     const uint4 B = philox4x32_10(p, 0u, t, k, key);
                     ++n_items;
                     uint32_t le, eq;
-                    level_compare(B, S.hpat[k], tie, &le, &eq);
+                    const uint32_t hk[4] = { lds_u32(hpat_addr + 16u * k), lds_u32(hpat_addr + 16u * k + 4u),
+                                             lds_u32(hpat_addr + 16u * k + 8u), lds_u32(hpat_addr + 16u * k + 12u) };
+                    level_compare(B, hk, tie, &le, &eq);
                     const uint32_t fire = k < 7u ? (le & ~eq) : le;        // last nibble: draw <= U
                     still = k < 7u ? eq : 0u;
                     claim(fire, x, 10u * z + y);
@@ -254,8 +277,8 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                 const uint32_t have = __ballot_sync(0xffffffffu, still != 0u);
                 if (still) {
                     const uint32_t slot = wpos + __popc(have & ((1u << lane) - 1u));
-                    my_queue[2 * slot] = v + (1u << 14);
-                    my_queue[2 * slot + 1] = still;
+                    sts_u32(queue_addr + 8u * slot, v + (1u << 14));
+                    sts_u32(queue_addr + 8u * slot + 4u, still);
                 }
                 wpos += __popc(have);
             }
@@ -273,7 +296,8 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                     for (uint32_t m = (uint32_t)(F >> (32 * half)); m; ++off) {
                         const uint32_t b = 31u - __clz(m);
                         m ^= 1u << b;
-                        if (off - pass0 < (uint32_t)kFrontCap) S.flist[off - pass0] = (uint16_t)(hh | b);
+                        if (off - pass0 < (uint32_t)kFrontCap)
+                            asm volatile("st.shared.u16 [%0], %1;" ::"r"(flist_addr + 2u * (off - pass0)), "h"((uint16_t)(hh | b)) : "memory");
                     }
                 }
             }
@@ -283,14 +307,19 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
             const uint32_t i = i0 + tid;
             uint32_t tie = 0, v = 0;
             if (i < n_pass) {
-                v = S.flist[i];
+                {
+                    uint16_t v16;
+                    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v16) : "r"(flist_addr + 2u * i) : "memory");
+                    v = v16;
+                }
                 const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = v >> 11;
                 const uint32_t k = (x * 2260u) >> 16;                       // x / 29: window k holds tile bits 29k-2 .. 29k+29
                 const uint32_t shr = 1u << (31u + 29u * k - x);            // umulhi(w, shr) = w >> (x - 29k + 1): a shift on the FMA pipe
                 uint32_t nb27 = 0;          // bit 9(dz+1) + 3(dy+1) + (dx+1): that neighbour is not void
+                const uint32_t wrow = win_addr + 4u * (kWin * (z * 10u + y) + k);
 #pragma unroll
                 for (int e = 0; e < 9; ++e)
-                    nb27 |= (__umulhi(S.win[(z + e / 3) * 10u + (y + e % 3)][k], shr) & 7u) << (3 * e);
+                    nb27 |= (__umulhi(lds_u32(wrow + 4u * kWin * (uint32_t)((e / 3) * 10 + e % 3)), shr) & 7u) << (3 * e);
                 const uint32_t void27 = ~nb27;
                 const uint32_t void26 = ((void27 & 0x1FFFu) | ((void27 >> 14) << 13)) & en26;
                 if (void26) {
@@ -311,8 +340,8 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                 while (qn + 32u > (uint32_t)kQueueCap) drain();
                 if (tie) {
                     const uint32_t slot = qn + __popc(have & ((1u << lane) - 1u));
-                    my_queue[2 * slot] = v | (1u << 14);   // next nibble level: 1
-                    my_queue[2 * slot + 1] = tie;
+                    sts_u32(queue_addr + 8u * slot, v | (1u << 14));   // next nibble level: 1
+                    sts_u32(queue_addr + 8u * slot + 4u, tie);
                 }
                 qn += __popc(have);
             }
@@ -413,14 +442,15 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
 int grow_tile_words() { return kTileW; }
 
 cudaError_t launch_grow_tile(liets_ctx* c) {
+    static_assert(sizeof(Smem) <= 48 * 1024, "static shared memory");
     static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_grow_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+    if (!attr_set) {                                        // 8 CTAs x 22.6 KB per SM
+        cudaError_t e = cudaFuncSetAttribute(k_grow_tile, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     const PhiloxKey key = philox_make_key(c->rng_seed);
-    k_grow_tile<<<c->tile_grid, kThreads, sizeof(Smem), c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->stamp, c->weight,
+    k_grow_tile<<<c->tile_grid, kThreads, 0, c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->stamp, c->weight,
                                                                       c->list[0], c->list[1], key);
     c->launches++;
     return cudaGetLastError();
