@@ -287,11 +287,23 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         };
         for (uint32_t pass0 = 0; pass0 < n_front; pass0 += (uint32_t)kFrontCap) {   // almost always a single pass
             if (pass0) __syncthreads();     // the previous pass no longer reads the list
-            {                               // list the front voxels pass0 .. pass0 + kFrontCap - 1
-                uint32_t off = off0;
+            if (n_front <= (uint32_t)kFrontCap) {       // the usual case, one pass: no capacity test, the address just advances
+                uint32_t addr = flist_addr + 2u * off0;
                 const uint32_t hi = ((uint32_t)f_row << 8) | (uint32_t)(64 * f_j);
 #pragma unroll
                 for (int half = 1; half >= 0; --half) {             // highest bit first: one FLO per voxel
+                    const uint32_t hh = hi | (uint32_t)(32 * half);
+                    for (uint32_t m = (uint32_t)(F >> (32 * half)); m; addr += 2u) {
+                        const uint32_t b = 31u - __clz(m);
+                        m ^= 1u << b;
+                        asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((uint16_t)(hh | b)) : "memory");
+                    }
+                }
+            } else {                        // list the front voxels pass0 .. pass0 + kFrontCap - 1
+                uint32_t off = off0;
+                const uint32_t hi = ((uint32_t)f_row << 8) | (uint32_t)(64 * f_j);
+#pragma unroll
+                for (int half = 1; half >= 0; --half) {
                     const uint32_t hh = hi | (uint32_t)(32 * half);
                     for (uint32_t m = (uint32_t)(F >> (32 * half)); m; ++off) {
                         const uint32_t b = 31u - __clz(m);
