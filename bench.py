@@ -312,7 +312,7 @@ PER_FRONT_VOXEL_OPS = 52
 KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_tile"}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/); None until a capture exists for the current kernel.
-TRAFFIC_BYTES_PER_LAUNCH = {0: None, 1: 18.08e6}     # profiles/r1_k_grow_tile_ncu.md (k_grow_tile, steps 18-20)
+TRAFFIC_BYTES_PER_LAUNCH = {0: None, 1: 18.09e6}     # profiles/r1_k_grow_tile_ncu.md (k_grow_tile, steps 18-20)
 
 
 def main():
