@@ -151,6 +151,17 @@ def run_reference(args):
     }))
 
 
+def bench_workload(args):
+    """workloads.BENCH (BASELINE.json's timing configuration) unless --workload names another config (its first
+    spacing, rng seed and target): the other configs are parity cases, timed for information only."""
+    if not args.workload:
+        return workloads.BENCH
+    c = workloads.CONFIGS[args.workload]
+    s = c["s"] if isinstance(c["s"], int) else c["s"][0]
+    return dict(name=args.workload, dims=c["dims"], periodic=c["periodic"], core=c["core"], s=s, seed=c["seeds"][0],
+                g=c["g"], target=c["targets"][0])
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -167,7 +178,7 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    w = workloads.BENCH
+    w = bench_workload(args)
     nx, ny, nz = w["dims"]
     N = nx * ny * nz
     storage = args.storage if args.storage is not None else DEFAULT_STORAGE
@@ -281,7 +292,7 @@ def run_ours(args):
                     "ms_per_step": t_e2e / args.steps, "note": "inputs are parameters only; output = uint8 phase array to pinned host"},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
         }
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.workload:
         out["cpu_baseline"] = cpu_baseline()
     if rank == 0:
         print(json.dumps(out))
@@ -323,6 +334,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--storage", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default=None, choices=sorted(workloads.CONFIGS), help="time another config (information only)")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = args.steps or 2
