@@ -82,7 +82,6 @@ struct Control {
     uint32_t claims;                 // voxels claimed by the live step (added to n_solid at finish)
     uint32_t n_cand;                 // seeding: candidates
     uint32_t pool_head;              // seeding: used entries of the adjacency pool
-    uint32_t n_rescan;               // seeding: candidates whose adjacency was not stored
     uint32_t pend3[3];               // seeding: pending candidates after round r, at index r % 3
     uint32_t spacing_slow;           // seeding: the adjacency lists do not fit the fast resolve -> rescan rounds
     uint32_t items;                  // Philox blocks evaluated by the live step (profiling counter)
@@ -182,9 +181,6 @@ __device__ __forceinline__ void level_compare(const uint4& B, const uint32_t* h,
     const uint32_t e0 = nib_eq(B.x, h[0]), e1 = nib_eq(B.y, h[1]), e2 = nib_eq(B.z, h[2]), e3 = nib_eq(B.w, h[3]);
     *le = interleave_dirs(l0, l1, l2, l3) & mask;
     *eq = interleave_dirs(e0, e1, e2, e3) & mask;
-}
-__device__ __forceinline__ uint32_t level_le(const uint4& B, const uint32_t* h, uint32_t mask) {
-    return interleave_dirs(nib_le(B.x, h[0]), nib_le(B.y, h[1]), nib_le(B.z, h[2]), nib_le(B.w, h[3])) & mask;
 }
 
 // all-zero thresholds nibbles (every class has probability < 1/16): "<=" is "== 0"; flag at bit 3 of zero nibbles

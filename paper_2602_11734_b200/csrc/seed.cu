@@ -33,7 +33,7 @@ __device__ __forceinline__ uint32_t ld_cg(const uint32_t* p) {
 __global__ void k_seed_reset(Control* c) {
     c->n_solid = 0; c->step = 0; c->steps_done = 0; c->active = 0; c->status = 0; c->cur = 0;
     c->count[0] = 0; c->count[1] = 0; c->count_back[0] = 0; c->count_back[1] = 0; c->claims = 0; c->n_cand = 0;
-    c->pool_head = 0; c->n_rescan = 0; c->pend3[0] = 0; c->pend3[1] = 0; c->pend3[2] = 0; c->spacing_slow = 0;
+    c->pool_head = 0; c->pend3[0] = 0; c->pend3[1] = 0; c->pend3[2] = 0; c->spacing_slow = 0;
 }
 
 // --- candidates: one thread per status word = 16 voxels = 4 Philox blocks -----------------------
