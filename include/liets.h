@@ -92,8 +92,8 @@ int liets_set_target(liets_ctx* ctx, double target_solid_fraction);
 int liets_step(liets_ctx* ctx, uint64_t* n_solid_out, uint64_t* n_front_out);
 
 /* set_target + "while phi_a < phi_s and A not empty" + at most max_steps steps,
- * the loop running on the device with no host synchronisation per step.  Bit-exactly equal to
- * repeated liets_step.  The fraction is tested between whole steps only.  Returns LIETS_OK /
+ * the loop running on the device (one CUDA graph with a WHILE node: growth kernel + control step per
+ * iteration) with no host involvement until it ends.  Bit-exactly equal to repeated liets_step.  The fraction is tested between whole steps only.  Returns LIETS_OK /
  * LIETS_FRONT_EMPTY / LIETS_MAX_STEPS; *steps_out = steps done by this call. */
 int liets_generate(liets_ctx* ctx, double target_solid_fraction, uint32_t max_steps,
                    uint32_t* steps_out, uint64_t* n_solid_out);

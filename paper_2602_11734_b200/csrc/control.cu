@@ -16,6 +16,23 @@ __global__ void k_control(Control* c, uint32_t flags) {
     control_step(c, flags);
 }
 
+// The control step inside the device-side WHILE loop of liets_generate's CUDA graph: closes the step that just ran,
+// prepares the next one and tells the loop whether to go round again.
+__global__ void k_control_loop(Control* c, cudaGraphConditionalHandle loop) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    control_step(c, kCtlFinish | kCtlPrepare);
+    cudaGraphSetConditional(loop, __ldcg(&c->active) ? 1u : 0u);
+}
+
+cudaError_t control_loop_node(liets_ctx* c, cudaGraph_t graph, cudaGraphNode_t after, cudaGraphConditionalHandle loop,
+                              cudaGraphNode_t* node) {
+    void* args[] = { &c->ctl, &loop };
+    cudaKernelNodeParams p = {};
+    p.func = reinterpret_cast<void*>(k_control_loop);
+    p.gridDim = dim3(1); p.blockDim = dim3(32); p.sharedMemBytes = 0; p.kernelParams = args;
+    return cudaGraphAddKernelNode(node, graph, &after, 1, &p);
+}
+
 __global__ void k_begin(Control* c, int generate, uint32_t max_steps) {
     c->steps_done = 0;
     c->max_steps = max_steps;

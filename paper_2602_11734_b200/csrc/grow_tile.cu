@@ -468,4 +468,17 @@ cudaError_t launch_grow_tile(liets_ctx* c) {
     return cudaGetLastError();
 }
 
+// The same launch as a kernel node of `graph` (exec == nullptr), or its parameters refreshed in an instantiated
+// graph (the Philox key changes with every liets_seed).
+cudaError_t grow_tile_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node) {
+    cudaError_t e = cudaFuncSetAttribute(k_grow_tile, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    PhiloxKey key = philox_make_key(c->rng_seed);
+    void* args[] = { &c->ctl, &c->geom, &c->G[0], &c->G[1], &c->stamp, &c->weight, &c->list[0], &c->list[1], &key };
+    cudaKernelNodeParams p = {};
+    p.func = reinterpret_cast<void*>(k_grow_tile);
+    p.gridDim = dim3(c->tile_grid); p.blockDim = dim3(kThreads); p.sharedMemBytes = 0; p.kernelParams = args;
+    return exec ? cudaGraphExecKernelNodeSetParams(exec, *node, &p) : cudaGraphAddKernelNode(node, graph, nullptr, 0, &p);
+}
+
 }  // namespace liets

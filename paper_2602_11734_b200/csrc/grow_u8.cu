@@ -152,4 +152,14 @@ cudaError_t launch_grow_u8(liets_ctx* c) {
     return cudaGetLastError();
 }
 
+cudaError_t grow_u8_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node) {
+    GridDims dims{ c->nx, c->ny, c->nz };
+    PhiloxKey key = philox_make_key(c->rng_seed);
+    void* args[] = { &c->ctl, &c->grid_u8, &c->list[0], &c->list[1], &dims, &key };
+    cudaKernelNodeParams p = {};
+    p.func = c->boundary ? reinterpret_cast<void*>(k_grow_u8<true>) : reinterpret_cast<void*>(k_grow_u8<false>);
+    p.gridDim = dim3(c->sm_count * 8); p.blockDim = dim3(256); p.sharedMemBytes = 0; p.kernelParams = args;
+    return exec ? cudaGraphExecKernelNodeSetParams(exec, *node, &p) : cudaGraphAddKernelNode(node, graph, nullptr, 0, &p);
+}
+
 }  // namespace liets

@@ -95,6 +95,53 @@ int launch_step_kernel(liets_ctx* c) {
     return 0;
 }
 
+// liets_generate's device-resident step loop as ONE CUDA graph: a WHILE node whose body is
+//   growth kernel ; control step (closes the step, prepares the next, sets the loop condition).
+// Built once per context; the growth node's parameters are refreshed when the rng seed (Philox key) changes.
+// Returns false if this runtime cannot do it (generate then enqueues batches of steps instead).
+bool ensure_loop_graph(liets_ctx* c) {
+    if (c->loop_exec) {
+        if (c->loop_seed == c->rng_seed) return true;
+        const cudaError_t e = c->storage == LIETS_STORAGE_U8 ? grow_u8_node(c, nullptr, c->loop_exec, &c->loop_grow_node)
+                                                            : grow_tile_node(c, nullptr, c->loop_exec, &c->loop_grow_node);
+        if (e == cudaSuccess) { c->loop_seed = c->rng_seed; return true; }
+        cudaGetLastError();
+        cudaGraphExecDestroy(c->loop_exec); cudaGraphDestroy(c->loop_graph);        // rebuild below
+        c->loop_exec = nullptr; c->loop_graph = nullptr; c->loop_tried = false;
+    }
+    if (c->loop_tried) return false;
+    c->loop_tried = true;
+    cudaGraph_t g = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaGraphConditionalHandle loop;
+    cudaGraphNode_t while_node, grow_node, ctl_node;
+    bool ok = cudaGraphCreate(&g, 0) == cudaSuccess &&
+              cudaGraphConditionalHandleCreate(&loop, g, 1u, cudaGraphCondAssignDefault) == cudaSuccess;
+    if (ok) {
+        cudaGraphNodeParams wp = {};
+        wp.type = cudaGraphNodeTypeConditional;
+        wp.conditional.handle = loop;
+        wp.conditional.type = cudaGraphCondTypeWhile;
+        wp.conditional.size = 1;
+        ok = cudaGraphAddNode(&while_node, g, nullptr, 0, &wp) == cudaSuccess;
+        if (ok) {
+            cudaGraph_t body = wp.conditional.phGraph_out[0];
+            ok = (c->storage == LIETS_STORAGE_U8 ? grow_u8_node(c, body, nullptr, &grow_node)
+                                                 : grow_tile_node(c, body, nullptr, &grow_node)) == cudaSuccess &&
+                 control_loop_node(c, body, grow_node, loop, &ctl_node) == cudaSuccess &&
+                 cudaGraphInstantiate(&exec, g, 0) == cudaSuccess;
+        }
+    }
+    if (!ok) {
+        cudaGetLastError();
+        if (exec) cudaGraphExecDestroy(exec);
+        if (g) cudaGraphDestroy(g);
+        return false;
+    }
+    c->loop_graph = g; c->loop_exec = exec; c->loop_grow_node = grow_node; c->loop_seed = c->rng_seed;
+    return true;
+}
+
 }  // namespace
 
 extern "C" {
@@ -178,6 +225,8 @@ void liets_destroy(liets_ctx* c) {
     if (c->pinned) cudaFreeHost(c->pinned);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->loop_exec) cudaGraphExecDestroy(c->loop_exec);
+    if (c->loop_graph) cudaGraphDestroy(c->loop_graph);
     if (c->prof_ev) {
         for (uint32_t k = 0; k < 2 * kProfCap; ++k)
             if (c->prof_ev[k]) cudaEventDestroy(c->prof_ev[k]);
@@ -271,7 +320,13 @@ int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps
     LIETS_CUDA_TRY(c, launch_begin(c, 1, max_steps));
     c->prof_n = 0;
     uint32_t enqueued = 0;
-    for (;;) {
+    if (!c->profiling && ensure_loop_graph(c)) {
+        // the whole loop on the device: first step prepared here, then WHILE(step armed) { grow ; control } as one graph
+        LIETS_CUDA_TRY(c, launch_control(c, kCtlPrepare));
+        LIETS_CUDA_TRY(c, cudaGraphLaunch(c->loop_exec, c->stream));
+        if (int rc = readback(c)) return rc;
+        c->launches += 2ull * c->pinned->steps_done + (c->pinned->steps_done ? 0 : 2);   // kernels the graph ran
+    } else for (;;) {
         // a batch of steps back to back; steps after the stop rule fired are no-ops on the device
         uint32_t batch = 32;
         if (max_steps - enqueued < batch) batch = max_steps - enqueued;

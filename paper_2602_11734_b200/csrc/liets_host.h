@@ -57,6 +57,12 @@ struct liets_ctx {
     bool profiling;
     cudaEvent_t* prof_ev;             // 2 * kProfCap events, created on first use
     uint32_t prof_n;                  // growth launches bracketed by the last call
+    // liets_generate's device-resident loop: WHILE(step armed) { growth kernel ; control step } as one CUDA graph
+    cudaGraph_t loop_graph;
+    cudaGraphExec_t loop_exec;
+    cudaGraphNode_t loop_grow_node;
+    uint64_t loop_seed;               // rng_seed whose Philox key the graph's growth node holds
+    bool loop_tried;                  // graph creation attempted (on failure generate keeps enqueueing batches)
     char err[256];
 };
 
@@ -78,10 +84,14 @@ constexpr size_t kControlScalarBytes = offsetof(Control, log_front);
 cudaError_t launch_control(liets_ctx* c, uint32_t flags);
 cudaError_t launch_begin(liets_ctx* c, int generate, uint32_t max_steps);
 cudaError_t launch_set_params(liets_ctx* c);
+cudaError_t control_loop_node(liets_ctx* c, cudaGraph_t graph, cudaGraphNode_t after, cudaGraphConditionalHandle loop,
+                              cudaGraphNode_t* node);
 // grow_u8.cu
 cudaError_t launch_grow_u8(liets_ctx* c);
+cudaError_t grow_u8_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);
 // grow_tile.cu
 cudaError_t launch_grow_tile(liets_ctx* c);
+cudaError_t grow_tile_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);
 int grow_tile_words();
 // seed.cu
 cudaError_t launch_seed_reset(liets_ctx* c);
