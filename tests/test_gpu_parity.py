@@ -206,3 +206,35 @@ def test_boundary_library_workspace_stream_and_capacity_errors(liets):
         assert (np.unpackbits(bits.cpu().numpy(), bitorder="little")[:N] == o.grid().ravel()).all()
         assert L.liets_launch_count(h) > 0
         L.liets_destroy(h)
+
+
+@pytest.mark.parametrize("storage", STORAGES)
+def test_concurrent_contexts_on_streams_bit_exact(liets, storage):
+    """Independent realisations as contexts on separate CUDA streams, driven from host threads at the same time
+    (replicas: SURVEY 8(e) / NEXT-2): each must equal its own oracle run, whatever the interleaving on the GPU."""
+    import threading
+    import torch
+    dims, core, s, g, phi = (72, 56, 64), 0.004, 6, (0.03, 0.01, 0.002), 0.6
+    seeds = [11, 12, 13, 14]
+    gens, out = [], {}
+    for _ in seeds:
+        L = liets.Liets(*dims, 0, storage, stream=torch.cuda.Stream())
+        L.set_growth(*g, liets.LAW_EQ1)
+        gens.append(L)
+
+    def run(L, seed):
+        n = L.seed(core, s, seed)
+        rc, steps, ns = L.generate(phi)
+        out[seed] = (n, rc, steps, ns, L.grid())
+    for rep in range(2):                                          # second round: graphs already built, keys refreshed
+        th = [threading.Thread(target=run, args=(L, seed + 100 * rep)) for L, seed in zip(gens, seeds)]
+        [t.start() for t in th]
+        [t.join() for t in th]
+        for seed in seeds:
+            o = oracle.Oracle(*dims, False)
+            o.set_growth(*g, 1)
+            n_o = o.seed(core, s, seed + 100 * rep)
+            rc_o, st_o = o.generate(phi, 10**6, True)
+            n, rc, steps, ns, grid = out[seed + 100 * rep]
+            assert (n, rc, steps, ns) == (n_o, rc_o, st_o, o.n_solid)
+            assert (grid == o.grid()).all()
