@@ -238,3 +238,25 @@ def test_concurrent_contexts_on_streams_bit_exact(liets, storage):
             n, rc, steps, ns, grid = out[seed + 100 * rep]
             assert (n, rc, steps, ns) == (n_o, rc_o, st_o, o.n_solid)
             assert (grid == o.grid()).all()
+
+
+def _fuzz_cases(n, seed=2024):
+    rng = np.random.default_rng(seed)
+    cases = []
+    for k in range(n):
+        dims = tuple(int(v) for v in rng.choice([1, 2, 3, 7, 8, 9, 15, 16, 17, 31, 33, 63, 64, 65, 70, 129, 140], 3))
+        if dims[0] * dims[1] * dims[2] > 300000:
+            dims = (dims[0], min(dims[1], 33), min(dims[2], 33))
+        cases.append(dict(dims=dims, periodic=bool(rng.integers(0, 2)), core=float(rng.choice([0.002, 0.01, 0.05, 0.3])),
+                          s=int(rng.choice([0, 1, 2, 3, 5, 9])), seed=int(rng.integers(0, 2**40)),
+                          g=tuple(float(v) for v in rng.choice([0.0, 0.003, 0.02, 0.07, 0.2, 0.6, 1.0], 3)),
+                          law=int(rng.integers(0, 2)), target=float(rng.choice([0.2, 0.5, 0.9, 1.0])), storage=k % 2))
+    return cases
+
+
+@pytest.mark.parametrize("case", _fuzz_cases(100), ids=lambda c: "%dx%dx%d-%s-s%d-st%d" % (*c["dims"], "per" if c["periodic"] else "wall", c["s"], c["storage"]))
+def test_random_parameters_bit_exact(liets, case):
+    """Seeded random shapes (1- and 2-cell axes, word and tile boundaries), boundaries, densities, spacings, probabilities
+    (0, tiny, above 1/16, 1), laws, targets and 40-bit rng seeds; at most 60 steps each."""
+    run_both(liets, case["dims"], case["periodic"], case["core"], case["s"], case["seed"], case["g"], case["law"],
+             case["target"], case["storage"], max_steps=60)
