@@ -260,3 +260,26 @@ def test_random_parameters_bit_exact(liets, case):
     (0, tiny, above 1/16, 1), laws, targets and 40-bit rng seeds; at most 60 steps each."""
     run_both(liets, case["dims"], case["periodic"], case["core"], case["s"], case["seed"], case["g"], case["law"],
              case["target"], case["storage"], max_steps=60)
+
+
+def test_oracle_philox_equals_curand_device_philox(liets, tmp_path):
+    """Pin P1 on the GPU box: the oracle's Philox4x32-10 against NVIDIA's own device implementation
+    (curand_Philox4x32_10 from curand_philox4x32_x.h, compiled here with nvcc) on 2000 random (counter, key) vectors."""
+    import os
+    import shutil
+    import subprocess
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not available on this box")
+    src = os.path.join(os.path.dirname(__file__), "curand_philox_check.cu")
+    exe = str(tmp_path / "curand_philox_check")
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-o", exe, src])
+    rng = np.random.default_rng(7)
+    vec = rng.integers(0, 2**32, size=(2000, 6), dtype=np.uint64)
+    vec[0] = 0
+    vec[1] = 2**32 - 1
+    text = "\n".join(" ".join("%x" % int(x) for x in row) for row in vec) + "\n"
+    out = subprocess.run([exe], input=text, capture_output=True, text=True, check=True).stdout.split("\n")
+    for row, line in zip(vec, out):
+        expect = oracle.philox4x32_10([int(x) for x in row[:4]], [int(x) for x in row[4:]])
+        assert tuple(int(t, 16) for t in line.split()) == expect
