@@ -40,7 +40,23 @@ __global__ void __launch_bounds__(256) k_unpack_rows_u8(const unsigned long long
         }
     }
 }
+// byte-aligned bit rows (nx % 8 == 0) -> the packed phase array: the rows without their padding words
+__global__ void __launch_bounds__(256) k_rows_to_bits(const uint8_t* __restrict__ G, uint8_t* __restrict__ dst,
+                                                       unsigned long long n_bytes, uint32_t row_bytes, uint32_t pitch) {
+    for (unsigned long long b = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; b < n_bytes;
+         b += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long row = b / row_bytes;
+        dst[b] = G[row * pitch + (b - row * row_bytes)];
+    }
+}
 }  // namespace
+
+cudaError_t launch_rows_to_bits(liets_ctx* c, uint8_t* dst_bits) {
+    k_rows_to_bits<<<c->sm_count * 8, 256, 0, c->stream>>>(reinterpret_cast<const uint8_t*>(c->G[c->host_step & 1u]), dst_bits,
+                                                           c->N / 8, (uint32_t)c->nx / 8, (uint32_t)c->geom.Wp * 8);
+    c->launches++;
+    return cudaGetLastError();
+}
 
 cudaError_t launch_pack_bits_u8(liets_ctx* c, const uint8_t* src_u8, uint8_t* dst_bits) {
     k_pack_bits_u8<<<c->sm_count * 8, 256, 0, c->stream>>>(src_u8, dst_bits, c->N);

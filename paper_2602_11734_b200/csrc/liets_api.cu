@@ -357,6 +357,17 @@ int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is
     if (c->storage == LIETS_STORAGE_TILE) {                 // bit rows -> linear uint8 (seeding scratch is idle)
         if (int rc = readback(c)) return rc;                // which grid copy is current
         c->host_step = c->pinned->step;
+        if (format == LIETS_FORMAT_BITS && c->nx % 8 == 0) {
+            // the x-rows are byte aligned: the packed output is the rows without their padding words
+            if (dst_is_device) {
+                LIETS_CUDA_TRY(c, launch_rows_to_bits(c, static_cast<uint8_t*>(dst)));
+            } else {                                        // gather into the (idle) seeding scratch, then one copy
+                LIETS_CUDA_TRY(c, launch_rows_to_bits(c, reinterpret_cast<uint8_t*>(c->status2)));
+                LIETS_CUDA_TRY(c, cudaMemcpyAsync(dst, c->status2, nb, kind, c->stream));
+                LIETS_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+            }
+            return LIETS_OK;
+        }
         uint8_t* lin = (format == LIETS_FORMAT_U8 && dst_is_device) ? static_cast<uint8_t*>(dst) : c->scratch_u8;
         LIETS_CUDA_TRY(c, launch_unpack_rows_u8(c, lin));
         u8 = lin;

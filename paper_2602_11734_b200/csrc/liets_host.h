@@ -102,4 +102,5 @@ cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n);
 // export.cu
 cudaError_t launch_pack_bits_u8(liets_ctx* c, const uint8_t* src_u8, uint8_t* dst_bits);
 cudaError_t launch_unpack_rows_u8(liets_ctx* c, uint8_t* dst_u8);
+cudaError_t launch_rows_to_bits(liets_ctx* c, uint8_t* dst_bits);
 }  // namespace liets
