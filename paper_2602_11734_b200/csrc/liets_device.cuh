@@ -61,6 +61,7 @@ struct Control {
     unsigned long long n_t;          // target count ceil(phi_s N) (R7)
     unsigned long long R[3];         // reference thresholds floor(G_ref 2^32 + .5): face, edge, corner (R8)
     unsigned long long N;
+    unsigned long long pool_head;    // seeding: entries handed out from the adjacency pool (64-bit: may run far past its size)
     uint32_t U[3];                   // T - 1 of the current step's thresholds T in [1, 2^32] (Eq. (1)):
                                      // a draw fires iff draw <= U
     uint32_t en[3];                  // T >= 1; a class with T == 0 never fires
@@ -81,7 +82,6 @@ struct Control {
     uint32_t list_cap;               // STORAGE_TILE: slots per list
     uint32_t claims;                 // voxels claimed by the live step (added to n_solid at finish)
     uint32_t n_cand;                 // seeding: candidates
-    uint32_t pool_head;              // seeding: used entries of the adjacency pool
     uint32_t pend3[3];               // seeding: pending candidates after round r, at index r % 3
     uint32_t spacing_slow;           // seeding: the adjacency lists do not fit the fast resolve -> rescan rounds
     uint32_t items;                  // Philox blocks evaluated by the live step (profiling counter)

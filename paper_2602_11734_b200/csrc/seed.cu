@@ -313,12 +313,12 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
         }
         __syncwarp();
         const uint32_t k = s_cnt[warp];
-        uint32_t base = 0;
+        unsigned long long base = 0;
         bool stored = k <= (uint32_t)kAdjBuf;
         if (stored && k) {
-            if (lane == 0) base = atomicAdd(&ctl->pool_head, k);
+            if (lane == 0) base = atomicAdd(&ctl->pool_head, (unsigned long long)k);
             base = __shfl_sync(0xffffffffu, base, 0);
-            stored = (unsigned long long)base + k <= a.pool_cap;
+            stored = base + k <= a.pool_cap;
         }
         if (stored) {
             bool far = false;
@@ -329,7 +329,7 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
                 far = far || (i - rk >= kRing && rk >= kHead);
             }
             if (far) ctl->spacing_slow = 1u;
-            if (lane == 0) { a.off[i] = base; a.cnt[i] = k; }
+            if (lane == 0) { a.off[i] = (uint32_t)base; a.cnt[i] = k; }
         } else if (lane == 0) {
             ctl->spacing_slow = 1u;
         }
