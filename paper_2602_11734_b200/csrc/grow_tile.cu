@@ -36,7 +36,7 @@ constexpr int kThreads = 128;
 constexpr int kWarps = kThreads / 32;
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
 constexpr int kWin = (64 * kTileW - 1) / 29 + 1;   // 32-bit windows per row; window k starts at tile bit 29 k - 2
-constexpr int kQueueCap = 128;                  // voxels with ties per warp queue
+constexpr int kQueueCap = 256;                  // voxels with ties per warp queue
 constexpr int kHeavyFront = 64 * 64 * kTileW / 8;  // a tile with at least this many front voxels (1/8 of its cells) is "heavy"
 constexpr int kFrontCap = 32 * 64 * kTileW;     // front voxels listed at a time (half the tile; more -> several passes)
 
