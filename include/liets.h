@@ -42,7 +42,7 @@ enum {
 
 enum { LIETS_BOUNDARY_WALL = 0, LIETS_BOUNDARY_PERIODIC = 1 };        /* R5 */
 enum { LIETS_STORAGE_U8 = 0,      /* uint8 grid + explicit list of front VOXELS (uint32 indices)  */
-       LIETS_STORAGE_TILE = 1 };  /* bit-packed x-rows + explicit list of active 256x8x8 TILES; the
+       LIETS_STORAGE_TILE = 1 };  /* bit-packed x-rows + explicit list of active 128x8x8 TILES; the
                                      front voxels of a tile are re-listed in shared memory each step */
 enum { LIETS_LAW_CONSTANT = 0, LIETS_LAW_EQ1 = 1 };
 enum { LIETS_FORMAT_U8 = 0,       /* one byte per voxel in {0,1}, x fastest, N bytes              */
@@ -77,7 +77,8 @@ int liets_set_growth(liets_ctx* ctx, double g_face, double g_edge, double g_corn
 int liets_seed(liets_ctx* ctx, double core_prob, int spacing_s, uint64_t rng_seed,
                uint64_t* n_seeds_out);
 
-/* Same reset, but the seeds are the n given voxel indices (HOST array, duplicates allowed). */
+/* Same reset, but the seeds are the n given voxel indices (HOST array, duplicates allowed).  The indices are
+ * staged in the library's seeding scratch: n <= max(8, N/2), else E_CAPACITY; an index >= N is E_ARG. */
 int liets_seed_explicit(liets_ctx* ctx, const uint64_t* idx, uint64_t n, uint64_t rng_seed);
 
 /* Target solid volume fraction phi_s in (0,1]: n_t = ceil(phi_s*N) (R7). Used by Eq. (1) and by
@@ -98,7 +99,8 @@ int liets_step(liets_ctx* ctx, uint64_t* n_solid_out, uint64_t* n_front_out);
 int liets_generate(liets_ctx* ctx, double target_solid_fraction, uint32_t max_steps,
                    uint32_t* steps_out, uint64_t* n_solid_out);
 
-/* Copy the phase array out: dst (HOST, or DEVICE if dst_is_device) in LIETS_FORMAT_*. */
+/* Copy the phase array out: dst (HOST, or DEVICE if dst_is_device) in LIETS_FORMAT_*.
+ * Errors: E_STATE before the first liets_seed / liets_seed_explicit, E_CAPACITY (dst_bytes), E_ARG. */
 int liets_grid(liets_ctx* ctx, void* dst, size_t dst_bytes, int format, int dst_is_device);
 
 /* Per-step counters of the steps done since the last seed (HOST arrays of capacity cap, may be
@@ -122,6 +124,29 @@ int liets_set_profiling(liets_ctx* ctx, int on);
 int liets_step_times(liets_ctx* ctx, float* ms, uint32_t cap);
 /* Number of kernels this ctx has launched since liets_create (memsets and copies not counted). */
 uint64_t liets_launch_count(const liets_ctx* ctx);
+
+/* After liets_seed: the number of keyed candidates before spacing, and whether the spacing was
+ * resolved by the rescan slow path (1) or by the adjacency lists (0); both may be NULL.  Errors: E_STATE. */
+int liets_seed_info(liets_ctx* ctx, uint32_t* n_candidates, uint32_t* slow_path);
+/* Test aid: shrink the status ring (a power of two in [2048, 2^17]) and the head table (<= 2^16) of the
+ * single-CTA spacing resolve so that small grids exercise the ring wrap; ring = 0 restores the defaults.
+ * The accepted seeds never depend on these sizes. */
+int liets_debug_spacing_ring(liets_ctx* ctx, uint32_t ring, uint32_t head);
+
+/* Measured roofs for the roofline report (SURVEY.md 8(d) "Which roofline": the working set of the growth steps
+ * is L2 resident and Philox makes the integer pipes a co-limit).  Runs probe `kind` `reps`
+ * times (after one warm-up launch) on cuda_stream, timed with CUDA events, and returns the best launch:
+ *   LIETS_PROBE_PHILOX   Philox4x32-10 blocks per second, nothing but the blocks
+ *   LIETS_PROBE_LOP3 / _IMAD / _MIX  thread-level integer instructions per second: three-input logic ops (ALU
+ *                        pipe), 32-bit multiply-adds (FMA pipe), and the two interleaved one to one
+ *   LIETS_PROBE_L2_READ  bytes per second of 16-byte ld.global.cg loads over an L2-resident 32 MiB window
+ *   LIETS_PROBE_HBM_READ bytes per second of the same loads over the whole scratch (make it >> L2)
+ * device_scratch: DEVICE buffer of scratch_bytes >= 1 MiB, caller-owned (contents are read, 4 KiB may be
+ * overwritten).  *ms_best (may be NULL) = duration of the best launch.  Needs no ctx.  Errors: E_ARG, E_CUDA. */
+enum { LIETS_PROBE_PHILOX = 0, LIETS_PROBE_LOP3 = 1, LIETS_PROBE_IMAD = 2, LIETS_PROBE_MIX = 3,
+       LIETS_PROBE_L2_READ = 4, LIETS_PROBE_HBM_READ = 5 };
+int liets_probe(int kind, void* device_scratch, size_t scratch_bytes, void* cuda_stream, int reps,
+                double* units_per_second, double* ms_best);
 
 void liets_destroy(liets_ctx* ctx);
 const char* liets_last_error(const liets_ctx* ctx);

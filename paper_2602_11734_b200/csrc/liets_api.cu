@@ -206,7 +206,9 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
             c->grid_u8 = nullptr;
             c->tile_grid = c->sm_count * kTileCtasPerSm;
         }
-        ok = cudaMemsetAsync(c->ctl, 0, sizeof(Control), c->stream) == cudaSuccess &&
+        // function attributes are per device: set them for the device of this context (cheap, idempotent)
+        ok = seed_kernel_attributes() == cudaSuccess && grow_tile_attributes() == cudaSuccess &&
+             cudaMemsetAsync(c->ctl, 0, sizeof(Control), c->stream) == cudaSuccess &&
              launch_set_params(c) == cudaSuccess;
     }
     if (!ok) {
@@ -282,7 +284,8 @@ int liets_seed(liets_ctx* c, double core_prob, int spacing_s, uint64_t rng_seed,
 
 int liets_seed_explicit(liets_ctx* c, const uint64_t* idx, uint64_t n, uint64_t rng_seed) {
     if (!c || (n && !idx)) return LIETS_E_ARG;
-    if (n * 8 > (c->N * 4 < 64 ? 64 : c->N * 4)) return fail(c, LIETS_E_CAPACITY, "too many explicit seeds for the staging buffer");
+    // the staging buffer is the 4 N-byte candidate region: at most N/2 (>= 8) indices; n is compared, not n * 8
+    if (n > (c->N * 4 < 64 ? 64 : c->N * 4) / 8) return fail(c, LIETS_E_CAPACITY, "too many explicit seeds for the staging buffer (max N/2)");
     for (uint64_t i = 0; i < n; ++i)
         if (idx[i] >= c->N) return fail(c, LIETS_E_ARG, "seed index outside the grid");
     c->rng_seed = rng_seed;
@@ -349,6 +352,7 @@ int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps
 
 int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is_device) {
     if (!c || !dst) return LIETS_E_ARG;
+    if (!c->seeded) return fail(c, LIETS_E_STATE, "liets_grid before liets_seed");
     const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     if (format != LIETS_FORMAT_U8 && format != LIETS_FORMAT_BITS) return fail(c, LIETS_E_ARG, "unknown grid format");
     const size_t nb = format == LIETS_FORMAT_U8 ? (size_t)c->N : (size_t)((c->N + 7) / 8);
@@ -430,5 +434,23 @@ int liets_step_times(liets_ctx* c, float* ms, uint32_t cap) {
 }
 
 uint64_t liets_launch_count(const liets_ctx* c) { return c ? c->launches : 0; }
+
+int liets_seed_info(liets_ctx* c, uint32_t* n_candidates, uint32_t* slow_path) {
+    if (!c) return LIETS_E_ARG;
+    if (!c->seeded) return fail(c, LIETS_E_STATE, "liets_seed_info before liets_seed");
+    if (int rc = readback(c)) return rc;
+    if (n_candidates) *n_candidates = c->pinned->n_cand;
+    if (slow_path) *slow_path = c->pinned->spacing_slow;
+    return LIETS_OK;
+}
+
+int liets_debug_spacing_ring(liets_ctx* c, uint32_t ring, uint32_t head) {
+    if (!c) return LIETS_E_ARG;
+    if (ring == 0) { c->spacing_ring = c->spacing_head = 0; return LIETS_OK; }
+    if (ring < 2048u || (ring & (ring - 1u)) || ring > (1u << 17) || head > (1u << 16))
+        return fail(c, LIETS_E_ARG, "ring must be a power of two in [2048, 2^17], head <= 2^16");
+    c->spacing_ring = ring; c->spacing_head = head;
+    return LIETS_OK;
+}
 
 }  // extern "C"

@@ -42,6 +42,7 @@ struct liets_ctx {
     uint8_t* scratch_u8;              // N bytes for format conversion (aliases the candidate buffer)
     uint32_t host_step;               // step counter as of the last read-back (selects the current grid copy)
     int resolve_grid;                 // CTAs of the cooperative spacing kernel (0 = not sized yet)
+    uint32_t spacing_ring, spacing_head;  // test hook (liets_debug_spacing_ring): 0 = the built-in sizes
     int tile_grid;                    // CTAs of the tile growth kernel
     uint64_t list_cap;                // slots per front list
     // host state
@@ -99,6 +100,8 @@ cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all
 cudaError_t launch_spacing(liets_ctx* c, int s);
 cudaError_t launch_seed_finalize(liets_ctx* c, int spaced);
 cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n);
+cudaError_t seed_kernel_attributes();
+cudaError_t grow_tile_attributes();
 // export.cu
 cudaError_t launch_pack_bits_u8(liets_ctx* c, const uint8_t* src_u8, uint8_t* dst_bits);
 cudaError_t launch_unpack_rows_u8(liets_ctx* c, uint8_t* dst_u8);

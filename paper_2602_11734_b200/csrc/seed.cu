@@ -232,6 +232,8 @@ __device__ __forceinline__ AdjView adj_view(uint32_t* cand, uint32_t n, unsigned
 // Ranks of the statuses kept in shared memory by k_spacing_resolve_cta: a ring of kRing candidates.  A candidate only
 // looks at candidates at most (candidates in s-1 slices) ranks below it; k_spacing_adjacency checks that this fits.
 constexpr uint32_t kRing = 1u << 17;             // one status byte per candidate: plain byte stores, no shared-memory atomics
+// (kRing / kHead are the defaults; the sizes are kernel arguments so that a test can shrink them until the ring wraps
+// after a few thousand candidates: liets_debug_spacing_ring)
 // On a periodic grid the candidates of the last slices also look at those of the first slices (ranks near 0): the
 // statuses of the first kHead ranks are kept for the whole run, next to the ring.
 constexpr uint32_t kHead = 1u << 16;
@@ -251,7 +253,7 @@ __global__ void __launch_bounds__(256) k_seed_rows(const Control* ctl, const uin
 // (consecutive ranks) and keeps those in range.  Sets ctl->spacing_slow if a list does not fit or a neighbour is
 // too far back in rank for the ring of k_spacing_resolve_cta.
 __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const uint32_t* __restrict__ rowoff, uint32_t* cand,
-                                                            Dims g, int s, unsigned long long N) {
+                                                            Dims g, int s, unsigned long long N, uint32_t ring, uint32_t head) {
     __shared__ uint32_t s_buf[8][kAdjBuf];
     __shared__ uint32_t s_cnt[8];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -326,7 +328,9 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
                 const uint32_t rk = s_buf[warp][e];
                 a.pool[base + e] = rk;
                 if (e < 8u) a.first8[(unsigned long long)e * n + i] = rk;
-                far = far || (i - rk >= kRing && rk >= kHead);
+                // the resolve re-arms the ring slots of a whole pass (1024 ranks) at once: rk's slot must survive until
+                // the END of i's pass, not just until i
+                far = far || ((i | 1023u) - rk >= ring && rk >= head);
             }
             if (far) ctl->spacing_slow = 1u;
             if (lane == 0) { a.off[i] = (uint32_t)base; a.cnt[i] = k; }
@@ -347,15 +351,16 @@ __device__ __forceinline__ uint32_t status_of(const uint32_t* status2, uint32_t 
 // A pending candidate is rejected as soon as a lower-rank neighbour is accepted, accepted once none of them is
 // pending, else it waits; neighbours of lower passes are already final.  The adjacency of the next passes is loaded
 // while the current one is resolved.  The final statuses go to st_rank (2 bits per candidate, by rank) for finalize.
-__global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, uint32_t* cand, unsigned long long N) {
-    extern __shared__ uint8_t s_st_raw[];                   // kRing + kHead status bytes: 1 pending, 3 accepted, 0 rejected
+__global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, uint32_t* cand, unsigned long long N,
+                                                                 uint32_t ring, uint32_t head) {
+    extern __shared__ uint8_t s_st_raw[];                   // ring + head status bytes: 1 pending, 3 accepted, 0 rejected
     volatile uint8_t* const s_st = s_st_raw;                // read afresh in every look: other warps write them meanwhile
     if (ctl->spacing_slow) return;
     const uint32_t n = ctl->n_cand;
     const AdjView a = adj_view(cand, n, N);
     uint8_t* const st_rank = reinterpret_cast<uint8_t*>(a.st_rank);    // n bytes of the n-word region
     const uint32_t tid = threadIdx.x;
-    constexpr uint32_t kMask = kRing - 1u;
+    const uint32_t kMask = ring - 1u;                       // ring is a power of two >= 2048
     // the next pass's lists (count, offset, first 8 ranks: coalesced) are loaded while this pass is resolved
     uint32_t kB = 0, offB = 0, nbrB[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
     auto load = [&](uint32_t i) {
@@ -372,9 +377,9 @@ __global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, u
         const uint32_t k = kB, off = offB;
         uint32_t slot[8];                                   // ring slot of each neighbour's status
 #pragma unroll
-        for (int e = 0; e < 8; ++e) slot[e] = nbrB[e] < kHead ? kRing + nbrB[e] : (nbrB[e] & kMask);
+        for (int e = 0; e < 8; ++e) slot[e] = nbrB[e] < head ? ring + nbrB[e] : (nbrB[e] & kMask);
         s_st[i & kMask] = 1u;                               // this pass's slots of the ring: all pending
-        if (i < kHead) s_st[kRing + i] = 1u;
+        if (i < head) s_st[ring + i] = 1u;
         load(i + 1024u);                                    // in flight while this pass is resolved
         __syncthreads();
         // every warp keeps looking until its 32 candidates are resolved -- no CTA barrier inside: a link of a chain costs
@@ -394,7 +399,7 @@ __global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, u
                 if (k > 8u && !accepted && !pending) {      // long lists: the rest from the pool (global memory), only once the
                     for (uint32_t e = 8; e < k; ++e) {      // first 8 are all rejected -- a pending one makes the candidate wait anyway
                         const uint32_t r = a.pool[off + e];
-                        const uint32_t sv = s_st[r < kHead ? kRing + r : (r & kMask)];
+                        const uint32_t sv = s_st[r < head ? ring + r : (r & kMask)];
                         accepted = accepted || sv == 3u;
                         pending = pending || sv == 1u;
                     }
@@ -402,7 +407,7 @@ __global__ void __launch_bounds__(1024, 1) k_spacing_resolve_cta(Control* ctl, u
                 if (accepted || !pending) {                 // pending -> rejected (0) / accepted (3)
                     const uint8_t fin = accepted ? 0u : 3u;
                     s_st[i & kMask] = fin;
-                    if (i < kHead) s_st[kRing + i] = fin;
+                    if (i < head) s_st[ring + i] = fin;
                     open = false;
                 }
             }
@@ -575,18 +580,13 @@ cudaError_t launch_spacing(liets_ctx* c, int s) {
     unsigned long long N = c->N;
     k_seed_rows<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->coff, c->rowoff, g);
     c->launches++;
-    k_spacing_adjacency<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->rowoff, c->cand, g, s, N);
+    const uint32_t ring = c->spacing_ring ? c->spacing_ring : kRing, head = c->spacing_ring ? c->spacing_head : kHead;
+    k_spacing_adjacency<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->rowoff, c->cand, g, s, N, ring, head);
     c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    static bool attr_set = false;
-    const int ring_bytes = (int)(kRing + kHead);
-    if (!attr_set) {
-        e = cudaFuncSetAttribute(k_spacing_resolve_cta, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_bytes);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
-    k_spacing_resolve_cta<<<1, 1024, ring_bytes, c->stream>>>(c->ctl, c->cand, N);
+    const int ring_bytes = (int)(ring + head);
+    k_spacing_resolve_cta<<<1, 1024, ring_bytes, c->stream>>>(c->ctl, c->cand, N, ring, head);
     c->launches++;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -601,6 +601,11 @@ cudaError_t launch_spacing(liets_ctx* c, int s) {
     e = cudaLaunchCooperativeKernel((const void*)k_spacing_resolve, dim3(c->resolve_grid), dim3(1024), args, 0, c->stream);
     c->launches++;
     return e;
+}
+
+// per-device function attributes, set once per context at liets_create (they are per device, not per process)
+cudaError_t seed_kernel_attributes() {
+    return cudaFuncSetAttribute(k_spacing_resolve_cta, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kRing + kHead));
 }
 
 cudaError_t launch_seed_finalize(liets_ctx* c, int spaced) {

@@ -17,7 +17,9 @@ FORMAT_U8, FORMAT_BITS = 0, 1
 # every symbol include/liets.h declares
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
            "liets_set_target", "liets_step", "liets_generate", "liets_grid", "liets_step_log", "liets_timings",
-           "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_destroy", "liets_last_error")
+           "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info",
+           "liets_debug_spacing_ring", "liets_probe", "liets_destroy", "liets_last_error")
+PROBE_PHILOX, PROBE_LOP3, PROBE_IMAD, PROBE_MIX, PROBE_L2_READ, PROBE_HBM_READ = range(6)
 
 
 class LietsError(RuntimeError):
@@ -73,12 +75,30 @@ def lib():
     L.liets_step_times.restype = ci
     L.liets_launch_count.argtypes = [vp]
     L.liets_launch_count.restype = u64
+    L.liets_seed_info.argtypes = [vp, P(u32), P(u32)]
+    L.liets_seed_info.restype = ci
+    L.liets_debug_spacing_ring.argtypes = [vp, u32, u32]
+    L.liets_debug_spacing_ring.restype = ci
+    L.liets_probe.argtypes = [ci, vp, sz, vp, ci, P(dbl), P(dbl)]
+    L.liets_probe.restype = ci
     L.liets_destroy.argtypes = [vp]
     L.liets_destroy.restype = None
     L.liets_last_error.argtypes = [vp]
     L.liets_last_error.restype = ctypes.c_char_p
     _lib = L
     return L
+
+
+def probe(kind, scratch, reps=5, stream=None):
+    """liets_probe on a torch uint8 CUDA tensor `scratch`: (units per second, milliseconds of the best launch)."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(scratch.device)
+    ups, ms = ctypes.c_double(0), ctypes.c_double(0)
+    rc = lib().liets_probe(kind, ctypes.c_void_p(scratch.data_ptr()), scratch.numel(), ctypes.c_void_p(st.cuda_stream),
+                           reps, ctypes.byref(ups), ctypes.byref(ms))
+    if rc < 0:
+        raise LietsError(rc, "liets_probe failed")
+    return float(ups.value), float(ms.value)
 
 
 class Liets:
@@ -188,6 +208,15 @@ class Liets:
         ms = (ctypes.c_float * cap)()
         n = self._check(self._L.liets_step_times(self._h, ms, cap))
         return np.array(ms[:n], dtype=np.float64)
+
+    def seed_info(self):
+        """(keyed candidates before spacing, 1 if the spacing took the rescan slow path)."""
+        n, slow = ctypes.c_uint32(0), ctypes.c_uint32(0)
+        self._check(self._L.liets_seed_info(self._h, ctypes.byref(n), ctypes.byref(slow)))
+        return int(n.value), int(slow.value)
+
+    def debug_spacing_ring(self, ring, head):
+        self._check(self._L.liets_debug_spacing_ring(self._h, ring, head))
 
     @property
     def launch_count(self):

@@ -5,8 +5,15 @@ the target and records the seed count, step count, final solid count and the SHA
 phase array (N bytes, x fastest).  The GPU tests compare the CUDA path's outputs with these.
 
     python tests/golden/make_fullsize_hashes.py cfg3_400 --target 0.80 [--seed 7] [--s 20]
+    python tests/golden/make_fullsize_hashes.py cfg5_1024 --seeds-only          # seeding + spacing only
+    python tests/golden/make_fullsize_hashes.py cfg5_1024 --target 0.80 --trace --hash-every 4
 
-Each run appends one JSON line; runs take minutes to hours of one CPU core (serial oracle).
+Each run appends one JSON line to fullsize_hashes.jsonl; runs take minutes to hours of one CPU core
+(serial oracle).  --seeds-only records the seed count and the SHA-256 of the grid right after seeding
+(kind "seeds").  --trace runs the same generation one step at a time (oracle_generate with max_steps = 1,
+which is the loop of PAPER.md:140 cut after every pass) and appends to fullsize_traces.jsonl, after
+EVERY step, the step index and solid count, plus the SHA-256 of the phase array every --hash-every
+steps: a run that is interrupted still leaves every completed step as an expected value.
 """
 import argparse
 import hashlib
@@ -22,12 +29,21 @@ import oracle  # noqa: E402
 from workloads import CONFIGS  # noqa: E402
 
 OUT = os.path.join(os.path.dirname(os.path.abspath(__file__)), "fullsize_hashes.jsonl")
+TRACE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "fullsize_traces.jsonl")
+
+
+def append(path, rec):
+    with open(path, "a") as f:
+        f.write(json.dumps(rec) + "\n")
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("config")
-    ap.add_argument("--target", type=float, required=True)
+    ap.add_argument("--target", type=float, default=None)
+    ap.add_argument("--seeds-only", action="store_true")
+    ap.add_argument("--trace", action="store_true")
+    ap.add_argument("--hash-every", type=int, default=4)
     ap.add_argument("--seed", type=int, default=None)
     ap.add_argument("--s", type=int, default=None)
     a = ap.parse_args()
@@ -40,13 +56,36 @@ def main():
     o.set_growth(*c["g"], 1)
     n_seeds = o.seed(c["core"], s, seed)
     t_seed = time.time() - t0
-    rc, steps = o.generate(a.target, 10**6, True)
+    base = dict(config=a.config, dims=[nx, ny, nz], periodic=c["periodic"], core=c["core"], s=s, rng_seed=seed,
+                g=list(c["g"]))
+    if a.seeds_only:
+        h = hashlib.sha256(o.grid().tobytes()).hexdigest()
+        rec = dict(base, kind="seeds", n_seeds=n_seeds, sha256=h, oracle_seconds=round(time.time() - t0, 1))
+        append(OUT, rec)
+        print(rec)
+        return
+    if a.target is None:
+        ap.error("--target is required unless --seeds-only")
+    if a.trace:
+        steps, rc = 0, oracle.MAX_STEPS
+        while rc == oracle.MAX_STEPS:
+            rc, done = o.generate(a.target, 1, True)
+            steps += done
+            if not done:
+                break
+            rec = dict(base, kind="trace", target=a.target, n_target=o.n_target, n_seeds=n_seeds, step=steps,
+                       n_solid=o.n_solid, oracle_seconds=round(time.time() - t0, 1))
+            if steps % a.hash_every == 0 or rc != oracle.MAX_STEPS:
+                rec["sha256"] = hashlib.sha256(o.grid().tobytes()).hexdigest()
+            append(TRACE, rec)
+            print(rec, flush=True)
+    else:
+        rc, steps = o.generate(a.target, 10**6, True)
     h = hashlib.sha256(o.grid().tobytes()).hexdigest()
     rec = dict(config=a.config, dims=[nx, ny, nz], periodic=c["periodic"], core=c["core"], s=s, rng_seed=seed,
                g=list(c["g"]), target=a.target, n_target=o.n_target, n_seeds=n_seeds, status=rc, steps=steps,
                n_solid=o.n_solid, sha256=h, oracle_seconds=round(time.time() - t0, 1), seed_seconds=round(t_seed, 1))
-    with open(OUT, "a") as f:
-        f.write(json.dumps(rec) + "\n")
+    append(OUT, rec)
     print(rec)
 
 

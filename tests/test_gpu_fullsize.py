@@ -18,16 +18,30 @@ from workloads import CONFIGS
 pytestmark = pytest.mark.gpu
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "fullsize_hashes.jsonl")
+TRACES = os.path.join(os.path.dirname(__file__), "golden", "fullsize_traces.jsonl")
 
 
-def records():
-    if not os.path.exists(GOLDEN):
+def read_jsonl(path):
+    if not os.path.exists(path):
         return []
-    return [json.loads(l) for l in open(GOLDEN) if l.strip()]
+    return [json.loads(l) for l in open(path) if l.strip()]
+
+
+def records(kind=None):
+    return [r for r in read_jsonl(GOLDEN) if r.get("kind") == kind]
 
 
 def ident(r):
-    return "%s-s%d-seed%d-phi%.2f" % (r["config"], r["s"], r["rng_seed"], r["target"])
+    return "%s-s%d-seed%d" % (r["config"], r["s"], r["rng_seed"]) + ("-phi%.2f" % r["target"] if "target" in r else "")
+
+
+def traces():
+    """Per-step traces (make_fullsize_hashes.py --trace), grouped by run: [(key record, [step records])]."""
+    runs = {}
+    for r in read_jsonl(TRACES):
+        key = (r["config"], r["s"], r["rng_seed"], r["target"])
+        runs.setdefault(key, []).append(r)
+    return [(v[0], sorted(v, key=lambda r: r["step"])) for v in runs.values()]
 
 
 @pytest.fixture(scope="module")
@@ -37,6 +51,49 @@ def liets():
         pytest.fail("gpu tests need a CUDA device")
     import paper_2602_11734_b200 as m
     return m
+
+
+@pytest.mark.parametrize("rec", records("seeds"), ids=ident)
+def test_fullsize_seeds_match_oracle_hash(liets, rec):
+    """Seeding + spacing alone at full size (config 5: 2.15e5 candidates, the only config whose ranks exceed the
+    2^17-rank status ring of the spacing resolve): seed count and SHA-256 of the grid right after liets_seed."""
+    nx, ny, nz = rec["dims"]
+    L = liets.Liets(nx, ny, nz, int(rec["periodic"]), 1)
+    assert L.seed(rec["core"], rec["s"], rec["rng_seed"]) == rec["n_seeds"]
+    n_cand, slow = L.seed_info()
+    g = L.grid()
+    assert int(g.sum(dtype=np.uint64)) == rec["n_seeds"]
+    assert hashlib.sha256(g.tobytes()).hexdigest() == rec["sha256"], "candidates %d, slow path %d" % (n_cand, slow)
+    L.close()
+
+
+@pytest.mark.parametrize("run", traces(), ids=lambda t: ident(t[0]) + "-trace")
+def test_fullsize_trace_matches_oracle_step_by_step(liets, run):
+    """Whole-run parity step by step (config 5 at 1024^3: a run of about ten CPU-hours of the serial oracle, recorded
+    one step at a time so that every completed step is an expected value): the solid count after EVERY recorded step
+    and the SHA-256 of the phase array at every step that carries one."""
+    head, steps = run
+    nx, ny, nz = head["dims"]
+    L = liets.Liets(nx, ny, nz, int(head["periodic"]), 1)
+    L.set_growth(*head["g"], liets.LAW_EQ1)
+    assert L.seed(head["core"], head["s"], head["rng_seed"]) == head["n_seeds"]
+    done = 0
+    hashed = [r for r in steps if "sha256" in r]
+    if nx * ny * nz > 2 * 10**8:                     # 1 GiB per hash: the last three recorded hashes only
+        hashed = hashed[-3:]
+    for r in hashed:
+        rc, n, n_solid = L.generate(head["target"], r["step"] - done)
+        done += n
+        assert done == r["step"] and n_solid == r["n_solid"]
+        assert hashlib.sha256(L.grid().tobytes()).hexdigest() == r["sha256"], "step %d" % r["step"]
+    last = steps[-1]
+    rc, n, n_solid = L.generate(head["target"], last["step"] - done)
+    done += n
+    front, solid_after, blocks = L.step_log()
+    assert done == last["step"] and len(solid_after) >= done
+    for r in steps:                                   # every recorded step's solid count
+        assert int(solid_after[r["step"] - 1]) == r["n_solid"], "step %d" % r["step"]
+    L.close()
 
 
 @pytest.mark.parametrize("rec", records(), ids=ident)

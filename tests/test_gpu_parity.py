@@ -60,6 +60,32 @@ def test_ragged_shapes_bit_exact(liets, storage, periodic, dims, core, s):
     run_both(liets, dims, periodic, core, s, 5, (0.05, 0.02, 0.01), 1, 0.55, storage)
 
 
+@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("s,expect_slow", [(5, 0), (8, 1), (6, None)])
+def test_spacing_ring_wrap_and_head_table(liets, periodic, s, expect_slow):
+    """The single-CTA spacing resolve keeps one status byte per candidate in a shared-memory ring (2^17 ranks, plus the
+    first 2^16 ranks for the periodic wrap).  No BASELINE config below 1024^3 has that many candidates, so the test
+    shrinks the ring to 2048 ranks and the head to 1024 (liets_debug_spacing_ring): 8192 candidates wrap it four
+    times.  s = 5: every neighbour is < 1024 ranks back -> adjacency-list path; s = 8: neighbours fall in the last 1023
+    ranks below the ring size, whose slots the resolve re-arms within the same pass -> must be sent to the rescan path
+    (the fit test compares against the END of the pass).  The accepted seeds equal the oracle's either way."""
+    dims, core, seed = (96, 96, 48), 0.02, 21                  # 184 candidates per z-slice, about 8800 in all
+    o = oracle.Oracle(*dims, periodic)
+    n_o = o.seed(core, s, seed)
+    L = liets.Liets(*dims, int(periodic), 1)
+    L.debug_spacing_ring(2048, 1024)
+    assert L.seed(core, s, seed) == n_o
+    n_cand, slow = L.seed_info()
+    assert n_cand > 3 * 2048
+    if expect_slow is not None:
+        assert slow == expect_slow
+    assert (L.grid() == o.grid()).all()
+    L.debug_spacing_ring(0, 0)                                  # built-in sizes: same seeds
+    assert L.seed(core, s, seed) == n_o and L.seed_info()[1] == 0
+    assert (L.grid() == o.grid()).all()
+    L.close()
+
+
 @pytest.mark.parametrize("storage", STORAGES)
 @pytest.mark.parametrize("periodic", [False, True])
 def test_dense_front_bit_exact(liets, storage, periodic):
