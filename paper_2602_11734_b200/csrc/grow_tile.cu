@@ -10,16 +10,18 @@
 //
 // One CTA owns one tile at a time (tiles are handed out through an atomic cursor):
 //   A  gather: the 10 x 10 rows of the tile's one-voxel neighbourhood, kTileW + 2 words each, as "not void"
-//      bits (solid, outside the domain, or padding), plus a copy in overlapping 32-bit windows so that
-//      any three x-adjacent bits come from one word (at a shift of 1..29, done as a multiply)
+//      bits (solid, outside the domain, or padding), kept as 18-bit windows at a stride of 16 voxels (window k of a
+//      row = tile bits 16k-1 .. 16k+16 in word bits 14..31), so that the three x-neighbours of any voxel come out of
+//      ONE word by a left shift of 15 - (x & 15), plus the x part of the front test per row
 //   B  front voxels: solid cells with a void neighbour, 64 cells per bit operation;
-//      their ids are compacted into a shared-memory list (popc + CTA-wide prefix sum)
-//   C  one thread per front voxel: its 26 void-target bits (Algorithm 3 lines 5-6) from nine window
-//      loads, ONE Philox4x32-10 block = the leading nibble of all 26 draws (R9), one carry-free
-//      per-nibble compare = the directions that fire or tie with the threshold (line 8); voxels with ties go
-//      to a per-warp queue
-//   D  one lane per queued voxel: the next blocks until no direction ties
-//      hits of C and D set bits in a shared-memory claim volume (atomicOr)
+//      their ids are compacted into a shared-memory list (popc + CTA-wide prefix sum).  A list entry is
+//      (15 - (x & 15)) | (8 row + x / 16) << 4: the shift count and the window index, ready to use
+//   C  one thread per front voxel: its 26 void-target bits (Algorithm 3 lines 5-6) from nine window loads, each
+//      aligned by one multiply and pushed into the mask by one funnel shift; ONE Philox4x32-10 block = the
+//      leading nibble of all 26 draws (R9), one carry-free per-nibble compare = the directions that fire or tie
+//      with the threshold (line 8); voxels with hits or ties go to a per-warp queue
+//   D  one lane per queued voxel: its hits are set in a shared-memory claim volume (atomicOr); for tied
+//      directions the next block decides, one direction at a time (there is almost always exactly one)
 //   E  claim + compact: own rows are OR-ed into G[next] together with the carried state, halo hits
 //      go to the neighbour tiles' rows with atomicOr; the returned old word tells who flipped the bit
 //      (line 9-10, "counted once" PAPER.md:77) for the solid count; a per-tile step stamp
@@ -35,23 +37,23 @@ constexpr int kTileW = 2;                       // 64-bit words per tile row
 constexpr int kThreads = 128;
 constexpr int kWarps = kThreads / 32;
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
-constexpr int kWin = (64 * kTileW - 1) / 29 + 1;   // 32-bit windows per row; window k starts at tile bit 29 k - 2
-constexpr int kQueueCap = 256;                  // voxels with ties per warp queue
+constexpr int kWin = 64 * kTileW / 16;          // 18-bit windows per row, one per 16 voxels
+constexpr int kQueueCap = 128;                  // voxels with hits or ties per warp queue
 constexpr int kHeavyFront = 64 * 64 * kTileW / 8;  // a tile with at least this many front voxels (1/8 of its cells) is "heavy"
 constexpr int kFrontCap = 32 * 64 * kTileW;     // front voxels listed at a time (half the tile; more -> several passes)
 
 struct Smem {
-    unsigned long long nv[100][kRowWords];      // not-void bits, row (z'+1)*10 + (y'+1)
-    uint32_t win[100][kWin];                    // the same rows as overlapping windows
+    uint32_t win[100 * kWin];                   // row (z'+1)*10 + (y'+1), window k: not-void bits of tile x = 16k-1 .. 16k+16 at bits 14..31
     unsigned long long vx[100][kTileW];         // per tile word: cells with a void cell at x-1, x or x+1 in the same row
-    uint32_t claims[100][2 * kRowWords];        // cells claimed in this step, same geometry as nv (32-bit view)
-    uint32_t queue[kWarps][2 * kQueueCap];      // (voxel id | nibble level << 14, tied directions)
+    unsigned long long own[64][kTileW];         // the tile's own not-void words (row y + 8 z)
+    uint32_t claims[100][2 * kRowWords];        // cells claimed in this step: row as in win, bit 64 + x of the row (32-bit view)
+    uint32_t queue[kWarps][3 * kQueueCap];      // (list entry | nibble level << 16, tied directions, firing directions)
     uint32_t hpat[8][4];
-    uint32_t dir[28];                           // direction d: (row delta + 11) | (dx + 1) << 8
-    uint32_t scan[33];
+    uint32_t dir[28];                           // direction d: claim-word offset 8 (10 dz + dy + 11) | (dx + 1) << 16
+    uint32_t ptab[100];                         // voxel index of tile x = 0 of each own row
     uint32_t tile[2], tile_id[2];               // list entry handed to the CTA, double-buffered by tile parity
     uint32_t wsum[2][kWarps];                   // per-warp front-voxel counts, double-buffered
-    uint16_t flist[kFrontCap];                  // x | (y | z << 3) << 8 of the tile's front voxels (x relative to the tile)
+    uint16_t flist[kFrontCap];                  // (15 - (x & 15)) | (8 row + x / 16) << 4 of the tile's front voxels
 };
 
 struct TileCoord {
@@ -107,6 +109,12 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
     return v;
 }
+template <int OFF>
+__device__ __forceinline__ uint32_t lds_u32_at(uint32_t addr) {            // [addr + OFF], OFF >= 0 an immediate
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(addr), "n"(OFF) : "memory");
+    return v;
+}
 __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v) {
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
@@ -149,11 +157,14 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         const int d = tid < 26 ? (int)tid : 25;
         const int raw = d + (d >= 13 ? 1 : 0);
         const int dx = raw % 3 - 1, dy = (raw / 3) % 3 - 1, dz = raw / 9 - 1;
-        S.dir[tid] = (uint32_t)(dz * 10 + dy + 11) | ((uint32_t)(dx + 1) << 8);
+        S.dir[tid] = (uint32_t)(2 * kRowWords * (dz * 10 + dy + 11)) | ((uint32_t)(dx + 1) << 16);
     }
     const uint32_t en26 = ctl->en26;
     const bool h0_any = ctl->h0_any != 0u;
     const uint32_t h0[4] = { ctl->hpat[0][0], ctl->hpat[0][1], ctl->hpat[0][2], ctl->hpat[0][3] };
+    constexpr uint32_t kM8 = 0x88888888u;
+    const uint32_t h0m[4] = { h0[0] & kM8, h0[1] & kM8, h0[2] & kM8, h0[3] & kM8 };     // level-0 compare: uniform parts
+    const uint32_t h08[4] = { h0[0] | kM8, h0[1] | kM8, h0[2] | kM8, h0[3] | kM8 };
     uint32_t new_solid = 0;                 // per thread: bits this thread flipped 0 -> 1
     uint32_t n_items = 0, n_items0 = 0;     // per thread: Philox blocks evaluated, front voxels with a void target
     // shared-window address of the voxel list, kept in a register: left to itself the compiler rebuilds it (S2R
@@ -161,6 +172,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
     const uint32_t flist_addr = opaque_shared_addr(S.flist), win_addr = opaque_shared_addr(S.win);
     const uint32_t claims_addr = opaque_shared_addr(S.claims), queue_addr = opaque_shared_addr(S.queue[warp]);
     const uint32_t hpat_addr = opaque_shared_addr(S.hpat), dir_addr = opaque_shared_addr(S.dir);
+    const uint32_t ptab_addr = opaque_shared_addr(S.ptab);
 
     uint32_t next_li = 0, next_id = 0;      // thread 0: the list entry fetched ahead
     if (tid == 0) {
@@ -181,28 +193,37 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         const TileCoord tc = tile_coord(id, g);
 
         // ---- A: gather ------------------------------------------------------------------------
+        const uint32_t p0 = (uint32_t)(64 * tc.w0) + (uint32_t)g.nx * ((uint32_t)tc.y0 + (uint32_t)g.ny * (uint32_t)tc.z0);
         for (int r = (int)tid; r < 100; r += kThreads) {    // one thread per row: the row's address once, its words as independent loads
-            const int zg = row_coord(r / 10 - 1, tc.z0, tc.wcz, g.nz, g.periodic);
-            const int yg = row_coord(r % 10 - 1, tc.y0, tc.wcy, g.ny, g.periodic);
+            const int zl = r / 10 - 1, yl = r % 10 - 1;
+            const int zg = row_coord(zl, tc.z0, tc.wcz, g.nz, g.periodic);
+            const int yg = row_coord(yl, tc.y0, tc.wcy, g.ny, g.periodic);
             const bool ok = zg >= 0 && yg >= 0;
             const unsigned long long row_base = ok ? (unsigned long long)g.Wp * ((unsigned long long)yg + (unsigned long long)g.ny * (unsigned long long)zg) : 0ull;
             unsigned long long w[kRowWords];
 #pragma unroll
             for (int c = 0; c < kRowWords; ++c) w[c] = not_void_word(Gc, g, ok, row_base, tc.w0 + c - 1);
+            if (zl >= 0 && zl < 8 && yl >= 0 && yl < 8) {           // an own row: its words for B and E, its first voxel's index
 #pragma unroll
-            for (int c = 0; c < kRowWords; ++c) S.nv[r][c] = w[c];
+                for (int j = 0; j < kTileW; ++j) S.own[zl * 8 + yl][j] = w[1 + j];
+                S.ptab[r] = p0 + (uint32_t)g.nx * ((uint32_t)yl + (uint32_t)g.ny * (uint32_t)zl);
+            }
 #pragma unroll
             for (int j = 0; j < kTileW; ++j) {                      // void at x-1, x or x+1 (the x part of the 3x3x3 dilation)
                 const unsigned long long v = ~w[1 + j];
                 S.vx[r][j] = v | (v << 1) | (~w[j] >> 63) | (v >> 1) | (~w[2 + j] << 63);
             }
 #pragma unroll
-            for (int k = 0; k < kWin; ++k) {                        // window k: 32 row bits from tile x = 29 k - 2
-                constexpr int kFirst = 62;
-                const int pos = kFirst + 29 * k, wd = pos >> 6, sh = pos & 63;
-                unsigned long long v = w[wd] >> sh;
-                if (sh > 32 && wd + 1 < kRowWords) v |= w[wd + 1] << (64 - sh);
-                S.win[r][k] = (uint32_t)v;
+            for (int k = 0; k < kWin; k += 4) {                     // window k: row bits 63 + 16 k .. 80 + 16 k (tile x = 16k-1 .. 16k+16) at bits 14..31
+                uint32_t wv[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int pos = 63 + 16 * (k + q), wd = pos >> 6, sh = pos & 63;
+                    unsigned long long v = w[wd] >> sh;
+                    if (sh + 18 > 64) v |= w[wd + 1] << (64 - sh);
+                    wv[q] = (uint32_t)v << 14;
+                }
+                *reinterpret_cast<uint4*>(&S.win[r * kWin + k]) = make_uint4(wv[0], wv[1], wv[2], wv[3]);
             }
         }
         for (int q = (int)tid; q < 100 * 2 * kRowWords / 4; q += kThreads)
@@ -217,7 +238,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
             const int y = f_row & 7, z = f_row >> 3;
             const int xbase = 64 * (tc.w0 + f_j);
             if (y < tc.wcy && z < tc.wcz && xbase < g.nx) {
-                unsigned long long src = S.nv[(z + 1) * 10 + (y + 1)][1 + f_j];
+                unsigned long long src = S.own[f_row][f_j];
                 if (xbase + 64 > g.nx) src &= ~(~0ull << (g.nx - xbase));               // padding is not a source
                 if (src) {                                                              // (sparse early steps: most words hold no solid)
                     unsigned long long anyvoid = 0ull;
@@ -240,45 +261,54 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                 if ((uint32_t)q < warp) off0 += v;
             }
         }
-        const uint32_t p0 = (uint32_t)(64 * tc.w0) + (uint32_t)g.nx * ((uint32_t)tc.y0 + (uint32_t)g.ny * (uint32_t)tc.z0);
 
         // ---- C + D -----------------------------------------------------------------------------------
-        auto claim = [&](uint32_t fire, uint32_t x, uint32_t zy) {
+        // the hits of voxel (x, row rr): bits of the claim volume
+        auto claim = [&](uint32_t fire, uint32_t x, uint32_t rr) {
+            const uint32_t cbase = claims_addr + 4u * (2u * kRowWords) * (rr - 11u);
             while (fire) {
-                const uint32_t d = __ffs(fire) - 1u;
-                fire &= fire - 1u;
+                const uint32_t d = 31u - __clz(fire);
+                fire ^= 1u << d;
                 const uint32_t lut = lds_u32(dir_addr + 4u * d);
-                const uint32_t xb = x + 63u + (lut >> 8);           // bit of the row: 64 + x + dx
-                atoms_or_u32(claims_addr + 4u * ((zy + (lut & 0xFFu)) * (2u * kRowWords) + (xb >> 5)), 1u << (xb & 31u));
+                const uint32_t xb = x + 63u + (lut >> 16);          // bit of the row: 64 + x + dx
+                atoms_or_u32(cbase + 4u * ((lut & 0xFFFFu) + (xb >> 5)), 1u << (xb & 31u));
             }
         };
         uint32_t qn = 0;                    // queue fill (warp-uniform)
-        auto drain = [&]() {                // D: one lane per queued voxel, one nibble level per visit
+        auto drain = [&]() {                // D: one lane per queued voxel: its hits, then one nibble level of its ties
             __syncwarp();
             uint32_t wpos = 0;              // entries that still tie are queued again, one level deeper
             for (uint32_t j0 = 0; j0 < qn; j0 += 32u) {
                 const uint32_t j = j0 + lane;
-                uint32_t v = 0, tie = 0, still = 0;
-                if (j < qn) { v = lds_u32(queue_addr + 8u * j); tie = lds_u32(queue_addr + 8u * j + 4u); }
+                uint32_t vk = 0, tie = 0, fire = 0, still = 0;
+                if (j < qn) { vk = lds_u32(queue_addr + 12u * j); tie = lds_u32(queue_addr + 12u * j + 4u); fire = lds_u32(queue_addr + 12u * j + 8u); }
                 __syncwarp();               // this round's entries are read before any slot is written again
-                if (tie) {
-                    const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = (v >> 11) & 7u, k = v >> 14;
-                    const uint32_t p = p0 + x + (uint32_t)g.nx * (y + (uint32_t)g.ny * z);
-                    const uint4 B = philox4x32_10(p, 0u, t, k, key);
-                    ++n_items;
-                    uint32_t le, eq;
-                    const uint32_t hk[4] = { lds_u32(hpat_addr + 16u * k), lds_u32(hpat_addr + 16u * k + 4u),
-                                             lds_u32(hpat_addr + 16u * k + 8u), lds_u32(hpat_addr + 16u * k + 12u) };
-                    level_compare(B, hk, tie, &le, &eq);
-                    const uint32_t fire = k < 7u ? (le & ~eq) : le;        // last nibble: draw <= U
-                    still = k < 7u ? eq : 0u;
-                    claim(fire, x, 10u * z + y);
+                if (tie | fire) {
+                    const uint32_t x = (vk & 0x7Fu) ^ 15u, rr = (vk >> 7) & 0x1FFu, k = vk >> 16;
+                    if (tie) {
+                        const uint32_t p = lds_u32(ptab_addr + 4u * rr) + x;
+                        const uint4 B = philox4x32_10(p, 0u, t, k, key);
+                        ++n_items;
+                        const uint32_t last = k == 7u ? 1u : 0u;                // last nibble: draw <= U
+                        do {                // one tied direction at a time: nibble k of its draw against the threshold's
+                            const uint32_t d = 31u - __clz(tie), bit = 1u << d;
+                            tie ^= bit;
+                            const uint32_t lo = (d & 1u) ? B.y : B.x, hi = (d & 1u) ? B.w : B.z;
+                            const uint32_t sh = d & 28u;
+                            const uint32_t a = (((d & 2u) ? hi : lo) >> sh) & 15u;
+                            const uint32_t h = (lds_u32(hpat_addr + 16u * k + 4u * (d & 3u)) >> sh) & 15u;
+                            if (a < h + last) fire |= bit;
+                            else if (a == h) still |= bit;
+                        } while (tie);
+                    }
+                    claim(fire, x, rr);
                 }
                 const uint32_t have = __ballot_sync(0xffffffffu, still != 0u);
                 if (still) {
                     const uint32_t slot = wpos + __popc(have & ((1u << lane) - 1u));
-                    sts_u32(queue_addr + 8u * slot, v + (1u << 14));
-                    sts_u32(queue_addr + 8u * slot + 4u, still);
+                    sts_u32(queue_addr + 12u * slot, vk + (1u << 16));
+                    sts_u32(queue_addr + 12u * slot + 4u, still);
+                    sts_u32(queue_addr + 12u * slot + 8u, 0u);
                 }
                 wpos += __popc(have);
             }
@@ -287,77 +317,84 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         };
         for (uint32_t pass0 = 0; pass0 < n_front; pass0 += (uint32_t)kFrontCap) {   // almost always a single pass
             if (pass0) __syncthreads();     // the previous pass no longer reads the list
-            if (n_front <= (uint32_t)kFrontCap) {       // the usual case, one pass: no capacity test, the address just advances
-                uint32_t addr = flist_addr + 2u * off0;
-                const uint32_t hi = ((uint32_t)f_row << 8) | (uint32_t)(64 * f_j);
+            {
+                // entry of bit b of half h of this thread's word: ((8 rr + 4 j + 2 h + b / 16) << 4) | (15 - b % 16) = base_h ^ b
+                const uint32_t rr = (uint32_t)((f_row >> 3) + 1) * 10u + (uint32_t)(f_row & 7) + 1u;
+                const uint32_t base = ((8u * rr + 4u * (uint32_t)f_j) << 4) | 15u;
+                if (n_front <= (uint32_t)kFrontCap) {   // the usual case, one pass: no capacity test, the address just advances
+                    uint32_t addr = flist_addr + 2u * off0;
 #pragma unroll
-                for (int half = 1; half >= 0; --half) {             // highest bit first: one FLO per voxel
-                    const uint32_t hh = hi | (uint32_t)(32 * half);
-                    for (uint32_t m = (uint32_t)(F >> (32 * half)); m; addr += 2u) {
-                        const uint32_t b = 31u - __clz(m);
-                        m ^= 1u << b;
-                        asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((uint16_t)(hh | b)) : "memory");
+                    for (int half = 1; half >= 0; --half) {         // highest bit first: one FLO per voxel
+                        const uint32_t hh = base | (uint32_t)(32 * half);
+                        for (uint32_t m = (uint32_t)(F >> (32 * half)); m; addr += 2u) {
+                            const uint32_t b = 31u - __clz(m);
+                            m ^= 1u << b;
+                            asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((uint16_t)(hh ^ b)) : "memory");
+                        }
                     }
-                }
-            } else {                        // list the front voxels pass0 .. pass0 + kFrontCap - 1
-                uint32_t off = off0;
-                const uint32_t hi = ((uint32_t)f_row << 8) | (uint32_t)(64 * f_j);
+                } else {                    // list the front voxels pass0 .. pass0 + kFrontCap - 1
+                    uint32_t off = off0;
 #pragma unroll
-                for (int half = 1; half >= 0; --half) {
-                    const uint32_t hh = hi | (uint32_t)(32 * half);
-                    for (uint32_t m = (uint32_t)(F >> (32 * half)); m; ++off) {
-                        const uint32_t b = 31u - __clz(m);
-                        m ^= 1u << b;
-                        if (off - pass0 < (uint32_t)kFrontCap)
-                            asm volatile("st.shared.u16 [%0], %1;" ::"r"(flist_addr + 2u * (off - pass0)), "h"((uint16_t)(hh | b)) : "memory");
+                    for (int half = 1; half >= 0; --half) {
+                        const uint32_t hh = base | (uint32_t)(32 * half);
+                        for (uint32_t m = (uint32_t)(F >> (32 * half)); m; ++off) {
+                            const uint32_t b = 31u - __clz(m);
+                            m ^= 1u << b;
+                            if (off - pass0 < (uint32_t)kFrontCap)
+                                asm volatile("st.shared.u16 [%0], %1;" ::"r"(flist_addr + 2u * (off - pass0)), "h"((uint16_t)(hh ^ b)) : "memory");
+                        }
                     }
                 }
             }
             __syncthreads();                // flist (and win) complete
             const uint32_t n_pass = min((uint32_t)kFrontCap, n_front - pass0);
-        for (uint32_t i0 = 0; i0 < n_pass; i0 += kThreads) {       // C: one thread per front voxel
-            const uint32_t i = i0 + tid;
-            uint32_t tie = 0, v = 0;
-            if (i < n_pass) {
-                {
-                    uint16_t v16;
-                    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v16) : "r"(flist_addr + 2u * i) : "memory");
-                    v = v16;
-                }
-                const uint32_t x = v & 255u, y = (v >> 8) & 7u, z = v >> 11;
-                const uint32_t k = (x * 2260u) >> 16;                       // x / 29: window k holds tile bits 29k-2 .. 29k+29
-                const uint32_t shr = 1u << (31u + 29u * k - x);            // umulhi(w, shr) = w >> (x - 29k + 1): a shift on the FMA pipe
-                uint32_t nb27 = 0;          // bit 9(dz+1) + 3(dy+1) + (dx+1): that neighbour is not void
-                const uint32_t wrow = win_addr + 4u * (kWin * (z * 10u + y) + k);
-#pragma unroll
-                for (int e = 0; e < 9; ++e)
-                    nb27 |= (__umulhi(lds_u32(wrow + 4u * kWin * (uint32_t)((e / 3) * 10 + e % 3)), shr) & 7u) << (3 * e);
-                const uint32_t void27 = ~nb27;
-                const uint32_t void26 = ((void27 & 0x1FFFu) | ((void27 >> 14) << 13)) & en26;
-                if (void26) {
-                    const uint32_t p = p0 + x + (uint32_t)g.nx * (y + (uint32_t)g.ny * z);
-                    const uint4 B0 = philox4x32_10(p, 0u, t, 0u, key);
-                    ++n_items0;
-                    if (h0_any) {           // some leading threshold nibble is non-zero: a draw can fire at level 0
-                        uint32_t le;
-                        level_compare(B0, h0, void26, &le, &tie);
-                        claim(le & ~tie, x, 10u * z + y);
-                    } else {                // all leading nibbles are 0: "<=" and "==" coincide with "== 0"
-                        tie = level_zero(B0, void26);
+            for (uint32_t i0 = 0; i0 < n_pass; i0 += kThreads) {   // C: one thread per front voxel
+                const uint32_t i = i0 + tid;
+                uint32_t tie = 0, fire = 0, v = 0;
+                if (i < n_pass) {
+                    {
+                        uint16_t v16;
+                        asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v16) : "r"(flist_addr + 2u * i) : "memory");
+                        v = v16;
+                    }
+                    // the nine rows of the neighbourhood: one window each, aligned so that x+1, x, x-1 are bits 31..29, pushed
+                    // into the mask three bits at a time (row dz = +1, dy = +1 first): bit 9(dz+1) + 3(dy+1) + (dx+1) = not void
+                    const uint32_t wa = win_addr + ((v >> 2) & 0xFFFCu) - 4u * kWin * 11u;
+                    const uint32_t mult = 1u << (v & 15u);
+                    uint32_t nb27 = 0;
+#define LIETS_ROW(E) nb27 = __funnelshift_l(lds_u32_at<4 * kWin * (((E) / 3) * 10 + (E) % 3)>(wa) * mult, nb27, 3)
+                    LIETS_ROW(8); LIETS_ROW(7); LIETS_ROW(6); LIETS_ROW(5); LIETS_ROW(4); LIETS_ROW(3); LIETS_ROW(2); LIETS_ROW(1); LIETS_ROW(0);
+#undef LIETS_ROW
+                    // the centre (bit 13) is solid, so ~nb27 has bit 13 clear: closing the gap is (v + (v & 0x1FFF)) >> 1
+                    const uint32_t lo13 = ~nb27 & 0x1FFFu;
+                    const uint32_t void26 = ((~nb27 + lo13) >> 1) & en26;
+                    if (void26) {
+                        const uint32_t x = (v & 0x7Fu) ^ 15u;
+                        const uint32_t p = lds_u32(ptab_addr + ((v >> 5) & 0x3FCu)) + x;
+                        const uint4 B0 = philox4x32_10(p, 0u, t, 0u, key);
+                        ++n_items0;
+                        if (h0_any) {       // some leading threshold nibble is non-zero: a draw can fire at level 0
+                            uint32_t le;
+                            level0_compare(B0, h0, h0m, h08, void26, &le, &tie);
+                            fire = le & ~tie;
+                        } else {            // all leading nibbles are 0: "<=" and "==" coincide with "== 0"
+                            tie = level_zero(B0, void26);
+                        }
                     }
                 }
-            }
-            const uint32_t have = __ballot_sync(0xffffffffu, tie != 0u);
-            if (have) {
-                while (qn + 32u > (uint32_t)kQueueCap) drain();
-                if (tie) {
-                    const uint32_t slot = qn + __popc(have & ((1u << lane) - 1u));
-                    sts_u32(queue_addr + 8u * slot, v | (1u << 14));   // next nibble level: 1
-                    sts_u32(queue_addr + 8u * slot + 4u, tie);
+                const uint32_t hit = tie | fire;
+                const uint32_t have = __ballot_sync(0xffffffffu, hit != 0u);
+                if (have) {
+                    while (qn + 32u > (uint32_t)kQueueCap) drain();
+                    if (hit) {
+                        const uint32_t slot = qn + __popc(have & ((1u << lane) - 1u));
+                        sts_u32(queue_addr + 12u * slot, v | (1u << 16));   // next nibble level: 1
+                        sts_u32(queue_addr + 12u * slot + 4u, tie);
+                        sts_u32(queue_addr + 12u * slot + 8u, fire);
+                    }
+                    qn += __popc(have);
                 }
-                qn += __popc(have);
             }
-        }
         }
         while (qn) drain();
         if (tid == 0) { S.tile[(kt + 1u) & 1u] = next_li; S.tile_id[(kt + 1u) & 1u] = next_id; }   // read after the next barrier but one
@@ -404,7 +441,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
             const int wg = tc.w0 + j, r = (z + 1) * 10 + (y + 1);
             if (y < tc.wcy && z < tc.wcz && 64 * wg < g.nx) {
                 const unsigned long long cw = (unsigned long long)S.claims[r][2 * (j + 1)] | ((unsigned long long)S.claims[r][2 * (j + 1) + 1] << 32);
-                unsigned long long curw = S.nv[r][j + 1], in_row = cw;
+                unsigned long long curw = S.own[row][j], in_row = cw;
                 if (64 * wg + 64 > g.nx) {                          // the row ends inside this word
                     const unsigned long long valid = ~(~0ull << (g.nx - 64 * wg));
                     curw &= valid;
@@ -453,14 +490,13 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
 
 int grow_tile_words() { return kTileW; }
 
-cudaError_t launch_grow_tile(liets_ctx* c) {
+// per-device function attribute, set once per context at liets_create: 8 CTAs x 26.8 KB of shared memory per SM
+cudaError_t grow_tile_attributes() {
     static_assert(sizeof(Smem) <= 48 * 1024, "static shared memory");
-    static bool attr_set = false;
-    if (!attr_set) {                                        // 8 CTAs x 22.6 KB per SM
-        cudaError_t e = cudaFuncSetAttribute(k_grow_tile, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    return cudaFuncSetAttribute(k_grow_tile, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+}
+
+cudaError_t launch_grow_tile(liets_ctx* c) {
     const PhiloxKey key = philox_make_key(c->rng_seed);
     k_grow_tile<<<c->tile_grid, kThreads, 0, c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->stamp, c->weight,
                                                                       c->list[0], c->list[1], key);
@@ -471,8 +507,6 @@ cudaError_t launch_grow_tile(liets_ctx* c) {
 // The same launch as a kernel node of `graph` (exec == nullptr), or its parameters refreshed in an instantiated
 // graph (the Philox key changes with every liets_seed).
 cudaError_t grow_tile_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node) {
-    cudaError_t e = cudaFuncSetAttribute(k_grow_tile, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
     PhiloxKey key = philox_make_key(c->rng_seed);
     void* args[] = { &c->ctl, &c->geom, &c->G[0], &c->G[1], &c->stamp, &c->weight, &c->list[0], &c->list[1], &key };
     cudaKernelNodeParams p = {};

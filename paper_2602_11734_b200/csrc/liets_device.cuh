@@ -183,6 +183,22 @@ __device__ __forceinline__ void level_compare(const uint4& B, const uint32_t* h,
     *eq = interleave_dirs(e0, e1, e2, e3) & mask;
 }
 
+// Level 0 with the uniform parts of the compare precomputed: hm = h & 0x8888.., h8 = h | 0x8888..
+__device__ __forceinline__ void level0_compare(const uint4& B, const uint32_t* h, const uint32_t* hm, const uint32_t* h8,
+                                               uint32_t mask, uint32_t* le, uint32_t* eq) {
+    const uint32_t a[4] = { B.x, B.y, B.z, B.w };
+    uint32_t l[4], e[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t dd = (h8[w] - (a[w] & 0x77777777u)) & 0x88888888u;      // bit 3: low 3 bits of h >= those of a
+        l[w] = (hm[w] & ~a[w]) | (~(hm[w] ^ a[w]) & dd);                        // only bit 3 of each nibble survives
+        const uint32_t z = a[w] ^ h[w];
+        e[w] = ~(((z & 0x77777777u) + 0x77777777u) | z | 0x77777777u);
+    }
+    *le = interleave_dirs(l[0], l[1], l[2], l[3]) & mask;
+    *eq = interleave_dirs(e[0], e[1], e[2], e[3]) & mask;
+}
+
 // all-zero thresholds nibbles (every class has probability < 1/16): "<=" is "== 0"; flag at bit 3 of zero nibbles
 __device__ __forceinline__ uint32_t nib_is_zero(uint32_t a) {
     return ~(((a & 0x77777777u) + 0x77777777u) | a | 0x77777777u);
