@@ -35,10 +35,14 @@ namespace {
 
 constexpr int kTileW = 2;                       // 64-bit words per tile row
 constexpr int kThreads = 128;
+#ifndef LIETS_TILE_CTAS
+#define LIETS_TILE_CTAS 8
+#endif
+constexpr int kCtasPerSm = LIETS_TILE_CTAS;       // resident CTAs per SM the kernel is compiled for (registers) and launched with
 constexpr int kWarps = kThreads / 32;
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
 constexpr int kWin = 64 * kTileW / 16;          // 18-bit windows per row, one per 16 voxels
-constexpr int kQueueCap = 128;                  // voxels with hits or ties per warp queue
+constexpr int kQueueCap = 128;                  // tied voxels per warp queue (a ring; power of two)
 constexpr int kHeavyFront = 64 * 64 * kTileW / 8;  // a tile with at least this many front voxels (1/8 of its cells) is "heavy"
 constexpr int kFrontCap = 32 * 64 * kTileW;     // front voxels listed at a time (half the tile; more -> several passes)
 
@@ -47,7 +51,7 @@ struct Smem {
     unsigned long long vx[100][kTileW];         // per tile word: cells with a void cell at x-1, x or x+1 in the same row
     unsigned long long own[64][kTileW];         // the tile's own not-void words (row y + 8 z)
     uint32_t claims[100][2 * kRowWords];        // cells claimed in this step: row as in win, bit 64 + x of the row (32-bit view)
-    uint32_t queue[kWarps][3 * kQueueCap];      // (list entry | nibble level << 16, tied directions, firing directions)
+    uint32_t queue[kWarps][2 * kQueueCap];      // ring of (list entry | nibble level << 16, tied directions)
     uint32_t hpat[8][4];
     uint32_t dir[28];                           // direction d: claim-word offset 8 (10 dz + dy + 11) | (dx + 1) << 16
     uint32_t ptab[100];                         // voxel index of tile x = 0 of each own row
@@ -115,6 +119,22 @@ __device__ __forceinline__ uint32_t lds_u32_at(uint32_t addr) {            // [a
     asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(addr), "n"(OFF) : "memory");
     return v;
 }
+__device__ __forceinline__ void lds_u64(uint32_t addr, uint32_t& a, uint32_t& b) {
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "r"(addr) : "memory");
+}
+__device__ __forceinline__ uint4 lds_u128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u64(uint32_t addr, uint32_t a, uint32_t b) {
+    asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(addr), "r"(a), "r"(b) : "memory");
+}
+__device__ __forceinline__ uint32_t mul_lo_u32(uint32_t a, uint32_t b) {     // a multiply the compiler does not turn into a shift
+    uint32_t r;
+    asm("mul.lo.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+    return r;
+}
 __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v) {
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
@@ -127,7 +147,7 @@ __device__ __forceinline__ uint32_t opaque_shared_addr(const void* p) {     // a
     return a;
 }
 
-__global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__ ctl, TileGeom g,
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(Control* __restrict__ ctl, TileGeom g,
                                                            unsigned long long* G0, unsigned long long* G1,
                                                            uint32_t* stamp, uint32_t* weight, uint32_t* list0, uint32_t* list1,
                                                            PhiloxKey key) {
@@ -150,6 +170,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
         else out[list_cap - 1u - atomicAdd(out_count_back, 1u)] = tile;
     };
     const uint32_t t = ctl->step;
+    const PhiloxStep ps = philox_step_uniform(t, key);
     const unsigned long long* __restrict__ Gc = (t & 1u) ? G1 : G0;     // g_t (read only)
     unsigned long long* Gn = (t & 1u) ? G0 : G1;                        // g_{t+1} (OR target)
     if (tid < 32) S.hpat[tid >> 2][tid & 3] = ctl->hpat[tid >> 2][tid & 3];
@@ -274,46 +295,35 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                 atoms_or_u32(cbase + 4u * ((lut & 0xFFFFu) + (xb >> 5)), 1u << (xb & 31u));
             }
         };
-        uint32_t qn = 0;                    // queue fill (warp-uniform)
-        auto drain = [&]() {                // D: one lane per queued voxel: its hits, then one nibble level of its ties
+        // D: tied voxels wait in a per-warp ring.  resolve() looks at the next nibble level of one entry: the directions that
+        // fire are claimed, the ones that tie again are returned.  round() takes the 32 oldest entries of the ring, one lane
+        // each, and appends the entries that still tie one level deeper; while the tile is being listed only full rounds run.
+        auto resolve = [&](uint32_t vk, uint32_t tie) -> uint32_t {
+            const uint32_t x = (vk & 0x7Fu) ^ 15u, rr = (vk >> 7) & 0x1FFu, k = vk >> 16;
+            const uint32_t p = lds_u32(ptab_addr + 4u * rr) + x;
+            const uint4 B = philox_growth_block(p, k, ps, key);
+            ++n_items;
+            const uint4 hk = lds_u128(hpat_addr + 16u * k);
+            const uint32_t h[4] = { hk.x, hk.y, hk.z, hk.w };
+            uint32_t le, eq;
+            level_compare(B, h, tie, &le, &eq);
+            const bool last = k == 7u;                                          // last nibble: draw <= U
+            claim(last ? le : (le & ~eq), x, rr);
+            return last ? 0u : eq;
+        };
+        uint32_t qh = 0, qn = 0;            // ring head and fill (warp-uniform)
+        auto round = [&](uint32_t n_take) {
+            constexpr uint32_t kMask = (uint32_t)kQueueCap - 1u;
+            uint32_t vk = 0, tie = 0, still = 0;
+            if (lane < n_take) lds_u64(queue_addr + 8u * ((qh + lane) & kMask), vk, tie);
+            __syncwarp();                   // this round's entries are read before any slot is written again
+            if (tie) still = resolve(vk, tie);
+            const uint32_t have = __ballot_sync(0xffffffffu, still != 0u);
+            qh = (qh + n_take) & kMask;
+            qn -= n_take;
+            if (still) sts_u64(queue_addr + 8u * ((qh + qn + __popc(have & ((1u << lane) - 1u))) & kMask), vk + (1u << 16), still);
+            qn += __popc(have);
             __syncwarp();
-            uint32_t wpos = 0;              // entries that still tie are queued again, one level deeper
-            for (uint32_t j0 = 0; j0 < qn; j0 += 32u) {
-                const uint32_t j = j0 + lane;
-                uint32_t vk = 0, tie = 0, fire = 0, still = 0;
-                if (j < qn) { vk = lds_u32(queue_addr + 12u * j); tie = lds_u32(queue_addr + 12u * j + 4u); fire = lds_u32(queue_addr + 12u * j + 8u); }
-                __syncwarp();               // this round's entries are read before any slot is written again
-                if (tie | fire) {
-                    const uint32_t x = (vk & 0x7Fu) ^ 15u, rr = (vk >> 7) & 0x1FFu, k = vk >> 16;
-                    if (tie) {
-                        const uint32_t p = lds_u32(ptab_addr + 4u * rr) + x;
-                        const uint4 B = philox4x32_10(p, 0u, t, k, key);
-                        ++n_items;
-                        const uint32_t last = k == 7u ? 1u : 0u;                // last nibble: draw <= U
-                        do {                // one tied direction at a time: nibble k of its draw against the threshold's
-                            const uint32_t d = 31u - __clz(tie), bit = 1u << d;
-                            tie ^= bit;
-                            const uint32_t lo = (d & 1u) ? B.y : B.x, hi = (d & 1u) ? B.w : B.z;
-                            const uint32_t sh = d & 28u;
-                            const uint32_t a = (((d & 2u) ? hi : lo) >> sh) & 15u;
-                            const uint32_t h = (lds_u32(hpat_addr + 16u * k + 4u * (d & 3u)) >> sh) & 15u;
-                            if (a < h + last) fire |= bit;
-                            else if (a == h) still |= bit;
-                        } while (tie);
-                    }
-                    claim(fire, x, rr);
-                }
-                const uint32_t have = __ballot_sync(0xffffffffu, still != 0u);
-                if (still) {
-                    const uint32_t slot = wpos + __popc(have & ((1u << lane) - 1u));
-                    sts_u32(queue_addr + 12u * slot, vk + (1u << 16));
-                    sts_u32(queue_addr + 12u * slot + 4u, still);
-                    sts_u32(queue_addr + 12u * slot + 8u, 0u);
-                }
-                wpos += __popc(have);
-            }
-            __syncwarp();
-            qn = wpos;
         };
         for (uint32_t pass0 = 0; pass0 < n_front; pass0 += (uint32_t)kFrontCap) {   // almost always a single pass
             if (pass0) __syncthreads();     // the previous pass no longer reads the list
@@ -357,21 +367,21 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                         asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v16) : "r"(flist_addr + 2u * i) : "memory");
                         v = v16;
                     }
-                    // the nine rows of the neighbourhood: one window each, aligned so that x+1, x, x-1 are bits 31..29, pushed
-                    // into the mask three bits at a time (row dz = +1, dy = +1 first): bit 9(dz+1) + 3(dy+1) + (dx+1) = not void
+                    // the nine rows of the neighbourhood: one window each, aligned so that x+1, x, x-1 are bits 31..29 (a multiply:
+                    // FMA pipe) and pushed into the mask three bits at a time (row dz = +1, dy = +1 first):
+                    // bit 9(dz+1) + 3(dy+1) + (dx+1) = not void
                     const uint32_t wa = win_addr + ((v >> 2) & 0xFFFCu) - 4u * kWin * 11u;
                     const uint32_t mult = 1u << (v & 15u);
                     uint32_t nb27 = 0;
-#define LIETS_ROW(E) nb27 = __funnelshift_l(lds_u32_at<4 * kWin * (((E) / 3) * 10 + (E) % 3)>(wa) * mult, nb27, 3)
+#define LIETS_ROW(E) nb27 = __funnelshift_l(mul_lo_u32(lds_u32_at<4 * kWin * (((E) / 3) * 10 + (E) % 3)>(wa), mult), nb27, 3)
                     LIETS_ROW(8); LIETS_ROW(7); LIETS_ROW(6); LIETS_ROW(5); LIETS_ROW(4); LIETS_ROW(3); LIETS_ROW(2); LIETS_ROW(1); LIETS_ROW(0);
 #undef LIETS_ROW
                     // the centre (bit 13) is solid, so ~nb27 has bit 13 clear: closing the gap is (v + (v & 0x1FFF)) >> 1
                     const uint32_t lo13 = ~nb27 & 0x1FFFu;
                     const uint32_t void26 = ((~nb27 + lo13) >> 1) & en26;
                     if (void26) {
-                        const uint32_t x = (v & 0x7Fu) ^ 15u;
-                        const uint32_t p = lds_u32(ptab_addr + ((v >> 5) & 0x3FCu)) + x;
-                        const uint4 B0 = philox4x32_10(p, 0u, t, 0u, key);
+                        const uint32_t p = lds_u32(ptab_addr + ((v >> 5) & 0x3FCu)) + ((v & 0x7Fu) ^ 15u);
+                        const uint4 B0 = philox_growth_block(p, 0u, ps, key);
                         ++n_items0;
                         if (h0_any) {       // some leading threshold nibble is non-zero: a draw can fire at level 0
                             uint32_t le;
@@ -382,21 +392,16 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
                         }
                     }
                 }
-                const uint32_t hit = tie | fire;
-                const uint32_t have = __ballot_sync(0xffffffffu, hit != 0u);
+                if (h0_any && __ballot_sync(0xffffffffu, fire != 0u)) claim(fire, (v & 0x7Fu) ^ 15u, (v >> 7) & 0x1FFu);
+                const uint32_t have = __ballot_sync(0xffffffffu, tie != 0u);
                 if (have) {
-                    while (qn + 32u > (uint32_t)kQueueCap) drain();
-                    if (hit) {
-                        const uint32_t slot = qn + __popc(have & ((1u << lane) - 1u));
-                        sts_u32(queue_addr + 12u * slot, v | (1u << 16));   // next nibble level: 1
-                        sts_u32(queue_addr + 12u * slot + 4u, tie);
-                        sts_u32(queue_addr + 12u * slot + 8u, fire);
-                    }
+                    if (qn + 32u > (uint32_t)kQueueCap) do round(32u); while (qn >= 32u);
+                    if (tie) sts_u64(queue_addr + 8u * ((qh + qn + __popc(have & ((1u << lane) - 1u))) & ((uint32_t)kQueueCap - 1u)), v | (1u << 16), tie);
                     qn += __popc(have);
                 }
             }
         }
-        while (qn) drain();
+        while (qn) round(min(qn, 32u));
         if (tid == 0) { S.tile[(kt + 1u) & 1u] = next_li; S.tile_id[(kt + 1u) & 1u] = next_id; }   // read after the next barrier but one
         __syncthreads();                    // all claims are in shared memory
 
@@ -489,6 +494,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_grow_tile(Control* __restrict__
 }  // namespace
 
 int grow_tile_words() { return kTileW; }
+int grow_tile_ctas_per_sm() { return kCtasPerSm; }
 
 // per-device function attribute, set once per context at liets_create: 8 CTAs x 26.8 KB of shared memory per SM
 cudaError_t grow_tile_attributes() {

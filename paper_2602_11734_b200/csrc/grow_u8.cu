@@ -80,7 +80,7 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
                 // next blocks only for the directions that still tie with the threshold
                 ++my_items;
                 ++my_items0;
-                const uint4 B0 = philox4x32_10(p, 0u, t, 0u, key);
+                const uint4 B0 = philox_growth_block(p, 0u, philox_step_uniform(t, key), key);
                 uint32_t le, eq;
                 level_compare(B0, s_hpat[0], mask & en26, &le, &eq);
                 uint32_t fire = le & ~eq;

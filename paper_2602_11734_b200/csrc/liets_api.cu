@@ -22,8 +22,6 @@ struct Layout {
     int Wp, ntx, nty, ntz;
 };
 
-constexpr int kTileCtasPerSm = 8;
-
 bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
     if (nx < 1 || ny < 1 || nz < 1) return false;
     const unsigned long long N = (unsigned long long)nx * (unsigned long long)ny * (unsigned long long)nz;
@@ -204,7 +202,7 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
             c->stamp = reinterpret_cast<uint32_t*>(base + L.stamp);
             c->weight = reinterpret_cast<uint32_t*>(base + L.weight);
             c->grid_u8 = nullptr;
-            c->tile_grid = c->sm_count * kTileCtasPerSm;
+            c->tile_grid = c->sm_count * grow_tile_ctas_per_sm();
         }
         // function attributes are per device: set them for the device of this context (cheap, idempotent)
         ok = seed_kernel_attributes() == cudaSuccess && grow_tile_attributes() == cudaSuccess &&

@@ -50,6 +50,46 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
+// The growth blocks B_k = philox(p, 0, t, k) of one step share t and the key: the halves of rounds 1-3 that do not
+// depend on the voxel are evaluated once per thread and launch (3 of the 40 multiply / xor pairs of a block).
+struct PhiloxStep { uint32_t k10, a, b, c; };
+
+__device__ __forceinline__ PhiloxStep philox_step_uniform(uint32_t t, const PhiloxKey& key) {
+    const unsigned long long p1 = (unsigned long long)kPhiloxM1 * t;            // round 1: c2 = t, c1 = 0
+    const uint32_t u0 = (uint32_t)(p1 >> 32) ^ key.k0[0], u1 = (uint32_t)p1;    // c0, c1 after round 1
+    const unsigned long long q0 = (unsigned long long)kPhiloxM0 * u0;           // round 2: M0 * c0
+    PhiloxStep s;
+    s.k10 = key.k1[0];                              // round 1: c2 = hi(M0 p) ^ k ^ k10
+    s.a = u1 ^ key.k0[1];                           // round 2: c0 = hi(M1 c2) ^ a
+    s.b = (uint32_t)(q0 >> 32) ^ key.k1[1];         // round 2: c2 = c3 ^ b
+    s.c = (uint32_t)q0 ^ key.k1[2];                 // round 3: c2 = hi(M0 c0) ^ c   (c3 after round 2 is lo(M0 u0))
+    return s;
+}
+
+__device__ __forceinline__ uint4 philox_growth_block(uint32_t p, uint32_t k, const PhiloxStep& s, const PhiloxKey& key) {
+    unsigned long long p0 = (unsigned long long)kPhiloxM0 * p;                  // round 1
+    uint32_t c2 = (uint32_t)(p0 >> 32) ^ k ^ s.k10, c3 = (uint32_t)p0;
+    unsigned long long p1 = (unsigned long long)kPhiloxM1 * c2;                 // round 2
+    uint32_t c0 = (uint32_t)(p1 >> 32) ^ s.a, c1 = (uint32_t)p1;
+    c2 = c3 ^ s.b;
+    p0 = (unsigned long long)kPhiloxM0 * c0;                                    // round 3
+    p1 = (unsigned long long)kPhiloxM1 * c2;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ key.k0[2];
+    c1 = (uint32_t)p1;
+    c2 = (uint32_t)(p0 >> 32) ^ s.c;
+    c3 = (uint32_t)p0;
+#pragma unroll
+    for (int r = 3; r < 10; ++r) {
+        p0 = (unsigned long long)kPhiloxM0 * c0;
+        p1 = (unsigned long long)kPhiloxM1 * c2;
+        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ key.k0[r];
+        c1 = (uint32_t)p1;
+        c2 = (uint32_t)(p0 >> 32) ^ c3 ^ key.k1[r];
+        c3 = (uint32_t)p0;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Control block: all loop state lives in HBM so that the step loop needs no host round trip.
 // ---------------------------------------------------------------------------------------------
@@ -201,7 +241,14 @@ __device__ __forceinline__ void level0_compare(const uint4& B, const uint32_t* h
 
 // all-zero thresholds nibbles (every class has probability < 1/16): "<=" is "== 0"; flag at bit 3 of zero nibbles
 __device__ __forceinline__ uint32_t nib_is_zero(uint32_t a) {
+#ifdef LIETS_ZERO_MUL
+    // bit 3 of a nibble of a | a<<1 | a<<2 | a<<3 is the OR of the nibble's four bits (nothing crosses into bit 3 from the
+    // nibble below); the left shifts are multiplies (FMA pipe), two three-input logic ops remain on the ALU pipe
+    const uint32_t u = a | (a * 2u);
+    return ~(u | (u * 4u)) & 0x88888888u;
+#else
     return ~(((a & 0x77777777u) + 0x77777777u) | a | 0x77777777u);
+#endif
 }
 __device__ __forceinline__ uint32_t level_zero(const uint4& B, uint32_t mask) {
     return interleave_dirs(nib_is_zero(B.x), nib_is_zero(B.y), nib_is_zero(B.z), nib_is_zero(B.w)) & mask;
@@ -211,8 +258,9 @@ __device__ __forceinline__ uint32_t level_zero(const uint4& B, uint32_t mask) {
 __device__ __forceinline__ uint32_t resolve_ties(uint32_t p, uint32_t t, uint32_t tie, const uint32_t (*hpat)[4],
                                                  const PhiloxKey& key, uint32_t* n_blocks) {
     uint32_t fire = 0;
+    const PhiloxStep ps = philox_step_uniform(t, key);
     for (uint32_t k = 1; k < 8u && tie; ++k) {
-        const uint4 B = philox4x32_10(p, 0u, t, k, key);
+        const uint4 B = philox_growth_block(p, k, ps, key);
         uint32_t le, eq;
         level_compare(B, hpat[k], tie, &le, &eq);
         ++*n_blocks;

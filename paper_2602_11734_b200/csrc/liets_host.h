@@ -94,6 +94,7 @@ cudaError_t grow_u8_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, 
 cudaError_t launch_grow_tile(liets_ctx* c);
 cudaError_t grow_tile_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);
 int grow_tile_words();
+int grow_tile_ctas_per_sm();
 // seed.cu
 cudaError_t launch_seed_reset(liets_ctx* c);
 cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all);
