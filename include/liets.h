@@ -132,6 +132,14 @@ int liets_seed_info(liets_ctx* ctx, uint32_t* n_candidates, uint32_t* slow_path)
  * single-CTA spacing resolve so that small grids exercise the ring wrap; ring = 0 restores the defaults.
  * The accepted seeds never depend on these sizes. */
 int liets_debug_spacing_ring(liets_ctx* ctx, uint32_t ring, uint32_t head);
+/* Test / tuning aid (STORAGE_TILE; a no-op for STORAGE_U8): the active set is kept as a list of front VOXELS while it
+ * is small ("the very early stages of growth") and as a list of tiles afterwards; a step that starts
+ * with more than max_front_voxels front voxels, or whose list did not fit `capacity` entries, runs on tiles, and so do
+ * all later ones.  max_front_voxels: 0 = tiles from the first step; UINT64_MAX = the default (max(N/128, 2^17), at most
+ * half the capacity); larger values are clamped to the capacity.  capacity: 0 = the allocated max(2^18, N/16) entries,
+ * smaller values shrink the list (so that small grids exercise the overflow hand-over).  The grid never depends on
+ * either value.  Takes effect from the next step; call it before liets_seed for a whole run. */
+int liets_debug_vox_list(liets_ctx* ctx, uint64_t max_front_voxels, uint32_t capacity);
 
 /* Measured roofs for the roofline report (SURVEY.md 8(d) "Which roofline": the working set of the growth steps
  * is L2 resident and Philox makes the integer pipes a co-limit).  Runs probe `kind` `reps`

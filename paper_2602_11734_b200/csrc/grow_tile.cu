@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(Control* __r
                                                            unsigned long long* G0, unsigned long long* G1,
                                                            uint32_t* stamp, uint32_t* weight, uint32_t* list0, uint32_t* list1,
                                                            PhiloxKey key) {
-    if (!ctl->active) return;
+    if (!ctl->active || (ctl->mode == 0u && !ctl->pending)) return;     // small fronts run in k_grow_vox
     __shared__ __align__(16) Smem S;        // static (< 48 KB): shared-memory addresses are immediates, not generic pointers
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
 

@@ -18,6 +18,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
     size_t ctl, grid, list0, list1, status2, coff, rowoff, cand, total;
     size_t g0, g1, stamp, weight;  // STORAGE_TILE (contiguous: G0 | G1 | stamp | weight)
+    size_t vox0, vox1, vox_cap;    // STORAGE_TILE: front voxel lists of the small-front steps
     size_t n_tiles, grid_words, list_cap;
     int Wp, ntx, nty, ntz;
 };
@@ -45,6 +46,9 @@ bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
         L->stamp = off;   off += L->n_tiles * 4;                // (memset together with G0 | G1 and the weights)
         L->weight = off;  off = align_up(off + L->n_tiles * 4);
         L->list_cap = L->n_tiles;                           // the step stamp admits every tile at most once per list
+        L->vox_cap = (size_t)N / 16 < ((size_t)1 << 18) ? ((size_t)1 << 18) : (size_t)N / 16;    // N/16, at least 2^18 entries (1 MiB)
+        L->vox0 = off;    off += align_up(L->vox_cap * 4);
+        L->vox1 = off;    off += align_up(L->vox_cap * 4);
     }
     L->list0 = off;   off += align_up(L->list_cap * 4);
     L->list1 = off;   off += align_up(L->list_cap * 4);
@@ -54,6 +58,14 @@ bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
     L->cand = off;    off += align_up((size_t)N * 4 < 64 ? 64 : (size_t)N * 4);
     L->total = off;
     return true;
+}
+
+// Steps that start with more front voxels than this run on tiles (measured cross-over on B200: one thread per voxel
+// with scattered row loads beats the tile kernel's fixed per-tile work up to about one front voxel per 128 cells, and on
+// small grids, whose few tiles cannot fill the GPU, up to about 10^5 front voxels).
+uint32_t default_vox_threshold(uint64_t N, uint32_t vox_cap) {
+    const uint64_t thr = N / 128 < ((uint64_t)1 << 17) ? ((uint64_t)1 << 17) : N / 128;
+    return (uint32_t)(thr < vox_cap / 2 ? thr : vox_cap / 2);
 }
 
 int fail(liets_ctx* c, int code, const char* msg) {
@@ -85,7 +97,13 @@ int launch_step_kernel(liets_ctx* c) {
             if (!c->prof_ev[2 * c->prof_n + k]) LIETS_CUDA_TRY(c, cudaEventCreate(&c->prof_ev[2 * c->prof_n + k]));
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream));
     }
-    LIETS_CUDA_TRY(c, c->storage == LIETS_STORAGE_U8 ? launch_grow_u8(c) : launch_grow_tile(c));
+    if (c->storage == LIETS_STORAGE_U8) {
+        LIETS_CUDA_TRY(c, launch_grow_u8(c));
+    } else {                                                // exactly one of the two growth kernels acts (Control::mode, pending)
+        LIETS_CUDA_TRY(c, launch_tiles_from_grid(c));
+        LIETS_CUDA_TRY(c, launch_grow_vox(c));
+        LIETS_CUDA_TRY(c, launch_grow_tile(c));
+    }
     if (prof) {
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream));
         c->prof_n++;
@@ -97,11 +115,29 @@ int launch_step_kernel(liets_ctx* c) {
 //   growth kernel ; control step (closes the step, prepares the next, sets the loop condition).
 // Built once per context; the growth node's parameters are refreshed when the rng seed (Philox key) changes.
 // Returns false if this runtime cannot do it (generate then enqueues batches of steps instead).
+// One WHILE node over { growth kernel ; control step }: adds the node to g after `after` (or at the root).
+bool add_loop(liets_ctx* c, cudaGraph_t g, const cudaGraphNode_t* after, int which, cudaGraphNode_t* while_node,
+              cudaGraphNode_t* grow_node) {
+    cudaGraphConditionalHandle loop;
+    if (cudaGraphConditionalHandleCreate(&loop, g, 1u, cudaGraphCondAssignDefault) != cudaSuccess) return false;
+    cudaGraphNodeParams wp = {};
+    wp.type = cudaGraphNodeTypeConditional;
+    wp.conditional.handle = loop;
+    wp.conditional.type = cudaGraphCondTypeWhile;
+    wp.conditional.size = 1;
+    if (cudaGraphAddNode(while_node, g, after, after ? 1 : 0, &wp) != cudaSuccess) return false;
+    cudaGraph_t body = wp.conditional.phGraph_out[0];
+    cudaGraphNode_t ctl_node;
+    const cudaError_t e = which == 0 ? grow_u8_node(c, body, nullptr, grow_node)
+                                     : grow_tile_node(c, body, nullptr, grow_node);
+    return e == cudaSuccess && control_loop_node(c, body, *grow_node, loop, &ctl_node) == cudaSuccess;
+}
+
 bool ensure_loop_graph(liets_ctx* c) {
     if (c->loop_exec) {
         if (c->loop_seed == c->rng_seed) return true;
-        const cudaError_t e = c->storage == LIETS_STORAGE_U8 ? grow_u8_node(c, nullptr, c->loop_exec, &c->loop_grow_node)
-                                                            : grow_tile_node(c, nullptr, c->loop_exec, &c->loop_grow_node);
+        cudaError_t e = c->storage == LIETS_STORAGE_U8 ? grow_u8_node(c, nullptr, c->loop_exec, &c->loop_grow_node)
+                                                      : grow_tile_node(c, nullptr, c->loop_exec, &c->loop_grow_node);
         if (e == cudaSuccess) { c->loop_seed = c->rng_seed; return true; }
         cudaGetLastError();
         cudaGraphExecDestroy(c->loop_exec); cudaGraphDestroy(c->loop_graph);        // rebuild below
@@ -111,25 +147,16 @@ bool ensure_loop_graph(liets_ctx* c) {
     c->loop_tried = true;
     cudaGraph_t g = nullptr;
     cudaGraphExec_t exec = nullptr;
-    cudaGraphConditionalHandle loop;
-    cudaGraphNode_t while_node, grow_node, ctl_node;
-    bool ok = cudaGraphCreate(&g, 0) == cudaSuccess &&
-              cudaGraphConditionalHandleCreate(&loop, g, 1u, cudaGraphCondAssignDefault) == cudaSuccess;
-    if (ok) {
-        cudaGraphNodeParams wp = {};
-        wp.type = cudaGraphNodeTypeConditional;
-        wp.conditional.handle = loop;
-        wp.conditional.type = cudaGraphCondTypeWhile;
-        wp.conditional.size = 1;
-        ok = cudaGraphAddNode(&while_node, g, nullptr, 0, &wp) == cudaSuccess;
-        if (ok) {
-            cudaGraph_t body = wp.conditional.phGraph_out[0];
-            ok = (c->storage == LIETS_STORAGE_U8 ? grow_u8_node(c, body, nullptr, &grow_node)
-                                                 : grow_tile_node(c, body, nullptr, &grow_node)) == cudaSuccess &&
-                 control_loop_node(c, body, grow_node, loop, &ctl_node) == cudaSuccess &&
-                 cudaGraphInstantiate(&exec, g, 0) == cudaSuccess;
-        }
+    cudaGraphNode_t while1, grow_node, switch_node;
+    bool ok = cudaGraphCreate(&g, 0) == cudaSuccess;
+    if (ok && c->storage == LIETS_STORAGE_U8) {
+        ok = add_loop(c, g, nullptr, 0, &while1, &grow_node);
+    } else if (ok) {
+        // STORAGE_TILE (after the steps on the voxel list, k_grow_vox_loop): k_tiles_from_grid -> WHILE(tiles) { k_grow_tile ; control }
+        ok = tiles_from_grid_node(c, g, nullptr, &switch_node) == cudaSuccess &&
+             add_loop(c, g, &switch_node, 2, &while1, &grow_node);
     }
+    ok = ok && cudaGraphInstantiate(&exec, g, 0) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
         if (exec) cudaGraphExecDestroy(exec);
@@ -201,6 +228,10 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
             c->G[1] = reinterpret_cast<unsigned long long*>(base + L.g1);
             c->stamp = reinterpret_cast<uint32_t*>(base + L.stamp);
             c->weight = reinterpret_cast<uint32_t*>(base + L.weight);
+            c->vox[0] = reinterpret_cast<uint32_t*>(base + L.vox0);
+            c->vox[1] = reinterpret_cast<uint32_t*>(base + L.vox1);
+            c->vox_cap = c->vox_cap_alloc = (uint32_t)L.vox_cap;
+            c->vox_thr = default_vox_threshold(c->N, c->vox_cap);
             c->grid_u8 = nullptr;
             c->tile_grid = c->sm_count * grow_tile_ctas_per_sm();
         }
@@ -308,7 +339,9 @@ int liets_step(liets_ctx* c, uint64_t* n_solid_out, uint64_t* n_front_out) {
         if (int rc = readback(c)) return rc;
         const uint64_t ns = c->pinned->n_solid;
         if (n_solid_out) *n_solid_out = ns;
-        if (n_front_out) *n_front_out = (ns == 0 || ns == c->N) ? 0 : c->pinned->count[c->pinned->cur] + c->pinned->count_back[c->pinned->cur];
+        const liets::Control* h = c->pinned;
+        const uint64_t nf = (h->mode == 0u && !h->pending) ? h->vox_count[h->cur] : (uint64_t)h->count[h->cur] + h->count_back[h->cur];
+        if (n_front_out) *n_front_out = (ns == 0 || ns == c->N) ? 0 : nf;
     }
     return LIETS_OK;
 }
@@ -324,9 +357,10 @@ int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps
     if (!c->profiling && ensure_loop_graph(c)) {
         // the whole loop on the device: first step prepared here, then WHILE(step armed) { grow ; control } as one graph
         LIETS_CUDA_TRY(c, launch_control(c, kCtlPrepare));
+        if (c->storage == LIETS_STORAGE_TILE) LIETS_CUDA_TRY(c, launch_grow_vox_loop(c));   // the steps on the voxel list, one launch
         LIETS_CUDA_TRY(c, cudaGraphLaunch(c->loop_exec, c->stream));
         if (int rc = readback(c)) return rc;
-        c->launches += 2ull * c->pinned->steps_done + (c->pinned->steps_done ? 0 : 2);   // kernels the graph ran
+        c->launches += 2ull * c->pinned->steps_done + (c->storage == LIETS_STORAGE_U8 ? 2 : 3);   // kernels the graph ran (incl. the loop's last, empty round)
     } else for (;;) {
         // a batch of steps back to back; steps after the stop rule fired are no-ops on the device
         uint32_t batch = 32;
@@ -439,6 +473,16 @@ int liets_seed_info(liets_ctx* c, uint32_t* n_candidates, uint32_t* slow_path) {
     if (int rc = readback(c)) return rc;
     if (n_candidates) *n_candidates = c->pinned->n_cand;
     if (slow_path) *slow_path = c->pinned->spacing_slow;
+    return LIETS_OK;
+}
+
+int liets_debug_vox_list(liets_ctx* c, uint64_t max_front_voxels, uint32_t capacity) {
+    if (!c) return LIETS_E_ARG;
+    if (c->storage != LIETS_STORAGE_TILE) return LIETS_OK;
+    c->vox_cap = capacity && capacity < c->vox_cap_alloc ? capacity : c->vox_cap_alloc;
+    c->vox_thr = max_front_voxels == UINT64_MAX ? default_vox_threshold(c->N, c->vox_cap)
+               : (uint32_t)(max_front_voxels > c->vox_cap ? c->vox_cap : max_front_voxels);
+    LIETS_CUDA_TRY(c, launch_set_params(c));
     return LIETS_OK;
 }
 

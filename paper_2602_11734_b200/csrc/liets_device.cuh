@@ -126,6 +126,13 @@ struct Control {
     uint32_t spacing_slow;           // seeding: the adjacency lists do not fit the fast resolve -> rescan rounds
     uint32_t items;                  // Philox blocks evaluated by the live step (profiling counter)
     uint32_t items0;                 // front voxels with a void target in the live step (= level-0 blocks)
+    // STORAGE_TILE keeps the active set as a voxel list while it is small (grow_vox.cu) and as a tile list afterwards
+    uint32_t mode;                   // 0: voxel list (both grid copies identical), 1: tile list (always 1 for STORAGE_U8)
+    uint32_t pending;                // the live step is the first one on tiles: k_tiles_from_grid fills its list
+    uint32_t vox_count[2];           // entries of each voxel list
+    uint32_t vox_cap;                // slots per voxel list
+    uint32_t vox_thr;                // hand over to tiles when a step starts with more front voxels than this
+    uint32_t vox_overflow;           // an append did not fit: the list is incomplete (the grid is exact)
     unsigned long long log_front[kLogCap];
     unsigned long long log_solid[kLogCap];
     unsigned long long log_items[kLogCap];
@@ -294,7 +301,11 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     const unsigned long long n_t = __ldcg(&c->n_t), N = __ldcg(&c->N);
     const unsigned long long R[3] = { __ldcg(&c->R[0]), __ldcg(&c->R[1]), __ldcg(&c->R[2]) };
     const uint32_t claims = __ldcg(&c->claims), items = __ldcg(&c->items), items0 = __ldcg(&c->items0);
-    const uint32_t count[2] = { __ldcg(&c->count[0]) + __ldcg(&c->count_back[0]), __ldcg(&c->count[1]) + __ldcg(&c->count_back[1]) };
+    uint32_t mode = __ldcg(&c->mode), pending = __ldcg(&c->pending);
+    const uint32_t vox_thr = __ldcg(&c->vox_thr), vox_overflow = __ldcg(&c->vox_overflow);
+    uint32_t count[2];
+    if (mode == 0u && !pending) { count[0] = __ldcg(&c->vox_count[0]); count[1] = __ldcg(&c->vox_count[1]); }
+    else { count[0] = __ldcg(&c->count[0]) + __ldcg(&c->count_back[0]); count[1] = __ldcg(&c->count[1]) + __ldcg(&c->count_back[1]); }
     const uint32_t law = __ldcg(&c->law), max_steps = __ldcg(&c->max_steps);
     uint32_t step = __ldcg(&c->step), steps_done = __ldcg(&c->steps_done), cur = __ldcg(&c->cur);
     uint32_t active = __ldcg(&c->active);
@@ -308,6 +319,7 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
         steps_done += 1;
         active = 0;
         c->cur = cur; c->step = step; c->steps_done = steps_done; c->active = 0; c->claims = 0;
+        if (pending) { mode = 1u; pending = 0u; c->mode = 1u; c->pending = 0u; }     // that was the first step on tiles
     }
     if (!(flags & (kCtlPrepare | kCtlEval))) return;
     if (!(flags & kCtlForce)) {                          // stop rule, between whole steps only
@@ -342,6 +354,14 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     c->tile_cursor = 0;
     c->count[cur ^ 1u] = 0;
     c->count_back[cur ^ 1u] = 0;
+    if (mode == 0u) {
+        c->vox_count[cur ^ 1u] = 0;
+        if (count[cur] > vox_thr || vox_overflow) {         // the front has outgrown the voxel list: this step runs on tiles
+            c->pending = 1u;
+            c->count[cur] = 0;                              // k_tiles_from_grid fills the list of this step
+            c->count_back[cur] = 0;
+        }
+    }
     c->claims = 0;
     c->items = 0;
     c->items0 = 0;

@@ -39,11 +39,16 @@ struct liets_ctx {
     unsigned long long* G[2];         // double-buffered bit grid, x-rows of Wp words
     uint32_t* stamp;                  // per tile: t+1 of the last step whose list holds it
     uint32_t* weight;                 // per tile: front voxels it had when it last ran (orders the list: heavy first)
+    uint32_t* vox[2];                 // front VOXEL lists of the small-front steps (grow_vox.cu)
+    uint32_t vox_cap;                 // slots per voxel list in use (<= vox_cap_alloc; a test hook shrinks it)
+    uint32_t vox_cap_alloc;           // slots per voxel list in the workspace
+    uint32_t vox_thr;                 // steps that start with more front voxels run on tiles
     uint8_t* scratch_u8;              // N bytes for format conversion (aliases the candidate buffer)
     uint32_t host_step;               // step counter as of the last read-back (selects the current grid copy)
     int resolve_grid;                 // CTAs of the cooperative spacing kernel (0 = not sized yet)
     uint32_t spacing_ring, spacing_head;  // test hook (liets_debug_spacing_ring): 0 = the built-in sizes
     int tile_grid;                    // CTAs of the tile growth kernel
+    int vox_grid;                     // CTAs of the cooperative voxel-list loop (0 = not sized yet)
     uint64_t list_cap;                // slots per front list
     // host state
     liets::Control* pinned;           // pinned host copy of the scalar part of Control
@@ -90,6 +95,12 @@ cudaError_t control_loop_node(liets_ctx* c, cudaGraph_t graph, cudaGraphNode_t a
 // grow_u8.cu
 cudaError_t launch_grow_u8(liets_ctx* c);
 cudaError_t grow_u8_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);
+// grow_vox.cu
+cudaError_t launch_grow_vox(liets_ctx* c);
+cudaError_t launch_grow_vox_loop(liets_ctx* c);
+cudaError_t launch_tiles_from_grid(liets_ctx* c);
+cudaError_t grow_vox_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);
+cudaError_t tiles_from_grid_node(liets_ctx* c, cudaGraph_t graph, const cudaGraphNode_t* after, cudaGraphNode_t* node);
 // grow_tile.cu
 cudaError_t launch_grow_tile(liets_ctx* c);
 cudaError_t grow_tile_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);

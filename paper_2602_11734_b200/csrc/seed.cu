@@ -34,6 +34,7 @@ __global__ void k_seed_reset(Control* c) {
     c->n_solid = 0; c->step = 0; c->steps_done = 0; c->active = 0; c->status = 0; c->cur = 0;
     c->count[0] = 0; c->count[1] = 0; c->count_back[0] = 0; c->count_back[1] = 0; c->claims = 0; c->n_cand = 0;
     c->pool_head = 0; c->pend3[0] = 0; c->pend3[1] = 0; c->pend3[2] = 0; c->spacing_slow = 0;
+    c->vox_count[0] = 0; c->vox_count[1] = 0; c->vox_overflow = 0; c->pending = 0;
 }
 
 // --- candidates: one thread per status word = 16 voxels = 4 Philox blocks -----------------------
@@ -486,41 +487,44 @@ __global__ void __launch_bounds__(256) k_seed_finalize_u8(Control* ctl, const ui
     }
 }
 
-__global__ void k_seed_close(Control* c) { c->n_solid = c->count[0]; c->cur = 0; }
+__global__ void k_seed_close(Control* c) { c->n_solid = c->count[0]; c->cur = 0; c->mode = 1; c->pending = 0; }
 
-// STORAGE_TILE: set the seed's bit in both grid copies; the tile enters the list of step 0 once
-// (stamp = 1).  The 0 -> 1 transition of the bit in G0 dedupes explicit seeds and counts them.
-__device__ __forceinline__ void place_seed_tile(Control* ctl, uint32_t v, TileGeom g, int tile_w, unsigned long long* G0,
-                                                unsigned long long* G1, uint32_t* stamp, uint32_t* front) {
+// STORAGE_TILE: set the seed's bit in both grid copies; A_0 = seeds as a voxel list (grow_vox.cu; a list that does
+// not fit only raises the overflow flag, and step 0 starts on tiles).  The 0 -> 1 transition of the bit in G0 dedupes
+// explicit seeds and counts them.
+__device__ __forceinline__ void place_seed_tile(Control* ctl, uint32_t v, TileGeom g, unsigned long long* G0,
+                                                unsigned long long* G1, uint32_t* vox, uint32_t vox_cap) {
     const uint32_t x = v % (uint32_t)g.nx, rest = v / (uint32_t)g.nx;
     const uint32_t y = rest % (uint32_t)g.ny, z = rest / (uint32_t)g.ny;
     const unsigned long long w = (unsigned long long)(x >> 6) + (unsigned long long)g.Wp * ((unsigned long long)y + (unsigned long long)g.ny * z);
     const unsigned long long bit = 1ull << (x & 63u);
     const unsigned long long old = atomicOr(G0 + w, bit);
     atomicOr(G1 + w, bit);
-    if (!(old & bit)) atomicAdd(&ctl->n_solid, 1ull);
-    const uint32_t tile = (x >> 6) / (uint32_t)tile_w + (uint32_t)g.ntx * ((y >> 3) + (uint32_t)g.nty * (z >> 3));
-    if (atomicMax(&stamp[tile], 1u) < 1u) front[atomicAdd(&ctl->count[0], 1u)] = tile;
+    if (old & bit) return;
+    atomicAdd(&ctl->n_solid, 1ull);
+    const uint32_t slot = atomicAdd(&ctl->vox_count[0], 1u);
+    if (slot < vox_cap) vox[slot] = v;
+    else ctl->vox_overflow = 1u;
 }
 
 __global__ void __launch_bounds__(256) k_seed_finalize_tile(Control* ctl, const uint32_t* status2, const uint32_t* cand,
-                                                             TileGeom g, int tile_w, unsigned long long* G0, unsigned long long* G1,
-                                                             uint32_t* stamp, uint32_t* front, unsigned long long N, uint32_t spaced) {
+                                                             TileGeom g, unsigned long long* G0, unsigned long long* G1,
+                                                             uint32_t* vox, uint32_t vox_cap, unsigned long long N, uint32_t spaced) {
     const uint32_t n = ctl->n_cand;
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
         const uint32_t v = cand[i];
-        if (seed_accepted(ctl, status2, cand, n, N, spaced, (uint32_t)i, v)) place_seed_tile(ctl, v, g, tile_w, G0, G1, stamp, front);
+        if (seed_accepted(ctl, status2, cand, n, N, spaced, (uint32_t)i, v)) place_seed_tile(ctl, v, g, G0, G1, vox, vox_cap);
     }
 }
 
-__global__ void k_seed_explicit_tile(Control* ctl, const unsigned long long* idx, unsigned long long n, TileGeom g, int tile_w,
-                                     unsigned long long* G0, unsigned long long* G1, uint32_t* stamp, uint32_t* front) {
+__global__ void k_seed_explicit_tile(Control* ctl, const unsigned long long* idx, unsigned long long n, TileGeom g,
+                                     unsigned long long* G0, unsigned long long* G1, uint32_t* vox, uint32_t vox_cap) {
     for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (unsigned long long)gridDim.x * blockDim.x)
-        place_seed_tile(ctl, (uint32_t)idx[i], g, tile_w, G0, G1, stamp, front);
+        place_seed_tile(ctl, (uint32_t)idx[i], g, G0, G1, vox, vox_cap);
 }
 
-__global__ void k_seed_close_tile(Control* c) { c->cur = 0; }
+__global__ void k_seed_close_tile(Control* c) { c->cur = 0; c->mode = 0; c->pending = 0; }
 
 // --- explicit seeds: dedupe with the 0 -> 1 transition of the grid byte -------------------------
 __global__ void k_seed_explicit_u8(Control* ctl, const unsigned long long* idx, unsigned long long n,
@@ -612,8 +616,8 @@ cudaError_t launch_seed_finalize(liets_ctx* c, int spaced) {
     if (c->storage == 0)
         k_seed_finalize_u8<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->grid_u8, c->list[0], c->N, (uint32_t)spaced);
     else
-        k_seed_finalize_tile<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->geom, grow_tile_words(),
-                                                                    c->G[0], c->G[1], c->stamp, c->list[0], c->N, (uint32_t)spaced);
+        k_seed_finalize_tile<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, c->geom, c->G[0], c->G[1],
+                                                                    c->vox[0], c->vox_cap, c->N, (uint32_t)spaced);
     c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -630,7 +634,7 @@ cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n) {
                                                                       c->grid_u8, c->list[0]);
         else
             k_seed_explicit_tile<<<c->sm_count * 2, 256, 0, c->stream>>>(c->ctl, (const unsigned long long*)c->explicit_idx, n,
-                                                                        c->geom, grow_tile_words(), c->G[0], c->G[1], c->stamp, c->list[0]);
+                                                                        c->geom, c->G[0], c->G[1], c->vox[0], c->vox_cap);
         c->launches++;
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;

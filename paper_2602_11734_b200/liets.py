@@ -18,7 +18,7 @@ FORMAT_U8, FORMAT_BITS = 0, 1
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
            "liets_set_target", "liets_step", "liets_generate", "liets_grid", "liets_step_log", "liets_timings",
            "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info",
-           "liets_debug_spacing_ring", "liets_probe", "liets_destroy", "liets_last_error")
+           "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_probe", "liets_destroy", "liets_last_error")
 PROBE_PHILOX, PROBE_LOP3, PROBE_IMAD, PROBE_MIX, PROBE_L2_READ, PROBE_HBM_READ = range(6)
 
 
@@ -79,6 +79,8 @@ def lib():
     L.liets_seed_info.restype = ci
     L.liets_debug_spacing_ring.argtypes = [vp, u32, u32]
     L.liets_debug_spacing_ring.restype = ci
+    L.liets_debug_vox_list.argtypes = [vp, u64, u32]
+    L.liets_debug_vox_list.restype = ci
     L.liets_probe.argtypes = [ci, vp, sz, vp, ci, P(dbl), P(dbl)]
     L.liets_probe.restype = ci
     L.liets_destroy.argtypes = [vp]
@@ -217,6 +219,11 @@ class Liets:
 
     def debug_spacing_ring(self, ring, head):
         self._check(self._L.liets_debug_spacing_ring(self._h, ring, head))
+
+    def debug_vox_list(self, max_front_voxels=None, capacity=0):
+        """max_front_voxels: None = the default, 0 = tiles from the first step; capacity: 0 = as allocated."""
+        v = 0xFFFFFFFFFFFFFFFF if max_front_voxels is None else int(max_front_voxels)
+        self._check(self._L.liets_debug_vox_list(self._h, v, int(capacity)))
 
     @property
     def launch_count(self):

@@ -19,6 +19,21 @@ def liets():
 
 
 STORAGES = [0, 1]
+# 2, 3, 4 are STORAGE_TILE with the hand-over from the voxel list to the tile list forced (liets_debug_vox_list):
+# 2 = tiles from the first step, 3 = a voxel list of 600 entries used for as long as it fits (the hand-over then happens
+# on overflow), 4 = the voxel list for the whole run (small grids fit the allocated 2^18 entries)
+STORAGES_ALL = [0, 1, 2, 3, 4]
+
+
+def make(liets, dims, periodic, storage, **kw):
+    L = liets.Liets(*dims, int(periodic), min(storage, 1), **kw)
+    if storage == 2:
+        L.debug_vox_list(0)
+    elif storage == 3:
+        L.debug_vox_list(1 << 40, 600)
+    elif storage == 4:
+        L.debug_vox_list(1 << 40)
+    return L
 
 
 def run_both(liets, dims, periodic, core, s, seed, g, law, target, storage, max_steps=100000):
@@ -26,7 +41,7 @@ def run_both(liets, dims, periodic, core, s, seed, g, law, target, storage, max_
     o = oracle.Oracle(nx, ny, nz, periodic)
     o.set_growth(*g, law)
     n_o = o.seed(core, s, seed)
-    L = liets.Liets(nx, ny, nz, int(periodic), storage)
+    L = make(liets, dims, periodic, storage)
     L.set_growth(*g, law)
     n_g = L.seed(core, s, seed)
     assert n_g == n_o
@@ -38,7 +53,7 @@ def run_both(liets, dims, periodic, core, s, seed, g, law, target, storage, max_
     return o, L
 
 
-@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("storage", STORAGES_ALL)
 def test_config1_bit_exact(liets, storage):
     c = CONFIGS["cfg1_64"]
     o, L = run_both(liets, c["dims"], c["periodic"], c["core"], c["s"], c["seeds"][0], c["g"], 1, c["targets"][0], storage)
@@ -51,7 +66,7 @@ def test_config1_bit_exact(liets, storage):
     assert len(f) == o.step_index and int(s[-1]) == o.n_solid
 
 
-@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("storage", STORAGES_ALL)
 @pytest.mark.parametrize("periodic", [False, True])
 @pytest.mark.parametrize("dims,core,s", [((37, 29, 41), 0.01, 4), ((70, 45, 33), 0.004, 7), ((5, 4, 3), 0.2, 2),
                                           ((1, 9, 2), 0.3, 0), ((96, 96, 96), 0.003, 9), ((17, 130, 9), 0.02, 3),
@@ -86,7 +101,7 @@ def test_spacing_ring_wrap_and_head_table(liets, periodic, s, expect_slow):
     L.close()
 
 
-@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("storage", STORAGES_ALL)
 @pytest.mark.parametrize("periodic", [False, True])
 def test_dense_front_bit_exact(liets, storage, periodic):
     # 55 % of the cells are seeds, nearly all of them front voxels: more than 4096 front voxels in one 128x8x8 tile,
@@ -94,20 +109,20 @@ def test_dense_front_bit_exact(liets, storage, periodic):
     run_both(liets, (130, 16, 16), periodic, 0.55, 0, 3, (0.3, 0.1, 0.02), 0, 0.97, storage)
 
 
-@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("storage", STORAGES_ALL)
 @pytest.mark.parametrize("periodic", [False, True])
 def test_step_by_step_equals_generate(liets, storage, periodic):
     dims, g = (48, 40, 52), (0.03, 0.01, 0.002)
     o = oracle.Oracle(*dims, periodic)
     o.set_growth(*g, 1); o.set_target(0.5); o.seed(0.004, 5, 9)
-    A = liets.Liets(*dims, int(periodic), storage)
+    A = make(liets, dims, periodic, storage)
     A.set_growth(*g, 1); A.set_target(0.5); A.seed(0.004, 5, 9)
     while o.n_solid < o.n_target:
         o.step(True)
         ns, nf = A.step()
         assert ns == o.n_solid and (nf == 0) == (o.n_front_exact == 0)
         assert (A.grid() == o.grid()).all(), o.step_index
-    B = liets.Liets(*dims, int(periodic), storage)
+    B = make(liets, dims, periodic, storage)
     B.set_growth(*g, 1); B.seed(0.004, 5, 9)
     rc, steps, ns = B.generate(0.5)
     assert rc == liets.OK and steps == o.step_index and (B.grid() == A.grid()).all()
@@ -119,7 +134,7 @@ def test_step_by_step_equals_generate(liets, storage, periodic):
     assert B.generate(0.7)[:2] == (liets.OK, 0)
 
 
-@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("storage", STORAGES_ALL)
 @pytest.mark.parametrize("periodic", [False, True])
 def test_closed_forms_on_gpu(liets, storage, periodic):
     nx, ny, nz = 23, 19, 21
@@ -130,7 +145,7 @@ def test_closed_forms_on_gpu(liets, storage, periodic):
         return np.minimum(d, n - d) if periodic else d
     seeds = [(0, 0, 0), (22, 18, 20), (11, 9, 10)]
     idx = [sx + nx * (sy + ny * sz) for sx, sy, sz in seeds]
-    L = liets.Liets(nx, ny, nz, int(periodic), storage)
+    L = make(liets, (nx, ny, nz), periodic, storage)
     L.set_growth(1.0, 0.0, 0.0, liets.LAW_CONSTANT)          # faces only, p = 1: union of L1 balls (P3)
     L.seed_explicit(idx + idx[:1])
     for k in range(1, 6):
@@ -150,9 +165,9 @@ def test_closed_forms_on_gpu(liets, storage, periodic):
     assert (rc, steps) == (liets.MAX_STEPS, 6) and (L.grid() == g0).all() and ns == g0.sum()
 
 
-@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("storage", STORAGES_ALL)
 def test_degenerate_cases(liets, storage):
-    L = liets.Liets(6, 6, 6, 0, storage)
+    L = make(liets, (6, 6, 6), 0, storage)
     L.set_growth(0.5, 0.5, 0.5, liets.LAW_CONSTANT)
     assert L.seed(0.0, 0, 1) == 0                             # no seeds: empty front
     assert L.generate(0.5, 10)[:2] == (liets.FRONT_EMPTY, 0)
@@ -163,11 +178,11 @@ def test_degenerate_cases(liets, storage):
     assert rc == liets.OK and ns == 216
     assert L.step() == (216, 0)                               # full grid: front is empty
     assert L.seed(1.0, 0, 1) == 216                           # every voxel a core
-    M = liets.Liets(12, 12, 12, 1, storage)
+    M = make(liets, (12, 12, 12), 1, storage)
     assert M.seed(1.0, 3, 1) == oracle_seed_count(12, True, 1.0, 3, 1)
     with pytest.raises(liets.LietsError):
         liets.Liets(0, 4, 4)
-    N = liets.Liets(4, 4, 4, 0, storage)
+    N = make(liets, (4, 4, 4), 0, storage)
     with pytest.raises(liets.LietsError):
         N.step()                                              # before seed
     with pytest.raises(liets.LietsError):
@@ -276,7 +291,7 @@ def _fuzz_cases(n, seed=2024):
         cases.append(dict(dims=dims, periodic=bool(rng.integers(0, 2)), core=float(rng.choice([0.002, 0.01, 0.05, 0.3])),
                           s=int(rng.choice([0, 1, 2, 3, 5, 9])), seed=int(rng.integers(0, 2**40)),
                           g=tuple(float(v) for v in rng.choice([0.0, 0.003, 0.02, 0.07, 0.2, 0.6, 1.0], 3)),
-                          law=int(rng.integers(0, 2)), target=float(rng.choice([0.2, 0.5, 0.9, 1.0])), storage=k % 2))
+                          law=int(rng.integers(0, 2)), target=float(rng.choice([0.2, 0.5, 0.9, 1.0])), storage=k % 5))
     return cases
 
 
