@@ -80,13 +80,15 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(s)}
 
 
-def algorithmic_bytes(storage, N, front, solid_after, n_seeds):
+def algorithmic_bytes(storage, N, front, solid_after, n_seeds, on_tiles=None, front_voxels=None):
     """bytes the list-indexed step itself must move, per step.
 
-    STORAGE_U8 (front = voxels):  4|A_t| + min(27|A_t|, N) + c_t + 4|A_{t+1}|
-    STORAGE_TILE (front = 128x8x8 tiles of 1 KiB): 4|L_t| + min(1625|L_t|, N/8) + 1024|L_t| + 4|L_{t+1}|
+    Voxel list (STORAGE_U8, b = w = 1 byte; or the small-front steps of STORAGE_TILE on the bit grid, b = 1/8, w = 8:
+    one 64-bit word per claim and grid copy):  4|A_t| + b min(27|A_t|, N) + w c_t + 4|A_{t+1}|
+    Tile list (STORAGE_TILE, 128x8x8 tiles of 1 KiB): 4|L_t| + min(1625|L_t|, N/8) + 1024|L_t| + 4|L_{t+1}|
       (read the tile list; each needed grid byte once -- a tile plus its one-voxel halo is 130x10x10
-      bits = 1625 B; write the tile's rows into the next buffer; write the next list)."""
+      bits = 1625 B; write the tile's rows into the next buffer; write the next list).
+    on_tiles[t]: step t of STORAGE_TILE ran on the tile list (default: all); front_voxels[t]: its front voxels."""
     out, prev = [], n_seeds
     for t in range(len(front)):
         a_t = int(front[t])
@@ -95,8 +97,11 @@ def algorithmic_bytes(storage, N, front, solid_after, n_seeds):
         prev = int(solid_after[t])
         if storage == 0:
             out.append(4 * a_t + min(27 * a_t, N) + c_t + 4 * a_n)
-        else:
+        elif on_tiles is None or on_tiles[t]:
             out.append(4 * a_t + min(1625 * a_t, N // 8) + 1024 * a_t + 4 * a_n)
+        else:
+            v_t = int(front_voxels[t]) if front_voxels is not None else a_t
+            out.append(4 * v_t + min(27 * v_t, N) // 8 + 2 * 8 * c_t + 4 * a_n)
     return out
 
 
@@ -127,14 +132,7 @@ def run_reference(args):
     N = nx * ny * nz
 
     def one():
-        o = oracle.Oracle(nx, ny, nz, w["periodic"])
-        o.set_growth(*w["g"], 1)
-        t0 = time.perf_counter()
-        o.seed(w["core"], w["s"], w["seed"])
-        o.generate(w["target"], 10**6, True)
-        dt = time.perf_counter() - t0
-        o.close()
-        return dt
+        return time_oracle(w, False)
     for _ in range(args.warmup):
         one()
     total = sum(one() for _ in range(args.steps))
@@ -240,45 +238,73 @@ def run_ours(args):
     clocks = sampler.stop()
     t_dev, t_e2e, t_bits = max_over_ranks([t_dev, t_e2e, t_bits], dist, "cuda")
 
-    # --- roofline of the dominant kernel (the growth kernel), timed live with CUDA events ---------
+    # --- roofline of the dominant kernel (the tile growth kernel), timed live with CUDA events ------------
     gen.set_profiling(True)
     gen.seed(w["core"], w["s"], rng_seed)
     gen.generate(w["target"])
     step_ms = gen.step_times()[:n_steps]
     gen.set_profiling(False)
     front, solid_after, philox_blocks = gen.step_log()
-    b_alg = algorithmic_bytes(storage, N, front[:n_steps], solid_after[:n_steps], n_seeds)
+    on_tiles = gen.step_on_tiles[:n_steps] if storage == 1 else np.ones(n_steps, dtype=bool)
+    handover = gen.step_handover[:n_steps] if storage == 1 else np.zeros(n_steps, dtype=bool)
+    front = front[:n_steps].astype(np.int64)
+    for t in np.flatnonzero(handover):                # the hand-over step's tile count: that of the step after it
+        front[t] = front[t + 1] if t + 1 < n_steps else front[t]
+    b_alg = np.array(algorithmic_bytes(storage, N, front, solid_after[:n_steps], n_seeds, on_tiles, gen.front_voxels[:n_steps]), dtype=np.float64)
+    dom = on_tiles                                    # launches of the dominant kernel that did a step
     peaks, peaks_kind = load_peaks()
-    grow_ms = float(np.sum(step_ms))
-    n_blocks = float(np.sum(philox_blocks[:n_steps]))
-    n_fvox = float(np.sum(gen.front_voxels[:n_steps]))
+    grow_ms = float(np.sum(step_ms[dom]))
+    n_dom = int(dom.sum())
+    n_blocks = float(np.sum(philox_blocks[:n_steps][dom]))
+    n_fvox = float(np.sum(gen.front_voxels[:n_steps][dom]))
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    # measured roofs of this box (liets_probe, csrc/probe.cu), taken after the timed legs
+    scratch = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    probes = {}
+    for kind, name in ((liets.liets.PROBE_PHILOX, "philox_blocks_per_s"), (liets.liets.PROBE_LOP3, "lop3_per_s"),
+                       (liets.liets.PROBE_IMAD, "imad_per_s"), (liets.liets.PROBE_MIX, "mix_per_s"),
+                       (liets.liets.PROBE_L2_READ, "l2_read_bytes_per_s"), (liets.liets.PROBE_HBM_READ, "hbm_read_bytes_per_s")):
+        probes[name] = liets.liets.probe(kind, scratch, reps=5)[0]
+    del scratch
     # the path is bound by integer issue, not by bytes.  Algorithmic work of a launch =
     #   40 integer instructions per Philox4x32-10 block the keyed draws need (20 32x32->64 multiplies + 20
     #   three-input XORs), plus 2 per (front voxel, direction): the void test of the target and the compare of the
     #   draw with the threshold (Algorithm 3 lines 6 and 8), 52 per front voxel that makes attempts.
-    # Peak = SMs x 4 schedulers x 32 lanes x 1 instruction/clock x the maximum SM clock.
-    alu_peak = sm_count * 4 * 32 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    # Peak = the MEASURED rate of an even multiply-add / logic-op mix on this box (liets_probe MIX); the figure derived
+    # from unit counts (SMs x 4 schedulers x 32 lanes x max clock) is quoted beside it.
+    derived_peak = sm_count * 4 * 32 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    alu_peak = probes["mix_per_s"] / 1e12
     alg_ops = n_blocks * PHILOX_INT_OPS + n_fvox * PER_FRONT_VOXEL_OPS
-    alu_achieved = alg_ops / (grow_ms * 1e-3) / 1e12 if grow_ms > 0 else 0.0
-    philox_only = n_blocks * PHILOX_INT_OPS / (grow_ms * 1e-3) / 1e12 if grow_ms > 0 else 0.0
-    hbm_achieved = sum(b_alg) / (grow_ms * 1e-3) / 1e9 if grow_ms > 0 else 0.0
+    sec = grow_ms * 1e-3 if grow_ms > 0 else float("inf")
+    alu_achieved = alg_ops / sec / 1e12
+    bytes_dom = float(np.sum(b_alg[dom]))
+    traffic, traffic_src = traffic_from_profile(w["name"], storage)
     roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Tiop/s (thread-level integer instructions)",
-                "frac": alu_achieved / alu_peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH[storage],
+                "frac": alu_achieved / alu_peak, "traffic": traffic, "traffic_source": traffic_src,
                 "kernel": KERNEL_NAMES[storage],
-                "peak_kind": "derived: %d SMs x 4 schedulers x 32 lanes x %.0f MHz (sm_max_mhz, %s)" % (
+                "peak_kind": "measured: liets_probe MIX (one 32-bit multiply-add per three-input logic op, 8 independent chains per "
+                             "thread, every warp slot) on this GPU, best of 5",
+                "peak_derived": derived_peak, "measured_over_derived": alu_peak / derived_peak,
+                "peak_derived_kind": "%d SMs x 4 schedulers x 32 lanes x %.0f MHz (sm_max_mhz, %s)" % (
                     sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peaks_kind),
-                "launches": int(n_steps), "philox_blocks_per_launch": n_blocks / max(n_steps, 1),
-                "front_voxels_per_launch": n_fvox / max(n_steps, 1),
+                "launches": n_dom, "launches_on_voxel_list": int(n_steps - n_dom),
+                "philox_blocks_per_launch": n_blocks / max(n_dom, 1), "front_voxels_per_launch": n_fvox / max(n_dom, 1),
                 "int_ops_per_philox_block": PHILOX_INT_OPS, "int_ops_per_front_voxel": PER_FRONT_VOXEL_OPS,
-                "frac_philox_only": philox_only / alu_peak,
-                "avg_launch_ms": grow_ms / max(n_steps, 1),
+                "avg_launch_ms": grow_ms / max(n_dom, 1),
                 "growth_kernel_share_of_generate": grow_ms / max(float(np.median(gen_ms)), 1e-9),
-                "hbm": {"bound": "hbm", "achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                        "frac": hbm_achieved / peaks["hbm_gbs"],
-                        "peak_kind": "%s (MEASURED_PEAKS.json hbm_gbs, burst copy)" % peaks_kind,
-                        "algorithmic_bytes_per_launch": sum(b_alg) / max(n_steps, 1),
-                        "note": "SURVEY.md 8(d) byte model; the grid (2 x %.1f MB) is L2 resident" % (N / 8e6)}}
+                "philox": {"bound": "alu", "achieved": n_blocks / sec, "peak": probes["philox_blocks_per_s"], "unit": "Philox4x32-10 blocks/s",
+                           "frac": n_blocks / sec / probes["philox_blocks_per_s"],
+                           "peak_kind": "measured: liets_probe PHILOX (blocks back to back, nothing else) on this GPU"},
+                "hbm": {"bound": "hbm", "achieved": bytes_dom / sec / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                        "frac": bytes_dom / sec / 1e9 / peaks["hbm_gbs"],
+                        "peak_kind": "%s (MEASURED_PEAKS.json hbm_gbs, burst copy); liets_probe HBM read: %.0f GB/s" % (
+                            peaks_kind, probes["hbm_read_bytes_per_s"] / 1e9),
+                        "algorithmic_bytes_per_launch": bytes_dom / max(n_dom, 1),
+                        "note": "SURVEY.md 8(d) byte model; the grid (2 x %.1f MB) is L2 resident" % (N / 8e6)},
+                "l2": {"bound": "l2", "achieved": bytes_dom / sec / 1e9, "peak": probes["l2_read_bytes_per_s"] / 1e9, "unit": "GB/s",
+                       "frac": bytes_dom / sec / probes["l2_read_bytes_per_s"],
+                       "peak_kind": "measured: liets_probe L2_READ (ld.cg of a 32 MiB window, 16 passes) on this GPU"},
+                "probes": probes}
 
     out = None
     if rank == 0:
@@ -310,30 +336,60 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def cpu_baseline():
-    """The oracle as it stands, on the box's host cores, on a bounded sample (one serial run)."""
+def time_oracle(w, omp):
+    """One run (seeding + growth to the target) of the CPU oracle on workload w; seconds."""
     import oracle
-    oracle.build()
-    w = workloads.BENCH_CPU_SAMPLE
     nx, ny, nz = w["dims"]
-    o = oracle.Oracle(nx, ny, nz, w["periodic"])
+    o = oracle.Oracle(nx, ny, nz, w["periodic"], omp=omp)
     o.set_growth(*w["g"], 1)
     t0 = time.perf_counter()
     o.seed(w["core"], w["s"], w["seed"])
     o.generate(w["target"], 10**6, True)
     dt = time.perf_counter() - t0
-    return {"value": nx * ny * nz / dt, "unit": "nodes/s", "cores": 1, "kind": "oracle", "seconds": dt,
-            "sample": "%s: %dx%dx%d sub-volume of %s with the same parameters (densities, spacing, target), "
-                      "one serial run of oracle/liets_oracle.c (gcc -O2)" % (w["name"], nx, ny, nz, workloads.BENCH["name"])}
+    o.close()
+    return dt
+
+
+def cpu_baseline():
+    """The oracle as it stands, on the box's host cores, on a bounded sample: one serial run (the checker of record)
+    and one run of the same source built with OpenMP over the front (liboracle_omp.so) on all host cores."""
+    import oracle
+    oracle.build()
+    oracle.build_omp()
+    w = workloads.BENCH_CPU_SAMPLE
+    nx, ny, nz = w["dims"]
+    n = nx * ny * nz
+    dt1 = time_oracle(w, False)
+    dtn = time_oracle(w, True)
+    cores = oracle.threads(True)
+    return {"value": n / dtn, "unit": "nodes/s", "cores": cores, "kind": "oracle", "seconds": dtn,
+            "value_1core": n / dt1, "seconds_1core": dt1, "value_allcores": n / dtn, "seconds_allcores": dtn,
+            "host_cpu_count": os.cpu_count(),
+            "sample": "%s: %dx%dx%d sub-volume of %s with the same parameters (densities, spacing, target); one serial run of "
+                      "oracle/liets_oracle.c (gcc -O2) and one run of the same source with OpenMP over the front on %d threads; "
+                      "seeding (brute-force greedy) is serial in both" % (w["name"], nx, ny, nz, workloads.BENCH["name"], cores)}
+
+
+def traffic_from_profile(workload, storage):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, averaged over all launches of one
+    generation, from the committed ncu capture of this round (profiles/*_dram.csv: launch, read bytes, write bytes).
+    Only for the workload and storage the capture was made on; None otherwise."""
+    import glob
+    if workload != workloads.BENCH["name"] or storage != 1:
+        return None, None
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_k_grow_tile_dram.csv")))
+    if not files:
+        return None, None
+    rows = [l.split(",") for l in open(files[-1]) if l.strip() and not l.startswith("#") and l[0].isdigit()]
+    if not rows:
+        return None, None
+    return sum(float(r[1]) + float(r[2]) for r in rows) / len(rows), os.path.relpath(files[-1], ROOT)
 
 
 DEFAULT_STORAGE = 1
 PHILOX_INT_OPS = 40
 PER_FRONT_VOXEL_OPS = 52
 KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_tile"}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
-# `ncu --set full` capture (profiles/); None until a capture exists for the current kernel.
-TRAFFIC_BYTES_PER_LAUNCH = {0: None, 1: 18.09e6}     # profiles/r1_k_grow_tile_ncu.md (k_grow_tile, steps 18-20)
 
 
 def main():
@@ -352,6 +408,17 @@ def main():
         return run_reference(args)
     args.steps = args.steps or 20
     args.warmup = 3 if args.warmup is None else max(args.warmup, 3)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and "RANK" not in os.environ:
+        # not under torchrun: spawn one rank per GPU ourselves, exactly as the driver would
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+                                  "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
+    if args.gpus != world:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE is %d" % (args.gpus, world))
     run_ours(args)
 
 

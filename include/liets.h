@@ -104,8 +104,9 @@ int liets_generate(liets_ctx* ctx, double target_solid_fraction, uint32_t max_st
 int liets_grid(liets_ctx* ctx, void* dst, size_t dst_bytes, int format, int dst_is_device);
 
 /* Per-step counters of the steps done since the last seed (HOST arrays of capacity cap, may be
- * NULL): front size at the start of step i (list entries: voxels for STORAGE_U8, tiles for
- * STORAGE_TILE), solid count after it, the number of Philox4x32-10 blocks the step evaluated
+ * NULL): front size at the start of step i (list entries: voxels for STORAGE_U8; for STORAGE_TILE voxels while the
+ * front is a voxel list, tiles afterwards -- bit 63 set: the step ran on the tile list; bit 62 set as well: it was
+ * the hand-over step and the count is still the voxel list's), solid count after it, the number of Philox4x32-10 blocks the step evaluated
  * (one per front voxel with a void target, plus one per further nibble level of its tied directions),
  * and the number of front voxels with a void target (the sources of Algorithm 3 that made attempts).
  * Returns the number of steps recorded (<= 4096 kept). */
@@ -132,6 +133,12 @@ int liets_seed_info(liets_ctx* ctx, uint32_t* n_candidates, uint32_t* slow_path)
  * single-CTA spacing resolve so that small grids exercise the ring wrap; ring = 0 restores the defaults.
  * The accepted seeds never depend on these sizes. */
 int liets_debug_spacing_ring(liets_ctx* ctx, uint32_t ring, uint32_t head);
+/* Test aid: the device's evaluation of Eq. (1) in counts (R6/R8),
+ *   T = min(2^32, floor(R max(0, 20 n_t - 19 n_solid) / n_t)),
+ * for n triples given as HOST arrays (R <= 2^32, 1 <= n_t <= 2^32, n_solid <= 2^32); T_out is a HOST array of n.
+ * It runs the same device function the control step uses (no 128-bit arithmetic on the device), on the default
+ * stream, and synchronises.  Errors: E_ARG, E_CUDA. */
+int liets_debug_thresholds(const uint64_t* R, const uint64_t* n_t, const uint64_t* n_solid, uint64_t* T_out, uint32_t n);
 /* Test / tuning aid (STORAGE_TILE; a no-op for STORAGE_U8): the active set is kept as a list of front VOXELS while it
  * is small ("the very early stages of growth") and as a list of tiles afterwards; a step that starts
  * with more than max_front_voxels front voxels, or whose list did not fit `capacity` entries, runs on tiles, and so do

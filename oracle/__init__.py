@@ -15,26 +15,39 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "liets_oracle.c")
 _DEPS = [_SRC, os.path.join(_HERE, "liets_oracle.h"), os.path.join(_HERE, "liets_oracle_directions.inc")]
 _LIB = os.path.join(_HERE, "liboracle.so")
+_LIB_OMP = os.path.join(_HERE, "liboracle_omp.so")
 
 OK, FRONT_EMPTY, MAX_STEPS = 0, 1, 2
 
 
 def build(force=False):
-    """Compile liboracle.so with gcc -O2 (no SIMD intrinsics, no OpenMP: the oracle is serial)."""
+    """Compile liboracle.so with gcc -O2 (no SIMD intrinsics, no OpenMP: the oracle of record is serial)."""
     if not force and os.path.exists(_LIB) and all(os.path.getmtime(_LIB) >= os.path.getmtime(d) for d in _DEPS):
         return _LIB
     subprocess.check_call(["gcc", "-O2", "-std=gnu99", "-Wall", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
     return _LIB
 
 
+def build_omp(force=False):
+    """The same source with -fopenmp: oracle_step_list shares the front among the host's cores (the all-cores CPU
+    baseline of bench.py).  The serial library stays the checker of record; tests prove the two equal."""
+    if not force and os.path.exists(_LIB_OMP) and all(os.path.getmtime(_LIB_OMP) >= os.path.getmtime(d) for d in _DEPS):
+        return _LIB_OMP
+    subprocess.check_call(["gcc", "-O2", "-fopenmp", "-std=gnu99", "-Wall", "-shared", "-fPIC", "-o", _LIB_OMP, _SRC, "-lm"])
+    return _LIB_OMP
+
+
 _lib = None
+_lib_omp = None
 
 
-def lib():
-    global _lib
-    if _lib is not None:
+def lib(omp=False):
+    global _lib, _lib_omp
+    if omp and _lib_omp is not None:
+        return _lib_omp
+    if not omp and _lib is not None:
         return _lib
-    L = ctypes.CDLL(build())
+    L = ctypes.CDLL(build_omp() if omp else build())
     u32, u64, i64, dbl, vp, ci = (ctypes.c_uint32, ctypes.c_uint64, ctypes.c_int64, ctypes.c_double,
                                   ctypes.c_void_p, ctypes.c_int)
     P = ctypes.POINTER
@@ -83,8 +96,18 @@ def lib():
     L.oracle_permute_front.restype = None
     L.oracle_s2.argtypes = [vp, ci, ci, ci, ci, ci, ci, P(u64), P(u64)]
     L.oracle_s2.restype = None
-    _lib = L
+    L.oracle_threads.argtypes = []
+    L.oracle_threads.restype = ci
+    if omp:
+        _lib_omp = L
+    else:
+        _lib = L
     return L
+
+
+def threads(omp=False):
+    """Host threads oracle_step_list uses in the chosen library."""
+    return int(lib(omp).oracle_threads())
 
 
 def philox4x32_10(ctr, key):
@@ -136,8 +159,8 @@ def s2(grid, periodic, axis, rmax):
 class Oracle:
     """One oracle run: create -> set_growth -> seed -> step/generate -> grid()."""
 
-    def __init__(self, nx, ny, nz, periodic=False):
-        self._L = lib()
+    def __init__(self, nx, ny, nz, periodic=False, omp=False):
+        self._L = lib(omp)
         self.nx, self.ny, self.nz, self.periodic = nx, ny, nz, bool(periodic)
         self.N = nx * ny * nz
         self._h = self._L.oracle_new(nx, ny, nz, int(periodic))

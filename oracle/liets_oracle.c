@@ -8,6 +8,9 @@
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 /* ------------------------------------------------------------------------------------------
  * Philox4x32-10 (R9).  One round:
@@ -295,6 +298,7 @@ int oracle_step_list(oracle_state* o) {
     int rc = step_thresholds(o, T);
     if (rc) return rc;
     uint64_t n_old = o->n_front;                       /* sources: A at the start of the step */
+#ifndef _OPENMP
     for (int d = 0; d < 26; ++d) {                     /* line 4: for each d in directions   */
         int cls = abs(ORACLE_DIRS[d][0]) + abs(ORACLE_DIRS[d][1]) + abs(ORACLE_DIRS[d][2]);
         for (uint64_t i = 0; i < n_old; ++i) {
@@ -314,6 +318,54 @@ int oracle_step_list(oracle_state* o) {
     for (uint64_t i = 0; i < o->n_front; ++i)
         if (has_void_neighbour(o, o->front[i])) o->front[kept++] = o->front[i];
     o->n_front = kept;
+#else
+    /* The same loops with the front shared among the host's cores (liboracle_omp.so, the all-cores
+     * CPU baseline of bench.py).  Legal because draws are keyed by (seed, t, p, d) and
+     * the update is an OR: line 6 reads the cell with an atomic load, line 9 is an atomic exchange
+     * whose old value says which thread flipped 0 -> 1 -- that thread alone appends q (line 10), to a
+     * list of its own; the lists are joined after each direction.  The order of A differs from the
+     * serial run, the grid cannot (pin P7).  tests/test_oracle_pins.py proves both libraries equal. */
+    int nth = omp_get_max_threads();
+    uint64_t** buf = (uint64_t**)calloc((size_t)nth, sizeof(uint64_t*));
+    uint64_t* nbuf = (uint64_t*)calloc((size_t)nth, sizeof(uint64_t));
+    uint64_t* cbuf = (uint64_t*)calloc((size_t)nth, sizeof(uint64_t));
+    for (int d = 0; d < 26; ++d) {                     /* line 4 */
+        int cls = abs(ORACLE_DIRS[d][0]) + abs(ORACLE_DIRS[d][1]) + abs(ORACLE_DIRS[d][2]);
+#pragma omp parallel
+        {
+            int me = omp_get_thread_num();
+            nbuf[me] = 0;
+#pragma omp for schedule(static)
+            for (uint64_t i = 0; i < n_old; ++i) {
+                uint64_t p = o->front[i], q;
+                if (!neighbour(o, p, d, &q)) continue;                                   /* line 5 */
+                if (__atomic_load_n(&o->grid[q], __ATOMIC_RELAXED) != 0) continue;       /* line 6 */
+                if ((uint64_t)oracle_growth_draw(o->rng_seed, o->step, p, d) < T[cls]) { /* line 8 */
+                    if (__atomic_exchange_n(&o->grid[q], 1, __ATOMIC_RELAXED) == 0) {    /* line 9 */
+                        if (nbuf[me] == cbuf[me]) {                                      /* line 10 */
+                            cbuf[me] = cbuf[me] ? 2 * cbuf[me] : 1024;
+                            buf[me] = (uint64_t*)realloc(buf[me], cbuf[me] * sizeof(uint64_t));
+                        }
+                        buf[me][nbuf[me]++] = q;
+                    }
+                }
+            }
+        }
+        for (int k = 0; k < nth; ++k)
+            for (uint64_t j = 0; j < nbuf[k]; ++j) { front_push(o, buf[k][j]); o->n_solid++; }
+    }
+    for (int k = 0; k < nth; ++k) free(buf[k]);
+    free(buf); free(nbuf); free(cbuf);
+    /* line 14: prune, the test in parallel, the compaction in order */
+    uint8_t* keep = (uint8_t*)malloc(o->n_front ? o->n_front : 1);
+#pragma omp parallel for schedule(static)
+    for (uint64_t i = 0; i < o->n_front; ++i) keep[i] = (uint8_t)has_void_neighbour(o, o->front[i]);
+    uint64_t kept = 0;
+    for (uint64_t i = 0; i < o->n_front; ++i)
+        if (keep[i]) o->front[kept++] = o->front[i];
+    free(keep);
+    o->n_front = kept;
+#endif
     o->step++;
     return 0;
 }
@@ -335,6 +387,15 @@ int oracle_generate(oracle_state* o, double phi_s, uint32_t max_steps, int use_l
     }
     if (steps_out) *steps_out = done;
     return status;
+}
+
+/* host threads oracle_step_list uses: 1 in liboracle.so, omp_get_max_threads() in liboracle_omp.so */
+int oracle_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
 }
 
 const uint8_t* oracle_grid(const oracle_state* o) { return o->grid; }

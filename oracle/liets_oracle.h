@@ -72,6 +72,7 @@ int oracle_step_list(oracle_state* o);
 int oracle_generate(oracle_state* o, double phi_s, uint32_t max_steps, int use_list,
                     uint32_t* steps_out);
 
+int oracle_threads(void);
 const uint8_t* oracle_grid(const oracle_state* o);          /* N bytes in {0,1}, x fastest */
 uint64_t oracle_n_solid(const oracle_state* o);
 uint64_t oracle_n_front_exact(const oracle_state* o);       /* #solid cells with a void neighbour */

@@ -48,6 +48,18 @@ __global__ void k_set_params(Control* c, unsigned long long R0, unsigned long lo
     c->vox_cap = vox_cap; c->vox_thr = vox_thr;
 }
 
+// test aid: eq1_threshold on the device for n (R, n_t, n_solid) triples (liets_debug_thresholds)
+__global__ void k_eq1_thresholds(const unsigned long long* R, const unsigned long long* n_t, const unsigned long long* n_solid,
+                                 unsigned long long* T, uint32_t n) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) T[i] = eq1_threshold(R[i], n_t[i], n_solid[i]);
+}
+
+cudaError_t launch_eq1_thresholds(const unsigned long long* dev_in, unsigned long long* dev_out, uint32_t n, cudaStream_t stream) {
+    k_eq1_thresholds<<<(n + 127) / 128, 128, 0, stream>>>(dev_in, dev_in + n, dev_in + 2ull * n, dev_out, n);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_control(liets_ctx* c, uint32_t flags) {
     k_control<<<1, 32, 0, c->stream>>>(c->ctl, flags);
     c->launches++;

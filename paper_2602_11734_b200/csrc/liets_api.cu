@@ -88,7 +88,11 @@ int readback(liets_ctx* c) {
 
 int launch_step_kernel(liets_ctx* c) {
     const bool prof = c->profiling && c->prof_n < kProfCap;
-    if (prof) {
+    if (c->storage == LIETS_STORAGE_TILE) {                 // exactly one of the two growth kernels acts (Control::mode, pending)
+        LIETS_CUDA_TRY(c, launch_tiles_from_grid(c));
+        LIETS_CUDA_TRY(c, launch_grow_vox(c));
+    }
+    if (prof) {                                             // the event pair brackets the dominant kernel (k_grow_tile / k_grow_u8) alone
         if (!c->prof_ev) {
             c->prof_ev = static_cast<cudaEvent_t*>(calloc(2 * kProfCap, sizeof(cudaEvent_t)));
             if (!c->prof_ev) return fail(c, LIETS_E_CUDA, "out of host memory");
@@ -97,13 +101,7 @@ int launch_step_kernel(liets_ctx* c) {
             if (!c->prof_ev[2 * c->prof_n + k]) LIETS_CUDA_TRY(c, cudaEventCreate(&c->prof_ev[2 * c->prof_n + k]));
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream));
     }
-    if (c->storage == LIETS_STORAGE_U8) {
-        LIETS_CUDA_TRY(c, launch_grow_u8(c));
-    } else {                                                // exactly one of the two growth kernels acts (Control::mode, pending)
-        LIETS_CUDA_TRY(c, launch_tiles_from_grid(c));
-        LIETS_CUDA_TRY(c, launch_grow_vox(c));
-        LIETS_CUDA_TRY(c, launch_grow_tile(c));
-    }
+    LIETS_CUDA_TRY(c, c->storage == LIETS_STORAGE_U8 ? launch_grow_u8(c) : launch_grow_tile(c));
     if (prof) {
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream));
         c->prof_n++;
@@ -111,10 +109,6 @@ int launch_step_kernel(liets_ctx* c) {
     return 0;
 }
 
-// liets_generate's device-resident step loop as ONE CUDA graph: a WHILE node whose body is
-//   growth kernel ; control step (closes the step, prepares the next, sets the loop condition).
-// Built once per context; the growth node's parameters are refreshed when the rng seed (Philox key) changes.
-// Returns false if this runtime cannot do it (generate then enqueues batches of steps instead).
 // One WHILE node over { growth kernel ; control step }: adds the node to g after `after` (or at the root).
 bool add_loop(liets_ctx* c, cudaGraph_t g, const cudaGraphNode_t* after, int which, cudaGraphNode_t* while_node,
               cudaGraphNode_t* grow_node) {
@@ -473,6 +467,22 @@ int liets_seed_info(liets_ctx* c, uint32_t* n_candidates, uint32_t* slow_path) {
     if (int rc = readback(c)) return rc;
     if (n_candidates) *n_candidates = c->pinned->n_cand;
     if (slow_path) *slow_path = c->pinned->spacing_slow;
+    return LIETS_OK;
+}
+
+int liets_debug_thresholds(const uint64_t* R, const uint64_t* n_t, const uint64_t* n_solid, uint64_t* T_out, uint32_t n) {
+    if (!R || !n_t || !n_solid || !T_out || n == 0) return LIETS_E_ARG;
+    for (uint32_t i = 0; i < n; ++i)
+        if (n_t[i] == 0 || n_t[i] > (1ull << 32) || R[i] > (1ull << 32) || n_solid[i] > (1ull << 32)) return LIETS_E_ARG;
+    unsigned long long* dev = nullptr;
+    if (cudaMalloc(&dev, 4ull * n * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); return LIETS_E_CUDA; }
+    bool ok = cudaMemcpy(dev, R, n * 8ull, cudaMemcpyHostToDevice) == cudaSuccess &&
+              cudaMemcpy(dev + n, n_t, n * 8ull, cudaMemcpyHostToDevice) == cudaSuccess &&
+              cudaMemcpy(dev + 2ull * n, n_solid, n * 8ull, cudaMemcpyHostToDevice) == cudaSuccess &&
+              launch_eq1_thresholds(dev, dev + 3ull * n, n, nullptr) == cudaSuccess &&
+              cudaMemcpy(T_out, dev + 3ull * n, n * 8ull, cudaMemcpyDeviceToHost) == cudaSuccess;
+    cudaFree(dev);
+    if (!ok) { cudaGetLastError(); return LIETS_E_CUDA; }
     return LIETS_OK;
 }
 

@@ -358,6 +358,7 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
         c->vox_count[cur ^ 1u] = 0;
         if (count[cur] > vox_thr || vox_overflow) {         // the front has outgrown the voxel list: this step runs on tiles
             c->pending = 1u;
+            pending = 2u;                                   // (2: handed over in this very call)
             c->count[cur] = 0;                              // k_tiles_from_grid fills the list of this step
             c->count_back[cur] = 0;
         }
@@ -365,7 +366,10 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     c->claims = 0;
     c->items = 0;
     c->items0 = 0;
-    if (step < kLogCap) c->log_front[step] = count[cur];
+    // entries of the list the step starts from; bit 63: the step runs on tiles (k_grow_tile); bit 62: it is the hand-over
+    // step, whose tile list k_tiles_from_grid has yet to fill -- the count is still the voxel list's
+    if (step < kLogCap)
+        c->log_front[step] = (unsigned long long)count[cur] | ((mode != 0u || pending) ? (1ull << 63) : 0ull) | (pending == 2u ? (1ull << 62) : 0ull);
     c->active = 1;
 }
 

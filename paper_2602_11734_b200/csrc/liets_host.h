@@ -90,6 +90,7 @@ constexpr size_t kControlScalarBytes = offsetof(Control, log_front);
 cudaError_t launch_control(liets_ctx* c, uint32_t flags);
 cudaError_t launch_begin(liets_ctx* c, int generate, uint32_t max_steps);
 cudaError_t launch_set_params(liets_ctx* c);
+cudaError_t launch_eq1_thresholds(const unsigned long long* dev_in, unsigned long long* dev_out, uint32_t n, cudaStream_t stream);
 cudaError_t control_loop_node(liets_ctx* c, cudaGraph_t graph, cudaGraphNode_t after, cudaGraphConditionalHandle loop,
                               cudaGraphNode_t* node);
 // grow_u8.cu

@@ -18,7 +18,7 @@ FORMAT_U8, FORMAT_BITS = 0, 1
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
            "liets_set_target", "liets_step", "liets_generate", "liets_grid", "liets_step_log", "liets_timings",
            "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info",
-           "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_probe", "liets_destroy", "liets_last_error")
+           "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_debug_thresholds", "liets_probe", "liets_destroy", "liets_last_error")
 PROBE_PHILOX, PROBE_LOP3, PROBE_IMAD, PROBE_MIX, PROBE_L2_READ, PROBE_HBM_READ = range(6)
 
 
@@ -81,6 +81,8 @@ def lib():
     L.liets_debug_spacing_ring.restype = ci
     L.liets_debug_vox_list.argtypes = [vp, u64, u32]
     L.liets_debug_vox_list.restype = ci
+    L.liets_debug_thresholds.argtypes = [P(u64), P(u64), P(u64), P(u64), u32]
+    L.liets_debug_thresholds.restype = ci
     L.liets_probe.argtypes = [ci, vp, sz, vp, ci, P(dbl), P(dbl)]
     L.liets_probe.restype = ci
     L.liets_destroy.argtypes = [vp]
@@ -101,6 +103,19 @@ def probe(kind, scratch, reps=5, stream=None):
     if rc < 0:
         raise LietsError(rc, "liets_probe failed")
     return float(ups.value), float(ms.value)
+
+
+def debug_thresholds(R, n_t, n_solid):
+    """liets_debug_thresholds on equally long sequences of Python ints: the device's T values as a list of ints."""
+    n = len(R)
+    arr = [np.ascontiguousarray(a, dtype=np.uint64) for a in (R, n_t, n_solid)]
+    out = np.zeros(n, dtype=np.uint64)
+    P64 = ctypes.POINTER(ctypes.c_uint64)
+    rc = lib().liets_debug_thresholds(arr[0].ctypes.data_as(P64), arr[1].ctypes.data_as(P64), arr[2].ctypes.data_as(P64),
+                                          out.ctypes.data_as(P64), n)
+    if rc < 0:
+        raise LietsError(rc, "liets_debug_thresholds failed")
+    return [int(v) for v in out]
 
 
 class Liets:
@@ -196,7 +211,9 @@ class Liets:
         n = self._check(self._L.liets_step_log(self._h, f.ctypes.data_as(P64), s.ctypes.data_as(P64),
                                                b.ctypes.data_as(P64), v.ctypes.data_as(P64), cap))
         self.front_voxels = v[:n].copy()      # front voxels with a void target per step
-        return f[:n].copy(), s[:n].copy(), b[:n].copy()
+        self.step_on_tiles = (f[:n] >> np.uint64(63)).astype(bool)        # the step ran in the tile kernel
+        self.step_handover = ((f[:n] >> np.uint64(62)) & np.uint64(1)).astype(bool)   # ... and its count is still in voxels
+        return (f[:n] & np.uint64((1 << 62) - 1)).copy(), s[:n].copy(), b[:n].copy()
 
     def timings(self):
         a, b = ctypes.c_float(0), ctypes.c_float(0)

@@ -324,3 +324,24 @@ def test_oracle_philox_equals_curand_device_philox(liets, tmp_path):
     for row, line in zip(vec, out):
         expect = oracle.philox4x32_10([int(x) for x in row[:4]], [int(x) for x in row[4:]])
         assert tuple(int(t, 16) for t in line.split()) == expect
+
+
+def test_eq1_thresholds_on_device_against_big_integers(liets):
+    """Row 1 of the path (Eq. (1) in counts, R6/R8) directly: the device function the control step uses
+    (q, r split, no 128-bit product) against Python big integers, including the extremes n_t = 1 and n_t = 2^32 - 1,
+    R = 2^32, n_solid = 0 / n_t - 1 / n_t / beyond 20/19 n_t, and random triples."""
+    rng = np.random.default_rng(7)
+    big = 1 << 32
+    R, n_t, n_s = [], [], []
+    for nt in (1, 2, 3, 19, 20, 21, 1000, 6_000_000, 51_200_000, 858_993_460, big - 2, big - 1, big):
+        for r in (0, 1, 2, 1 << 16, 42_949_673, 1_073_742, (1 << 31) + 12345, big - 1, big):
+            for ns in (0, 1, nt // 2, max(nt - 1, 0), nt, min(nt + 1, big), min(20 * nt // 19, big), min(20 * nt // 19 + 1, big), big):
+                R.append(r); n_t.append(nt); n_s.append(ns)
+    for _ in range(4000):
+        nt = int(rng.integers(1, big + 1))
+        R.append(int(rng.integers(0, big + 1))); n_t.append(nt); n_s.append(int(rng.integers(0, min(2 * nt, big) + 1)))
+    got = liets.liets.debug_thresholds(R, n_t, n_s)
+    for r, nt, ns, T in zip(R, n_t, n_s, got):
+        expect = min(big, r * max(0, 20 * nt - 19 * ns) // nt)
+        assert T == expect, (r, nt, ns, T, expect)
+        assert T == oracle.step_threshold(r, 1, nt, ns)

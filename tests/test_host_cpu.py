@@ -123,3 +123,6 @@ def test_algorithmic_bytes_model():
     # STORAGE_TILE: 4|L_t| + min(1625|L_t|, N/8) + 1024|L_t| + 4|L_{t+1}|
     assert bench.algorithmic_bytes(1, 10**6, [2, 3], [0, 0], 0)[0] == 8 + 3250 + 2048 + 12
     assert bench.algorithmic_bytes(1, 8000, [2, 3], [0, 0], 0)[0] == 8 + 1000 + 2048 + 12
+    # STORAGE_TILE with the first step on the voxel list of the bit grid: 4|A_t| + min(27|A_t|, N)/8 + 2 words per claim + 4|L_{t+1}|
+    b = bench.algorithmic_bytes(1, 10**6, [10, 3], [25, 60], 10, on_tiles=[False, True], front_voxels=[10, 999])
+    assert b == [40 + 270 // 8 + 16 * 15 + 12, 12 + 3 * 1625 + 3 * 1024 + 12]

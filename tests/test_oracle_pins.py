@@ -428,3 +428,27 @@ def test_p12_two_point_correlation(periodic):
     phi = pairs[0] / valid[0]
     for r in range(1, 6):
         assert abs(pairs[r] / valid[r] - phi**2) < 0.01
+
+
+@pytest.mark.parametrize("dims,periodic,core,s,seed,g,phi", [
+    ((64, 64, 64), False, 0.005, 0, 1, (0.02, 0.005, 0.0005), 0.30),
+    ((70, 45, 33), True, 0.004, 7, 5, (0.05, 0.02, 0.01), 0.55),
+    ((5, 4, 3), True, 0.2, 2, 5, (0.3, 0.2, 0.1), 0.9),
+    ((96, 96, 96), False, 0.003, 9, 3, (0.01, 0.0025, 0.00025), 0.6)])
+def test_openmp_build_of_the_list_oracle_equals_the_serial_oracle(dims, periodic, core, s, seed, g, phi):
+    """liboracle_omp.so (the same source with the front of oracle_step_list shared among the host's cores; the all-cores
+    CPU baseline of bench.py) against liboracle.so, the checker of record: seeds, status, steps, solid count and the
+    grid after EVERY step are identical, whatever order the threads append the new front in (P7)."""
+    a = oracle.Oracle(*dims, periodic)
+    b = oracle.Oracle(*dims, periodic, omp=True)
+    assert oracle.threads(False) == 1 and oracle.threads(True) >= 1
+    for o in (a, b):
+        o.set_growth(*g, 1)
+        o.set_target(phi)
+    assert a.seed(core, s, seed) == b.seed(core, s, seed)
+    while a.n_solid < a.n_target and a.n_front_exact:
+        a.step(True)
+        b.step(True)
+        assert a.n_solid == b.n_solid and (a.grid() == b.grid()).all(), a.step_index
+    ra, rb = a.generate(min(1.0, phi + 0.2)), b.generate(min(1.0, phi + 0.2))
+    assert ra == rb and a.n_solid == b.n_solid and (a.grid() == b.grid()).all()
