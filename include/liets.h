@@ -103,6 +103,14 @@ int liets_generate(liets_ctx* ctx, double target_solid_fraction, uint32_t max_st
  * Errors: E_STATE before the first liets_seed / liets_seed_explicit, E_CAPACITY (dst_bytes), E_ARG. */
 int liets_grid(liets_ctx* ctx, void* dst, size_t dst_bytes, int format, int dst_is_device);
 
+/* Two-point correlation of the VOID phase of the current grid along one axis (0 = x, 1 = y, 2 = z), as exact integer
+ * pair counts (R16; BASELINE.json asks for it, the paper does not define it): for r = 0 .. rmax,
+ *   pairs[r] = #{ x : void(x) and void(x + r e_axis) },   valid[r] = #{ x : the pair (x, x + r e_axis) is counted },
+ * with pairs inside the domain only on a walled grid and wrapped per coordinate on a periodic one; S2(r) = pairs / valid,
+ * S2(0) = porosity.  pairs and valid are HOST arrays of rmax + 1 entries, rmax <= 65534.  Computed on the device from
+ * the bit rows; synchronises.  Errors: E_ARG, E_STATE before the first seed, E_CUDA. */
+int liets_s2(liets_ctx* ctx, int axis, int rmax, uint64_t* pairs, uint64_t* valid);
+
 /* Per-step counters of the steps done since the last seed (HOST arrays of capacity cap, may be
  * NULL): front size at the start of step i (list entries: voxels for STORAGE_U8; for STORAGE_TILE voxels while the
  * front is a voxel list, tiles afterwards -- bit 63 set: the step ran on the tile list; bit 62 set as well: it was

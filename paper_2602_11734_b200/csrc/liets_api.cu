@@ -418,6 +418,28 @@ int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is
     return LIETS_OK;
 }
 
+int liets_s2(liets_ctx* c, int axis, int rmax, uint64_t* pairs, uint64_t* valid) {
+    if (!c || !pairs || !valid) return LIETS_E_ARG;
+    if (axis < 0 || axis > 2 || rmax < 0 || rmax > 65534) return fail(c, LIETS_E_ARG, "axis must be 0..2 and rmax 0..65534");
+    if (!c->seeded) return fail(c, LIETS_E_STATE, "liets_s2 before liets_seed");
+    if (int rc = readback(c)) return rc;                    // which grid copy is current
+    c->host_step = c->pinned->step;
+    const size_t n_words = (size_t)((c->nx + 63) / 64) * c->ny * c->nz;
+    const size_t bytes = (size_t)(rmax + 1) * 8 + (c->storage == LIETS_STORAGE_U8 ? n_words * 8 : 0);
+    unsigned long long* dev = nullptr;
+    if (cudaMalloc(&dev, bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, LIETS_E_CUDA, "cudaMalloc failed in liets_s2"); }
+    bool ok = cudaMemsetAsync(dev, 0, (size_t)(rmax + 1) * 8, c->stream) == cudaSuccess &&
+              launch_s2(c, axis, rmax, dev, dev + rmax + 1) == cudaSuccess &&
+              cudaMemcpyAsync(pairs, dev, (size_t)(rmax + 1) * 8, cudaMemcpyDeviceToHost, c->stream) == cudaSuccess &&
+              cudaStreamSynchronize(c->stream) == cudaSuccess;
+    cudaFree(dev);
+    if (!ok) { cudaGetLastError(); return fail(c, LIETS_E_CUDA, "liets_s2 failed on the device"); }
+    const uint64_t n[3] = { (uint64_t)c->nx, (uint64_t)c->ny, (uint64_t)c->nz };
+    for (int r = 0; r <= rmax; ++r)                         // positions counted: all of them if periodic, else those with x + r inside
+        valid[r] = c->boundary == LIETS_BOUNDARY_PERIODIC ? c->N : ((uint64_t)r < n[axis] ? c->N / n[axis] * (n[axis] - (uint64_t)r) : 0);
+    return LIETS_OK;
+}
+
 int liets_step_log(liets_ctx* c, uint64_t* front_in, uint64_t* solid_after, uint64_t* philox_blocks,
                    uint64_t* front_voxels, uint32_t cap) {
     if (!c) return LIETS_E_ARG;

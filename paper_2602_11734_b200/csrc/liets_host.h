@@ -115,6 +115,8 @@ cudaError_t launch_seed_finalize(liets_ctx* c, int spaced);
 cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n);
 cudaError_t seed_kernel_attributes();
 cudaError_t grow_tile_attributes();
+// s2.cu
+cudaError_t launch_s2(liets_ctx* c, int axis, int rmax, unsigned long long* pairs_dev, unsigned long long* rows_scratch);
 // export.cu
 cudaError_t launch_pack_bits_u8(liets_ctx* c, const uint8_t* src_u8, uint8_t* dst_bits);
 cudaError_t launch_unpack_rows_u8(liets_ctx* c, uint8_t* dst_u8);

@@ -16,7 +16,7 @@ FORMAT_U8, FORMAT_BITS = 0, 1
 
 # every symbol include/liets.h declares
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
-           "liets_set_target", "liets_step", "liets_generate", "liets_grid", "liets_step_log", "liets_timings",
+           "liets_set_target", "liets_step", "liets_generate", "liets_grid", "liets_s2", "liets_step_log", "liets_timings",
            "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info",
            "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_debug_thresholds", "liets_probe", "liets_destroy", "liets_last_error")
 PROBE_PHILOX, PROBE_LOP3, PROBE_IMAD, PROBE_MIX, PROBE_L2_READ, PROBE_HBM_READ = range(6)
@@ -65,6 +65,8 @@ def lib():
     L.liets_generate.restype = ci
     L.liets_grid.argtypes = [vp, vp, sz, ci, ci]
     L.liets_grid.restype = ci
+    L.liets_s2.argtypes = [vp, ci, ci, P(u64), P(u64)]
+    L.liets_s2.restype = ci
     L.liets_step_log.argtypes = [vp, P(u64), P(u64), P(u64), P(u64), u32]
     L.liets_step_log.restype = ci
     L.liets_timings.argtypes = [vp, P(ctypes.c_float), P(ctypes.c_float)]
@@ -201,6 +203,14 @@ class Liets:
         out = self._torch.empty(n, dtype=self._torch.uint8, device=self.device)
         self._check(self._L.liets_grid(self._h, ctypes.c_void_p(out.data_ptr()), n, format, 1))
         return out
+
+    def s2(self, axis, rmax):
+        """Exact void-void pair counts at lags 0..rmax along `axis` (0 = x, 1 = y, 2 = z): (pairs, valid) uint64 arrays."""
+        pairs = np.zeros(rmax + 1, dtype=np.uint64)
+        valid = np.zeros(rmax + 1, dtype=np.uint64)
+        P64 = ctypes.POINTER(ctypes.c_uint64)
+        self._check(self._L.liets_s2(self._h, axis, rmax, pairs.ctypes.data_as(P64), valid.ctypes.data_as(P64)))
+        return pairs, valid
 
     def step_log(self, cap=4096):
         f = np.zeros(cap, dtype=np.uint64)

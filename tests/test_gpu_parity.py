@@ -208,6 +208,9 @@ def test_config2_bit_exact(liets, storage, seed):
         po, vo = oracle.s2(o.grid(), False, axis, 16)
         assert (pg == po).all() and (vg == vo).all()
         assert pg[0] == L.N - o.n_solid
+        XX
+        po, vo = oracle.s2(o.grid(), False, axis, 100)
+        assert (pd == po).all() and (vd == vo).all()
 
 
 def test_boundary_library_workspace_stream_and_capacity_errors(liets):
@@ -345,3 +348,19 @@ def test_eq1_thresholds_on_device_against_big_integers(liets):
         expect = min(big, r * max(0, 20 * nt - 19 * ns) // nt)
         assert T == expect, (r, nt, ns, T, expect)
         assert T == oracle.step_threshold(r, 1, nt, ns)
+
+
+@pytest.mark.parametrize("storage", STORAGES)
+@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("dims", [(70, 45, 33), (130, 9, 17), (5, 4, 3), (1, 9, 2), (64, 64, 8), (191, 3, 2)])
+def test_device_two_point_correlation_equals_oracle(liets, storage, periodic, dims):
+    """liets_s2 (exact void-void pair counts on the device, R16) against the oracle's plain triple loop, every axis, lags
+    beyond the grid size included, on shapes whose rows end inside a word and on axes of 1, 2 and 3 cells."""
+    o, L = run_both(liets, dims, periodic, 0.02, 2, 11, (0.08, 0.03, 0.01), 1, 0.45, storage)
+    for axis in range(3):
+        rmax = 2 * max(dims) + 3
+        pd, vd = L.s2(axis, rmax)
+        po, vo = oracle.s2(o.grid(), periodic, axis, rmax)
+        assert (vd == vo).all(), (axis, vd, vo)
+        assert (pd == po).all(), (axis, np.flatnonzero(pd != po)[:5])
+        assert pd[0] == L.N - o.n_solid
