@@ -42,8 +42,12 @@ enum {
 
 enum { LIETS_BOUNDARY_WALL = 0, LIETS_BOUNDARY_PERIODIC = 1 };        /* R5 */
 enum { LIETS_STORAGE_U8 = 0,      /* uint8 grid + explicit list of front VOXELS (uint32 indices)  */
-       LIETS_STORAGE_TILE = 1 };  /* bit-packed x-rows + explicit list of active 128x8x8 TILES; the
-                                     front voxels of a tile are re-listed in shared memory each step */
+       LIETS_STORAGE_TILE = 1,    /* bit-packed x-rows; the active set is an explicit list of front VOXELS while it
+                                     is small and an explicit list of active 128x8x8 TILES afterwards, whose front
+                                     voxels are re-listed in shared memory each step                               */
+       LIETS_STORAGE_FULL = 2 };  /* bit-packed x-rows and NO active set: every step sweeps the full field
+                                     (Algorithm 2, the paper's "vectorized QSGS"; same keyed draws, so
+                                     the same grid).  Kept as the same-box comparison of :181; cost ~ N per step.      */
 enum { LIETS_LAW_CONSTANT = 0, LIETS_LAW_EQ1 = 1 };
 enum { LIETS_FORMAT_U8 = 0,       /* one byte per voxel in {0,1}, x fastest, N bytes              */
        LIETS_FORMAT_BITS = 1 };   /* bit idx%8 (LSB first) of byte idx/8, ceil(N/8) bytes         */

@@ -27,7 +27,7 @@ bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
     if (nx < 1 || ny < 1 || nz < 1) return false;
     const unsigned long long N = (unsigned long long)nx * (unsigned long long)ny * (unsigned long long)nz;
     if (N >= (1ull << 32)) return false;
-    if (storage != LIETS_STORAGE_U8 && storage != LIETS_STORAGE_TILE) return false;
+    if (storage != LIETS_STORAGE_U8 && storage != LIETS_STORAGE_TILE && storage != LIETS_STORAGE_FULL) return false;
     memset(L, 0, sizeof(*L));
     size_t off = 0;
     L->ctl = off;     off += align_up(sizeof(Control));
@@ -101,7 +101,7 @@ int launch_step_kernel(liets_ctx* c) {
             if (!c->prof_ev[2 * c->prof_n + k]) LIETS_CUDA_TRY(c, cudaEventCreate(&c->prof_ev[2 * c->prof_n + k]));
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream));
     }
-    LIETS_CUDA_TRY(c, c->storage == LIETS_STORAGE_U8 ? launch_grow_u8(c) : launch_grow_tile(c));
+    LIETS_CUDA_TRY(c, c->storage == LIETS_STORAGE_U8 ? launch_grow_u8(c) : c->storage == LIETS_STORAGE_FULL ? launch_grow_full(c) : launch_grow_tile(c));
     if (prof) {
         LIETS_CUDA_TRY(c, cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream));
         c->prof_n++;
@@ -123,6 +123,7 @@ bool add_loop(liets_ctx* c, cudaGraph_t g, const cudaGraphNode_t* after, int whi
     cudaGraph_t body = wp.conditional.phGraph_out[0];
     cudaGraphNode_t ctl_node;
     const cudaError_t e = which == 0 ? grow_u8_node(c, body, nullptr, grow_node)
+                        : which == 1 ? grow_full_node(c, body, nullptr, grow_node)
                                      : grow_tile_node(c, body, nullptr, grow_node);
     return e == cudaSuccess && control_loop_node(c, body, *grow_node, loop, &ctl_node) == cudaSuccess;
 }
@@ -131,7 +132,8 @@ bool ensure_loop_graph(liets_ctx* c) {
     if (c->loop_exec) {
         if (c->loop_seed == c->rng_seed) return true;
         cudaError_t e = c->storage == LIETS_STORAGE_U8 ? grow_u8_node(c, nullptr, c->loop_exec, &c->loop_grow_node)
-                                                      : grow_tile_node(c, nullptr, c->loop_exec, &c->loop_grow_node);
+                      : c->storage == LIETS_STORAGE_FULL ? grow_full_node(c, nullptr, c->loop_exec, &c->loop_grow_node)
+                                                         : grow_tile_node(c, nullptr, c->loop_exec, &c->loop_grow_node);
         if (e == cudaSuccess) { c->loop_seed = c->rng_seed; return true; }
         cudaGetLastError();
         cudaGraphExecDestroy(c->loop_exec); cudaGraphDestroy(c->loop_graph);        // rebuild below
@@ -143,8 +145,8 @@ bool ensure_loop_graph(liets_ctx* c) {
     cudaGraphExec_t exec = nullptr;
     cudaGraphNode_t while1, grow_node, switch_node;
     bool ok = cudaGraphCreate(&g, 0) == cudaSuccess;
-    if (ok && c->storage == LIETS_STORAGE_U8) {
-        ok = add_loop(c, g, nullptr, 0, &while1, &grow_node);
+    if (ok && c->storage != LIETS_STORAGE_TILE) {
+        ok = add_loop(c, g, nullptr, c->storage == LIETS_STORAGE_U8 ? 0 : 1, &while1, &grow_node);
     } else if (ok) {
         // STORAGE_TILE (after the steps on the voxel list, k_grow_vox_loop): k_tiles_from_grid -> WHILE(tiles) { k_grow_tile ; control }
         ok = tiles_from_grid_node(c, g, nullptr, &switch_node) == cudaSuccess &&
@@ -214,7 +216,7 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
         c->explicit_idx = reinterpret_cast<uint64_t*>(base + L.cand);
         c->scratch_u8 = reinterpret_cast<uint8_t*>(base + L.cand);
         c->list_cap = L.list_cap;
-        if (storage == LIETS_STORAGE_TILE) {
+        if (storage != LIETS_STORAGE_U8) {
             c->geom = TileGeom{ nx, ny, nz, L.Wp, L.ntx, L.nty, L.ntz, boundary };
             c->n_tiles = L.n_tiles;
             c->grid_words = L.grid_words;
@@ -334,7 +336,7 @@ int liets_step(liets_ctx* c, uint64_t* n_solid_out, uint64_t* n_front_out) {
         const uint64_t ns = c->pinned->n_solid;
         if (n_solid_out) *n_solid_out = ns;
         const liets::Control* h = c->pinned;
-        const uint64_t nf = (h->mode == 0u && !h->pending) ? h->vox_count[h->cur] : (uint64_t)h->count[h->cur] + h->count_back[h->cur];
+        const uint64_t nf = h->mode == 2u ? 1u : (h->mode == 0u && !h->pending) ? h->vox_count[h->cur] : (uint64_t)h->count[h->cur] + h->count_back[h->cur];
         if (n_front_out) *n_front_out = (ns == 0 || ns == c->N) ? 0 : nf;
     }
     return LIETS_OK;
@@ -354,7 +356,7 @@ int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps
         if (c->storage == LIETS_STORAGE_TILE) LIETS_CUDA_TRY(c, launch_grow_vox_loop(c));   // the steps on the voxel list, one launch
         LIETS_CUDA_TRY(c, cudaGraphLaunch(c->loop_exec, c->stream));
         if (int rc = readback(c)) return rc;
-        c->launches += 2ull * c->pinned->steps_done + (c->storage == LIETS_STORAGE_U8 ? 2 : 3);   // kernels the graph ran (incl. the loop's last, empty round)
+        c->launches += 2ull * c->pinned->steps_done + (c->storage == LIETS_STORAGE_TILE ? 3 : 2);   // kernels the graph ran (incl. the loop's last, empty round)
     } else for (;;) {
         // a batch of steps back to back; steps after the stop rule fired are no-ops on the device
         uint32_t batch = 32;
@@ -384,7 +386,7 @@ int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is
     const size_t nb = format == LIETS_FORMAT_U8 ? (size_t)c->N : (size_t)((c->N + 7) / 8);
     if (dst_bytes < nb) return fail(c, LIETS_E_CAPACITY, "dst buffer too small for the requested format");
     const uint8_t* u8 = c->grid_u8;
-    if (c->storage == LIETS_STORAGE_TILE) {                 // bit rows -> linear uint8 (seeding scratch is idle)
+    if (c->storage != LIETS_STORAGE_U8) {                   // bit rows -> linear uint8 (seeding scratch is idle)
         if (int rc = readback(c)) return rc;                // which grid copy is current
         c->host_step = c->pinned->step;
         if (format == LIETS_FORMAT_BITS && c->nx % 8 == 0) {

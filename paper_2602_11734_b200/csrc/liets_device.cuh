@@ -127,7 +127,7 @@ struct Control {
     uint32_t items;                  // Philox blocks evaluated by the live step (profiling counter)
     uint32_t items0;                 // front voxels with a void target in the live step (= level-0 blocks)
     // STORAGE_TILE keeps the active set as a voxel list while it is small (grow_vox.cu) and as a tile list afterwards
-    uint32_t mode;                   // 0: voxel list (both grid copies identical), 1: tile list (always 1 for STORAGE_U8)
+    uint32_t mode;                   // 0: voxel list (both grid copies identical), 1: tile list (always 1 for STORAGE_U8), 2: no list (STORAGE_FULL)
     uint32_t pending;                // the live step is the first one on tiles: k_tiles_from_grid fills its list
     uint32_t vox_count[2];           // entries of each voxel list
     uint32_t vox_cap;                // slots per voxel list
@@ -305,6 +305,7 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     const uint32_t vox_thr = __ldcg(&c->vox_thr), vox_overflow = __ldcg(&c->vox_overflow);
     uint32_t count[2];
     if (mode == 0u && !pending) { count[0] = __ldcg(&c->vox_count[0]); count[1] = __ldcg(&c->vox_count[1]); }
+    else if (mode == 2u) { count[0] = count[1] = (n_solid != 0ull) ? 1u : 0u; }      // the full-field sweep keeps no list
     else { count[0] = __ldcg(&c->count[0]) + __ldcg(&c->count_back[0]); count[1] = __ldcg(&c->count[1]) + __ldcg(&c->count_back[1]); }
     const uint32_t law = __ldcg(&c->law), max_steps = __ldcg(&c->max_steps);
     uint32_t step = __ldcg(&c->step), steps_done = __ldcg(&c->steps_done), cur = __ldcg(&c->cur);

@@ -524,7 +524,7 @@ __global__ void k_seed_explicit_tile(Control* ctl, const unsigned long long* idx
         place_seed_tile(ctl, (uint32_t)idx[i], g, G0, G1, vox, vox_cap);
 }
 
-__global__ void k_seed_close_tile(Control* c) { c->cur = 0; c->mode = 0; c->pending = 0; }
+__global__ void k_seed_close_tile(Control* c, uint32_t mode) { c->cur = 0; c->mode = mode; c->pending = 0; }
 
 // --- explicit seeds: dedupe with the 0 -> 1 transition of the grid byte -------------------------
 __global__ void k_seed_explicit_u8(Control* ctl, const unsigned long long* idx, unsigned long long n,
@@ -622,7 +622,7 @@ cudaError_t launch_seed_finalize(liets_ctx* c, int spaced) {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (c->storage == 0) k_seed_close<<<1, 1, 0, c->stream>>>(c->ctl);
-    else k_seed_close_tile<<<1, 1, 0, c->stream>>>(c->ctl);
+    else k_seed_close_tile<<<1, 1, 0, c->stream>>>(c->ctl, c->storage == 2 ? 2u : 0u);
     c->launches++;
     return cudaGetLastError();
 }
@@ -640,7 +640,7 @@ cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n) {
         if (e != cudaSuccess) return e;
     }
     if (c->storage == 0) k_seed_close<<<1, 1, 0, c->stream>>>(c->ctl);
-    else k_seed_close_tile<<<1, 1, 0, c->stream>>>(c->ctl);
+    else k_seed_close_tile<<<1, 1, 0, c->stream>>>(c->ctl, c->storage == 2 ? 2u : 0u);
     c->launches++;
     return cudaGetLastError();
 }

@@ -21,12 +21,13 @@ def liets():
 STORAGES = [0, 1]
 # 2, 3, 4 are STORAGE_TILE with the hand-over from the voxel list to the tile list forced (liets_debug_vox_list):
 # 2 = tiles from the first step, 3 = a voxel list of 600 entries used for as long as it fits (the hand-over then happens
-# on overflow), 4 = the voxel list for the whole run (small grids fit the allocated 2^18 entries)
-STORAGES_ALL = [0, 1, 2, 3, 4]
+# on overflow), 4 = the voxel list for the whole run (small grids fit the allocated 2^18 entries);
+# 5 is STORAGE_FULL, the full-field sweep of Algorithm 2 (no active set)
+STORAGES_ALL = [0, 1, 2, 3, 4, 5]
 
 
 def make(liets, dims, periodic, storage, **kw):
-    L = liets.Liets(*dims, int(periodic), min(storage, 1), **kw)
+    L = liets.Liets(*dims, int(periodic), 2 if storage == 5 else min(storage, 1), **kw)
     if storage == 2:
         L.debug_vox_list(0)
     elif storage == 3:
@@ -294,7 +295,7 @@ def _fuzz_cases(n, seed=2024):
         cases.append(dict(dims=dims, periodic=bool(rng.integers(0, 2)), core=float(rng.choice([0.002, 0.01, 0.05, 0.3])),
                           s=int(rng.choice([0, 1, 2, 3, 5, 9])), seed=int(rng.integers(0, 2**40)),
                           g=tuple(float(v) for v in rng.choice([0.0, 0.003, 0.02, 0.07, 0.2, 0.6, 1.0], 3)),
-                          law=int(rng.integers(0, 2)), target=float(rng.choice([0.2, 0.5, 0.9, 1.0])), storage=k % 5))
+                          law=int(rng.integers(0, 2)), target=float(rng.choice([0.2, 0.5, 0.9, 1.0])), storage=k % 6))
     return cases
 
 
