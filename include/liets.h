@@ -107,6 +107,30 @@ int liets_generate(liets_ctx* ctx, double target_solid_fraction, uint32_t max_st
  * Errors: E_STATE before the first liets_seed / liets_seed_explicit, E_CAPACITY (dst_bytes), E_ARG. */
 int liets_grid(liets_ctx* ctx, void* dst, size_t dst_bytes, int format, int dst_is_device);
 
+/* ---- Batched realisations ----------------------------------------------------------------------
+ * The paper's use of the generator is a sweep: "five independent realizations ... for each value of s",
+ * fifteen porosities (:217).  A batch is n <= 16 equally shaped LIETS_STORAGE_TILE generators on one stream whose step
+ * loops run as ONE device-side loop: each iteration is one launch of the tile kernel over the tile lists of ALL grids (a
+ * CTA that finds one grid's list used up moves on to the next grid) and one control step per grid; the loop ends when
+ * every grid has stopped.  Small grids, whose few tiles cannot fill the GPU and whose steps are bound by launch latency,
+ * share both.  Every grid's result is exactly that of its own liets_generate (draws are keyed per grid by its rng_seed).
+ *
+ * liets_create_batch: workspace = DEVICE memory of n * liets_workspace_bytes(.., LIETS_STORAGE_TILE) bytes, 256-byte
+ *   aligned, or NULL (the library allocates).  Errors: E_ARG (n outside 1..16, bad dims), E_CAPACITY, E_CUDA.
+ * liets_batch_ctx(b, i): the i-th generator, owned by the batch -- use it with liets_set_growth, liets_seed,
+ *   liets_seed_explicit, liets_grid, liets_s2, liets_step_log (NOT liets_destroy); NULL if i is out of range.
+ * liets_generate_batch: target_solid_fraction = HOST array of n; status_out / steps_out / n_solid_out = HOST arrays of n
+ *   (may be NULL): per grid what liets_generate returns and reports; device_ms_out (may be NULL) = device time of the
+ *   whole call.  Returns LIETS_OK or an error (E_ARG, E_STATE if a grid is not seeded, E_CUDA); synchronises. */
+typedef struct liets_batch liets_batch;
+int liets_create_batch(liets_batch** out, int n, int nx, int ny, int nz, int boundary, void* workspace, size_t workspace_bytes,
+                       void* cuda_stream);
+liets_ctx* liets_batch_ctx(liets_batch* batch, int i);
+int liets_generate_batch(liets_batch* batch, const double* target_solid_fraction, uint32_t max_steps, int* status_out,
+                         uint32_t* steps_out, uint64_t* n_solid_out, float* device_ms_out);
+void liets_destroy_batch(liets_batch* batch);
+const char* liets_batch_last_error(const liets_batch* batch);
+
 /* Two-point correlation of the VOID phase of the current grid along one axis (0 = x, 1 = y, 2 = z), as exact integer
  * pair counts (R16; BASELINE.json asks for it, the paper does not define it): for r = 0 .. rmax,
  *   pairs[r] = #{ x : void(x) and void(x + r e_axis) },   valid[r] = #{ x : the pair (x, x + r e_axis) is counted },

@@ -5,7 +5,7 @@ Everything the method computes runs in the hand-written sm_100a kernels behind t
 (the workspace and output buffers) and the CUDA stream.  There is no CPU fallback: loading fails
 loudly if the library has not been built, and every call fails without a CUDA device.
 """
-from .liets import (Liets, LietsError, lib, library_path, OK, FRONT_EMPTY, MAX_STEPS,  # noqa: F401
+from .liets import (Liets, LietsBatch, LietsError, lib, library_path, OK, FRONT_EMPTY, MAX_STEPS,  # noqa: F401
                     E_ARG, E_STATE, E_CAPACITY, E_CUDA,
                     BOUNDARY_WALL, BOUNDARY_PERIODIC, STORAGE_U8, STORAGE_TILE, STORAGE_FULL, LAW_CONSTANT, LAW_EQ1,
                     FORMAT_U8, FORMAT_BITS, EXPORTS)

@@ -33,6 +33,32 @@ cudaError_t control_loop_node(liets_ctx* c, cudaGraph_t graph, cudaGraphNode_t a
     return cudaGraphAddKernelNode(node, graph, &after, 1, &p);
 }
 
+// The same for the grids of a batch (liets_generate_batch): thread i steps grid i; the loop goes round while any grid is live.
+struct ControlBatch { int n; Control* ctl[32]; };
+
+__global__ void k_control_loop_batch(ControlBatch b, cudaGraphConditionalHandle loop) {
+    int live = 0;
+    if ((int)threadIdx.x < b.n) {
+        control_step(b.ctl[threadIdx.x], kCtlFinish | kCtlPrepare);
+        live = __ldcg(&b.ctl[threadIdx.x]->active) ? 1 : 0;
+    }
+    live = __syncthreads_or(live);
+    if (threadIdx.x == 0) cudaGraphSetConditional(loop, live ? 1u : 0u);
+}
+
+cudaError_t control_loop_batch_node(liets_ctx* const* ctx, int n, cudaGraph_t graph, cudaGraphNode_t after,
+                                    cudaGraphConditionalHandle loop, cudaGraphNode_t* node) {
+    if (n < 1 || n > 32) return cudaErrorInvalidValue;
+    ControlBatch b = {};
+    b.n = n;
+    for (int i = 0; i < n; ++i) b.ctl[i] = ctx[i]->ctl;
+    void* args[] = { &b, &loop };
+    cudaKernelNodeParams p = {};
+    p.func = reinterpret_cast<void*>(k_control_loop_batch);
+    p.gridDim = dim3(1); p.blockDim = dim3(32); p.sharedMemBytes = 0; p.kernelParams = args;
+    return cudaGraphAddKernelNode(node, graph, &after, 1, &p);
+}
+
 __global__ void k_begin(Control* c, int generate, uint32_t max_steps) {
     c->steps_done = 0;
     c->max_steps = max_steps;

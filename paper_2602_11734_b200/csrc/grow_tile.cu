@@ -40,6 +40,7 @@ constexpr int kThreads = 128;
 #endif
 constexpr int kCtasPerSm = LIETS_TILE_CTAS;       // resident CTAs per SM the kernel is compiled for (registers) and launched with
 constexpr int kWarps = kThreads / 32;
+constexpr int kMaxBatch = 16;                   // grids per launch of the batched kernel (kernel parameters: 2.2 KB)
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
 constexpr int kWin = 64 * kTileW / 16;          // 18-bit windows per row, one per 16 voxels
 constexpr int kQueueCap = 128;                  // tied voxels per warp queue (a ring; power of two)
@@ -147,13 +148,39 @@ __device__ __forceinline__ uint32_t opaque_shared_addr(const void* p) {     // a
     return a;
 }
 
-__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(Control* __restrict__ ctl, TileGeom g,
-                                                           unsigned long long* G0, unsigned long long* G1,
-                                                           uint32_t* stamp, uint32_t* weight, uint32_t* list0, uint32_t* list1,
-                                                           PhiloxKey key) {
-    if (!ctl->active || (ctl->mode == 0u && !ctl->pending)) return;     // small fronts run in k_grow_vox
+// The grids of one launch: one for liets_step / liets_generate, up to kMaxBatch equally shaped grids for
+// liets_generate_batch (independent realisations).  A CTA starts with grid blockIdx.x mod n and then
+// visits the others in turn: each grid hands its tiles out through its own cursor, so CTAs that find a grid's list used
+// up move on and the whole GPU works on whatever is left -- small grids, whose few tiles cannot fill it, overlap.
+template <int MAXB>
+struct TileBatch {
+    int n;
+    Control* ctl[MAXB];
+    unsigned long long* G0[MAXB];
+    unsigned long long* G1[MAXB];
+    uint32_t* stamp[MAXB];
+    uint32_t* weight[MAXB];
+    uint32_t* list0[MAXB];
+    uint32_t* list1[MAXB];
+    PhiloxKey key[MAXB];
+};
+
+template <int MAXB>
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid_constant__ TileBatch<MAXB> B, const TileGeom g) {
     __shared__ __align__(16) Smem S;        // static (< 48 KB): shared-memory addresses are immediates, not generic pointers
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  for (int bk = 0; bk < (MAXB == 1 ? 1 : B.n); ++bk) {
+    const int gi = MAXB == 1 ? 0 : (int)((blockIdx.x + (uint32_t)bk) % (uint32_t)B.n);
+    if (MAXB > 1) __syncthreads();          // the previous grid's last tile is no longer read
+    Control* __restrict__ ctl = B.ctl[gi];
+    if (!ctl->active || (ctl->mode == 0u && !ctl->pending)) continue;   // small fronts run in k_grow_vox
+    unsigned long long* const G0 = B.G0[gi];
+    unsigned long long* const G1 = B.G1[gi];
+    uint32_t* const stamp = B.stamp[gi];
+    uint32_t* const weight = B.weight[gi];
+    uint32_t* const list0 = B.list0[gi];
+    uint32_t* const list1 = B.list1[gi];
+    const PhiloxKey& key = B.key[gi];
 
     const uint32_t cur = ctl->cur;
     // the list of step t: heavy tiles in slots [0, n_head), light ones in the last n_back slots; heavy ones are handed
@@ -489,23 +516,37 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(Control* __r
     }
     if (lane == 0 && new_solid) atomicAdd(&ctl->claims, new_solid);
     if (lane == 0 && n_items0) { atomicAdd(&ctl->items, n_items + n_items0); atomicAdd(&ctl->items0, n_items0); }
+  }
 }
 
 }  // namespace
 
 int grow_tile_words() { return kTileW; }
 int grow_tile_ctas_per_sm() { return kCtasPerSm; }
+int grow_tile_max_batch() { return kMaxBatch; }
 
-// per-device function attribute, set once per context at liets_create: 8 CTAs x 26.8 KB of shared memory per SM
+// per-device function attribute, set once per context at liets_create: the SM's shared memory to the CTAs
 cudaError_t grow_tile_attributes() {
     static_assert(sizeof(Smem) <= 48 * 1024, "static shared memory");
-    return cudaFuncSetAttribute(k_grow_tile, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    cudaError_t e = cudaFuncSetAttribute(k_grow_tile<1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_grow_tile<kMaxBatch>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+}
+
+template <int MAXB>
+static void fill_batch(TileBatch<MAXB>* b, liets_ctx* const* ctx, int n) {
+    b->n = n;
+    for (int i = 0; i < n; ++i) {
+        liets_ctx* c = ctx[i];
+        b->ctl[i] = c->ctl; b->G0[i] = c->G[0]; b->G1[i] = c->G[1]; b->stamp[i] = c->stamp; b->weight[i] = c->weight;
+        b->list0[i] = c->list[0]; b->list1[i] = c->list[1]; b->key[i] = philox_make_key(c->rng_seed);
+    }
 }
 
 cudaError_t launch_grow_tile(liets_ctx* c) {
-    const PhiloxKey key = philox_make_key(c->rng_seed);
-    k_grow_tile<<<c->tile_grid, kThreads, 0, c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->stamp, c->weight,
-                                                                      c->list[0], c->list[1], key);
+    TileBatch<1> b;
+    fill_batch(&b, &c, 1);
+    k_grow_tile<1><<<c->tile_grid, kThreads, 0, c->stream>>>(b, c->geom);
     c->launches++;
     return cudaGetLastError();
 }
@@ -513,11 +554,24 @@ cudaError_t launch_grow_tile(liets_ctx* c) {
 // The same launch as a kernel node of `graph` (exec == nullptr), or its parameters refreshed in an instantiated
 // graph (the Philox key changes with every liets_seed).
 cudaError_t grow_tile_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node) {
-    PhiloxKey key = philox_make_key(c->rng_seed);
-    void* args[] = { &c->ctl, &c->geom, &c->G[0], &c->G[1], &c->stamp, &c->weight, &c->list[0], &c->list[1], &key };
+    TileBatch<1> b;
+    fill_batch(&b, &c, 1);
+    void* args[] = { &b, &c->geom };
     cudaKernelNodeParams p = {};
-    p.func = reinterpret_cast<void*>(k_grow_tile);
+    p.func = reinterpret_cast<void*>(k_grow_tile<1>);
     p.gridDim = dim3(c->tile_grid); p.blockDim = dim3(kThreads); p.sharedMemBytes = 0; p.kernelParams = args;
+    return exec ? cudaGraphExecKernelNodeSetParams(exec, *node, &p) : cudaGraphAddKernelNode(node, graph, nullptr, 0, &p);
+}
+
+// n equally shaped grids (n <= kMaxBatch) in one kernel node; the launch is the first grid's
+cudaError_t grow_tile_batch_node(liets_ctx* const* ctx, int n, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node) {
+    if (n < 1 || n > kMaxBatch) return cudaErrorInvalidValue;
+    TileBatch<kMaxBatch> b = {};
+    fill_batch(&b, ctx, n);
+    void* args[] = { &b, &ctx[0]->geom };
+    cudaKernelNodeParams p = {};
+    p.func = reinterpret_cast<void*>(k_grow_tile<kMaxBatch>);
+    p.gridDim = dim3(ctx[0]->tile_grid); p.blockDim = dim3(kThreads); p.sharedMemBytes = 0; p.kernelParams = args;
     return exec ? cudaGraphExecKernelNodeSetParams(exec, *node, &p) : cudaGraphAddKernelNode(node, graph, nullptr, 0, &p);
 }
 

@@ -494,6 +494,138 @@ int liets_seed_info(liets_ctx* c, uint32_t* n_candidates, uint32_t* slow_path) {
     return LIETS_OK;
 }
 
+// ---- batched realisations ---------------------------------------------------
+int liets_create_batch(liets_batch** out, int n, int nx, int ny, int nz, int boundary, void* workspace, size_t workspace_bytes,
+                       void* cuda_stream) {
+    if (!out) return LIETS_E_ARG;
+    *out = nullptr;
+    if (n < 1 || n > grow_tile_max_batch()) return LIETS_E_ARG;
+    const size_t each = liets_workspace_bytes(nx, ny, nz, LIETS_STORAGE_TILE);
+    if (each == 0) return LIETS_E_ARG;
+    if (workspace && workspace_bytes < each * (size_t)n) return LIETS_E_CAPACITY;
+    liets_batch* b = new (std::nothrow) liets_batch();
+    if (!b) return LIETS_E_CUDA;
+    memset(b, 0, sizeof(*b));
+    b->n = n;
+    b->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    int rc = LIETS_OK;
+    for (int i = 0; i < n && rc == LIETS_OK; ++i)
+        rc = liets_create(&b->ctx[i], nx, ny, nz, boundary, LIETS_STORAGE_TILE,
+                          workspace ? static_cast<char*>(workspace) + each * (size_t)i : nullptr, workspace ? each : 0, cuda_stream);
+    if (rc == LIETS_OK && (cudaEventCreate(&b->ev0) != cudaSuccess || cudaEventCreate(&b->ev1) != cudaSuccess)) rc = LIETS_E_CUDA;
+    if (rc != LIETS_OK) { cudaGetLastError(); liets_destroy_batch(b); return rc; }
+    *out = b;
+    return LIETS_OK;
+}
+
+void liets_destroy_batch(liets_batch* b) {
+    if (!b) return;
+    cudaStreamSynchronize(b->stream);
+    if (b->exec) cudaGraphExecDestroy(b->exec);
+    if (b->graph) cudaGraphDestroy(b->graph);
+    if (b->ev0) cudaEventDestroy(b->ev0);
+    if (b->ev1) cudaEventDestroy(b->ev1);
+    for (int i = 0; i < b->n; ++i) liets_destroy(b->ctx[i]);
+    delete b;
+}
+
+liets_ctx* liets_batch_ctx(liets_batch* b, int i) { return (b && i >= 0 && i < b->n) ? b->ctx[i] : nullptr; }
+
+const char* liets_batch_last_error(const liets_batch* b) { return b ? b->err : "null batch"; }
+
+// WHILE(any grid live) { k_grow_tile over all grids ; one control step per grid }, built once, keys refreshed after re-seeding
+static bool ensure_batch_graph(liets_batch* b) {
+    bool same = b->exec != nullptr;
+    for (int i = 0; i < b->n && same; ++i) same = b->graph_seed[i] == b->ctx[i]->rng_seed;
+    if (same) return true;
+    if (b->exec) {
+        if (grow_tile_batch_node(b->ctx, b->n, nullptr, b->exec, &b->grow_node) == cudaSuccess) {
+            for (int i = 0; i < b->n; ++i) b->graph_seed[i] = b->ctx[i]->rng_seed;
+            return true;
+        }
+        cudaGetLastError();
+        cudaGraphExecDestroy(b->exec); cudaGraphDestroy(b->graph);
+        b->exec = nullptr; b->graph = nullptr;
+    }
+    cudaGraph_t g = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaGraphConditionalHandle loop;
+    cudaGraphNode_t while_node, grow_node, ctl_node;
+    bool ok = cudaGraphCreate(&g, 0) == cudaSuccess &&
+              cudaGraphConditionalHandleCreate(&loop, g, 1u, cudaGraphCondAssignDefault) == cudaSuccess;
+    if (ok) {
+        cudaGraphNodeParams wp = {};
+        wp.type = cudaGraphNodeTypeConditional;
+        wp.conditional.handle = loop;
+        wp.conditional.type = cudaGraphCondTypeWhile;
+        wp.conditional.size = 1;
+        ok = cudaGraphAddNode(&while_node, g, nullptr, 0, &wp) == cudaSuccess;
+        if (ok) {
+            cudaGraph_t body = wp.conditional.phGraph_out[0];
+            ok = grow_tile_batch_node(b->ctx, b->n, body, nullptr, &grow_node) == cudaSuccess &&
+                 control_loop_batch_node(b->ctx, b->n, body, grow_node, loop, &ctl_node) == cudaSuccess &&
+                 cudaGraphInstantiate(&exec, g, 0) == cudaSuccess;
+        }
+    }
+    if (!ok) {
+        cudaGetLastError();
+        if (exec) cudaGraphExecDestroy(exec);
+        if (g) cudaGraphDestroy(g);
+        return false;
+    }
+    b->graph = g; b->exec = exec; b->grow_node = grow_node;
+    for (int i = 0; i < b->n; ++i) b->graph_seed[i] = b->ctx[i]->rng_seed;
+    return true;
+}
+
+#define LIETS_BATCH_TRY(b, expr)                                                                       \
+    do {                                                                                               \
+        cudaError_t e__ = (expr);                                                                      \
+        if (e__ != cudaSuccess) {                                                                      \
+            snprintf((b)->err, sizeof((b)->err), "%s:%d: %s: %s", __FILE__, __LINE__, #expr, cudaGetErrorString(e__)); \
+            return LIETS_E_CUDA;                                                                       \
+        }                                                                                              \
+    } while (0)
+
+int liets_generate_batch(liets_batch* b, const double* target_solid_fraction, uint32_t max_steps, int* status_out,
+                         uint32_t* steps_out, uint64_t* n_solid_out, float* device_ms_out) {
+    if (!b || !target_solid_fraction) return LIETS_E_ARG;
+    for (int i = 0; i < b->n; ++i) {
+        liets_ctx* c = b->ctx[i];
+        if (!(target_solid_fraction[i] > 0.0 && target_solid_fraction[i] <= 1.0)) { snprintf(b->err, sizeof(b->err), "target solid fraction of grid %d outside (0,1]", i); return LIETS_E_ARG; }
+        if (!c->seeded) { snprintf(b->err, sizeof(b->err), "liets_generate_batch before liets_seed of grid %d", i); return LIETS_E_STATE; }
+    }
+    LIETS_BATCH_TRY(b, cudaEventRecord(b->ev0, b->stream));
+    for (int i = 0; i < b->n; ++i) {
+        liets_ctx* c = b->ctx[i];
+        const uint32_t thr = c->vox_thr;
+        c->vox_thr = 0;                                     // the batched loop runs on tiles from its first step
+        int rc = liets_set_target(c, target_solid_fraction[i]);             // (also sends vox_thr to the device)
+        c->vox_thr = thr;
+        if (rc) { snprintf(b->err, sizeof(b->err), "grid %d: %s", i, c->err); return rc; }
+        LIETS_BATCH_TRY(b, launch_begin(c, 1, max_steps));
+        c->prof_n = 0;
+        LIETS_BATCH_TRY(b, launch_control(c, kCtlPrepare));
+        LIETS_BATCH_TRY(b, launch_tiles_from_grid(c));
+    }
+    if (!ensure_batch_graph(b)) { snprintf(b->err, sizeof(b->err), "the batch graph could not be built"); return LIETS_E_CUDA; }
+    LIETS_BATCH_TRY(b, cudaGraphLaunch(b->exec, b->stream));
+    for (int i = 0; i < b->n; ++i) LIETS_BATCH_TRY(b, launch_set_params(b->ctx[i]));      // the contexts' own thresholds again
+    LIETS_BATCH_TRY(b, cudaEventRecord(b->ev1, b->stream));
+    for (int i = 0; i < b->n; ++i) {
+        liets_ctx* c = b->ctx[i];
+        if (int rc = readback(c)) { snprintf(b->err, sizeof(b->err), "grid %d: %s", i, c->err); return rc; }
+        c->launches += 1ull + c->pinned->steps_done;        // its share of the batched loop: one control step per step
+        if (status_out) status_out[i] = c->pinned->status;
+        if (steps_out) steps_out[i] = c->pinned->steps_done;
+        if (n_solid_out) n_solid_out[i] = c->pinned->n_solid;
+    }
+    LIETS_BATCH_TRY(b, cudaEventSynchronize(b->ev1));
+    LIETS_BATCH_TRY(b, cudaEventElapsedTime(&b->gen_ms, b->ev0, b->ev1));
+    if (device_ms_out) *device_ms_out = b->gen_ms;
+    return LIETS_OK;
+}
+
 int liets_debug_thresholds(const uint64_t* R, const uint64_t* n_t, const uint64_t* n_solid, uint64_t* T_out, uint32_t n) {
     if (!R || !n_t || !n_solid || !T_out || n == 0) return LIETS_E_ARG;
     for (uint32_t i = 0; i < n; ++i)

@@ -72,6 +72,20 @@ struct liets_ctx {
     char err[256];
 };
 
+// liets_create_batch: equally shaped STORAGE_TILE contexts on one stream whose step loops run as ONE graph
+struct liets_batch {
+    int n;
+    liets_ctx* ctx[16];
+    cudaStream_t stream;
+    cudaGraph_t graph;
+    cudaGraphExec_t exec;
+    cudaGraphNode_t grow_node;
+    uint64_t graph_seed[16];          // rng seeds whose Philox keys the graph's growth node holds
+    cudaEvent_t ev0, ev1;
+    float gen_ms;
+    char err[256];
+};
+
 #define LIETS_CUDA_TRY(ctx, expr)                                                                 \
     do {                                                                                          \
         cudaError_t e__ = (expr);                                                                 \
@@ -93,6 +107,8 @@ cudaError_t launch_set_params(liets_ctx* c);
 cudaError_t launch_eq1_thresholds(const unsigned long long* dev_in, unsigned long long* dev_out, uint32_t n, cudaStream_t stream);
 cudaError_t control_loop_node(liets_ctx* c, cudaGraph_t graph, cudaGraphNode_t after, cudaGraphConditionalHandle loop,
                               cudaGraphNode_t* node);
+cudaError_t control_loop_batch_node(liets_ctx* const* ctx, int n, cudaGraph_t graph, cudaGraphNode_t after,
+                                    cudaGraphConditionalHandle loop, cudaGraphNode_t* node);
 // grow_u8.cu
 cudaError_t launch_grow_u8(liets_ctx* c);
 cudaError_t grow_u8_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);
@@ -108,6 +124,8 @@ cudaError_t grow_full_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec
 // grow_tile.cu
 cudaError_t launch_grow_tile(liets_ctx* c);
 cudaError_t grow_tile_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);
+cudaError_t grow_tile_batch_node(liets_ctx* const* ctx, int n, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);
+int grow_tile_max_batch();
 int grow_tile_words();
 int grow_tile_ctas_per_sm();
 // seed.cu

@@ -18,7 +18,8 @@ FORMAT_U8, FORMAT_BITS = 0, 1
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
            "liets_set_target", "liets_step", "liets_generate", "liets_grid", "liets_s2", "liets_step_log", "liets_timings",
            "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info",
-           "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_debug_thresholds", "liets_probe", "liets_destroy", "liets_last_error")
+           "liets_create_batch", "liets_batch_ctx", "liets_generate_batch", "liets_destroy_batch",
+           "liets_batch_last_error", "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_debug_thresholds", "liets_probe", "liets_destroy", "liets_last_error")
 PROBE_PHILOX, PROBE_LOP3, PROBE_IMAD, PROBE_MIX, PROBE_L2_READ, PROBE_HBM_READ = range(6)
 
 
@@ -85,6 +86,16 @@ def lib():
     L.liets_debug_vox_list.restype = ci
     L.liets_debug_thresholds.argtypes = [P(u64), P(u64), P(u64), P(u64), u32]
     L.liets_debug_thresholds.restype = ci
+    L.liets_create_batch.argtypes = [P(vp), ci, ci, ci, ci, ci, vp, sz, vp]
+    L.liets_create_batch.restype = ci
+    L.liets_batch_ctx.argtypes = [vp, ci]
+    L.liets_batch_ctx.restype = vp
+    L.liets_generate_batch.argtypes = [vp, P(dbl), u32, P(ci), P(u32), P(u64), P(ctypes.c_float)]
+    L.liets_generate_batch.restype = ci
+    L.liets_destroy_batch.argtypes = [vp]
+    L.liets_destroy_batch.restype = None
+    L.liets_batch_last_error.argtypes = [vp]
+    L.liets_batch_last_error.restype = ctypes.c_char_p
     L.liets_probe.argtypes = [ci, vp, sz, vp, ci, P(dbl), P(dbl)]
     L.liets_probe.restype = ci
     L.liets_destroy.argtypes = [vp]
@@ -147,9 +158,24 @@ class Liets:
             raise LietsError(rc, "liets_create failed")
         self._h = h
 
+    @classmethod
+    def _borrowed(cls, owner, handle, nx, ny, nz, boundary, device):
+        """A view of a generator owned by a LietsBatch (never destroyed from here)."""
+        import torch
+        self = cls.__new__(cls)
+        self._L, self._torch, self._owner = lib(), torch, owner
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self.N = nx * ny * nz
+        self.boundary, self.storage, self.device = boundary, STORAGE_TILE, device
+        self._ws, self._stream = None, None
+        self._h = ctypes.c_void_p(handle)
+        self._is_borrowed = True
+        return self
+
     def close(self):
         if getattr(self, "_h", None):
-            self._L.liets_destroy(self._h)
+            if not getattr(self, "_is_borrowed", False):
+                self._L.liets_destroy(self._h)
             self._h = None
             self._ws = None
 
@@ -255,3 +281,59 @@ class Liets:
     @property
     def launch_count(self):
         return int(self._L.liets_launch_count(self._h))
+
+
+class LietsBatch:
+    """n equally shaped STORAGE_TILE generators whose step loops run as one device-side loop (liets_create_batch).
+    batch[i] is the i-th generator: set_growth / seed / grid / s2 / step_log as usual; generate() runs them all."""
+
+    def __init__(self, n, nx, ny, nz, boundary=BOUNDARY_WALL, device="cuda:0", stream=None):
+        import torch
+        self._L = lib()
+        if not torch.cuda.is_available():
+            raise LietsError(E_CUDA, "no CUDA device (there is no CPU fallback)")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        each = self._L.liets_workspace_bytes(int(nx), int(ny), int(nz), STORAGE_TILE)
+        if each == 0 or n < 1:
+            raise LietsError(E_ARG, "bad batch size, grid dimensions")
+        self._ws = torch.empty(each * n + 256, dtype=torch.uint8, device=self.device)
+        base = (self._ws.data_ptr() + 255) // 256 * 256
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = ctypes.c_void_p()
+        rc = self._L.liets_create_batch(ctypes.byref(h), n, int(nx), int(ny), int(nz), int(boundary), ctypes.c_void_p(base), each * n,
+                                        ctypes.c_void_p(self._stream.cuda_stream))
+        if rc < 0:
+            raise LietsError(rc, "liets_create_batch failed")
+        self._h, self.n = h, n
+        self._items = [Liets._borrowed(self, self._L.liets_batch_ctx(h, i), int(nx), int(ny), int(nz), int(boundary), self.device)
+                       for i in range(n)]
+
+    def __getitem__(self, i):
+        return self._items[i]
+
+    def __len__(self):
+        return self.n
+
+    def generate(self, targets, max_steps=100000):
+        """targets: one solid fraction per grid (or one for all). Returns [(status, steps, n_solid)] and sets .device_ms."""
+        t = [float(targets)] * self.n if np.isscalar(targets) else [float(v) for v in targets]
+        arr = (ctypes.c_double * self.n)(*t)
+        st, steps, ns = (ctypes.c_int * self.n)(), (ctypes.c_uint32 * self.n)(), (ctypes.c_uint64 * self.n)()
+        ms = ctypes.c_float(0)
+        rc = self._L.liets_generate_batch(self._h, arr, max_steps, st, steps, ns, ctypes.byref(ms))
+        if rc < 0:
+            raise LietsError(rc, self._L.liets_batch_last_error(self._h).decode())
+        self.device_ms = float(ms.value)
+        return [(int(st[i]), int(steps[i]), int(ns[i])) for i in range(self.n)]
+
+    def close(self):
+        if getattr(self, "_h", None):
+            for it in self._items:
+                it._h = None
+            self._L.liets_destroy_batch(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        self.close()

@@ -365,3 +365,76 @@ def test_device_two_point_correlation_equals_oracle(liets, storage, periodic, di
         assert (vd == vo).all(), (axis, vd, vo)
         assert (pd == po).all(), (axis, np.flatnonzero(pd != po)[:5])
         assert pd[0] == L.N - o.n_solid
+
+
+def _batch_against_singles(liets, name, seeds, spacing=None):
+    """n realisations of one BASELINE.json config in ONE batched loop: every grid equals its own oracle run (stored hash
+    or live oracle) and its own liets_generate."""
+    import hashlib
+    import json
+    import os
+    c = CONFIGS[name]
+    s = spacing if spacing is not None else (c["s"] if isinstance(c["s"], int) else c["s"][0])
+    gold = {}
+    path = os.path.join(os.path.dirname(__file__), "golden", "fullsize_hashes.jsonl")
+    for l in open(path):
+        r = json.loads(l)
+        if r["config"] == name and r.get("kind") is None and r["s"] == s and r["target"] == c["targets"][0]:
+            gold[r["rng_seed"]] = r
+    B = liets.LietsBatch(len(seeds), *c["dims"], int(c["periodic"]))
+    n_seeds = []
+    for i, seed in enumerate(seeds):
+        B[i].set_growth(*c["g"], liets.LAW_EQ1)
+        n_seeds.append(B[i].seed(c["core"], s, seed))
+    res = B.generate(c["targets"][0])
+    for i, seed in enumerate(seeds):
+        rc, steps, n_solid = res[i]
+        g = B[i].grid()
+        if seed in gold:
+            r = gold[seed]
+            assert (n_seeds[i], rc, steps, n_solid) == (r["n_seeds"], r["status"], r["steps"], r["n_solid"])
+            assert hashlib.sha256(g.tobytes()).hexdigest() == r["sha256"], seed
+        else:
+            o = oracle.Oracle(*c["dims"], c["periodic"])
+            o.set_growth(*c["g"], 1)
+            assert o.seed(c["core"], s, seed) == n_seeds[i]
+            rc_o, st_o = o.generate(c["targets"][0])
+            assert (rc, steps, n_solid) == (rc_o, st_o, o.n_solid) and (g == o.grid()).all(), seed
+        f, sol, blocks = B[i].step_log()
+        assert len(sol) == steps and int(sol[-1]) == n_solid
+    # a second batched run after re-seeding half of the grids (the graph's keys are refreshed), and resuming the others
+    for i in range(0, len(seeds), 2):
+        B[i].seed(c["core"], s, seeds[i] + 100)
+    res2 = B.generate(min(1.0, c["targets"][0] + 0.05))
+    L = liets.Liets(*c["dims"], int(c["periodic"]), 1)
+    L.set_growth(*c["g"], liets.LAW_EQ1)
+    for i in (0, 1):
+        L.seed(c["core"], s, seeds[i] + (100 if i % 2 == 0 else 0))
+        if i % 2:
+            L.generate(c["targets"][0])
+        rc, steps, n_solid = L.generate(min(1.0, c["targets"][0] + 0.05))
+        assert (rc, n_solid) == (res2[i][0], res2[i][2]) and (L.grid() == B[i].grid()).all()
+    B.close()
+
+
+def test_batched_generate_config1_eight_realisations(liets):
+    _batch_against_singles(liets, "cfg1_64", [1, 2, 3, 4, 5, 6, 7, 8])
+
+
+def test_batched_generate_config2_seeds_1_to_4(liets):
+    _batch_against_singles(liets, "cfg2_200", [1, 2, 3, 4])
+
+
+def test_batch_argument_errors(liets):
+    with pytest.raises(liets.LietsError):
+        liets.LietsBatch(17, 8, 8, 8)
+    B = liets.LietsBatch(2, 8, 8, 8)
+    B[0].set_growth(0.1, 0.1, 0.1, 0)
+    B[0].seed(0.1, 0, 1)
+    with pytest.raises(liets.LietsError):                 # grid 1 is not seeded
+        B.generate(0.5)
+    B[1].set_growth(0.1, 0.1, 0.1, 0)
+    B[1].seed(0.0, 0, 1)                                   # no seeds at all: FRONT_EMPTY at once
+    res = B.generate([0.5, 0.5])
+    assert res[1][0] == liets.FRONT_EMPTY and res[1][1] == 0 and res[0][0] == liets.OK
+    B.close()

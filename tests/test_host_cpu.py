@@ -21,7 +21,7 @@ def liets():
 def test_library_exports_every_declared_symbol(liets):
     header = open(os.path.join(ROOT, "include", "liets.h")).read()
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
-    declared = set(re.findall(r"\b(liets_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(liets_[a-z0-9_]+)\s*\(", header))
     assert declared == set(liets.EXPORTS), declared ^ set(liets.EXPORTS)
     L = liets.lib()
     for name in declared:
