@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- whole-generation throughput of the LIETS growth path on B200 (one JSON line).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--storage 0|1]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--storage 0|1|2]
 
 A "step" is one pass of the whole hot path over one synthetic workload: liets_seed (keyed seeding +
 L1 seed spacing) followed by liets_generate (device-resident growth loop to the target fraction)
@@ -97,6 +97,8 @@ def algorithmic_bytes(storage, N, front, solid_after, n_seeds, on_tiles=None, fr
         prev = int(solid_after[t])
         if storage == 0:
             out.append(4 * a_t + min(27 * a_t, N) + c_t + 4 * a_n)
+        elif storage == 2:                            # full-field sweep: read g_t once, write g_{t+1} once
+            out.append(2 * ((N + 7) // 8))
         elif on_tiles is None or on_tiles[t]:
             out.append(4 * a_t + min(1625 * a_t, N // 8) + 1024 * a_t + 4 * a_n)
         else:
@@ -317,7 +319,7 @@ def run_ours(args):
             "dtype": "u32", "data": "synthetic",
             "config": {"workload": w["name"], "grid": [nx, ny, nz], "core_prob": w["core"], "spacing_s": w["s"],
                        "g_face_edge_corner": list(w["g"]), "target_solid_fraction": w["target"], "rng_seed": w["seed"],
-                       "storage": ["u8+voxel-list", "bit-rows+tile-list"][storage], "parallelism": "replicas" if world > 1 else "1gpu",
+                       "storage": ["u8+voxel-list", "bit-rows+voxel-list/tile-list", "bit-rows+full-field sweep (Algorithm 2)"][storage], "parallelism": "replicas" if world > 1 else "1gpu",
                        "l2": "flushed between iterations (256 MiB memset outside the timed events)",
                        "growth_steps": int(n_steps), "seeds": int(n_seeds), "final_solid": int(n_solid)},
             "seconds_per_generation": t_dev / args.steps * 1e-3,
@@ -422,7 +424,7 @@ BATCH_WORKLOADS = {"cfg1_64": (1, 2, 3, 4, 5, 6, 7, 8), "cfg2_200": (1, 2, 3, 4)
 DEFAULT_STORAGE = 1
 PHILOX_INT_OPS = 40
 PER_FRONT_VOXEL_OPS = 52
-KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_tile"}
+KERNEL_NAMES = {0: "k_grow_u8", 1: "k_grow_tile", 2: "k_grow_full"}
 
 
 def main():
