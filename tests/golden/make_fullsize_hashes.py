@@ -13,7 +13,11 @@ Each run appends one JSON line to fullsize_hashes.jsonl; runs take minutes to ho
 (kind "seeds").  --trace runs the same generation one step at a time (oracle_generate with max_steps = 1,
 which is the loop of PAPER.md:140 cut after every pass) and appends to fullsize_traces.jsonl, after
 EVERY step, the step index and solid count, plus the SHA-256 of the phase array every --hash-every
-steps: a run that is interrupted still leaves every completed step as an expected value.
+steps: a run that is interrupted still leaves every completed step as an expected value.  Steps that the trace file
+already holds for the same run are re-computed, CHECKED against the stored values and not written again, so a run can be
+repeated to extend an interrupted trace.  --omp uses liboracle_omp.so (the same oracle source compiled with -fopenmp, the
+front of the list step shared among the host's cores; tests/test_oracle_pins.py proves it equal to the serial library
+after every step): records made with it carry "oracle": "omp".
 """
 import argparse
 import hashlib
@@ -46,13 +50,14 @@ def main():
     ap.add_argument("--hash-every", type=int, default=4)
     ap.add_argument("--seed", type=int, default=None)
     ap.add_argument("--s", type=int, default=None)
+    ap.add_argument("--omp", action="store_true")
     a = ap.parse_args()
     c = CONFIGS[a.config]
     seed = a.seed if a.seed is not None else c["seeds"][0]
     s = a.s if a.s is not None else (c["s"] if isinstance(c["s"], int) else c["s"][0])
     nx, ny, nz = c["dims"]
     t0 = time.time()
-    o = oracle.Oracle(nx, ny, nz, c["periodic"])
+    o = oracle.Oracle(nx, ny, nz, c["periodic"], omp=a.omp)
     o.set_growth(*c["g"], 1)
     n_seeds = o.seed(c["core"], s, seed)
     t_seed = time.time() - t0
@@ -67,6 +72,12 @@ def main():
     if a.target is None:
         ap.error("--target is required unless --seeds-only")
     if a.trace:
+        have = {}
+        if os.path.exists(TRACE):
+            for line in open(TRACE):
+                r = json.loads(line)
+                if (r["config"], r["s"], r["rng_seed"], r["target"]) == (a.config, s, seed, a.target):
+                    have[r["step"]] = r
         steps, rc = 0, oracle.MAX_STEPS
         while rc == oracle.MAX_STEPS:
             rc, done = o.generate(a.target, 1, True)
@@ -75,8 +86,16 @@ def main():
                 break
             rec = dict(base, kind="trace", target=a.target, n_target=o.n_target, n_seeds=n_seeds, step=steps,
                        n_solid=o.n_solid, oracle_seconds=round(time.time() - t0, 1))
-            if steps % a.hash_every == 0 or rc != oracle.MAX_STEPS:
+            if a.omp:
+                rec["oracle"] = "omp"
+            old = have.get(steps)
+            if steps % a.hash_every == 0 or rc != oracle.MAX_STEPS or (old is not None and "sha256" in old):
                 rec["sha256"] = hashlib.sha256(o.grid().tobytes()).hexdigest()
+            if old is not None:                        # already recorded: check, do not write again
+                assert old["n_solid"] == rec["n_solid"] and old["n_seeds"] == rec["n_seeds"], (old, rec)
+                assert "sha256" not in old or old["sha256"] == rec["sha256"], (old, rec)
+                print("step %d agrees with the stored record" % steps, flush=True)
+                continue
             append(TRACE, rec)
             print(rec, flush=True)
     else:
@@ -85,6 +104,8 @@ def main():
     rec = dict(config=a.config, dims=[nx, ny, nz], periodic=c["periodic"], core=c["core"], s=s, rng_seed=seed,
                g=list(c["g"]), target=a.target, n_target=o.n_target, n_seeds=n_seeds, status=rc, steps=steps,
                n_solid=o.n_solid, sha256=h, oracle_seconds=round(time.time() - t0, 1), seed_seconds=round(t_seed, 1))
+    if a.omp:
+        rec["oracle"] = "omp"
     append(OUT, rec)
     print(rec)
 
