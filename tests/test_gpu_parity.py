@@ -209,8 +209,8 @@ def test_config2_bit_exact(liets, storage, seed):
         po, vo = oracle.s2(o.grid(), False, axis, 16)
         assert (pg == po).all() and (vg == vo).all()
         assert pg[0] == L.N - o.n_solid
-        XX
-        po, vo = oracle.s2(o.grid(), False, axis, 100)
+        pd, vd = L.s2(axis, 40)                        # the device's own pair counts (liets_s2)
+        po, vo = oracle.s2(o.grid(), False, axis, 40)
         assert (pd == po).all() and (vd == vo).all()
 
 
