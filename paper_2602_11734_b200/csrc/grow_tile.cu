@@ -36,16 +36,23 @@ namespace {
 constexpr int kTileW = 2;                       // 64-bit words per tile row
 constexpr int kThreads = 128;
 #ifndef LIETS_TILE_CTAS
-#define LIETS_TILE_CTAS 8
+#define LIETS_TILE_CTAS 10
 #endif
 constexpr int kCtasPerSm = LIETS_TILE_CTAS;       // resident CTAs per SM the kernel is compiled for (registers) and launched with
 constexpr int kWarps = kThreads / 32;
+#ifndef LIETS_VOX_PER_THREAD
+#define LIETS_VOX_PER_THREAD 2
+#endif
+constexpr int kVoxPerThread = LIETS_VOX_PER_THREAD;     // front voxels a thread handles per trip of phase C
 constexpr int kMaxBatch = 16;                   // grids per launch of the batched kernel (kernel parameters: 2.2 KB)
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
 constexpr int kWin = 64 * kTileW / 16;          // 18-bit windows per row, one per 16 voxels
 constexpr int kQueueCap = 128;                  // tied voxels per warp queue (a ring; power of two)
 constexpr int kHeavyFront = 64 * 64 * kTileW / 8;  // a tile with at least this many front voxels (1/8 of its cells) is "heavy"
-constexpr int kFrontCap = 32 * 64 * kTileW;     // front voxels listed at a time (half the tile; more -> several passes)
+#ifndef LIETS_FRONT_CAP
+#define LIETS_FRONT_CAP (32 * 64 * kTileW)
+#endif
+constexpr int kFrontCap = LIETS_FRONT_CAP;      // front voxels listed at a time (half the tile; more -> several passes)
 
 struct Smem {
     uint32_t win[100 * kWin];                   // row (z'+1)*10 + (y'+1), window k: not-void bits of tile x = 16k-1 .. 16k+16 at bits 14..31
@@ -169,6 +176,7 @@ template <int MAXB>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid_constant__ TileBatch<MAXB> B, const TileGeom g) {
     __shared__ __align__(16) Smem S;        // static (< 48 KB): shared-memory addresses are immediates, not generic pointers
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t lanes_below = (1u << lane) - 1u;
   for (int bk = 0; bk < (MAXB == 1 ? 1 : B.n); ++bk) {
     const int gi = MAXB == 1 ? 0 : (int)((blockIdx.x + (uint32_t)bk) % (uint32_t)B.n);
     if (MAXB > 1) __syncthreads();          // the previous grid's last tile is no longer read
@@ -385,9 +393,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
             }
             __syncthreads();                // flist (and win) complete
             const uint32_t n_pass = min((uint32_t)kFrontCap, n_front - pass0);
-            for (uint32_t i0 = 0; i0 < n_pass; i0 += kThreads) {   // C: one thread per front voxel
-                const uint32_t i = i0 + tid;
-                uint32_t tie = 0, fire = 0, v = 0;
+            // C: one thread per front voxel, kVoxPerThread voxels per thread and trip (their Philox chains interleave, the loop
+            // and ring bookkeeping is shared)
+            auto level0 = [&](uint32_t i, uint32_t& v, uint32_t& tie, uint32_t& fire) {
+                tie = 0; fire = 0; v = 0;
                 if (i < n_pass) {
                     {
                         uint16_t v16;
@@ -419,13 +428,22 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                         }
                     }
                 }
+            };
+            auto settle = [&](uint32_t v, uint32_t tie, uint32_t fire) {       // level-0 hits to the claim volume, ties to the ring
                 if (h0_any && __ballot_sync(0xffffffffu, fire != 0u)) claim(fire, (v & 0x7Fu) ^ 15u, (v >> 7) & 0x1FFu);
                 const uint32_t have = __ballot_sync(0xffffffffu, tie != 0u);
                 if (have) {
                     if (qn + 32u > (uint32_t)kQueueCap) do round(32u); while (qn >= 32u);
-                    if (tie) sts_u64(queue_addr + 8u * ((qh + qn + __popc(have & ((1u << lane) - 1u))) & ((uint32_t)kQueueCap - 1u)), v | (1u << 16), tie);
+                    if (tie) sts_u64(queue_addr + 8u * ((qh + qn + __popc(have & lanes_below)) & ((uint32_t)kQueueCap - 1u)), v | (1u << 16), tie);
                     qn += __popc(have);
                 }
+            };
+            for (uint32_t i0 = 0; i0 < n_pass; i0 += kVoxPerThread * kThreads) {
+                uint32_t v[kVoxPerThread], tie[kVoxPerThread], fire[kVoxPerThread];
+#pragma unroll
+                for (int u = 0; u < kVoxPerThread; ++u) level0(i0 + (uint32_t)u * kThreads + tid, v[u], tie[u], fire[u]);
+#pragma unroll
+                for (int u = 0; u < kVoxPerThread; ++u) settle(v[u], tie[u], fire[u]);
             }
         }
         while (qn) round(min(qn, 32u));
