@@ -40,7 +40,12 @@ enum {
     LIETS_E_CUDA = -4        /* CUDA runtime error or no device                                   */
 };
 
-enum { LIETS_BOUNDARY_WALL = 0, LIETS_BOUNDARY_PERIODIC = 1 };        /* R5 */
+enum { LIETS_BOUNDARY_WALL = 0,          /* neighbours outside the domain are dropped                  */
+       LIETS_BOUNDARY_PERIODIC = 1,      /* every coordinate wraps ("roll"), also on axes of length 1 or 2 (R5) */
+       LIETS_BOUNDARY_PERIODIC_XY = 2 }; /* x and y wrap, walls in z: a slab -- and with nz = 1 the TWO-DIMENSIONAL periodic
+                                            grid of Algorithm 2: the 8 in-plane directions only, because the
+                                            18 directions with dz != 0 have no target.  (nz = 1 with LIETS_BOUNDARY_WALL is the
+                                            2D grid of Algorithms 1 and 3, :53, :145.)                                     */
 enum { LIETS_STORAGE_U8 = 0,      /* uint8 grid + explicit list of front VOXELS (uint32 indices)  */
        LIETS_STORAGE_TILE = 1,    /* bit-packed x-rows; the active set is an explicit list of front VOXELS while it
                                      is small and an explicit list of active 128x8x8 TILES afterwards, whose front

@@ -145,15 +145,22 @@ def step_threshold(R, law, n_t, n_solid):
 
 
 def s2(grid, periodic, axis, rmax):
-    """grid: uint8 array of shape (nz, ny, nx). Returns (pairs, valid) uint64 arrays of r = 0..rmax."""
+    """grid: uint8 array of shape (nz, ny, nx); periodic: the boundary mode (0 walls, 1 torus, 2 periodic in x and y).
+    Returns (pairs, valid) uint64 arrays of r = 0..rmax."""
     g = np.ascontiguousarray(grid, dtype=np.uint8)
     nz, ny, nx = g.shape
     pairs = np.zeros(rmax + 1, dtype=np.uint64)
     valid = np.zeros(rmax + 1, dtype=np.uint64)
     P64 = ctypes.POINTER(ctypes.c_uint64)
-    lib().oracle_s2(g.ctypes.data, nx, ny, nz, int(periodic), axis, rmax,
+    lib().oracle_s2(g.ctypes.data, nx, ny, nz, (periodic_mask(periodic) >> axis) & 1, axis, rmax,
                     pairs.ctypes.data_as(P64), valid.ctypes.data_as(P64))
     return pairs, valid
+
+
+def periodic_mask(periodic):
+    """Boundary argument of the callers -> the oracle's per-axis mask: False / 0 = walls, True / 1 = torus (7),
+    2 = periodic in x and y between walls in z (3)."""
+    return {0: 0, 1: 7, 2: 3}[int(periodic)]
 
 
 class Oracle:
@@ -161,9 +168,9 @@ class Oracle:
 
     def __init__(self, nx, ny, nz, periodic=False, omp=False):
         self._L = lib(omp)
-        self.nx, self.ny, self.nz, self.periodic = nx, ny, nz, bool(periodic)
+        self.nx, self.ny, self.nz, self.periodic = nx, ny, nz, int(periodic)
         self.N = nx * ny * nz
-        self._h = self._L.oracle_new(nx, ny, nz, int(periodic))
+        self._h = self._L.oracle_new(nx, ny, nz, periodic_mask(periodic))
         if not self._h:
             raise ValueError("bad dimensions")
 

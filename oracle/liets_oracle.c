@@ -125,7 +125,7 @@ struct oracle_state {
 oracle_state* oracle_new(int nx, int ny, int nz, int periodic) {
     if (nx < 1 || ny < 1 || nz < 1) return NULL;
     oracle_state* o = (oracle_state*)calloc(1, sizeof(*o));
-    o->nx = nx; o->ny = ny; o->nz = nz; o->periodic = periodic ? 1 : 0;
+    o->nx = nx; o->ny = ny; o->nz = nz; o->periodic = periodic & 7;    /* bit 0: x wraps, bit 1: y, bit 2: z (R5) */
     o->N = (uint64_t)nx * (uint64_t)ny * (uint64_t)nz;
     o->grid = (uint8_t*)calloc(o->N, 1);
     o->cap_front = 1024;
@@ -170,13 +170,10 @@ static int neighbour(const oracle_state* o, uint64_t p, int d, uint64_t* q) {
     int64_t y = (int64_t)((p / (uint64_t)o->nx) % (uint64_t)o->ny);
     int64_t z = (int64_t)(p / ((uint64_t)o->nx * (uint64_t)o->ny));
     x += ORACLE_DIRS[d][0]; y += ORACLE_DIRS[d][1]; z += ORACLE_DIRS[d][2];
-    if (o->periodic) {
-        x = (x % o->nx + o->nx) % o->nx;
-        y = (y % o->ny + o->ny) % o->ny;
-        z = (z % o->nz + o->nz) % o->nz;
-    } else if (x < 0 || x >= o->nx || y < 0 || y >= o->ny || z < 0 || z >= o->nz) {
-        return 0;
-    }
+    /* per axis: wrapped if that axis is periodic ("roll"), else the neighbour must lie inside (:53, :145) */
+    if (o->periodic & 1) x = (x % o->nx + o->nx) % o->nx; else if (x < 0 || x >= o->nx) return 0;
+    if (o->periodic & 2) y = (y % o->ny + o->ny) % o->ny; else if (y < 0 || y >= o->ny) return 0;
+    if (o->periodic & 4) z = (z % o->nz + o->nz) % o->nz; else if (z < 0 || z >= o->nz) return 0;
     *q = (uint64_t)x + (uint64_t)o->nx * ((uint64_t)y + (uint64_t)o->ny * (uint64_t)z);
     return 1;
 }
@@ -213,8 +210,8 @@ static int64_t l1_dist(const oracle_state* o, uint64_t v, uint64_t w) {
     int64_t vx = (int64_t)(v % (uint64_t)o->nx), wx = (int64_t)(w % (uint64_t)o->nx);
     int64_t vy = (int64_t)((v / (uint64_t)o->nx) % (uint64_t)o->ny), wy = (int64_t)((w / (uint64_t)o->nx) % (uint64_t)o->ny);
     int64_t vz = (int64_t)(v / ((uint64_t)o->nx * (uint64_t)o->ny)), wz = (int64_t)(w / ((uint64_t)o->nx * (uint64_t)o->ny));
-    return axis_dist(vx, wx, o->nx, o->periodic) + axis_dist(vy, wy, o->ny, o->periodic) +
-           axis_dist(vz, wz, o->nz, o->periodic);
+    return axis_dist(vx, wx, o->nx, o->periodic & 1) + axis_dist(vy, wy, o->ny, o->periodic & 2) +
+           axis_dist(vz, wz, o->nz, o->periodic & 4);
 }
 
 int64_t oracle_seed(oracle_state* o, double core_prob, int spacing_s, uint64_t rng_seed) {

@@ -50,6 +50,8 @@ uint64_t oracle_target_count(double phi_s, uint64_t N);
  * law 0 = constant probability: T = R. */
 uint64_t oracle_step_threshold(uint64_t R, int law, uint64_t n_t, uint64_t n_solid);
 
+/* periodic: bit 0 = x wraps, bit 1 = y wraps, bit 2 = z wraps (R5); 0 = walls all round, 7 = torus, 3 = periodic in
+ * the x-y plane between walls in z (with nz = 1: the two-dimensional periodic grid of Algorithm 2) */
 oracle_state* oracle_new(int nx, int ny, int nz, int periodic);
 void oracle_free(oracle_state* o);
 

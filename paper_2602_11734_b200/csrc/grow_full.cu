@@ -37,7 +37,7 @@ __device__ __forceinline__ unsigned long long window34(const unsigned long long*
     unsigned long long left;
     if (b) left = (cur >> (b - 1)) & 1ull;
     else if (w > 0) left = __ldg(G + rb + w - 1) >> 63;
-    else left = g.periodic ? (__ldg(G + rb + ((g.nx - 1) >> 6)) >> ((g.nx - 1) & 63)) & 1ull : 1ull;
+    else left = (g.periodic & 1) ? (__ldg(G + rb + ((g.nx - 1) >> 6)) >> ((g.nx - 1) & 63)) & 1ull : 1ull;
     win |= left;
     // cell x0 + 32
     if (b) {                                                // it is in the next word, or across the row end
@@ -49,7 +49,7 @@ __device__ __forceinline__ unsigned long long window34(const unsigned long long*
     // the cell just beyond the row end, x = nx, is cell 0 of a periodic row
     const int iend = g.nx - (x0 - 1);                       // window bit of cell x = nx
     if (iend >= 0 && iend <= 33) {
-        const unsigned long long wrap = g.periodic ? __ldg(G + rb) & 1ull : 1ull;
+        const unsigned long long wrap = (g.periodic & 1) ? __ldg(G + rb) & 1ull : 1ull;
         win = (win & ~(1ull << iend)) | (wrap << iend);
     }
     return win & 0x3FFFFFFFFull;
@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(kFullThreads) k_grow_full(Control* __restrict_
         unsigned long long all_or = 0ull, all_and = ~0ull;
 #pragma unroll
         for (int e = 0; e < 9; ++e) {
-            const int Z = full_wrap(z + e / 3 - 1, g.nz, g.periodic), Y = full_wrap(y + e % 3 - 1, g.ny, g.periodic);
+            const int Z = full_wrap(z + e / 3 - 1, g.nz, g.periodic & 4), Y = full_wrap(y + e % 3 - 1, g.ny, g.periodic & 2);
             win[e] = (Z >= 0 && Y >= 0)
                    ? window34(Gc, (unsigned long long)g.Wp * ((unsigned long long)Y + (unsigned long long)g.ny * (unsigned long long)Z), x0, g)
                    : 0x3FFFFFFFFull;
@@ -122,9 +122,9 @@ __global__ void __launch_bounds__(kFullThreads) k_grow_full(Control* __restrict_
             const uint32_t d = __ffs(fire) - 1u;
             fire &= fire - 1u;
             const uint32_t raw = d + (d >= 13u ? 1u : 0u);
-            const int X = full_wrap(x + (int)(raw % 3u) - 1, g.nx, g.periodic);
-            const int Y = full_wrap(y + (int)((raw / 3u) % 3u) - 1, g.ny, g.periodic);
-            const int Z = full_wrap(z + (int)(raw / 9u) - 1, g.nz, g.periodic);
+            const int X = full_wrap(x + (int)(raw % 3u) - 1, g.nx, g.periodic & 1);
+            const int Y = full_wrap(y + (int)((raw / 3u) % 3u) - 1, g.ny, g.periodic & 2);
+            const int Z = full_wrap(z + (int)(raw / 9u) - 1, g.nz, g.periodic & 4);
             const unsigned long long w = (unsigned long long)(X >> 6) + (unsigned long long)g.Wp * ((unsigned long long)Y + (unsigned long long)g.ny * (unsigned long long)Z);
             const unsigned long long bit = 1ull << (X & 63);
             const unsigned long long old = atomicOr(Gn + w, bit);

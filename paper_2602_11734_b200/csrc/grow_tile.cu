@@ -47,7 +47,10 @@ constexpr int kVoxPerThread = LIETS_VOX_PER_THREAD;     // front voxels a thread
 constexpr int kMaxBatch = 16;                   // grids per launch of the batched kernel (kernel parameters: 2.2 KB)
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
 constexpr int kWin = 64 * kTileW / 16;          // 18-bit windows per row, one per 16 voxels
-constexpr int kQueueCap = 128;                  // tied voxels per warp queue (a ring; power of two)
+#ifndef LIETS_QUEUE_CAP
+#define LIETS_QUEUE_CAP 128
+#endif
+constexpr int kQueueCap = LIETS_QUEUE_CAP;      // tied voxels per warp queue (a ring; power of two, at least 64)
 constexpr int kHeavyFront = 64 * 64 * kTileW / 8;  // a tile with at least this many front voxels (1/8 of its cells) is "heavy"
 #ifndef LIETS_FRONT_CAP
 #define LIETS_FRONT_CAP (32 * 64 * kTileW)
@@ -79,7 +82,7 @@ __device__ __forceinline__ unsigned long long not_void_word(const unsigned long 
                                                             bool yz_ok, unsigned long long row_base, int wg) {
     if (!yz_ok) return ~0ull;
     if (wg < 0) {                               // only bit 63 (x = -1) is ever looked at
-        if (!g.periodic) return ~0ull;
+        if (!(g.periodic & 1)) return ~0ull;
         const int xl = g.nx - 1;
         return ((__ldcg(G + row_base + (xl >> 6)) >> (xl & 63)) & 1ull) << 63;
     }
@@ -88,7 +91,7 @@ __device__ __forceinline__ unsigned long long not_void_word(const unsigned long 
     unsigned long long v = xbase < g.nx ? __ldcg(G + row_base + wg) : 0ull;
     if (xbase + 64 > g.nx) {                    // the row ends inside this word: halo bit at x = nx, ones above
         const int nvalid = g.nx - xbase;        // 0..63
-        const unsigned long long halo = g.periodic ? (__ldcg(G + row_base) & 1ull) : 1ull;
+        const unsigned long long halo = (g.periodic & 1) ? (__ldcg(G + row_base) & 1ull) : 1ull;
         v |= (~0ull << nvalid);
         if (!halo) v &= ~(1ull << nvalid);
     }
@@ -252,8 +255,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
         const uint32_t p0 = (uint32_t)(64 * tc.w0) + (uint32_t)g.nx * ((uint32_t)tc.y0 + (uint32_t)g.ny * (uint32_t)tc.z0);
         for (int r = (int)tid; r < 100; r += kThreads) {    // one thread per row: the row's address once, its words as independent loads
             const int zl = r / 10 - 1, yl = r % 10 - 1;
-            const int zg = row_coord(zl, tc.z0, tc.wcz, g.nz, g.periodic);
-            const int yg = row_coord(yl, tc.y0, tc.wcy, g.ny, g.periodic);
+            const int zg = row_coord(zl, tc.z0, tc.wcz, g.nz, g.periodic & 4);
+            const int yg = row_coord(yl, tc.y0, tc.wcy, g.ny, g.periodic & 2);
             const bool ok = zg >= 0 && yg >= 0;
             const unsigned long long row_base = ok ? (unsigned long long)g.Wp * ((unsigned long long)yg + (unsigned long long)g.ny * (unsigned long long)zg) : 0ull;
             unsigned long long w[kRowWords];
@@ -456,8 +459,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
         auto halo_word = [&](int r, int c, unsigned long long cw) {
             const int zl = r / 10 - 1, yl = r % 10 - 1;
             const int wg = tc.w0 + c - 1;
-            const int zg = row_coord(zl, tc.z0, tc.wcz, g.nz, g.periodic);
-            const int yg = row_coord(yl, tc.y0, tc.wcy, g.ny, g.periodic);
+            const int zg = row_coord(zl, tc.z0, tc.wcz, g.nz, g.periodic & 4);
+            const int yg = row_coord(yl, tc.y0, tc.wcy, g.ny, g.periodic & 2);
             const unsigned long long row_base = (unsigned long long)g.Wp * ((unsigned long long)yg + (unsigned long long)g.ny * (unsigned long long)zg);
             unsigned long long in_row = 0ull, wrap = 0ull;
             int x_wrap = 0;

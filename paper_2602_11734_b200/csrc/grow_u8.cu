@@ -15,20 +15,20 @@ namespace liets {
 
 namespace {
 
-struct GridDims { int nx, ny, nz; };
+struct GridDims { int nx, ny, nz, periodic; };    // periodic: bit 0 = x wraps, bit 1 = y, bit 2 = z (R5)
 
 template <bool PERIODIC>
 __device__ __forceinline__ bool neighbour(int d, uint32_t p, int x, int y, int z, const GridDims& g,
                                           uint32_t* q) {
     const int dx = dir_dx(d), dy = dir_dy(d), dz = dir_dz(d);
     int X = x + dx, Y = y + dy, Z = z + dz;
-    if (PERIODIC) {
-        if (dx < 0 && X < 0) X = g.nx - 1;
-        if (dx > 0 && X >= g.nx) X = 0;
-        if (dy < 0 && Y < 0) Y = g.ny - 1;
-        if (dy > 0 && Y >= g.ny) Y = 0;
-        if (dz < 0 && Z < 0) Z = g.nz - 1;
-        if (dz > 0 && Z >= g.nz) Z = 0;
+    if (PERIODIC) {                         // some axis wraps: per axis, wrap or stay inside
+        if (X < 0) { if (!(g.periodic & 1)) return false; X = g.nx - 1; }
+        if (X >= g.nx) { if (!(g.periodic & 1)) return false; X = 0; }
+        if (Y < 0) { if (!(g.periodic & 2)) return false; Y = g.ny - 1; }
+        if (Y >= g.ny) { if (!(g.periodic & 2)) return false; Y = 0; }
+        if (Z < 0) { if (!(g.periodic & 4)) return false; Z = g.nz - 1; }
+        if (Z >= g.nz) { if (!(g.periodic & 4)) return false; Z = 0; }
         *q = (uint32_t)X + (uint32_t)g.nx * ((uint32_t)Y + (uint32_t)g.ny * (uint32_t)Z);
         return true;
     } else {
@@ -141,10 +141,10 @@ __global__ void __launch_bounds__(256) k_grow_u8(Control* __restrict__ ctl, uint
 }  // namespace
 
 cudaError_t launch_grow_u8(liets_ctx* c) {
-    const GridDims dims{ c->nx, c->ny, c->nz };
+    const GridDims dims{ c->nx, c->ny, c->nz, c->periodic };
     const PhiloxKey key = philox_make_key(c->rng_seed);
     const int grid = c->sm_count * 8;
-    if (c->boundary)
+    if (c->periodic)
         k_grow_u8<true><<<grid, 256, 0, c->stream>>>(c->ctl, c->grid_u8, c->list[0], c->list[1], dims, key);
     else
         k_grow_u8<false><<<grid, 256, 0, c->stream>>>(c->ctl, c->grid_u8, c->list[0], c->list[1], dims, key);
@@ -153,11 +153,11 @@ cudaError_t launch_grow_u8(liets_ctx* c) {
 }
 
 cudaError_t grow_u8_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node) {
-    GridDims dims{ c->nx, c->ny, c->nz };
+    GridDims dims{ c->nx, c->ny, c->nz, c->periodic };
     PhiloxKey key = philox_make_key(c->rng_seed);
     void* args[] = { &c->ctl, &c->grid_u8, &c->list[0], &c->list[1], &dims, &key };
     cudaKernelNodeParams p = {};
-    p.func = c->boundary ? reinterpret_cast<void*>(k_grow_u8<true>) : reinterpret_cast<void*>(k_grow_u8<false>);
+    p.func = c->periodic ? reinterpret_cast<void*>(k_grow_u8<true>) : reinterpret_cast<void*>(k_grow_u8<false>);
     p.gridDim = dim3(c->sm_count * 8); p.blockDim = dim3(256); p.sharedMemBytes = 0; p.kernelParams = args;
     return exec ? cudaGraphExecKernelNodeSetParams(exec, *node, &p) : cudaGraphAddKernelNode(node, graph, nullptr, 0, &p);
 }

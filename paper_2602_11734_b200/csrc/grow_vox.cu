@@ -81,10 +81,10 @@ __device__ __forceinline__ void vox_step(Control* __restrict__ ctl, const TileGe
             uint32_t raw27 = 0;                             // bit 9(dz+1) + 3(dy+1) + (dx+1): that neighbour exists and is void
 #pragma unroll
             for (int e = 0; e < 9; ++e) {                   // N_d, C_d (Algorithm 3 lines 5-6), one x-row at a time
-                const int Z = wrap_coord(z + e / 3 - 1, g.nz, g.periodic), Y = wrap_coord(y + e % 3 - 1, g.ny, g.periodic);
+                const int Z = wrap_coord(z + e / 3 - 1, g.nz, g.periodic & 4), Y = wrap_coord(y + e % 3 - 1, g.ny, g.periodic & 2);
                 if (Z >= 0 && Y >= 0)
                     raw27 |= void3(G0, (unsigned long long)g.Wp * ((unsigned long long)Y + (unsigned long long)g.ny * (unsigned long long)Z),
-                                   x, g.nx, g.periodic) << (3 * e);
+                                   x, g.nx, g.periodic & 1) << (3 * e);
             }
             mask = (raw27 & 0x1FFFu) | ((raw27 >> 14) << 13);          // the centre (bit 13) is p itself
             if (mask & en26) {
@@ -104,9 +104,9 @@ __device__ __forceinline__ void vox_step(Control* __restrict__ ctl, const TileGe
                         const uint32_t d = __ffs(fire) - 1u;
                         fire &= fire - 1u;
                         const uint32_t raw = d + (d >= 13u ? 1u : 0u);
-                        const int X = wrap_coord(x + (int)(raw % 3u) - 1, g.nx, g.periodic);
-                        const int Y = wrap_coord(y + (int)((raw / 3u) % 3u) - 1, g.ny, g.periodic);
-                        const int Z = wrap_coord(z + (int)(raw / 9u) - 1, g.nz, g.periodic);
+                        const int X = wrap_coord(x + (int)(raw % 3u) - 1, g.nx, g.periodic & 1);
+                        const int Y = wrap_coord(y + (int)((raw / 3u) % 3u) - 1, g.ny, g.periodic & 2);
+                        const int Z = wrap_coord(z + (int)(raw / 9u) - 1, g.nz, g.periodic & 4);
                         const unsigned long long w = (unsigned long long)(X >> 6) + (unsigned long long)g.Wp * ((unsigned long long)Y + (unsigned long long)g.ny * (unsigned long long)Z);
                         bb[k] = 1ull << (X & 63);
                         dd[k] = d;
@@ -138,9 +138,9 @@ __device__ __forceinline__ void vox_step(Control* __restrict__ ctl, const TileGe
                 const uint32_t d = __ffs(won) - 1u;
                 won &= won - 1u;
                 const uint32_t raw = d + (d >= 13u ? 1u : 0u);
-                const int X = wrap_coord(x + (int)(raw % 3u) - 1, g.nx, g.periodic);
-                const int Y = wrap_coord(y + (int)((raw / 3u) % 3u) - 1, g.ny, g.periodic);
-                const int Z = wrap_coord(z + (int)(raw / 9u) - 1, g.nz, g.periodic);
+                const int X = wrap_coord(x + (int)(raw % 3u) - 1, g.nx, g.periodic & 1);
+                const int Y = wrap_coord(y + (int)((raw / 3u) % 3u) - 1, g.ny, g.periodic & 2);
+                const int Z = wrap_coord(z + (int)(raw / 9u) - 1, g.nz, g.periodic & 4);
                 out[off++] = (uint32_t)X + (uint32_t)g.nx * ((uint32_t)Y + (uint32_t)g.ny * (uint32_t)Z);
             }
         }

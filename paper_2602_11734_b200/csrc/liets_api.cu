@@ -178,7 +178,7 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
     *out = nullptr;
     Layout L;
     if (!make_layout(nx, ny, nz, storage, &L)) return LIETS_E_ARG;
-    if (boundary != LIETS_BOUNDARY_WALL && boundary != LIETS_BOUNDARY_PERIODIC) return LIETS_E_ARG;
+    if (boundary != LIETS_BOUNDARY_WALL && boundary != LIETS_BOUNDARY_PERIODIC && boundary != LIETS_BOUNDARY_PERIODIC_XY) return LIETS_E_ARG;
     if (workspace && workspace_bytes < L.total) return LIETS_E_CAPACITY;
     if (workspace && (reinterpret_cast<uintptr_t>(workspace) % kAlign)) return LIETS_E_ARG;
     int n_dev = 0;
@@ -188,6 +188,7 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
     if (!c) return LIETS_E_CUDA;
     memset(c, 0, sizeof(*c));
     c->nx = nx; c->ny = ny; c->nz = nz; c->boundary = boundary; c->storage = storage;
+    c->periodic = boundary == LIETS_BOUNDARY_PERIODIC ? 7 : boundary == LIETS_BOUNDARY_PERIODIC_XY ? 3 : 0;
     c->N = (uint64_t)nx * (uint64_t)ny * (uint64_t)nz;
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     c->law = LIETS_LAW_EQ1;
@@ -217,7 +218,7 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
         c->scratch_u8 = reinterpret_cast<uint8_t*>(base + L.cand);
         c->list_cap = L.list_cap;
         if (storage != LIETS_STORAGE_U8) {
-            c->geom = TileGeom{ nx, ny, nz, L.Wp, L.ntx, L.nty, L.ntz, boundary };
+            c->geom = TileGeom{ nx, ny, nz, L.Wp, L.ntx, L.nty, L.ntz, c->periodic };
             c->n_tiles = L.n_tiles;
             c->grid_words = L.grid_words;
             c->G[0] = reinterpret_cast<unsigned long long*>(base + L.g0);
@@ -438,7 +439,7 @@ int liets_s2(liets_ctx* c, int axis, int rmax, uint64_t* pairs, uint64_t* valid)
     if (!ok) { cudaGetLastError(); return fail(c, LIETS_E_CUDA, "liets_s2 failed on the device"); }
     const uint64_t n[3] = { (uint64_t)c->nx, (uint64_t)c->ny, (uint64_t)c->nz };
     for (int r = 0; r <= rmax; ++r)                         // positions counted: all of them if periodic, else those with x + r inside
-        valid[r] = c->boundary == LIETS_BOUNDARY_PERIODIC ? c->N : ((uint64_t)r < n[axis] ? c->N / n[axis] * (n[axis] - (uint64_t)r) : 0);
+        valid[r] = ((c->periodic >> axis) & 1) ? c->N : ((uint64_t)r < n[axis] ? c->N / n[axis] * (n[axis] - (uint64_t)r) : 0);
     return LIETS_OK;
 }
 

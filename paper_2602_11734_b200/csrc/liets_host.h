@@ -12,11 +12,13 @@ struct HostReadback {                 // pinned; filled by cudaMemcpyAsync from 
 };
 
 namespace liets {
-struct TileGeom { int nx, ny, nz, Wp, ntx, nty, ntz, periodic; };   // Wp = 64-bit words per x-row; nt* = tiles per axis
+struct TileGeom { int nx, ny, nz, Wp, ntx, nty, ntz, periodic; };   // Wp = 64-bit words per x-row; nt* = tiles per axis;
+                                                                    // periodic: bit 0 = x wraps, bit 1 = y, bit 2 = z (R5)
 }
 
 struct liets_ctx {
     int nx, ny, nz, boundary, storage;
+    int periodic;                     // per-axis mask of the boundary mode: bit 0 = x wraps, bit 1 = y, bit 2 = z
     uint64_t N;
     cudaStream_t stream;
     void* ws;

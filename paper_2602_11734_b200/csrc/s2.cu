@@ -112,7 +112,7 @@ __global__ void k_u8_to_rows(const uint8_t* __restrict__ grid, S2Geom g, unsigne
 
 // pairs_dev: rmax + 1 zeroed 64-bit counters on the device; rows: the bit rows to use (nullptr = the ctx's current grid)
 cudaError_t launch_s2(liets_ctx* c, int axis, int rmax, unsigned long long* pairs_dev, unsigned long long* rows_scratch) {
-    S2Geom g{ c->nx, c->ny, c->nz, (c->nx + 63) / 64, c->boundary };
+    S2Geom g{ c->nx, c->ny, c->nz, (c->nx + 63) / 64, (c->periodic >> axis) & 1 };      // only the lag axis's boundary matters
     const unsigned long long* G;
     if (c->storage == LIETS_STORAGE_U8) {
         k_u8_to_rows<<<c->sm_count * 8, 256, 0, c->stream>>>(c->grid_u8, g, rows_scratch);

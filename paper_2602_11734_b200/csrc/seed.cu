@@ -146,7 +146,7 @@ __device__ __forceinline__ uint32_t rank_of(const uint32_t* status2, const uint3
 }
 
 // --- seed spacing -------------------------------------------------------------------------------
-struct Dims { int nx, ny, nz, periodic; };
+struct Dims { int nx, ny, nz, periodic; };      // periodic: bit 0 = x wraps, bit 1 = y, bit 2 = z (R5)
 
 constexpr int kAdjBuf = 96;                     // neighbours a warp can buffer per candidate
 
@@ -178,24 +178,23 @@ __device__ __forceinline__ void scan_diamond(const uint32_t* status2, uint32_t v
     const int y = (int)(rest % (uint32_t)g.ny), z = (int)(rest / (uint32_t)g.ny);
     const int r = s - 1;                                    // diamond radius: L1 <= s-1  <=>  L1 < s
     const int side = 2 * r + 1;
-    // without wrap-around, lower-index voxels have dz < 0, or dz = 0 and dy <= 0
+    // without any wrap-around, lower-index voxels have dz < 0, or dz = 0 and dy <= 0; with a periodic axis the whole
+    // diamond is walked and `limit` (on_word sees indices below v only) keeps the lower ones
+    const int px = g.periodic & 1, py = g.periodic & 2, pz = g.periodic & 4;
     const int n_rows = g.periodic ? side * side : (r + 1) * side;
     for (int j = (int)lane; j < n_rows; j += 32) {
         const int dz = j / side - r, dy = j % side - r;
         const int rem = r - abs(dz) - abs(dy);
         if (rem < 0) continue;
         int Y = y + dy, Z = z + dz;
-        if (g.periodic) {
-            Y %= g.ny; if (Y < 0) Y += g.ny;
-            Z %= g.nz; if (Z < 0) Z += g.nz;
-        } else if (Y < 0 || Y >= g.ny || Z < 0 || Z >= g.nz || (dz == 0 && dy > 0)) {
-            continue;
-        }
+        if (!g.periodic && dz == 0 && dy > 0) continue;
+        if (py) { Y %= g.ny; if (Y < 0) Y += g.ny; } else if (Y < 0 || Y >= g.ny) continue;
+        if (pz) { Z %= g.nz; if (Z < 0) Z += g.nz; } else if (Z < 0 || Z >= g.nz) continue;
         const unsigned long long row = ((unsigned long long)Z * g.ny + Y) * (unsigned long long)g.nx;
         int xa = x - rem, xb = x + rem;
-        if (g.periodic && 2 * rem + 1 >= g.nx) {            // the range covers the whole row
+        if (px && 2 * rem + 1 >= g.nx) {                    // the range covers the whole row
             scan_segment(status2, row, row + g.nx - 1, v, on_word);
-        } else if (!g.periodic) {                           // clipped at the walls
+        } else if (!px) {                                   // clipped at the walls
             xa = xa < 0 ? 0 : xa;
             xb = xb >= g.nx ? g.nx - 1 : xb;
             scan_segment(status2, row + xa, row + xb, v, on_word);
@@ -266,7 +265,8 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
     const int r = s - 1;                                    // diamond radius: L1 <= s-1  <=>  L1 < s
     // slices to visit: dz = -r..0 between walls (lower index = lower z, or same z and lower row), all slices within r
     // on the torus (each once)
-    const int n_slices = g.periodic ? min(2 * r + 1, g.nz) : r + 1;
+    const int px = g.periodic & 1, py = g.periodic & 2, pz = g.periodic & 4;
+    const int n_slices = pz ? min(2 * r + 1, g.nz) : r + 1;
     for (uint32_t i = warp_global; i < n; i += n_warps) {
         const uint32_t v = cand[i];
         const int x = (int)(v % (uint32_t)g.nx);
@@ -276,7 +276,7 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
         __syncwarp();
         for (int t = (int)lane; t < n_slices; t += 32) {
             int Z = z - r + t, dz;
-            if (g.periodic) {
+            if (pz) {
                 if (n_slices == g.nz) Z = t;                // the diamond covers every slice
                 Z %= g.nz; if (Z < 0) Z += g.nz;
                 dz = abs(Z - z); dz = min(dz, g.nz - dz);
@@ -288,9 +288,9 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
             if (rho < 0) continue;
             int ya = y - rho, yb = y + rho;
             int run_lo[2], run_hi[2], n_runs = 1;           // row runs [lo, hi] inside the slice
-            if (!g.periodic) {
+            if (!py) {
                 run_lo[0] = max(ya, 0); run_hi[0] = min(yb, g.ny - 1);
-                if (Z == z) run_hi[0] = min(run_hi[0], y);  // same slice: only rows up to the candidate's own
+                if (Z == z && !g.periodic) run_hi[0] = min(run_hi[0], y);   // same slice, no wrap anywhere: only rows up to the candidate's own
             } else if (2 * rho + 1 >= g.ny) {
                 run_lo[0] = 0; run_hi[0] = g.ny - 1;
             } else {
@@ -306,7 +306,8 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
                     const int wx = (int)(w % (uint32_t)g.nx);
                     const int wy = (int)((w / (uint32_t)g.nx) % (uint32_t)g.ny);
                     int dx = abs(wx - x), dy = abs(wy - y);
-                    if (g.periodic) { dx = min(dx, g.nx - dx); dy = min(dy, g.ny - dy); }
+                    if (px) dx = min(dx, g.nx - dx);
+                    if (py) dy = min(dy, g.ny - dy);
                     if (dx + dy + dz <= r) {
                         const uint32_t slot = atomicAdd(&s_cnt[warp], 1u);
                         if (slot < (uint32_t)kAdjBuf) s_buf[warp][slot] = k;
@@ -580,7 +581,7 @@ cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all
 // candidates resolved in rank order by one CTA with the statuses in shared memory; a cooperative rescan kernel
 // takes over only when the lists do not fit (it returns at once otherwise)
 cudaError_t launch_spacing(liets_ctx* c, int s) {
-    Dims g{ c->nx, c->ny, c->nz, c->boundary };
+    Dims g{ c->nx, c->ny, c->nz, c->periodic };
     unsigned long long N = c->N;
     k_seed_rows<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->coff, c->rowoff, g);
     c->launches++;

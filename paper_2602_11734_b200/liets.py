@@ -9,7 +9,7 @@ _LIB_PATH = os.path.join(_HERE, "libliets.so")
 
 OK, FRONT_EMPTY, MAX_STEPS = 0, 1, 2
 E_ARG, E_STATE, E_CAPACITY, E_CUDA = -1, -2, -3, -4
-BOUNDARY_WALL, BOUNDARY_PERIODIC = 0, 1
+BOUNDARY_WALL, BOUNDARY_PERIODIC, BOUNDARY_PERIODIC_XY = 0, 1, 2
 STORAGE_U8, STORAGE_TILE, STORAGE_FULL = 0, 1, 2
 LAW_CONSTANT, LAW_EQ1 = 0, 1
 FORMAT_U8, FORMAT_BITS = 0, 1

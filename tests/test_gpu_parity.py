@@ -68,7 +68,7 @@ def test_config1_bit_exact(liets, storage):
 
 
 @pytest.mark.parametrize("storage", STORAGES_ALL)
-@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("periodic", [False, True, 2])      # 2 = LIETS_BOUNDARY_PERIODIC_XY: x and y wrap, walls in z
 @pytest.mark.parametrize("dims,core,s", [((37, 29, 41), 0.01, 4), ((70, 45, 33), 0.004, 7), ((5, 4, 3), 0.2, 2),
                                           ((1, 9, 2), 0.3, 0), ((96, 96, 96), 0.003, 9), ((17, 130, 9), 0.02, 3),
                                           ((24, 20, 28), 0.5, 8)])    # > 96 lower neighbours per candidate: the rescan path of the spacing
@@ -292,7 +292,7 @@ def _fuzz_cases(n, seed=2024):
         dims = tuple(int(v) for v in rng.choice([1, 2, 3, 7, 8, 9, 15, 16, 17, 31, 33, 63, 64, 65, 70, 129, 140], 3))
         if dims[0] * dims[1] * dims[2] > 300000:
             dims = (dims[0], min(dims[1], 33), min(dims[2], 33))
-        cases.append(dict(dims=dims, periodic=bool(rng.integers(0, 2)), core=float(rng.choice([0.002, 0.01, 0.05, 0.3])),
+        cases.append(dict(dims=dims, periodic=int(rng.integers(0, 3)), core=float(rng.choice([0.002, 0.01, 0.05, 0.3])),
                           s=int(rng.choice([0, 1, 2, 3, 5, 9])), seed=int(rng.integers(0, 2**40)),
                           g=tuple(float(v) for v in rng.choice([0.0, 0.003, 0.02, 0.07, 0.2, 0.6, 1.0], 3)),
                           law=int(rng.integers(0, 2)), target=float(rng.choice([0.2, 0.5, 0.9, 1.0])), storage=k % 6))
@@ -352,7 +352,7 @@ def test_eq1_thresholds_on_device_against_big_integers(liets):
 
 
 @pytest.mark.parametrize("storage", STORAGES)
-@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("periodic", [False, True, 2])
 @pytest.mark.parametrize("dims", [(70, 45, 33), (130, 9, 17), (5, 4, 3), (1, 9, 2), (64, 64, 8), (191, 3, 2)])
 def test_device_two_point_correlation_equals_oracle(liets, storage, periodic, dims):
     """liets_s2 (exact void-void pair counts on the device, R16) against the oracle's plain triple loop, every axis, lags
@@ -438,3 +438,12 @@ def test_batch_argument_errors(liets):
     res = B.generate([0.5, 0.5])
     assert res[1][0] == liets.FRONT_EMPTY and res[1][1] == 0 and res[0][0] == liets.OK
     B.close()
+
+
+@pytest.mark.parametrize("storage", STORAGES_ALL)
+@pytest.mark.parametrize("periodic", [0, 2])
+@pytest.mark.parametrize("dims", [(150, 97, 1), (64, 200, 1), (9, 1, 1)])
+def test_two_dimensional_grids_bit_exact(liets, storage, periodic, dims):
+    """Two-dimensional grids (Algorithms 1-3 are stated in 2D): nz = 1 between walls (mode 0) or periodic in
+    the plane (mode 2, the "roll" of :76), seeding with spacing and growth to the target against the oracle."""
+    run_both(liets, dims, periodic, 0.01, 5, 4, (0.08, 0.03, 0.01), 1, 0.6, storage)

@@ -452,3 +452,92 @@ def test_openmp_build_of_the_list_oracle_equals_the_serial_oracle(dims, periodic
         assert a.n_solid == b.n_solid and (a.grid() == b.grid()).all(), a.step_index
     ra, rb = a.generate(min(1.0, phi + 0.2)), b.generate(min(1.0, phi + 0.2))
     assert ra == rb and a.n_solid == b.n_solid and (a.grid() == b.grid()).all()
+
+
+# ------------------------------------------------------------------------------------------ boundary mode 2 (R5)
+def _mask(periodic):
+    return {0: (False, False, False), 1: (True, True, True), 2: (True, True, False)}[int(periodic)]
+
+
+def test_two_dimensional_periodic_grid_uses_the_eight_in_plane_directions():
+    """PAPER.md:68 / :76: Algorithm 2 is stated for a two-dimensional grid with "roll" (periodic) shifts.  nz = 1 with
+    x and y periodic between walls in z (boundary mode 2) is that grid: the 18 directions with dz != 0 have no target,
+    so they are never attempted; face growth at probability 1 gives wrapped 2D diamonds of 2k^2 + 2k + 1 cells, all eight
+    in-plane directions give wrapped squares of (2k + 1)^2 cells; edge only (the four diagonals) keeps parity."""
+    nx, ny = 31, 27
+    x, y, _ = coords((1, ny, nx))
+    c = (2, 25)
+    ax, ay = axis_d(x, c[0], nx, True), axis_d(y, c[1], ny, True)
+    o = oracle.Oracle(nx, ny, 1, 2)
+    o.set_growth(1.0, 0.0, 0.0, 0)
+    o.seed_explicit([c[0] + nx * c[1]])
+    for k in range(1, 12):
+        o.step(False)                                   # the full-field definition (it also counts the attempts)
+        assert (o.grid() == (ax + ay <= k)).all(), k
+        assert o.n_solid == 2 * k * k + 2 * k + 1
+    attempts, successes = o.rates()
+    for d in range(26):
+        dx, dy, dz, cls = oracle.direction(d)
+        assert (attempts[d] > 0) == (dz == 0), d        # a void target was only ever seen in the eight in-plane directions
+        assert (successes[d] > 0) == (dz == 0 and cls == 1), d   # and only the four faces could fire
+    o.set_growth(1.0, 1.0, 1.0, 0)
+    o.seed_explicit([c[0] + nx * c[1]])
+    for k in range(1, 10):
+        o.step(True)
+        assert (o.grid() == (np.maximum(ax, ay) <= k)).all() and o.n_solid == (2 * k + 1) ** 2
+    o.set_growth(0.0, 1.0, 0.0, 0)
+    o.seed_explicit([c[0] + nx * c[1]])
+    for k in range(1, 6):
+        o.step(True)
+    assert (o.grid() == ((ax <= 5) & (ay <= 5) & ((ax + ay) % 2 == 0))).all()
+    # the same plane with walls all round (nz = 1, mode 0) clips instead of wrapping
+    w = oracle.Oracle(nx, ny, 1, 0)
+    w.set_growth(1.0, 0.0, 0.0, 0)
+    w.seed_explicit([c[0] + nx * c[1]])
+    for k in range(1, 6):
+        w.step(True)
+    assert (w.grid() == (np.abs(x - c[0]) + np.abs(y - c[1]) <= 5)).all()
+
+
+@pytest.mark.parametrize("use_list", [True, False])
+def test_slab_periodic_in_plane_walls_in_z_against_brute_force_distances(use_list):
+    nx, ny, nz = 19, 13, 6
+    x, y, z = coords((nz, ny, nx))
+    seeds = [(0, 0, 0), (18, 12, 5), (9, 1, 3)]
+    for g, metric in (((1.0, 0.0, 0.0), "l1"), ((1.0, 1.0, 1.0), "cheb")):
+        o = oracle.Oracle(nx, ny, nz, 2)
+        o.set_growth(*g, 0)
+        o.seed_explicit([sx + nx * (sy + ny * sz) for sx, sy, sz in seeds])
+        for k in range(1, 7):
+            o.step(use_list)
+            per = []
+            for sx, sy, sz in seeds:
+                dx, dy, dz = axis_d(x, sx, nx, True), axis_d(y, sy, ny, True), axis_d(z, sz, nz, False)
+                per.append(dx + dy + dz if metric == "l1" else np.maximum(np.maximum(dx, dy), dz))
+            assert (o.grid() == (np.min(per, axis=0) <= k)).all(), (metric, k)
+
+
+@pytest.mark.parametrize("s", [2, 4, 7])
+def test_spacing_with_in_plane_periodicity_equals_brute_force_greedy(s):
+    """Seed spacing when only x and y wrap: the accepted set is the ascending-index greedy under the L1
+    distance that wraps in x and y and not in z -- brute force over all pairs."""
+    nx, ny, nz = 18, 11, 9
+    N = nx * ny * nz
+    seed, c = 21 + s, 0.03
+    Tc = oracle.prob_to_threshold(c)
+    cand = [v for v in range(N) if oracle.seed_draw(seed, v) < Tc]
+    dims = np.array([nx, ny, nz])
+    wrap = np.array([True, True, False])
+
+    def dist(a, b):
+        d = np.abs(np.asarray(a) - np.asarray(b))
+        return int(np.where(wrap, np.minimum(d, dims - d), d).sum())
+    acc = []
+    for v in cand:
+        p = (v % nx, (v // nx) % ny, v // (nx * ny))
+        if all(dist(p, q) >= s for q in acc):
+            acc.append(p)
+    o = oracle.Oracle(nx, ny, nz, 2)
+    assert o.seed(c, s, seed) == len(acc)
+    got = np.flatnonzero(o.grid().ravel())
+    assert [(v % nx, (v // nx) % ny, v // (nx * ny)) for v in got] == acc
