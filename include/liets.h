@@ -90,6 +90,20 @@ int liets_seed(liets_ctx* ctx, double core_prob, int spacing_s, uint64_t rng_see
  * staged in the library's seeding scratch: n <= max(8, N/2), else E_CAPACITY; an index >= N is E_ARG. */
 int liets_seed_explicit(liets_ctx* ctx, const uint64_t* idx, uint64_t n, uint64_t rng_seed);
 
+/* Multi-phase growth, independent phases (PAPER.md:40 step 4: "The remaining phases are generated on the still unassigned
+ * cells ... its cores are placed and grown in the same way as for the first phase, using its own core probability and
+ * growth probabilities"): hand over the cells the phases grown before have taken.  mask: N bytes, non-zero = taken
+ * (LIETS_FORMAT_U8) or ceil(N/8) bytes, bit idx%8 of byte idx/8 (LIETS_FORMAT_BITS) -- what liets_grid writes, so one
+ * phase's output is the next phase's input; HOST or DEVICE memory (mask_is_device); the library keeps a copy.  Those cells
+ * are NOT VOID (never cores, never claimed, and they close a front voxel's neighbourhood like solid cells) and NOT OF THIS
+ * PHASE (never sources, not counted in n_solid, not in liets_grid's output; liets_s2 counts the cells no phase has taken).
+ * The target fraction stays a fraction of all N cells.  mask = NULL clears.  Takes effect at the next liets_seed /
+ * liets_seed_explicit (E_STATE from step / generate / grid until then).  A front that dies inside an enclosure of taken
+ * cells may be found empty one (claim-less) step after the serial algorithm would: status and grid are the same.
+ * Phase-interaction probabilities I_i^{n,m} (growth of a phase ON the surface of another) are not provided.
+ * Errors: E_ARG (format), E_CAPACITY (mask_bytes), E_CUDA.  Synchronises. */
+int liets_set_blocked(liets_ctx* ctx, const void* mask, size_t mask_bytes, int format, int mask_is_device);
+
 /* Target solid volume fraction phi_s in (0,1]: n_t = ceil(phi_s*N) (R7). Used by Eq. (1) and by
  * the stopping rule. */
 int liets_set_target(liets_ctx* ctx, double target_solid_fraction);

@@ -96,6 +96,8 @@ def lib(omp=False):
     L.oracle_permute_front.restype = None
     L.oracle_s2.argtypes = [vp, ci, ci, ci, ci, ci, ci, P(u64), P(u64)]
     L.oracle_s2.restype = None
+    L.oracle_set_blocked.argtypes = [vp, vp]
+    L.oracle_set_blocked.restype = ci
     L.oracle_threads.argtypes = []
     L.oracle_threads.restype = ci
     if omp:
@@ -215,10 +217,23 @@ class Oracle:
             raise RuntimeError("oracle generate: error %d" % rc)
         return rc, int(steps.value)
 
-    def grid(self):
-        """uint8 copy of the phase array, shape (nz, ny, nx), 1 = solid."""
+    def set_blocked(self, mask):
+        """Cells of earlier growing phases (array of N entries, non-zero = taken; None clears). Seed again afterwards."""
+        if mask is None:
+            self._L.oracle_set_blocked(self._h, None)
+        else:
+            m = np.ascontiguousarray(np.asarray(mask).ravel() != 0, dtype=np.uint8)
+            assert m.size == self.N
+            self._L.oracle_set_blocked(self._h, m.ctypes.data)
+
+    def phase_map(self):
+        """uint8 copy of the raw phase array: 0 void, 1 this phase, 2 an earlier phase (set_blocked)."""
         ptr = self._L.oracle_grid(self._h)
         return np.ctypeslib.as_array(ptr, shape=(self.N,)).reshape(self.nz, self.ny, self.nx).copy()
+
+    def grid(self):
+        """uint8 copy of the phase array of THIS phase, shape (nz, ny, nx), 1 = solid."""
+        return (self.phase_map() == 1).astype(np.uint8)
 
     @property
     def n_solid(self):

@@ -108,7 +108,8 @@ uint64_t oracle_step_threshold(uint64_t R, int law, uint64_t n_t, uint64_t n_sol
 struct oracle_state {
     int nx, ny, nz, periodic;
     uint64_t N;
-    uint8_t* grid;            /* phase array, 1 = solid, 0 = void */
+    uint8_t* grid;            /* phase array, 1 = solid, 0 = void; 2 = a cell of an earlier phase (PAPER.md:40 step 4) */
+    uint8_t* blocked;         /* NULL, or N bytes: 1 = the cell belongs to an earlier growing phase */
     uint64_t* front;          /* active set A */
     uint64_t n_front, cap_front;
     uint64_t n_solid;
@@ -135,7 +136,7 @@ oracle_state* oracle_new(int nx, int ny, int nz, int periodic) {
 
 void oracle_free(oracle_state* o) {
     if (!o) return;
-    free(o->grid); free(o->front); free(o);
+    free(o->grid); free(o->blocked); free(o->front); free(o);
 }
 
 int oracle_set_growth(oracle_state* o, double g_face, double g_edge, double g_corner, int law) {
@@ -187,8 +188,26 @@ static int has_void_neighbour(const oracle_state* o, uint64_t p) {
     return 0;
 }
 
+/* Multi-phase growth, independent phases (PAPER.md:40 step 4: "The remaining phases are generated on the still
+ * unassigned cells ... its cores are placed and grown in the same way as for the first phase"): cells of the phases grown
+ * before are given as a mask.  They are not void -- never cores, never claimed -- and not of this phase -- never sources,
+ * not counted in n_solid.  mask = NULL clears.  Takes effect at the next seeding. */
+int oracle_set_blocked(oracle_state* o, const uint8_t* mask) {
+    free(o->blocked);
+    o->blocked = NULL;
+    if (mask) {
+        o->blocked = (uint8_t*)malloc(o->N);
+        for (uint64_t v = 0; v < o->N; ++v) o->blocked[v] = mask[v] ? 1 : 0;
+    }
+    o->seeded = 0;
+    return 0;
+}
+
 static void reset_run(oracle_state* o, uint64_t rng_seed) {
     memset(o->grid, 0, o->N);
+    if (o->blocked)
+        for (uint64_t v = 0; v < o->N; ++v)
+            if (o->blocked[v]) o->grid[v] = 2;
     o->n_front = 0; o->n_solid = 0; o->step = 0; o->rng_seed = rng_seed; o->seeded = 1;
     memset(o->attempts, 0, sizeof(o->attempts));
     memset(o->successes, 0, sizeof(o->successes));
@@ -219,6 +238,7 @@ int64_t oracle_seed(oracle_state* o, double core_prob, int spacing_s, uint64_t r
     reset_run(o, rng_seed);
     uint64_t T_core = oracle_prob_to_threshold(core_prob);
     for (uint64_t v = 0; v < o->N; ++v) {
+        if (o->grid[v] != 0) continue;                                     /* an earlier phase's cell: not unassigned */
         if ((uint64_t)oracle_seed_draw(rng_seed, v) >= T_core) continue;   /* not a candidate */
         int ok = 1;
         if (spacing_s > 1) {
@@ -280,7 +300,7 @@ int oracle_step_full(oracle_state* o) {
     free(next);
     /* phi_a recomputed from the phase array; the front is rebuilt by definition */
     o->n_solid = 0; o->n_front = 0;
-    for (uint64_t p = 0; p < o->N; ++p) o->n_solid += o->grid[p];
+    for (uint64_t p = 0; p < o->N; ++p) o->n_solid += (o->grid[p] == 1);
     for (uint64_t p = 0; p < o->N; ++p)
         if (o->grid[p] == 1 && has_void_neighbour(o, p)) front_push(o, p);
     o->step++;

@@ -75,6 +75,9 @@ int oracle_generate(oracle_state* o, double phi_s, uint32_t max_steps, int use_l
                     uint32_t* steps_out);
 
 int oracle_threads(void);
+/* cells of earlier growing phases (N bytes, non-zero = taken; NULL clears): not void, not of this phase (PAPER.md:40 step 4,
+ * independent phases).  oracle_grid then holds 2 in those cells.  Takes effect at the next oracle_seed. */
+int oracle_set_blocked(oracle_state* o, const uint8_t* mask);
 const uint8_t* oracle_grid(const oracle_state* o);          /* N bytes in {0,1}, x fastest */
 uint64_t oracle_n_solid(const oracle_state* o);
 uint64_t oracle_n_front_exact(const oracle_state* o);       /* #solid cells with a void neighbour */

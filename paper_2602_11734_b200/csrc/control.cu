@@ -68,9 +68,10 @@ __global__ void k_begin(Control* c, int generate, uint32_t max_steps) {
 
 __global__ void k_set_params(Control* c, unsigned long long R0, unsigned long long R1,
                              unsigned long long R2, uint32_t law, unsigned long long n_t,
-                             uint32_t has_target, unsigned long long N, uint32_t list_cap, uint32_t vox_cap, uint32_t vox_thr) {
+                             uint32_t has_target, unsigned long long N, unsigned long long n_free, uint32_t list_cap,
+                             uint32_t vox_cap, uint32_t vox_thr) {
     c->R[0] = R0; c->R[1] = R1; c->R[2] = R2;
-    c->law = law; c->n_t = n_t; c->has_target = has_target; c->N = N; c->list_cap = list_cap;
+    c->law = law; c->n_t = n_t; c->has_target = has_target; c->N = N; c->n_free = n_free; c->list_cap = list_cap;
     c->vox_cap = vox_cap; c->vox_thr = vox_thr;
 }
 
@@ -100,7 +101,8 @@ cudaError_t launch_begin(liets_ctx* c, int generate, uint32_t max_steps) {
 
 cudaError_t launch_set_params(liets_ctx* c) {
     k_set_params<<<1, 1, 0, c->stream>>>(c->ctl, c->R[0], c->R[1], c->R[2], (uint32_t)c->law, c->n_t,
-                                         c->has_target ? 1u : 0u, c->N, (uint32_t)c->list_cap, c->vox_cap, c->vox_thr);
+                                         c->has_target ? 1u : 0u, c->N, c->N - (c->has_blocked ? c->n_blocked : 0), (uint32_t)c->list_cap,
+                                         c->vox_cap, c->vox_thr);
     c->launches++;
     return cudaGetLastError();
 }

@@ -56,7 +56,8 @@ __device__ __forceinline__ unsigned long long window34(const unsigned long long*
 }
 
 __global__ void __launch_bounds__(kFullThreads) k_grow_full(Control* __restrict__ ctl, TileGeom g, unsigned long long* G0,
-                                                             unsigned long long* G1, PhiloxKey key) {
+                                                             unsigned long long* G1, const unsigned long long* __restrict__ P,
+                                                             PhiloxKey key) {
     if (!ctl->active) return;
     __shared__ __align__(16) uint32_t s_hpat[8][4];
     const uint32_t t = ctl->step;
@@ -94,9 +95,10 @@ __global__ void __launch_bounds__(kFullThreads) k_grow_full(Control* __restrict_
         const uint32_t own32 = (uint32_t)(win[4] >> 1);                     // cells x0 .. x0+31 (not-void = solid or beyond the row)
         uint32_t in_row = 0xFFFFFFFFu;
         if (x0 + 32 > g.nx) in_row = ~(~0u << (g.nx - x0));
-        const uint32_t solid32 = own32 & in_row;
+        uint32_t solid32 = own32 & in_row;
         // carry g_t into g_{t+1} (one atomic per segment that holds solid cells)
         if (lane == 0 && solid32) atomicOr(Gn + own_word_idx, (unsigned long long)solid32 << (x0 & 63));
+        if (P) solid32 &= ~(uint32_t)(__ldg(P + own_word_idx) >> (x0 & 63));   // cells of earlier phases are carried, but are no sources
         // nothing solid in the centre row's cells, or no void cell anywhere around: no attempt can exist here
         if (solid32 == 0u || all_and == 0x3FFFFFFFFull || all_or == 0ull) continue;
         const int x = x0 + (int)lane;
@@ -147,14 +149,15 @@ __global__ void __launch_bounds__(kFullThreads) k_grow_full(Control* __restrict_
 
 cudaError_t launch_grow_full(liets_ctx* c) {
     const PhiloxKey key = philox_make_key(c->rng_seed);
-    k_grow_full<<<c->sm_count * 8, kFullThreads, 0, c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], key);
+    k_grow_full<<<c->sm_count * 8, kFullThreads, 0, c->stream>>>(c->ctl, c->geom, c->G[0], c->G[1], c->has_blocked ? c->prow : nullptr, key);
     c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t grow_full_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node) {
     PhiloxKey key = philox_make_key(c->rng_seed);
-    void* args[] = { &c->ctl, &c->geom, &c->G[0], &c->G[1], &key };
+    const unsigned long long* P = c->has_blocked ? c->prow : nullptr;
+    void* args[] = { &c->ctl, &c->geom, &c->G[0], &c->G[1], &P, &key };
     cudaKernelNodeParams p = {};
     p.func = reinterpret_cast<void*>(k_grow_full);
     p.gridDim = dim3(c->sm_count * 8); p.blockDim = dim3(kFullThreads); p.sharedMemBytes = 0; p.kernelParams = args;

@@ -172,6 +172,7 @@ struct TileBatch {
     uint32_t* weight[MAXB];
     uint32_t* list0[MAXB];
     uint32_t* list1[MAXB];
+    const unsigned long long* P[MAXB];      // cells of earlier phases in row layout (liets_set_blocked), or nullptr
     PhiloxKey key[MAXB];
 };
 
@@ -191,6 +192,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
     uint32_t* const weight = B.weight[gi];
     uint32_t* const list0 = B.list0[gi];
     uint32_t* const list1 = B.list1[gi];
+    const unsigned long long* const P = B.P[gi];
     const PhiloxKey& key = B.key[gi];
 
     const uint32_t cur = ctl->cur;
@@ -299,6 +301,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
             if (y < tc.wcy && z < tc.wcz && xbase < g.nx) {
                 unsigned long long src = S.own[f_row][f_j];
                 if (xbase + 64 > g.nx) src &= ~(~0ull << (g.nx - xbase));               // padding is not a source
+                if (P) src &= ~__ldg(P + (unsigned long long)g.Wp * ((unsigned long long)(tc.y0 + y) + (unsigned long long)g.ny * (unsigned long long)(tc.z0 + z)) + (unsigned long long)(tc.w0 + f_j));   // nor is a cell of an earlier phase
                 if (src) {                                                              // (sparse early steps: most words hold no solid)
                     unsigned long long anyvoid = 0ull;
 #pragma unroll
@@ -560,7 +563,8 @@ static void fill_batch(TileBatch<MAXB>* b, liets_ctx* const* ctx, int n) {
     for (int i = 0; i < n; ++i) {
         liets_ctx* c = ctx[i];
         b->ctl[i] = c->ctl; b->G0[i] = c->G[0]; b->G1[i] = c->G[1]; b->stamp[i] = c->stamp; b->weight[i] = c->weight;
-        b->list0[i] = c->list[0]; b->list1[i] = c->list[1]; b->key[i] = philox_make_key(c->rng_seed);
+        b->list0[i] = c->list[0]; b->list1[i] = c->list[1]; b->P[i] = c->has_blocked ? c->prow : nullptr;
+        b->key[i] = philox_make_key(c->rng_seed);
     }
 }
 

@@ -16,7 +16,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t ctl, grid, list0, list1, status2, coff, rowoff, cand, total;
+    size_t ctl, grid, list0, list1, status2, coff, rowoff, cand, pbits, prow, total;
     size_t g0, g1, stamp, weight;  // STORAGE_TILE (contiguous: G0 | G1 | stamp | weight)
     size_t vox0, vox1, vox_cap;    // STORAGE_TILE: front voxel lists of the small-front steps
     size_t n_tiles, grid_words, list_cap;
@@ -56,6 +56,8 @@ bool make_layout(int nx, int ny, int nz, int storage, Layout* L) {
     L->coff = off;    off += align_up((((size_t)N + 15) / 16 + 31) / 32 * 32 / 8 * 4 + 64);
     L->rowoff = off;  off += align_up(((size_t)ny * nz + 2) * 4);
     L->cand = off;    off += align_up((size_t)N * 4 < 64 ? 64 : (size_t)N * 4);
+    L->pbits = off;   off += align_up(((size_t)N + 7) / 8 + 8);             // liets_set_blocked: N/8 bytes, and the same in row layout
+    L->prow = off;    off += align_up(L->grid_words * 8);
     L->total = off;
     return true;
 }
@@ -130,11 +132,11 @@ bool add_loop(liets_ctx* c, cudaGraph_t g, const cudaGraphNode_t* after, int whi
 
 bool ensure_loop_graph(liets_ctx* c) {
     if (c->loop_exec) {
-        if (c->loop_seed == c->rng_seed) return true;
+        if (c->loop_seed == c->rng_seed && c->loop_blocked == c->has_blocked) return true;
         cudaError_t e = c->storage == LIETS_STORAGE_U8 ? grow_u8_node(c, nullptr, c->loop_exec, &c->loop_grow_node)
                       : c->storage == LIETS_STORAGE_FULL ? grow_full_node(c, nullptr, c->loop_exec, &c->loop_grow_node)
                                                          : grow_tile_node(c, nullptr, c->loop_exec, &c->loop_grow_node);
-        if (e == cudaSuccess) { c->loop_seed = c->rng_seed; return true; }
+        if (e == cudaSuccess) { c->loop_seed = c->rng_seed; c->loop_blocked = c->has_blocked; return true; }
         cudaGetLastError();
         cudaGraphExecDestroy(c->loop_exec); cudaGraphDestroy(c->loop_graph);        // rebuild below
         c->loop_exec = nullptr; c->loop_graph = nullptr; c->loop_tried = false;
@@ -159,7 +161,7 @@ bool ensure_loop_graph(liets_ctx* c) {
         if (g) cudaGraphDestroy(g);
         return false;
     }
-    c->loop_graph = g; c->loop_exec = exec; c->loop_grow_node = grow_node; c->loop_seed = c->rng_seed;
+    c->loop_graph = g; c->loop_exec = exec; c->loop_grow_node = grow_node; c->loop_seed = c->rng_seed; c->loop_blocked = c->has_blocked;
     return true;
 }
 
@@ -216,6 +218,8 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
         c->rowoff = reinterpret_cast<uint32_t*>(base + L.rowoff);
         c->explicit_idx = reinterpret_cast<uint64_t*>(base + L.cand);
         c->scratch_u8 = reinterpret_cast<uint8_t*>(base + L.cand);
+        c->pbits = reinterpret_cast<uint8_t*>(base + L.pbits);
+        c->prow = reinterpret_cast<unsigned long long*>(base + L.prow);
         c->list_cap = L.list_cap;
         if (storage != LIETS_STORAGE_U8) {
             c->geom = TileGeom{ nx, ny, nz, L.Wp, L.ntx, L.nty, L.ntz, c->periodic };
@@ -274,6 +278,35 @@ int liets_set_growth(liets_ctx* c, double g_face, double g_edge, double g_corner
     for (int k = 0; k < 3; ++k) c->R[k] = prob_to_threshold(g[k]);
     c->law = law;
     c->growth_set = true;
+    LIETS_CUDA_TRY(c, launch_set_params(c));
+    return LIETS_OK;
+}
+
+int liets_set_blocked(liets_ctx* c, const void* mask, size_t mask_bytes, int format, int mask_is_device) {
+    if (!c) return LIETS_E_ARG;
+    c->seeded = false;                                      // takes effect at the next seeding
+    if (!mask) {
+        c->has_blocked = false;
+        c->n_blocked = 0;
+        LIETS_CUDA_TRY(c, launch_set_params(c));
+        return LIETS_OK;
+    }
+    if (format != LIETS_FORMAT_U8 && format != LIETS_FORMAT_BITS) return fail(c, LIETS_E_ARG, "unknown mask format");
+    const size_t nb = format == LIETS_FORMAT_U8 ? (size_t)c->N : (size_t)((c->N + 7) / 8);
+    if (mask_bytes < nb) return fail(c, LIETS_E_CAPACITY, "mask buffer too small for the format");
+    const uint8_t* src = static_cast<const uint8_t*>(mask);
+    unsigned long long* count_dev = reinterpret_cast<unsigned long long*>(c->status2);       // seeding scratch is idle here
+    LIETS_CUDA_TRY(c, cudaMemsetAsync(count_dev, 0, 8, c->stream));
+    if (!mask_is_device) {                                  // stage in the seeding scratch (4 N bytes)
+        LIETS_CUDA_TRY(c, cudaMemcpyAsync(c->scratch_u8, mask, nb, cudaMemcpyHostToDevice, c->stream));
+        src = c->scratch_u8;
+    }
+    LIETS_CUDA_TRY(c, launch_blocked_set(c, src, format, count_dev));
+    unsigned long long n = 0;
+    LIETS_CUDA_TRY(c, cudaMemcpyAsync(&n, count_dev, 8, cudaMemcpyDeviceToHost, c->stream));
+    LIETS_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->has_blocked = true;
+    c->n_blocked = n;
     LIETS_CUDA_TRY(c, launch_set_params(c));
     return LIETS_OK;
 }
@@ -338,7 +371,7 @@ int liets_step(liets_ctx* c, uint64_t* n_solid_out, uint64_t* n_front_out) {
         if (n_solid_out) *n_solid_out = ns;
         const liets::Control* h = c->pinned;
         const uint64_t nf = h->mode == 2u ? 1u : (h->mode == 0u && !h->pending) ? h->vox_count[h->cur] : (uint64_t)h->count[h->cur] + h->count_back[h->cur];
-        if (n_front_out) *n_front_out = (ns == 0 || ns == c->N) ? 0 : nf;
+        if (n_front_out) *n_front_out = (ns == 0 || ns == c->N - c->n_blocked) ? 0 : nf;
     }
     return LIETS_OK;
 }
@@ -405,7 +438,11 @@ int liets_grid(liets_ctx* c, void* dst, size_t dst_bytes, int format, int dst_is
         LIETS_CUDA_TRY(c, launch_unpack_rows_u8(c, lin));
         u8 = lin;
     }
-    if (format == LIETS_FORMAT_U8) {
+    if (format == LIETS_FORMAT_U8 && c->storage == LIETS_STORAGE_U8 && c->has_blocked) {      // bytes of value 2 are another phase's
+        uint8_t* lin = dst_is_device ? static_cast<uint8_t*>(dst) : c->scratch_u8;
+        LIETS_CUDA_TRY(c, launch_u8_this_phase(c, lin));
+        if (lin != dst) LIETS_CUDA_TRY(c, cudaMemcpyAsync(dst, lin, c->N, kind, c->stream));
+    } else if (format == LIETS_FORMAT_U8) {
         if (u8 != dst) LIETS_CUDA_TRY(c, cudaMemcpyAsync(dst, u8, c->N, kind, c->stream));
     } else if (format == LIETS_FORMAT_BITS) {
         if (dst_is_device) {
@@ -537,11 +574,11 @@ const char* liets_batch_last_error(const liets_batch* b) { return b ? b->err : "
 // WHILE(any grid live) { k_grow_tile over all grids ; one control step per grid }, built once, keys refreshed after re-seeding
 static bool ensure_batch_graph(liets_batch* b) {
     bool same = b->exec != nullptr;
-    for (int i = 0; i < b->n && same; ++i) same = b->graph_seed[i] == b->ctx[i]->rng_seed;
+    for (int i = 0; i < b->n && same; ++i) same = b->graph_seed[i] == b->ctx[i]->rng_seed && b->graph_blocked[i] == b->ctx[i]->has_blocked;
     if (same) return true;
     if (b->exec) {
         if (grow_tile_batch_node(b->ctx, b->n, nullptr, b->exec, &b->grow_node) == cudaSuccess) {
-            for (int i = 0; i < b->n; ++i) b->graph_seed[i] = b->ctx[i]->rng_seed;
+            for (int i = 0; i < b->n; ++i) { b->graph_seed[i] = b->ctx[i]->rng_seed; b->graph_blocked[i] = b->ctx[i]->has_blocked; }
             return true;
         }
         cudaGetLastError();
@@ -575,7 +612,7 @@ static bool ensure_batch_graph(liets_batch* b) {
         return false;
     }
     b->graph = g; b->exec = exec; b->grow_node = grow_node;
-    for (int i = 0; i < b->n; ++i) b->graph_seed[i] = b->ctx[i]->rng_seed;
+    for (int i = 0; i < b->n; ++i) { b->graph_seed[i] = b->ctx[i]->rng_seed; b->graph_blocked[i] = b->ctx[i]->has_blocked; }
     return true;
 }
 

@@ -101,6 +101,7 @@ struct Control {
     unsigned long long n_t;          // target count ceil(phi_s N) (R7)
     unsigned long long R[3];         // reference thresholds floor(G_ref 2^32 + .5): face, edge, corner (R8)
     unsigned long long N;
+    unsigned long long n_free;       // N minus the cells of earlier phases (liets_set_blocked): the most this phase can hold
     unsigned long long pool_head;    // seeding: entries handed out from the adjacency pool (64-bit: may run far past its size)
     uint32_t U[3];                   // T - 1 of the current step's thresholds T in [1, 2^32] (Eq. (1)):
                                      // a draw fires iff draw <= U
@@ -298,7 +299,7 @@ __device__ __forceinline__ unsigned long long eq1_threshold(unsigned long long R
 // atomics must not come from L1), the logic runs on registers, the results are stored at the end.
 static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     unsigned long long n_solid = __ldcg(&c->n_solid);
-    const unsigned long long n_t = __ldcg(&c->n_t), N = __ldcg(&c->N);
+    const unsigned long long n_t = __ldcg(&c->n_t), N = __ldcg(&c->n_free);     // (cells this phase can ever hold)
     const unsigned long long R[3] = { __ldcg(&c->R[0]), __ldcg(&c->R[1]), __ldcg(&c->R[2]) };
     const uint32_t claims = __ldcg(&c->claims), items = __ldcg(&c->items), items0 = __ldcg(&c->items0);
     uint32_t mode = __ldcg(&c->mode), pending = __ldcg(&c->pending);

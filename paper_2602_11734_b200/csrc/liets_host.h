@@ -46,6 +46,10 @@ struct liets_ctx {
     uint32_t vox_cap_alloc;           // slots per voxel list in the workspace
     uint32_t vox_thr;                 // steps that start with more front voxels run on tiles
     uint8_t* scratch_u8;              // N bytes for format conversion (aliases the candidate buffer)
+    uint8_t* pbits;                   // liets_set_blocked: cells of earlier phases, one bit per voxel in linear order
+    unsigned long long* prow;         // the same cells in the grid's row layout (bit-row storages)
+    bool has_blocked;
+    uint64_t n_blocked;
     uint32_t host_step;               // step counter as of the last read-back (selects the current grid copy)
     int resolve_grid;                 // CTAs of the cooperative spacing kernel (0 = not sized yet)
     uint32_t spacing_ring, spacing_head;  // test hook (liets_debug_spacing_ring): 0 = the built-in sizes
@@ -70,6 +74,7 @@ struct liets_ctx {
     cudaGraphExec_t loop_exec;
     cudaGraphNode_t loop_grow_node;
     uint64_t loop_seed;               // rng_seed whose Philox key the graph's growth node holds
+    bool loop_blocked;                // ... and whether it holds the blocked-cell plane
     bool loop_tried;                  // graph creation attempted (on failure generate keeps enqueueing batches)
     char err[256];
 };
@@ -83,6 +88,7 @@ struct liets_batch {
     cudaGraphExec_t exec;
     cudaGraphNode_t grow_node;
     uint64_t graph_seed[16];          // rng seeds whose Philox keys the graph's growth node holds
+    bool graph_blocked[16];           // ... and whether it holds each grid's blocked-cell plane
     cudaEvent_t ev0, ev1;
     float gen_ms;
     char err[256];
@@ -138,6 +144,10 @@ cudaError_t launch_seed_finalize(liets_ctx* c, int spaced);
 cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n);
 cudaError_t seed_kernel_attributes();
 cudaError_t grow_tile_attributes();
+// blocked.cu
+cudaError_t launch_blocked_set(liets_ctx* c, const uint8_t* src_dev, int format, unsigned long long* count_dev);
+cudaError_t launch_blocked_apply(liets_ctx* c);
+cudaError_t launch_u8_this_phase(liets_ctx* c, uint8_t* dst);
 // s2.cu
 cudaError_t launch_s2(liets_ctx* c, int axis, int rmax, unsigned long long* pairs_dev, unsigned long long* rows_scratch);
 // export.cu

@@ -49,7 +49,7 @@ __device__ __forceinline__ uint32_t candidate_fields(uint32_t status_word) {    
 __global__ void __launch_bounds__(256) k_seed_candidates(uint32_t* status2, uint32_t* ccount,
                                                           unsigned long long N, uint32_t T_core,
                                                           uint32_t always, uint32_t accept_all,
-                                                          PhiloxKey key) {
+                                                          const uint16_t* __restrict__ blocked16, PhiloxKey key) {
     const unsigned long long n_words = (N + 15ull) / 16ull;
     const unsigned long long n_padded = (n_words + 31ull) / 32ull * 32ull;      // whole warps: the chunk shuffles need every lane
     for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < n_padded;
@@ -66,6 +66,7 @@ __global__ void __launch_bounds__(256) k_seed_candidates(uint32_t* status2, uint
                 for (int k = 0; k < 4; ++k)
                     if (blk * 4ull + k < N && (always || d[k] < T_core)) bits |= 1u << (4 * b + k);
             }
+            if (blocked16) bits &= ~(uint32_t)blocked16[w];  // cells of earlier phases are not unassigned (PAPER.md:40 step 4)
             uint32_t word = 0;                              // spread: bit k -> field 2k
             for (uint32_t m = bits; m; m &= m - 1) {
                 const int k = __ffs(m) - 1;
@@ -549,6 +550,7 @@ cudaError_t launch_seed_reset(liets_ctx* c) {
         e = cudaMemsetAsync(c->G[0], 0, c->grid_words * 16 + c->n_tiles * 8, c->stream);
     }
     if (e != cudaSuccess) return e;
+    if (c->has_blocked && (e = launch_blocked_apply(c)) != cudaSuccess) return e;      // the earlier phases' cells go back in
     k_seed_reset<<<1, 1, 0, c->stream>>>(c->ctl);
     c->launches++;
     return cudaGetLastError();
@@ -558,7 +560,8 @@ cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all
     const PhiloxKey key = philox_make_key(c->rng_seed);
     const uint32_t always = t_core >= (1ull << 32);
     const uint32_t T = always ? 0xFFFFFFFFu : (uint32_t)t_core;
-    k_seed_candidates<<<c->sm_count * 8, 256, 0, c->stream>>>(c->status2, c->coff, c->N, T, always, (uint32_t)accept_all, key);
+    k_seed_candidates<<<c->sm_count * 8, 256, 0, c->stream>>>(c->status2, c->coff, c->N, T, always, (uint32_t)accept_all,
+                                                              c->has_blocked ? reinterpret_cast<const uint16_t*>(c->pbits) : nullptr, key);
     c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;

@@ -16,7 +16,7 @@ FORMAT_U8, FORMAT_BITS = 0, 1
 
 # every symbol include/liets.h declares
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
-           "liets_set_target", "liets_step", "liets_generate", "liets_grid", "liets_s2", "liets_step_log", "liets_timings",
+           "liets_set_target", "liets_set_blocked", "liets_step", "liets_generate", "liets_grid", "liets_s2", "liets_step_log", "liets_timings",
            "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info",
            "liets_create_batch", "liets_batch_ctx", "liets_generate_batch", "liets_destroy_batch",
            "liets_batch_last_error", "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_debug_thresholds", "liets_probe", "liets_destroy", "liets_last_error")
@@ -58,6 +58,8 @@ def lib():
     L.liets_seed.restype = ci
     L.liets_seed_explicit.argtypes = [vp, P(u64), u64, u64]
     L.liets_seed_explicit.restype = ci
+    L.liets_set_blocked.argtypes = [vp, vp, sz, ci, ci]
+    L.liets_set_blocked.restype = ci
     L.liets_set_target.argtypes = [vp, dbl]
     L.liets_set_target.restype = ci
     L.liets_step.argtypes = [vp, P(u64), P(u64)]
@@ -199,6 +201,18 @@ class Liets:
         a = np.ascontiguousarray(idx, dtype=np.uint64)
         self._check(self._L.liets_seed_explicit(self._h, a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)),
                                                 a.size, rng_seed))
+
+    def set_blocked(self, mask, format=FORMAT_U8):
+        """Cells of earlier growing phases: a numpy array (host) or a torch CUDA uint8 tensor, N bytes (FORMAT_U8, non-zero =
+        taken) or ceil(N/8) packed bytes (FORMAT_BITS); None clears.  Seed again afterwards."""
+        if mask is None:
+            self._check(self._L.liets_set_blocked(self._h, None, 0, format, 0))
+            return
+        if hasattr(mask, "data_ptr"):                       # torch tensor on the device
+            self._check(self._L.liets_set_blocked(self._h, ctypes.c_void_p(mask.data_ptr()), mask.numel(), format, 1))
+        else:
+            a = np.ascontiguousarray(np.asarray(mask).ravel(), dtype=np.uint8)
+            self._check(self._L.liets_set_blocked(self._h, a.ctypes.data, a.size, format, 0))
 
     def set_target(self, phi):
         self._check(self._L.liets_set_target(self._h, phi))

@@ -447,3 +447,51 @@ def test_two_dimensional_grids_bit_exact(liets, storage, periodic, dims):
     """Two-dimensional grids (Algorithms 1-3 are stated in 2D): nz = 1 between walls (mode 0) or periodic in
     the plane (mode 2, the "roll" of :76), seeding with spacing and growth to the target against the oracle."""
     run_both(liets, dims, periodic, 0.01, 5, 4, (0.08, 0.03, 0.01), 1, 0.6, storage)
+
+
+@pytest.mark.parametrize("storage", STORAGES_ALL)
+@pytest.mark.parametrize("periodic", [False, True])
+def test_two_growing_phases_bit_exact(liets, storage, periodic):
+    """Multi-phase growth, independent phases (PAPER.md:40 step 4): phase 1 is generated, its cells are handed to a second
+    generator (liets_set_blocked: uint8 from the host, packed bits from the device), phase 2 grows on the unassigned cells with
+    its own core and growth probabilities.  Seeds, every step's solid count and the final grid equal the oracle's; no cell
+    belongs to both phases; re-seeding keeps the mask, clearing it restores the plain run."""
+    import torch
+    dims = (70, 45, 33)
+    nx, ny, nz = dims
+    o1, L1 = run_both(liets, dims, periodic, 0.004, 6, 3, (0.05, 0.02, 0.01), 1, 0.35, storage)
+    p1 = o1.grid()
+    o2 = oracle.Oracle(nx, ny, nz, periodic)
+    o2.set_blocked(p1)
+    o2.set_growth(0.08, 0.01, 0.0, 1)
+    n2 = o2.seed(0.01, 4, 17)
+    rc_o, st_o = o2.generate(0.30)
+    for how in ("host_u8", "device_bits"):
+        L2 = make(liets, dims, periodic, storage)
+        L2.set_growth(0.08, 0.01, 0.0, 1)
+        if how == "host_u8":
+            L2.set_blocked(L1.grid())
+        else:
+            L2.set_blocked(L1.grid_device(liets.FORMAT_BITS), liets.FORMAT_BITS)
+        with pytest.raises(liets.LietsError):
+            L2.step()                                      # not seeded since the mask changed
+        assert L2.seed(0.01, 4, 17) == n2
+        rc, st, ns = L2.generate(0.30)
+        assert (rc, ns) == (rc_o, o2.n_solid) and st in (st_o, st_o + (1 if rc == liets.FRONT_EMPTY else 0))
+        g2 = L2.grid()
+        assert (g2 == o2.grid()).all() and not (g2 & p1).any()
+        bits = np.unpackbits(L2.grid(liets.FORMAT_BITS), bitorder="little")[: L2.N]
+        assert (bits == o2.grid().ravel()).all()
+        f, sol, blocks = L2.step_log()
+        assert int(sol[min(st_o, len(sol)) - 1]) == o2.n_solid
+        # free cells of the two-phase map, by the device's two-point correlation at lag 0
+        pairs, valid = L2.s2(0, 3)
+        assert pairs[0] == L2.N - int(p1.sum()) - ns
+        L2.close()
+    L3 = make(liets, dims, periodic, storage)
+    L3.set_growth(0.05, 0.02, 0.01, 1)
+    L3.set_blocked(p1)
+    L3.set_blocked(None)                                   # cleared: the plain phase-1 run again
+    L3.seed(0.004, 6, 3)
+    L3.generate(0.35)
+    assert (L3.grid() == p1).all()

@@ -541,3 +541,71 @@ def test_spacing_with_in_plane_periodicity_equals_brute_force_greedy(s):
     assert o.seed(c, s, seed) == len(acc)
     got = np.flatnonzero(o.grid().ravel())
     assert [(v % nx, (v // nx) % ny, v // (nx * ny)) for v in got] == acc
+
+
+# ------------------------------------------------------------------------------------------ earlier phases (PAPER.md:40 step 4)
+def _bfs_steps(free, starts, neigh):
+    """Breadth-first distance (in growth steps) from the start cells through `free` cells with the given neighbour offsets."""
+    nz, ny, nx = free.shape
+    dist = np.full(free.shape, -1, dtype=np.int64)
+    frontier = []
+    for (x, y, z) in starts:
+        dist[z, y, x] = 0
+        frontier.append((x, y, z))
+    k = 0
+    while frontier:
+        k += 1
+        nxt = []
+        for (x, y, z) in frontier:
+            for dx, dy, dz in neigh:
+                X, Y, Z = x + dx, y + dy, z + dz
+                if 0 <= X < nx and 0 <= Y < ny and 0 <= Z < nz and free[Z, Y, X] and dist[Z, Y, X] < 0:
+                    dist[Z, Y, X] = k
+                    nxt.append((X, Y, Z))
+        frontier = nxt
+    return dist
+
+
+@pytest.mark.parametrize("use_list", [True, False])
+def test_cells_of_an_earlier_phase_are_neither_void_nor_sources(use_list):
+    """PAPER.md:40 step 4, independent phases: the new phase grows on the still unassigned cells.  With probability 1 the
+    cells of the new phase after k steps are exactly the unassigned cells within k moves of a seed along paths that avoid
+    the earlier phase (breadth-first search); the earlier phase's cells never change, are never counted, are never cores."""
+    nx, ny, nz = 17, 13, 9
+    rng = np.random.default_rng(5)
+    taken = rng.random((nz, ny, nx)) < 0.3
+    taken[:, 6, :] = True                                 # a wall with a hole: the phase has to go round
+    taken[4, 6, 8] = False
+    seeds = [(2, 2, 2), (15, 11, 7)]
+    for s in seeds:
+        taken[s[2], s[1], s[0]] = False
+    faces = [(1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)]
+    alld = [(a, b, c) for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1) if (a, b, c) != (0, 0, 0)]
+    for g, neigh in (((1.0, 0.0, 0.0), faces), ((1.0, 1.0, 1.0), alld)):
+        o = oracle.Oracle(nx, ny, nz, False)
+        o.set_blocked(taken)
+        o.set_growth(*g, 0)
+        o.seed_explicit([x + nx * (y + ny * z) for x, y, z in seeds] + [8 + nx * (6 + ny * 0)])    # the last one is taken: no seed
+        assert o.n_solid == 2
+        dist = _bfs_steps(~taken, seeds, neigh)
+        for k in range(1, 30):
+            o.step(use_list)
+            assert (o.grid() == ((dist >= 0) & (dist <= k))).all(), k
+            assert ((o.phase_map() == 2) == taken).all() and o.n_solid == int(o.grid().sum())
+        if neigh is alld:
+            assert o.n_front_exact == 0                    # everything reachable is taken: no solid cell has a void neighbour left
+    # keyed cores: the candidates are the unassigned cells whose draw is below the threshold
+    o = oracle.Oracle(nx, ny, nz, False)
+    o.set_blocked(taken)
+    n = o.seed(0.05, 0, 3)
+    Tc = oracle.prob_to_threshold(0.05)
+    expect = [v for v in range(nx * ny * nz) if not taken.ravel()[v] and oracle.seed_draw(3, v) < Tc]
+    assert n == len(expect) and (np.flatnonzero(o.grid().ravel()) == np.array(expect)).all()
+    # no earlier phase at all == the plain run
+    a, b = oracle.Oracle(nx, ny, nz, True), oracle.Oracle(nx, ny, nz, True)
+    b.set_blocked(np.zeros((nz, ny, nx), np.uint8))
+    for o in (a, b):
+        o.set_growth(0.1, 0.05, 0.02, 1)
+        o.seed(0.01, 3, 9)
+        o.generate(0.4)
+    assert (a.grid() == b.grid()).all() and a.n_solid == b.n_solid
