@@ -146,9 +146,6 @@ __device__ __forceinline__ uint32_t mul_lo_u32(uint32_t a, uint32_t b) {     // 
     asm("mul.lo.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
     return r;
 }
-__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v) {
-    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
-}
 __device__ __forceinline__ void atoms_or_u32(uint32_t addr, uint32_t v) {
     asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }

@@ -247,17 +247,7 @@ cudaError_t launch_tiles_from_grid(liets_ctx* c) {
     return cudaGetLastError();
 }
 
-// the same launches as kernel nodes of `graph` (exec == nullptr) or refreshed in an instantiated graph
-cudaError_t grow_vox_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node) {
-    PhiloxKey key = philox_make_key(c->rng_seed);
-    void* args[7];
-    vox_args(c, &key, args);
-    cudaKernelNodeParams p = {};
-    p.func = reinterpret_cast<void*>(k_grow_vox);
-    p.gridDim = dim3(c->sm_count * 4); p.blockDim = dim3(kVoxThreads); p.sharedMemBytes = 0; p.kernelParams = args;
-    return exec ? cudaGraphExecKernelNodeSetParams(exec, *node, &p) : cudaGraphAddKernelNode(node, graph, nullptr, 0, &p);
-}
-
+// the hand-over as a kernel node of liets_generate's graph
 cudaError_t tiles_from_grid_node(liets_ctx* c, cudaGraph_t graph, const cudaGraphNode_t* after, cudaGraphNode_t* node) {
     int tile_w = grow_tile_words();
     void* args[] = { &c->ctl, &c->geom, &tile_w, &c->G[0], &c->stamp, &c->weight, &c->list[0], &c->list[1] };

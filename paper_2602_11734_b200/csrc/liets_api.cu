@@ -640,7 +640,7 @@ int liets_generate_batch(liets_batch* b, const double* target_solid_fraction, ui
         c->vox_thr = 0;                                     // the batched loop runs on tiles from its first step
         int rc = liets_set_target(c, target_solid_fraction[i]);             // (also sends vox_thr to the device)
         c->vox_thr = thr;
-        if (rc) { snprintf(b->err, sizeof(b->err), "grid %d: %s", i, c->err); return rc; }
+        if (rc) { snprintf(b->err, sizeof(b->err), "grid %d: %.200s", i, c->err); return rc; }
         LIETS_BATCH_TRY(b, launch_begin(c, 1, max_steps));
         c->prof_n = 0;
         LIETS_BATCH_TRY(b, launch_control(c, kCtlPrepare));
@@ -652,7 +652,7 @@ int liets_generate_batch(liets_batch* b, const double* target_solid_fraction, ui
     LIETS_BATCH_TRY(b, cudaEventRecord(b->ev1, b->stream));
     for (int i = 0; i < b->n; ++i) {
         liets_ctx* c = b->ctx[i];
-        if (int rc = readback(c)) { snprintf(b->err, sizeof(b->err), "grid %d: %s", i, c->err); return rc; }
+        if (int rc = readback(c)) { snprintf(b->err, sizeof(b->err), "grid %d: %.200s", i, c->err); return rc; }
         c->launches += 1ull + c->pinned->steps_done;        // its share of the batched loop: one control step per step
         if (status_out) status_out[i] = c->pinned->status;
         if (steps_out) steps_out[i] = c->pinned->steps_done;

@@ -124,7 +124,6 @@ cudaError_t grow_u8_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, 
 cudaError_t launch_grow_vox(liets_ctx* c);
 cudaError_t launch_grow_vox_loop(liets_ctx* c);
 cudaError_t launch_tiles_from_grid(liets_ctx* c);
-cudaError_t grow_vox_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec, cudaGraphNode_t* node);
 cudaError_t tiles_from_grid_node(liets_ctx* c, cudaGraph_t graph, const cudaGraphNode_t* after, cudaGraphNode_t* node);
 // grow_full.cu
 cudaError_t launch_grow_full(liets_ctx* c);
