@@ -201,3 +201,34 @@ def test_config5_1024_periodic_sampled_transitions_and_properties(liets):
     assert (np.diff(solid_after.astype(np.int64)) > 0).all()
     assert solid_after[-1] == n_solid >= n_t and solid_after[-2] < n_t
     L.close()
+
+
+def test_near_maximum_grid_counts_are_consistent(liets):
+    """A grid close to the largest the ABI admits (N < 2^32): 1500^3 = 3.375e9 voxels, voxel indices beyond 2^31, 18 GB of
+    workspace.  No oracle run exists at this size; what must hold at any size is checked on the device: the stop rule,
+    strictly growing solid counts, the popcount of the packed output == n_solid, S2 at lag 0 == the void count, and the
+    number of counted pairs at lags 1, 2 (walls: (n - r) n^2, periodic: n^3)."""
+    import torch
+    n = 1500
+    N = n ** 3
+    lut = torch.tensor([bin(i).count("1") for i in range(256)], dtype=torch.int64, device="cuda")
+    for boundary in (0, 1):
+        L = liets.Liets(n, n, n, boundary, 1)
+        L.set_growth(0.01, 0.0025, 0.00025, liets.LAW_EQ1)
+        n_seeds = L.seed(0.0002, 30, 5)
+        n_cand, slow = L.seed_info()
+        assert 0 < n_seeds < n_cand and abs(n_cand - 0.0002 * N) < 6 * (0.0002 * N) ** 0.5
+        rc, steps, n_solid = L.generate(0.8)
+        front, solid_after, blocks = L.step_log()
+        n_t = oracle.target_count(0.8, N)
+        assert rc == liets.OK and len(solid_after) == steps
+        assert (np.diff(solid_after.astype(np.int64)) > 0).all()
+        assert solid_after[-1] == n_solid >= n_t and solid_after[-2] < n_t
+        bits = L.grid_device(liets.FORMAT_BITS)
+        tot = sum(int(lut[bits[i:i + (1 << 28)].long()].sum()) for i in range(0, bits.numel(), 1 << 28))
+        assert tot == n_solid
+        pairs, valid = L.s2(2, 2)
+        assert int(pairs[0]) == N - n_solid
+        assert [int(v) for v in valid] == ([N, N, N] if boundary else [N, (n - 1) * n * n, (n - 2) * n * n])
+        del bits
+        L.close()
