@@ -13,6 +13,7 @@ using namespace liets;
 namespace {
 
 constexpr size_t kAlign = 256;
+constexpr uint64_t kSmallGrid = 1ull << 22;     // grids up to this many voxels can finish on the voxel list (its capacity is 2^18 entries)
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
@@ -387,9 +388,18 @@ int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps
     if (!c->profiling && ensure_loop_graph(c)) {
         // the whole loop on the device: first step prepared here, then WHILE(step armed) { grow ; control } as one graph
         LIETS_CUDA_TRY(c, launch_control(c, kCtlPrepare));
-        if (c->storage == LIETS_STORAGE_TILE) LIETS_CUDA_TRY(c, launch_grow_vox_loop(c));   // the steps on the voxel list, one launch
-        LIETS_CUDA_TRY(c, cudaGraphLaunch(c->loop_exec, c->stream));
-        if (int rc = readback(c)) return rc;
+        bool done = false;
+        if (c->storage == LIETS_STORAGE_TILE) {
+            LIETS_CUDA_TRY(c, launch_grow_vox_loop(c));     // the steps on the voxel list, one launch
+            if (c->N <= kSmallGrid) {                       // a small grid often ends on the voxel list: look before launching the graph
+                if (int rc = readback(c)) return rc;
+                done = c->pinned->status != kStatusRunning;
+            }
+        }
+        if (!done) {
+            LIETS_CUDA_TRY(c, cudaGraphLaunch(c->loop_exec, c->stream));
+            if (int rc = readback(c)) return rc;
+        }
         c->launches += 2ull * c->pinned->steps_done + (c->storage == LIETS_STORAGE_TILE ? 3 : 2);   // kernels the graph ran (incl. the loop's last, empty round)
     } else for (;;) {
         // a batch of steps back to back; steps after the stop rule fired are no-ops on the device
