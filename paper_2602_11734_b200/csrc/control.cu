@@ -1,27 +1,28 @@
 // control.cu -- the device-resident step loop: thresholds (Eq. (1)), stop rule, list swap, counters.
 //
 // One growth step is  control_step(PREPARE) ; grow kernel ; control_step(FINISH ...)  (liets_device.cuh).
-// control_step is a single thread: it turns the solid count into the three integer thresholds of the
+// control_step is run by a single warp: it turns the solid count into the three integer thresholds of the
 // step (R6/R8), evaluates "while phi_a < phi_s and A not empty" and
 // arms or disarms the grow kernel through Control::active, so a batch of steps can be enqueued
-// without the host looking at the device in between.  It runs as the one-thread kernel k_control between the
+// without the host looking at the device in between.  It runs as the one-warp kernel k_control between the
 // growth kernels: enqueued ahead, its launch overlaps the previous kernel's tail (folding it into the last CTA of
 // the growth kernel was measured slower: the whole GPU idles behind one thread).
 #include "liets_host.h"
 
 namespace liets {
 
-__global__ void k_control(Control* c, uint32_t flags) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+__global__ void k_control(Control* c, uint32_t flags) {     // one warp
+    if (blockIdx.x != 0 || threadIdx.x >= 32) return;
     control_step(c, flags);
 }
 
 // The control step inside the device-side WHILE loop of liets_generate's CUDA graph: closes the step that just ran,
 // prepares the next one and tells the loop whether to go round again.
-__global__ void k_control_loop(Control* c, cudaGraphConditionalHandle loop) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+__global__ void k_control_loop(Control* c, cudaGraphConditionalHandle loop) {      // one warp
+    if (blockIdx.x != 0 || threadIdx.x >= 32) return;
     control_step(c, kCtlFinish | kCtlPrepare);
-    cudaGraphSetConditional(loop, __ldcg(&c->active) ? 1u : 0u);
+    __syncwarp();
+    if (threadIdx.x == 0) cudaGraphSetConditional(loop, __ldcg(&c->active) ? 1u : 0u);
 }
 
 cudaError_t control_loop_node(liets_ctx* c, cudaGraph_t graph, cudaGraphNode_t after, cudaGraphConditionalHandle loop,
@@ -33,14 +34,16 @@ cudaError_t control_loop_node(liets_ctx* c, cudaGraph_t graph, cudaGraphNode_t a
     return cudaGraphAddKernelNode(node, graph, &after, 1, &p);
 }
 
-// The same for the grids of a batch (liets_generate_batch): thread i steps grid i; the loop goes round while any grid is live.
+// The same for the grids of a batch (liets_generate_batch): warp i steps grid i; the loop goes round while any grid is live.
 struct ControlBatch { int n; Control* ctl[32]; };
 
 __global__ void k_control_loop_batch(ControlBatch b, cudaGraphConditionalHandle loop) {
+    const int grid_i = (int)(threadIdx.x >> 5);
     int live = 0;
-    if ((int)threadIdx.x < b.n) {
-        control_step(b.ctl[threadIdx.x], kCtlFinish | kCtlPrepare);
-        live = __ldcg(&b.ctl[threadIdx.x]->active) ? 1 : 0;
+    if (grid_i < b.n) {
+        control_step(b.ctl[grid_i], kCtlFinish | kCtlPrepare);
+        __syncwarp();
+        live = __ldcg(&b.ctl[grid_i]->active) ? 1 : 0;
     }
     live = __syncthreads_or(live);
     if (threadIdx.x == 0) cudaGraphSetConditional(loop, live ? 1u : 0u);
@@ -55,7 +58,7 @@ cudaError_t control_loop_batch_node(liets_ctx* const* ctx, int n, cudaGraph_t gr
     void* args[] = { &b, &loop };
     cudaKernelNodeParams p = {};
     p.func = reinterpret_cast<void*>(k_control_loop_batch);
-    p.gridDim = dim3(1); p.blockDim = dim3(32); p.sharedMemBytes = 0; p.kernelParams = args;
+    p.gridDim = dim3(1); p.blockDim = dim3(32 * n); p.sharedMemBytes = 0; p.kernelParams = args;
     return cudaGraphAddKernelNode(node, graph, &after, 1, &p);
 }
 

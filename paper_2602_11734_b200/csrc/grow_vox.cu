@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(kVoxThreads) k_grow_vox_loop(Control* __restri
         if (!__ldcg(&ctl->active) || __ldcg(&ctl->mode) != 0u || __ldcg(&ctl->pending)) return;    // the same for every thread
         vox_step(ctl, g, G0, G1, vox0, vox1, key, S);
         grid.sync();
-        if (blockIdx.x == 0 && threadIdx.x == 0) control_step(ctl, kCtlFinish | kCtlPrepare);
+        if (blockIdx.x == 0 && threadIdx.x < 32) control_step(ctl, kCtlFinish | kCtlPrepare);      // one warp
         grid.sync();
     }
 }

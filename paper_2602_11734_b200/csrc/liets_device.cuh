@@ -295,12 +295,17 @@ __device__ __forceinline__ unsigned long long eq1_threshold(unsigned long long R
     return T > (1ull << 32) ? (1ull << 32) : T;
 }
 
-// One call by ONE thread between two growth kernels.  All inputs are read up front in one batch of L2 loads (fields that other CTAs update with
-// atomics must not come from L1), the logic runs on registers, the results are stored at the end.
+// One call by ONE WARP (all 32 lanes, converged) between two growth kernels.  All inputs are read up front in one batch of
+// L2 loads, the same by every lane (fields that other CTAs update with atomics must not come from L1); the scalar logic
+// runs redundantly on registers and lane 0 stores its results; the two parts that cost time on a single thread are spread:
+// the three thresholds of Eq. (1) (64-bit divisions) on lanes 0-2, the 32 words of the nibble layout one per lane.  This
+// call sits on the critical path of every step (between two growth launches, or between two grid barriers).
 static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
+    const uint32_t lane = threadIdx.x & 31u;
+    const bool lead = lane == 0u;
     unsigned long long n_solid = __ldcg(&c->n_solid);
     const unsigned long long n_t = __ldcg(&c->n_t), N = __ldcg(&c->n_free);     // (cells this phase can ever hold)
-    const unsigned long long R[3] = { __ldcg(&c->R[0]), __ldcg(&c->R[1]), __ldcg(&c->R[2]) };
+    const unsigned long long R_mine = __ldcg(&c->R[lane < 3u ? lane : 0u]);
     const uint32_t claims = __ldcg(&c->claims), items = __ldcg(&c->items), items0 = __ldcg(&c->items0);
     uint32_t mode = __ldcg(&c->mode), pending = __ldcg(&c->pending);
     const uint32_t vox_thr = __ldcg(&c->vox_thr), vox_overflow = __ldcg(&c->vox_overflow);
@@ -312,16 +317,22 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     uint32_t step = __ldcg(&c->step), steps_done = __ldcg(&c->steps_done), cur = __ldcg(&c->cur);
     uint32_t active = __ldcg(&c->active);
     int32_t status = __ldcg(&c->status);
+    __syncwarp();                                        // every lane has read the state before lane 0 changes it
     if ((flags & kCtlFinish) && active) {                // close the step that just ran
         n_solid += claims;                               // phi_a update
-        c->n_solid = n_solid;
-        if (step < kLogCap) { c->log_solid[step] = n_solid; c->log_items[step] = items; c->log_items0[step] = items0; }
+        if (lead) {
+            c->n_solid = n_solid;
+            if (step < kLogCap) { c->log_solid[step] = n_solid; c->log_items[step] = items; c->log_items0[step] = items0; }
+        }
         cur ^= 1u;                                       // A <- prune(A U A_new) (R4)
         step += 1;
         steps_done += 1;
         active = 0;
-        c->cur = cur; c->step = step; c->steps_done = steps_done; c->active = 0; c->claims = 0;
-        if (pending) { mode = 1u; pending = 0u; c->mode = 1u; c->pending = 0u; }     // that was the first step on tiles
+        if (lead) { c->cur = cur; c->step = step; c->steps_done = steps_done; c->active = 0; c->claims = 0; }
+        if (pending) {                                   // that was the first step on tiles
+            mode = 1u; pending = 0u;
+            if (lead) { c->mode = 1u; c->pending = 0u; }
+        }
     }
     if (!(flags & (kCtlPrepare | kCtlEval))) return;
     if (!(flags & kCtlForce)) {                          // stop rule, between whole steps only
@@ -329,50 +340,61 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
         if (n_solid >= n_t) status = 0;                                      // LIETS_OK
         else if (count[cur] == 0 || n_solid == N) status = 1;                // FRONT_EMPTY
         else if (steps_done >= max_steps) status = 2;                        // MAX_STEPS
-        if (status != kStatusRunning) { c->status = status; return; }
+        if (status != kStatusRunning) { if (lead) c->status = status; return; }
     }
     if (!(flags & kCtlPrepare)) return;
+    // Eq. (1): lane k < 3 evaluates class k
+    uint32_t U_mine = 0, en_mine = 0;
+    if (lane < 3u) {
+        const unsigned long long T = law ? eq1_threshold(R_mine, n_t, n_solid) : R_mine;
+        en_mine = T >= 1ull;                                                 // T in [0, 2^32]
+        U_mine = T >= 1ull ? (uint32_t)(T - 1ull) : 0u;                      // draw < T  <=>  draw <= T - 1
+        c->en[lane] = en_mine;
+        c->U[lane] = U_mine;
+    }
     uint32_t U[3], en[3], en26 = 0, h0_any = 0;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        const unsigned long long T = law ? eq1_threshold(R[k], n_t, n_solid) : R[k];
-        en[k] = T >= 1ull;                                                   // T in [0, 2^32]
-        U[k] = T >= 1ull ? (uint32_t)(T - 1ull) : 0u;                        // draw < T  <=>  draw <= T - 1
-        c->en[k] = en[k];
-        c->U[k] = U[k];
+        U[k] = __shfl_sync(0xffffffffu, U_mine, k);
+        en[k] = __shfl_sync(0xffffffffu, en_mine, k);
         if (en[k]) en26 |= class_dir_mask(k);
         if (en[k] && (U[k] >> 28)) h0_any = 1;
     }
-    // the thresholds nibble by nibble, laid out like the draws (direction d: nibble d>>2 of word d&3)
+    // the thresholds nibble by nibble, laid out like the draws (direction d: nibble d>>2 of word d&3): lane = 4 level + word
+    {
+        const uint32_t lv = lane >> 2, w = lane & 3u;
+        uint32_t ones[3];
 #pragma unroll
-    for (int lv = 0; lv < 8; ++lv)
-#pragma unroll
-        for (int w = 0; w < 4; ++w)
-            c->hpat[lv][w] = ((U[0] >> (28 - 4 * lv)) & 15u) * class_nibble_ones(w, 0) +
-                             ((U[1] >> (28 - 4 * lv)) & 15u) * class_nibble_ones(w, 1) +
-                             ((U[2] >> (28 - 4 * lv)) & 15u) * class_nibble_ones(w, 2);
-    c->en26 = en26;
-    c->h0_any = h0_any;
-    c->tile_cursor = 0;
-    c->count[cur ^ 1u] = 0;
-    c->count_back[cur ^ 1u] = 0;
-    if (mode == 0u) {
-        c->vox_count[cur ^ 1u] = 0;
-        if (count[cur] > vox_thr || vox_overflow) {         // the front has outgrown the voxel list: this step runs on tiles
-            c->pending = 1u;
-            pending = 2u;                                   // (2: handed over in this very call)
-            c->count[cur] = 0;                              // k_tiles_from_grid fills the list of this step
-            c->count_back[cur] = 0;
-        }
+        for (int k = 0; k < 3; ++k)
+            ones[k] = w == 0u ? class_nibble_ones(0, k) : w == 1u ? class_nibble_ones(1, k) : w == 2u ? class_nibble_ones(2, k) : class_nibble_ones(3, k);
+        c->hpat[lv][w] = ((U[0] >> (28u - 4u * lv)) & 15u) * ones[0] + ((U[1] >> (28u - 4u * lv)) & 15u) * ones[1] +
+                         ((U[2] >> (28u - 4u * lv)) & 15u) * ones[2];
     }
-    c->claims = 0;
-    c->items = 0;
-    c->items0 = 0;
-    // entries of the list the step starts from; bit 63: the step runs on tiles (k_grow_tile); bit 62: it is the hand-over
-    // step, whose tile list k_tiles_from_grid has yet to fill -- the count is still the voxel list's
-    if (step < kLogCap)
-        c->log_front[step] = (unsigned long long)count[cur] | ((mode != 0u || pending) ? (1ull << 63) : 0ull) | (pending == 2u ? (1ull << 62) : 0ull);
-    c->active = 1;
+    if (mode == 0u && (count[cur] > vox_thr || vox_overflow)) pending = 2u;  // the front has outgrown the voxel list: this step
+                                                                             // runs on tiles (2: handed over in this very call)
+    if (lead) {
+        c->en26 = en26;
+        c->h0_any = h0_any;
+        c->tile_cursor = 0;
+        c->count[cur ^ 1u] = 0;
+        c->count_back[cur ^ 1u] = 0;
+        if (mode == 0u) {
+            c->vox_count[cur ^ 1u] = 0;
+            if (pending == 2u) {
+                c->pending = 1u;
+                c->count[cur] = 0;                          // k_tiles_from_grid fills the list of this step
+                c->count_back[cur] = 0;
+            }
+        }
+        c->claims = 0;
+        c->items = 0;
+        c->items0 = 0;
+        // entries of the list the step starts from; bit 63: the step runs on tiles (k_grow_tile); bit 62: it is the
+        // hand-over step, whose tile list k_tiles_from_grid has yet to fill -- the count is still the voxel list's
+        if (step < kLogCap)
+            c->log_front[step] = (unsigned long long)count[cur] | ((mode != 0u || pending) ? (1ull << 63) : 0ull) | (pending == 2u ? (1ull << 62) : 0ull);
+        c->active = 1;
+    }
 }
 
 }  // namespace liets
