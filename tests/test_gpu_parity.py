@@ -495,3 +495,34 @@ def test_two_growing_phases_bit_exact(liets, storage, periodic):
     L3.seed(0.004, 6, 3)
     L3.generate(0.35)
     assert (L3.grid() == p1).all()
+
+
+def test_second_phases_in_a_batch_equal_single_runs(liets):
+    """liets_set_blocked on the generators of a batch: two second phases (different earlier phases, different seeds) in one
+    batched loop equal their single runs."""
+    dims = (64, 40, 24)
+    firsts = []
+    for seed in (3, 4):
+        L = liets.Liets(*dims, 0, 1)
+        L.set_growth(0.05, 0.02, 0.01, 1)
+        L.seed(0.005, 5, seed)
+        L.generate(0.3)
+        firsts.append(L.grid())
+    singles = []
+    for i, p1 in enumerate(firsts):
+        L = liets.Liets(*dims, 0, 1)
+        L.set_growth(0.06, 0.01, 0.002, 1)
+        L.set_blocked(p1)
+        n = L.seed(0.01, 3, 20 + i)
+        singles.append((n, L.generate(0.25), L.grid()))
+    B = liets.LietsBatch(2, *dims, 0)
+    for i, p1 in enumerate(firsts):
+        B[i].set_growth(0.06, 0.01, 0.002, 1)
+        B[i].set_blocked(p1)
+        assert B[i].seed(0.01, 3, 20 + i) == singles[i][0]
+    res = B.generate(0.25)
+    for i in range(2):
+        rc, st, ns = singles[i][1]
+        assert (res[i][0], res[i][2]) == (rc, ns) and (B[i].grid() == singles[i][2]).all()
+        assert not (B[i].grid() & firsts[i]).any()
+    B.close()
