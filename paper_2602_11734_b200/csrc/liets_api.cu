@@ -234,6 +234,8 @@ int liets_create(liets_ctx** out, int nx, int ny, int nz, int boundary, int stor
             c->vox[1] = reinterpret_cast<uint32_t*>(base + L.vox1);
             c->vox_cap = c->vox_cap_alloc = (uint32_t)L.vox_cap;
             c->vox_thr = default_vox_threshold(c->N, c->vox_cap);
+            int coop = 0;                                   // the voxel-list loop is a cooperative launch: without it, tiles from step 0
+            if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) { cudaGetLastError(); c->vox_thr = 0; c->no_coop = true; }
             c->grid_u8 = nullptr;
             c->tile_grid = c->sm_count * grow_tile_ctas_per_sm();
         }
@@ -390,7 +392,7 @@ int liets_generate(liets_ctx* c, double phi, uint32_t max_steps, uint32_t* steps
         LIETS_CUDA_TRY(c, launch_control(c, kCtlPrepare));
         bool done = false;
         if (c->storage == LIETS_STORAGE_TILE) {
-            LIETS_CUDA_TRY(c, launch_grow_vox_loop(c));     // the steps on the voxel list, one launch
+            if (!c->no_coop) LIETS_CUDA_TRY(c, launch_grow_vox_loop(c));     // the steps on the voxel list, one launch
             if (c->N <= kSmallGrid) {                       // a small grid often ends on the voxel list: look before launching the graph
                 if (int rc = readback(c)) return rc;
                 done = c->pinned->status != kStatusRunning;
@@ -696,6 +698,7 @@ int liets_debug_vox_list(liets_ctx* c, uint64_t max_front_voxels, uint32_t capac
     c->vox_cap = capacity && capacity < c->vox_cap_alloc ? capacity : c->vox_cap_alloc;
     c->vox_thr = max_front_voxels == UINT64_MAX ? default_vox_threshold(c->N, c->vox_cap)
                : (uint32_t)(max_front_voxels > c->vox_cap ? c->vox_cap : max_front_voxels);
+    if (c->no_coop) c->vox_thr = 0;
     LIETS_CUDA_TRY(c, launch_set_params(c));
     return LIETS_OK;
 }

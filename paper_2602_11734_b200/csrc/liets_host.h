@@ -49,6 +49,7 @@ struct liets_ctx {
     uint8_t* pbits;                   // liets_set_blocked: cells of earlier phases, one bit per voxel in linear order
     unsigned long long* prow;         // the same cells in the grid's row layout (bit-row storages)
     bool has_blocked;
+    bool no_coop;                     // the device cannot launch cooperative kernels: no voxel-list loop, tiles from step 0
     uint64_t n_blocked;
     uint32_t host_step;               // step counter as of the last read-back (selects the current grid copy)
     int resolve_grid;                 // CTAs of the cooperative spacing kernel (0 = not sized yet)
