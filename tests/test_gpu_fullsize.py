@@ -232,3 +232,18 @@ def test_near_maximum_grid_counts_are_consistent(liets):
         assert [int(v) for v in valid] == ([N, N, N] if boundary else [N, (n - 1) * n * n, (n - 2) * n * n])
         del bits
         L.close()
+
+
+def test_repeated_generations_are_identical(liets):
+    """The same context, seeded and grown ten times at full size: every run reproduces the stored oracle hash (inter-CTA
+    communication is by idempotent atomics only, so no schedule can change the grid; compute-sanitizer is closed on
+    the pool)."""
+    rec = [r for r in records() if r["config"] == "cfg3_400" and r["target"] == 0.8][0]
+    L = liets.Liets(*rec["dims"], int(rec["periodic"]), 1)
+    L.set_growth(*rec["g"], liets.LAW_EQ1)
+    for rep in range(10):
+        assert L.seed(rec["core"], rec["s"], rec["rng_seed"]) == rec["n_seeds"]
+        rc, steps, n_solid = L.generate(rec["target"])
+        assert (rc, steps, n_solid) == (rec["status"], rec["steps"], rec["n_solid"])
+        assert hashlib.sha256(L.grid().tobytes()).hexdigest() == rec["sha256"], rep
+    L.close()
