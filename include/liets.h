@@ -158,6 +158,19 @@ const char* liets_batch_last_error(const liets_batch* batch);
  * the bit rows; synchronises.  Errors: E_ARG, E_STATE before the first seed, E_CUDA. */
 int liets_s2(liets_ctx* ctx, int axis, int rmax, uint64_t* pairs, uint64_t* valid);
 
+/* liets_s2 for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it):
+ * the same pair counts (R16), same arguments and outputs, but the per-lag counters that liets_s2 takes from
+ * cudaMalloc on every call sit in one file-scope device array of LIETS_S2_STATIC_MAX_LAGS 64-bit counters (32 KiB; every
+ * GPU that loads the library holds it until the process exits).  The call makes no cudaMalloc, cudaFree or allocating
+ * library call.  Limits: rmax + 1 <= LIETS_S2_STATIC_MAX_LAGS, else LIETS_E_CAPACITY; bit-row storages only
+ * (LIETS_STORAGE_TILE, LIETS_STORAGE_FULL; a STORAGE_U8 grid would need N/8 bytes of packing scratch: LIETS_E_ARG).
+ * The ctx's device must be current.  All calls on a device share the array, which keeps the last call's counts: every
+ * call zeroes the counters it uses first.  Calls that overlap on the GPU would race on it; this entry point holds a
+ * host mutex and synchronises the ctx's stream before it returns, so its own calls never overlap within a process.
+ * pairs and valid are HOST arrays of rmax + 1 entries.  Errors: E_ARG, E_CAPACITY, E_STATE before the first seed, E_CUDA. */
+#define LIETS_S2_STATIC_MAX_LAGS 4096
+int liets_s2_static(liets_ctx* ctx, int axis, int rmax, uint64_t* pairs, uint64_t* valid);
+
 /* Per-step counters of the steps done since the last seed (HOST arrays of capacity cap, may be
  * NULL): front size at the start of step i (list entries: voxels for STORAGE_U8; for STORAGE_TILE voxels while the
  * front is a voxel list, tiles afterwards -- bit 63 set: the step ran on the tile list; bit 62 set as well: it was

@@ -13,10 +13,11 @@ BOUNDARY_WALL, BOUNDARY_PERIODIC, BOUNDARY_PERIODIC_XY = 0, 1, 2
 STORAGE_U8, STORAGE_TILE, STORAGE_FULL = 0, 1, 2
 LAW_CONSTANT, LAW_EQ1 = 0, 1
 FORMAT_U8, FORMAT_BITS = 0, 1
+S2_STATIC_MAX_LAGS = 4096
 
 # every symbol include/liets.h declares
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
-           "liets_set_target", "liets_set_blocked", "liets_step", "liets_generate", "liets_grid", "liets_s2", "liets_step_log", "liets_timings",
+           "liets_set_target", "liets_set_blocked", "liets_step", "liets_generate", "liets_grid", "liets_s2", "liets_s2_static", "liets_step_log", "liets_timings",
            "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info",
            "liets_create_batch", "liets_batch_ctx", "liets_generate_batch", "liets_destroy_batch",
            "liets_batch_last_error", "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_debug_thresholds", "liets_probe", "liets_destroy", "liets_last_error")
@@ -70,6 +71,8 @@ def lib():
     L.liets_grid.restype = ci
     L.liets_s2.argtypes = [vp, ci, ci, P(u64), P(u64)]
     L.liets_s2.restype = ci
+    L.liets_s2_static.argtypes = [vp, ci, ci, P(u64), P(u64)]
+    L.liets_s2_static.restype = ci
     L.liets_step_log.argtypes = [vp, P(u64), P(u64), P(u64), P(u64), u32]
     L.liets_step_log.restype = ci
     L.liets_timings.argtypes = [vp, P(ctypes.c_float), P(ctypes.c_float)]
@@ -250,6 +253,14 @@ class Liets:
         valid = np.zeros(rmax + 1, dtype=np.uint64)
         P64 = ctypes.POINTER(ctypes.c_uint64)
         self._check(self._L.liets_s2(self._h, axis, rmax, pairs.ctypes.data_as(P64), valid.ctypes.data_as(P64)))
+        return pairs, valid
+
+    def s2_static(self, axis, rmax):
+        """s2() through liets_s2_static: no cudaMalloc in the call, counters in a static device array (rmax < S2_STATIC_MAX_LAGS)."""
+        pairs = np.zeros(rmax + 1, dtype=np.uint64)
+        valid = np.zeros(rmax + 1, dtype=np.uint64)
+        P64 = ctypes.POINTER(ctypes.c_uint64)
+        self._check(self._L.liets_s2_static(self._h, axis, rmax, pairs.ctypes.data_as(P64), valid.ctypes.data_as(P64)))
         return pairs, valid
 
     def step_log(self, cap=4096):
