@@ -68,7 +68,7 @@ struct Smem {
     uint32_t ptab[100];                         // voxel index of tile x = 0 of each own row
     uint32_t tile[2], tile_id[2];               // list entry handed to the CTA, double-buffered by tile parity
     uint32_t wsum[2][kWarps];                   // per-warp front-voxel counts, double-buffered
-    uint16_t flist[kFrontCap];                  // (15 - (x & 15)) | (8 row + x / 16) << 4 of the tile's front voxels
+    alignas(4) uint16_t flist[kFrontCap];                  // (15 - (x & 15)) | (8 row + x / 16) << 4 of the tile's front voxels
 };
 
 struct TileCoord {
@@ -237,7 +237,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
         next_li = atomicAdd(&ctl->tile_cursor, 1u);
         if (next_li < n_list) next_id = list_entry(next_li);
     }
-    unsigned long long own_new = 0ull, own_old = 0ull;      // the own word's atomicOr of the previous tile, looked at late
     if (tid == 0) { S.tile[0] = next_li; S.tile_id[0] = next_id; }
     for (uint32_t kt = 0;; ++kt) {
         __syncthreads();                    // the previous tile's shared memory is no longer read; this tile's slot is written
@@ -396,6 +395,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
             }
             __syncthreads();                // flist (and win) complete
             const uint32_t n_pass = min((uint32_t)kFrontCap, n_front - pass0);
+#ifdef LIETS_OLD_C
             // C: one thread per front voxel, kVoxPerThread voxels per thread and trip (their Philox chains interleave, the loop
             // and ring bookkeeping is shared)
             auto level0 = [&](uint32_t i, uint32_t& v, uint32_t& tie, uint32_t& fire) {
@@ -432,6 +432,57 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                     }
                 }
             };
+#else
+            // C: front voxels, two CONSECUTIVE list entries per thread and trip (one 32-bit load), worked without a branch in
+            // one basic block: the two Philox chains interleave and share the round keys.  A warp covers 64 entries, so the
+            // test that skips a warp beyond the list's end is warp-uniform; a lane beyond the end works on a harmless
+            // entry and its result is dropped.  Every listed voxel has a void target unless its directions are disabled
+            // (en26), so the block is evaluated unconditionally and the compare masks by void26.
+            auto gather26 = [&](uint32_t v) -> uint32_t {
+                // the nine rows of the neighbourhood: one window each, aligned so that x+1, x, x-1 are bits 31..29 (a multiply:
+                // FMA pipe) and pushed into the mask three bits at a time (row dz = +1, dy = +1 first):
+                // bit 9(dz+1) + 3(dy+1) + (dx+1) = not void
+                const uint32_t wa = win_addr + ((v >> 2) & 0xFFFCu) - 4u * kWin * 11u;
+                const uint32_t mult = 1u << (v & 15u);
+                uint32_t nb27 = 0;
+#define LIETS_ROW(E) nb27 = __funnelshift_l(mul_lo_u32(lds_u32_at<4 * kWin * (((E) / 3) * 10 + (E) % 3)>(wa), mult), nb27, 3)
+                LIETS_ROW(8); LIETS_ROW(7); LIETS_ROW(6); LIETS_ROW(5); LIETS_ROW(4); LIETS_ROW(3); LIETS_ROW(2); LIETS_ROW(1); LIETS_ROW(0);
+#undef LIETS_ROW
+                // the centre (bit 13) is solid, so ~nb27 has bit 13 clear: closing the gap is (v + (v & 0x1FFF)) >> 1
+                const uint32_t lo13 = ~nb27 & 0x1FFFu;
+                return ((~nb27 + lo13) >> 1) & en26;
+            };
+            constexpr uint32_t kSafeEntry = (8u * 11u) << 4;        // row (0, 0), window 0: a list entry that is always addressable
+            auto level0_pair = [&](uint32_t i, uint32_t* v, uint32_t* tie, uint32_t* fire) {
+                const uint32_t pair = lds_u32(flist_addr + 2u * i);             // i is even
+                const bool live0 = i < n_pass, live1 = i + 1u < n_pass;
+                v[0] = live0 ? (pair & 0xFFFFu) : kSafeEntry;
+                v[1] = live1 ? (pair >> 16) : kSafeEntry;
+                uint32_t void26[2];
+                uint4 B0[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) void26[u] = gather26(v[u]);
+                void26[0] = live0 ? void26[0] : 0u;
+                void26[1] = live1 ? void26[1] : 0u;
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const uint32_t p = lds_u32(ptab_addr + ((v[u] >> 5) & 0x3FCu)) + ((v[u] & 0x7Fu) ^ 15u);
+                    B0[u] = philox_growth_block(p, 0u, ps, key);
+                    n_items0 += void26[u] ? 1u : 0u;
+                }
+                if (h0_any) {               // some leading threshold nibble is non-zero: a draw can fire at level 0
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        uint32_t le;
+                        level0_compare(B0[u], h0, h0m, h08, void26[u], &le, &tie[u]);
+                        fire[u] = le & ~tie[u];
+                    }
+                } else {                    // all leading nibbles are 0: "<=" and "==" coincide with "== 0"
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) tie[u] = level_zero(B0[u], void26[u]);
+                }
+            };
+#endif
             auto settle = [&](uint32_t v, uint32_t tie, uint32_t fire) {       // level-0 hits to the claim volume, ties to the ring
                 if (h0_any && __ballot_sync(0xffffffffu, fire != 0u)) claim(fire, (v & 0x7Fu) ^ 15u, (v >> 7) & 0x1FFu);
                 const uint32_t have = __ballot_sync(0xffffffffu, tie != 0u);
@@ -441,6 +492,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                     qn += __popc(have);
                 }
             };
+#ifdef LIETS_OLD_C
             for (uint32_t i0 = 0; i0 < n_pass; i0 += kVoxPerThread * kThreads) {
                 uint32_t v[kVoxPerThread], tie[kVoxPerThread], fire[kVoxPerThread];
 #pragma unroll
@@ -449,6 +501,15 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                 for (int u = 0; u < kVoxPerThread; ++u) settle(v[u], tie[u], fire[u]);
             }
         }
+#else
+            for (uint32_t i0 = 0; i0 < n_pass; i0 += 2u * kThreads) {
+                uint32_t v[2] = { 0u, 0u }, tie[2] = { 0u, 0u }, fire[2] = { 0u, 0u };
+                if (i0 + 64u * warp < n_pass) level0_pair(i0 + 2u * tid, v, tie, fire);     // warp-uniform
+#pragma unroll
+                for (int u = 0; u < 2; ++u) settle(v[u], tie[u], fire[u]);
+            }
+        }
+#endif
         while (qn) round(min(qn, 32u));
         if (tid == 0) { S.tile[(kt + 1u) & 1u] = next_li; S.tile_id[(kt + 1u) & 1u] = next_id; }   // read after the next barrier but one
         __syncthreads();                    // all claims are in shared memory
@@ -485,9 +546,13 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                 if (nb != id && atomicMax(&stamp[nb], t + 2u) < t + 2u) emit_tile(nb, weight[nb]);
             }
         };
-        // own words first, one per thread: carry g_t and add the hits; the old word is looked at after the halo pass
-        new_solid += __popcll(own_new & ~own_old);                  // the previous tile's own word
-        own_new = 0ull;
+        // A tile is "x-plain" when no claim of it can cross the x border of the grid: always between walls (cells outside
+        // are never void, so they are never claimed), and on a grid that wraps in x when the tile touches neither end of
+        // the row.  Its claim words map one to one to words of the grid.
+        const bool x_plain = !(g.periodic & 1) || (tc.w0 >= 1 && 64 * (tc.w0 + kTileW) < g.nx);
+        // own words first, one per thread: carry g_t and add the hits.  The atomic's old word (who flipped the bit) comes
+        // back while the halo rows are worked on and is looked at after them.
+        unsigned long long own_hits = 0ull, own_old = ~0ull;
         {
             static_assert(64 * kTileW == kThreads, "one own word per thread");
             const int row = (int)tid / kTileW, j = (int)tid - row * kTileW, y = row & 7, z = row >> 3;
@@ -499,36 +564,80 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                     const unsigned long long valid = ~(~0ull << (g.nx - 64 * wg));
                     curw &= valid;
                     in_row &= valid;
-                    if (cw & ~valid) halo_word(r, j + 1, cw & ~valid);       // the cell at x = nx (periodic wrap)
+                    if (!x_plain && (cw & ~valid)) halo_word(r, j + 1, cw & ~valid);       // the cell at x = nx (periodic wrap)
                 }
                 unsigned long long* dst = Gn + (unsigned long long)g.Wp * ((unsigned long long)(tc.y0 + y) + (unsigned long long)g.ny * (unsigned long long)(tc.z0 + z)) + wg;
-                if (in_row) { own_old = atomicOr(dst, curw | in_row); own_new = in_row; }
+                if (in_row) { own_old = atomicOr(dst, curw | in_row); own_hits = in_row; }
                 else if (curw) atomicOr(dst, curw);
             }
         }
-        for (int r = (int)tid; r < 100; r += kThreads) {    // halo words, one thread per row: rarely non-zero
+        // newly active neighbour tile: the first claim of the step into it lists it
+        auto wake = [&](uint32_t nb) {
+            if (nb != id && atomicMax(&stamp[nb], t + 2u) < t + 2u) emit_tile(nb, weight[nb]);
+        };
+        for (int r = (int)tid; r < 100; r += kThreads) {    // halo words, one thread per row
             unsigned long long cw[kRowWords], any = 0ull;
 #pragma unroll
             for (int c = 0; c < kRowWords; ++c) {
                 cw[c] = (unsigned long long)S.claims[r][2 * c] | ((unsigned long long)S.claims[r][2 * c + 1] << 32);
                 any |= cw[c];
             }
-            if (any) {
-                const int zl = r / 10 - 1, yl = r % 10 - 1;
-                const bool own_row = zl >= 0 && zl < tc.wcz && yl >= 0 && yl < tc.wcy;
+            const int zl = r / 10 - 1, yl = r % 10 - 1;
+            const bool own_row = zl >= 0 && zl < tc.wcz && yl >= 0 && yl < tc.wcy;
+            if (own_row) {                                  // the tile words of an own row went out above
+#pragma unroll
+                for (int c = 1; c <= kTileW; ++c)
+                    if (64 * (tc.w0 + c - 1) < g.nx) cw[c] = 0ull;
+                any = 0ull;
+#pragma unroll
+                for (int c = 0; c < kRowWords; ++c) any |= cw[c];
+            }
+            if (!any) continue;
+            if (x_plain) {
+                // all atomics of the row go out together, with plain loads of the stamps of the (at most three) tiles they
+                // fall into; only a tile whose stamp is still old takes the atomicMax
+                const int zg = row_coord(zl, tc.z0, tc.wcz, g.nz, g.periodic & 4);
+                const int yg = row_coord(yl, tc.y0, tc.wcy, g.ny, g.periodic & 2);
+                unsigned long long* rowp = Gn + (unsigned long long)g.Wp * ((unsigned long long)yg + (unsigned long long)g.ny * (unsigned long long)zg) + (tc.w0 - 1);
+                const uint32_t nb_mid = (uint32_t)(tc.w0 / kTileW) + (uint32_t)g.ntx * ((uint32_t)(yg >> 3) + (uint32_t)g.nty * (uint32_t)(zg >> 3));
+                cw[0] &= 1ull << 63;                        // (only the cell next to the tile can be claimed in a halo word)
+                cw[kRowWords - 1] &= 1ull;
+                unsigned long long mid = 0ull;
+#pragma unroll
+                for (int c = 1; c <= kTileW; ++c) mid |= cw[c];
+                unsigned long long old[kRowWords];
+                uint32_t st[3] = { ~0u, ~0u, ~0u };
 #pragma unroll
                 for (int c = 0; c < kRowWords; ++c) {
+                    old[c] = ~0ull;
+                    if (cw[c]) old[c] = atomicOr(rowp + c, cw[c]);
+                }
+                if (cw[0]) st[0] = __ldcg(&stamp[nb_mid - 1u]);
+                if (mid) st[1] = __ldcg(&stamp[nb_mid]);
+                if (cw[kRowWords - 1]) st[2] = __ldcg(&stamp[nb_mid + 1u]);
+#pragma unroll
+                for (int c = 0; c < kRowWords; ++c) new_solid += __popcll(cw[c] & ~old[c]);
+                uint32_t need = (st[0] < t + 2u ? 1u : 0u) | (st[1] < t + 2u ? 2u : 0u) | (st[2] < t + 2u ? 4u : 0u);
+                while (need) {                              // rare: at most once per neighbour tile and step
+                    const uint32_t k = 31u - __clz(need);
+                    need ^= 1u << k;
+                    wake(nb_mid + k - 1u);
+                }
+            } else {
+#pragma unroll 1
+                for (int c = 0; c < kRowWords; ++c) {       // (the words are read again: no register array indexed at run time)
                     const bool own_word = own_row && c >= 1 && c <= kTileW && 64 * (tc.w0 + c - 1) < g.nx;
-                    if (cw[c] && !own_word) halo_word(r, c, cw[c]);
+                    const unsigned long long cwv = (unsigned long long)S.claims[r][2 * c] | ((unsigned long long)S.claims[r][2 * c + 1] << 32);
+                    if (cwv && !own_word) halo_word(r, c, cwv);
                 }
             }
         }
+        new_solid += __popcll(own_hits & ~own_old);
         if (tid == 0 && n_front) {                                  // this tile still has front voxels
             weight[id] = n_front;                                   // whoever lists the tile for the next step sorts it by this
             if (atomicMax(&stamp[id], t + 2u) < t + 2u) emit_tile(id, n_front);
         }
     }
-    new_solid += __popcll(own_new & ~own_old);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         new_solid += __shfl_xor_sync(0xffffffffu, new_solid, o);
