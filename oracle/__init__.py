@@ -75,6 +75,12 @@ def lib(omp=False):
     L.oracle_set_target.restype = ci
     L.oracle_seed.argtypes = [vp, dbl, ci, u64]
     L.oracle_seed.restype = i64
+    L.oracle_seed_by_dilation.argtypes = [vp, dbl, ci, u64]
+    L.oracle_seed_by_dilation.restype = i64
+    L.oracle_set_spacing_order.argtypes = [vp, ci]
+    L.oracle_set_spacing_order.restype = ci
+    L.oracle_seed_priority.argtypes = [u64, u64]
+    L.oracle_seed_priority.restype = u32
     L.oracle_seed_explicit.argtypes = [vp, P(u64), u64, u64]
     L.oracle_seed_explicit.restype = i64
     L.oracle_step_full.argtypes = [vp]
@@ -126,6 +132,11 @@ def growth_draw(rng_seed, t, p, d):
 
 def seed_draw(rng_seed, v):
     return int(lib().oracle_seed_draw(rng_seed, v))
+
+
+def seed_priority(rng_seed, v):
+    """R19: the key of voxel v in the keyed acceptance order of the spacing filter."""
+    return int(lib().oracle_seed_priority(rng_seed, v))
 
 
 def direction(d):
@@ -194,6 +205,18 @@ class Oracle:
 
     def seed(self, core_prob, spacing_s, rng_seed):
         n = self._L.oracle_seed(self._h, core_prob, spacing_s, rng_seed)
+        if n < 0:
+            raise ValueError("bad seed parameters")
+        return int(n)
+
+    def set_spacing_order(self, order):
+        """0 = ascending index (R12), 1 = ascending (seed_priority, index) (R19); used by the next seed()."""
+        if self._L.oracle_set_spacing_order(self._h, order) != 0:
+            raise ValueError("bad spacing order")
+
+    def seed_by_dilation(self, core_prob, spacing_s, rng_seed):
+        """seed() with the spacing filter done by literal diamond dilation; ascending index order."""
+        n = self._L.oracle_seed_by_dilation(self._h, core_prob, spacing_s, rng_seed)
         if n < 0:
             raise ValueError("bad seed parameters")
         return int(n)

@@ -65,6 +65,19 @@ uint32_t oracle_seed_draw(uint64_t rng_seed, uint64_t v) {
     return out[v % 4];
 }
 
+/* R19 (the order kept in reserve there): the key of voxel v in the keyed acceptance order of the
+ * spacing filter.  The paper does not say in which order candidate cores are tried; with this key the
+ * order is a random permutation fixed by the seed.  Counter (v/4, 0, 1, 2^32-1): the core draw uses (v/4, 0, 0, 2^32-1),
+ * the growth draws have a last word <= 7, so the three streams never meet. */
+uint32_t oracle_seed_priority(uint64_t rng_seed, uint64_t v) {
+    uint32_t key[2] = { (uint32_t)(rng_seed & 0xFFFFFFFFu), (uint32_t)(rng_seed >> 32) };
+    uint64_t blk = v / 4;
+    uint32_t ctr[4] = { (uint32_t)(blk & 0xFFFFFFFFu), (uint32_t)(blk >> 32), 1u, 0xFFFFFFFFu };
+    uint32_t out[4];
+    oracle_philox4x32_10(ctr, key, out);
+    return out[v % 4];
+}
+
 /* ------------------------------------------------------------------------------------------
  * R1: the 26 directions.  See DESIGN.md "Readings" R1 for the order; class = |dx|+|dy|+|dz|.
  * ------------------------------------------------------------------------------------------ */
@@ -121,6 +134,7 @@ struct oracle_state {
     int has_target;
     uint64_t n_t;
     uint64_t attempts[26], successes[26];
+    int spacing_order;        /* 0: candidates are tried in ascending index (R12); 1: in ascending (key, index) (R19) */
 };
 
 oracle_state* oracle_new(int nx, int ny, int nz, int periodic) {
@@ -233,10 +247,52 @@ static int64_t l1_dist(const oracle_state* o, uint64_t v, uint64_t w) {
            axis_dist(vz, wz, o->nz, o->periodic & 4);
 }
 
+int oracle_set_spacing_order(oracle_state* o, int order) {
+    if (order != 0 && order != 1) return -1;
+    o->spacing_order = order;
+    return 0;
+}
+
+typedef struct { uint32_t key; uint64_t v; } keyed_cand;
+
+static int keyed_cmp(const void* a, const void* b) {
+    const keyed_cand* p = (const keyed_cand*)a;
+    const keyed_cand* q = (const keyed_cand*)b;
+    if (p->key != q->key) return p->key < q->key ? -1 : 1;
+    return p->v < q->v ? -1 : (p->v > q->v ? 1 : 0);
+}
+
+static int u64_cmp(const void* a, const void* b) {
+    uint64_t p = *(const uint64_t*)a, q = *(const uint64_t*)b;
+    return p < q ? -1 : (p > q ? 1 : 0);
+}
+
 int64_t oracle_seed(oracle_state* o, double core_prob, int spacing_s, uint64_t rng_seed) {
     if (core_prob < 0.0 || core_prob > 1.0 || spacing_s < 0) return -1;
     reset_run(o, rng_seed);
     uint64_t T_core = oracle_prob_to_threshold(core_prob);
+    if (o->spacing_order == 1 && spacing_s > 1) {
+        /* R19: the same candidates, tried in ascending (key, index) instead of ascending index */
+        uint64_t n = 0, cap = 1024;
+        keyed_cand* c = (keyed_cand*)malloc(cap * sizeof(*c));
+        for (uint64_t v = 0; v < o->N; ++v) {
+            if (o->grid[v] != 0) continue;
+            if ((uint64_t)oracle_seed_draw(rng_seed, v) >= T_core) continue;
+            if (n == cap) { cap *= 2; c = (keyed_cand*)realloc(c, cap * sizeof(*c)); }
+            c[n].key = oracle_seed_priority(rng_seed, v); c[n].v = v; ++n;
+        }
+        qsort(c, n, sizeof(*c), keyed_cmp);
+        for (uint64_t k = 0; k < n; ++k) {
+            int ok = 1;
+            for (uint64_t i = 0; i < o->n_front; ++i)                       /* accepted so far */
+                if (l1_dist(o, c[k].v, o->front[i]) < (int64_t)spacing_s) { ok = 0; break; }
+            if (ok) { o->grid[c[k].v] = 1; front_push(o, c[k].v); }
+        }
+        free(c);
+        qsort(o->front, o->n_front, sizeof(uint64_t), u64_cmp);             /* A_0 listed in ascending index, as always */
+        o->n_solid = o->n_front;
+        return (int64_t)o->n_solid;
+    }
     for (uint64_t v = 0; v < o->N; ++v) {
         if (o->grid[v] != 0) continue;                                     /* an earlier phase's cell: not unassigned */
         if ((uint64_t)oracle_seed_draw(rng_seed, v) >= T_core) continue;   /* not a candidate */
@@ -249,6 +305,47 @@ int64_t oracle_seed(oracle_state* o, double core_prob, int spacing_s, uint64_t r
         if (ok) { o->grid[v] = 1; front_push(o, v); }
     }
     o->n_solid = o->n_front;       /* A_0 = seeds (R3) */
+    return (int64_t)o->n_solid;
+}
+
+/* The spacing filter as the paper words it (Fig. 1(D): "diamond dilation is conducted with a small
+ * kernel but multiple iterations"): a candidate is accepted iff it is not covered, and every accepted seed covers its
+ * diamond, grown literally by s-1 passes of the 6-neighbour kernel (pass: every covered cell covers its face
+ * neighbours; walls or wrap per axis as the grid's boundary says).  Ascending index order only.  Same result as
+ * oracle_seed (pin P5d); cost O(s^3) per seed, for small cases. */
+int64_t oracle_seed_by_dilation(oracle_state* o, double core_prob, int spacing_s, uint64_t rng_seed) {
+    static const int FACE[6] = { 4, 10, 12, 13, 15, 21 };                  /* the six directions of class 1 (R1) */
+    if (core_prob < 0.0 || core_prob > 1.0 || spacing_s < 0) return -1;
+    for (int k = 0; k < 6; ++k)
+        if (abs(ORACLE_DIRS[FACE[k]][0]) + abs(ORACLE_DIRS[FACE[k]][1]) + abs(ORACLE_DIRS[FACE[k]][2]) != 1) return -3;
+    reset_run(o, rng_seed);
+    uint64_t T_core = oracle_prob_to_threshold(core_prob);
+    uint8_t* covered = (uint8_t*)calloc(o->N, 1);
+    uint64_t* wave = (uint64_t*)malloc(o->N * sizeof(uint64_t));
+    for (uint64_t v = 0; v < o->N; ++v) {
+        if (o->grid[v] != 0) continue;
+        if ((uint64_t)oracle_seed_draw(rng_seed, v) >= T_core) continue;
+        if (spacing_s > 1 && covered[v]) continue;
+        o->grid[v] = 1; front_push(o, v);
+        if (spacing_s > 1) {
+            uint8_t* mine = (uint8_t*)calloc(o->N, 1);                     /* this seed's diamond */
+            uint64_t n_wave = 1, lo = 0;
+            wave[0] = v; mine[v] = 1;
+            for (int pass = 1; pass < spacing_s; ++pass) {                 /* s-1 passes */
+                uint64_t hi = n_wave;
+                for (uint64_t i = lo; i < hi; ++i)
+                    for (int k = 0; k < 6; ++k) {
+                        uint64_t q;
+                        if (neighbour(o, wave[i], FACE[k], &q) && !mine[q]) { mine[q] = 1; wave[n_wave++] = q; }
+                    }
+                lo = hi;
+            }
+            for (uint64_t i = 0; i < n_wave; ++i) covered[wave[i]] = 1;
+            free(mine);
+        }
+    }
+    free(covered); free(wave);
+    o->n_solid = o->n_front;
     return (int64_t)o->n_solid;
 }
 

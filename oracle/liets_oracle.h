@@ -60,6 +60,13 @@ int oracle_set_target(oracle_state* o, double phi_s);
 
 /* Seeding + seed spacing (R11, R12). Resets grid, front, step. */
 int64_t oracle_seed(oracle_state* o, double core_prob, int spacing_s, uint64_t rng_seed);
+/* R19: 0 (default) = candidates are tried in ascending index (R12); 1 = in ascending (oracle_seed_priority, index), a
+ * random order fixed by the seed.  Used by the next oracle_seed. */
+int oracle_set_spacing_order(oracle_state* o, int order);
+uint32_t oracle_seed_priority(uint64_t rng_seed, uint64_t v);
+/* The spacing filter by literal diamond dilation (s-1 passes of the 6-neighbour kernel per accepted seed),
+ * ascending index order: the same seeds as oracle_seed. */
+int64_t oracle_seed_by_dilation(oracle_state* o, double core_prob, int spacing_s, uint64_t rng_seed);
 /* Same candidates, but place an explicit list of seeds instead (for closed-form tests). */
 int64_t oracle_seed_explicit(oracle_state* o, const uint64_t* idx, uint64_t n, uint64_t rng_seed);
 

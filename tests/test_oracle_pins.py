@@ -609,3 +609,85 @@ def test_cells_of_an_earlier_phase_are_neither_void_nor_sources(use_list):
         o.seed(0.01, 3, 9)
         o.generate(0.4)
     assert (a.grid() == b.grid()).all() and a.n_solid == b.n_solid
+
+
+# ------------------------------------------------------------------------- P5d, P5k (NEXT-1: R19)
+@pytest.mark.parametrize("periodic", [0, 1, 2])
+@pytest.mark.parametrize("s", [0, 2, 4, 7])
+def test_p5d_seeding_by_literal_dilation_passes_equals_the_distance_rule(periodic, s):
+    """PAPER.md:131 Fig. 1(D): diamond dilation 'with a small kernel but multiple iterations'.  The oracle's literal
+    form (every accepted seed covers what s-1 passes of the 6-neighbour kernel reach, walls or wrap per axis) accepts
+    exactly the seeds of the distance rule of oracle_seed."""
+    nx, ny, nz = 23, 14, 9
+    a = oracle.Oracle(nx, ny, nz, periodic)
+    b = oracle.Oracle(nx, ny, nz, periodic)
+    na, nb = a.seed(0.03, s, 21 + s), b.seed_by_dilation(0.03, s, 21 + s)
+    assert na == nb and (a.grid() == b.grid()).all()
+    if s > 1:
+        assert na < int((np.array([oracle.seed_draw(21 + s, v) for v in range(nx * ny * nz)]) < oracle.prob_to_threshold(0.03)).sum())
+
+
+def test_p5k_priority_is_a_word_of_its_own_philox_block():
+    """R19: key(v) = word v % 4 of Philox4x32-10 at counter (v / 4, 0, 1, 2^32 - 1) -- the block function itself is
+    pinned by the known answers (P1); the core draw sits at (v / 4, 0, 0, 2^32 - 1)."""
+    for seed in (0, 7, 0x123456789ABCDEF0):
+        key = (seed & 0xFFFFFFFF, seed >> 32)
+        for v in (0, 1, 2, 3, 4, 1000003, 2**32 + 5, 2**34 + 2):
+            blk = v // 4
+            ctr = (blk & 0xFFFFFFFF, blk >> 32, 1, 0xFFFFFFFF)
+            assert oracle.seed_priority(seed, v) == oracle.philox4x32_10(ctr, key)[v % 4]
+            ctr0 = (blk & 0xFFFFFFFF, blk >> 32, 0, 0xFFFFFFFF)
+            assert oracle.seed_draw(seed, v) == oracle.philox4x32_10(ctr0, key)[v % 4]
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("s", [0, 1, 2, 3, 5, 8])
+def test_p5k_keyed_order_equals_the_greedy_in_key_order(periodic, s):
+    """The keyed acceptance order (R19): the same candidates as in index order, tried in ascending (key, index).
+    Against the independent dilation greedy fed with the candidates in that order; the result keeps every pair at
+    L1 >= s and is maximal: every rejected candidate has an accepted seed EARLIER in the order within L1 < s."""
+    nx, ny, nz = 20, 17, 14
+    N = nx * ny * nz
+    seed, c = 31 + s, 0.02
+    Tc = oracle.prob_to_threshold(c)
+    cand = [v for v in range(N) if oracle.seed_draw(seed, v) < Tc]
+    order = sorted(cand, key=lambda v: (oracle.seed_priority(seed, v), v))
+    expect = sorted(_dilation_greedy((nz, ny, nx), periodic, order, s))
+    o = oracle.Oracle(nx, ny, nz, periodic)
+    o.set_spacing_order(1)
+    n = o.seed(c, s, seed)
+    got = np.flatnonzero(o.grid().ravel())
+    assert n == len(expect) and (got == np.array(expect)).all()
+    if s <= 1:
+        assert list(got) == cand
+        return
+    pos = {v: k for k, v in enumerate(order)}
+    pts = {v: np.array((v % nx, (v // nx) % ny, v // (nx * ny))) for v in cand}
+    dims = np.array([nx, ny, nz])
+
+    def dist(a, b):
+        d = np.abs(a - b)
+        if periodic:
+            d = np.minimum(d, dims - d)
+        return int(d.sum())
+    acc = [int(v) for v in got]
+    for i, v in enumerate(acc):
+        for w in acc[:i]:
+            assert dist(pts[v], pts[w]) >= s
+    for v in set(cand) - set(acc):
+        assert any(pos[w] < pos[v] and dist(pts[v], pts[w]) < s for w in acc)
+    # the order matters: index order accepts another maximal set (same candidates, another permutation)
+    o2 = oracle.Oracle(nx, ny, nz, periodic)
+    o2.seed(c, s, seed)
+    if s >= 3:
+        assert (o2.grid() != o.grid()).any()
+    # and growth goes on from the keyed seeds like from any others: list step == full-field step
+    for q in (o, o2):
+        q.set_growth(0.1, 0.05, 0.02, 0)
+    a = oracle.Oracle(nx, ny, nz, periodic)
+    a.set_spacing_order(1)
+    a.set_growth(0.1, 0.05, 0.02, 0)
+    a.seed(c, s, seed)
+    o.step(use_list=True)
+    a.step(use_list=False)
+    assert (o.grid() == a.grid()).all()
