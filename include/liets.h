@@ -194,6 +194,25 @@ int liets_step_times(liets_ctx* ctx, float* ms, uint32_t cap);
 /* Number of kernels this ctx has launched since liets_create (memsets and copies not counted). */
 uint64_t liets_launch_count(const liets_ctx* ctx);
 
+/* Variants of the spacing filter of liets_seed, used from the next liets_seed on.
+ * order  LIETS_ORDER_INDEX (default): candidates are tried in ascending linear index (R12).
+ *        LIETS_ORDER_KEYED: in ascending (key, index), key(v) = word v % 4 of Philox4x32-10 at counter
+ *        (v / 4, 0, 1, 2^32 - 1) under the rng_seed's key: a random order fixed by the seed (R19; the paper does not say
+ *        in which order cores are tried).  Another maximal set of seeds at pairwise L1 >= s; the
+ *        dependency chains are a handful of rounds long instead of a sweep through the grid.
+ * method LIETS_SPACING_SPARSE (default): works on the list of candidates.
+ *        LIETS_SPACING_DENSE: the paper's mechanism (Fig. 1(D), "a small kernel but multiple iterations"):
+ *        every round dilates bit planes of the WHOLE grid by s-1 passes of the 6-neighbour kernel.  Same seeds as the
+ *        default (index order); LIETS_BOUNDARY_WALL only; kept as the same-box comparison for the paper's "seed spacing
+ *        halves the generation rate" (:189).  liets_seed then synchronises once per round and may return E_CAPACITY when
+ *        the candidate list and 8 bit planes (ceil(nx/64) * 8 * ny * nz bytes each) exceed the 4 N bytes of seeding scratch.
+ * Errors: E_ARG (unknown value, DENSE with KEYED, DENSE on a periodic grid). */
+enum { LIETS_ORDER_INDEX = 0, LIETS_ORDER_KEYED = 1 };
+enum { LIETS_SPACING_SPARSE = 0, LIETS_SPACING_DENSE = 1 };
+int liets_set_spacing(liets_ctx* ctx, int order, int method);
+/* After liets_seed: rounds the keyed-order or dense-dilation spacing took (0 for the default path).  Errors: E_STATE. */
+int liets_spacing_rounds(liets_ctx* ctx, uint32_t* rounds);
+
 /* After liets_seed: the number of keyed candidates before spacing, and whether the spacing was
  * resolved by the rescan slow path (1) or by the adjacency lists (0); both may be NULL.  Errors: E_STATE. */
 int liets_seed_info(liets_ctx* ctx, uint32_t* n_candidates, uint32_t* slow_path);

@@ -8,4 +8,4 @@ loudly if the library has not been built, and every call fails without a CUDA de
 from .liets import (Liets, LietsBatch, LietsError, lib, library_path, OK, FRONT_EMPTY, MAX_STEPS,  # noqa: F401
                     E_ARG, E_STATE, E_CAPACITY, E_CUDA,
                     BOUNDARY_WALL, BOUNDARY_PERIODIC, BOUNDARY_PERIODIC_XY, STORAGE_U8, STORAGE_TILE, STORAGE_FULL, LAW_CONSTANT, LAW_EQ1,
-                    FORMAT_U8, FORMAT_BITS, S2_STATIC_MAX_LAGS, EXPORTS)
+                    FORMAT_U8, FORMAT_BITS, S2_STATIC_MAX_LAGS, ORDER_INDEX, ORDER_KEYED, SPACING_SPARSE, SPACING_DENSE, EXPORTS)

@@ -40,10 +40,12 @@ constexpr int kThreads = 128;
 #endif
 constexpr int kCtasPerSm = LIETS_TILE_CTAS;       // resident CTAs per SM the kernel is compiled for (registers) and launched with
 constexpr int kWarps = kThreads / 32;
+#ifdef LIETS_OLD_C
 #ifndef LIETS_VOX_PER_THREAD
 #define LIETS_VOX_PER_THREAD 2
 #endif
 constexpr int kVoxPerThread = LIETS_VOX_PER_THREAD;     // front voxels a thread handles per trip of phase C
+#endif
 constexpr int kMaxBatch = 16;                   // grids per launch of the batched kernel (kernel parameters: 2.2 KB)
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
 constexpr int kWin = 64 * kTileW / 16;          // 18-bit windows per row, one per 16 voxels

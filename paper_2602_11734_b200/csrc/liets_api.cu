@@ -334,13 +334,38 @@ int liets_seed(liets_ctx* c, double core_prob, int spacing_s, uint64_t rng_seed,
     LIETS_CUDA_TRY(c, launch_seed_reset(c));
     const int accept_all = spacing_s <= 1;
     LIETS_CUDA_TRY(c, launch_seed_candidates(c, prob_to_threshold(core_prob), accept_all));
-    if (!accept_all) LIETS_CUDA_TRY(c, launch_spacing(c, spacing_s));
+    if (!accept_all) {
+        if (c->spacing_method == LIETS_SPACING_DENSE) {     // the bit rows go behind the candidate list: its length first
+            if (int rc = readback(c)) return rc;
+            const uint32_t n_cand = c->pinned->n_cand;
+            const size_t need = (((size_t)n_cand * 4u + 255u) & ~(size_t)255u) + 8u * spacing_dense_bytes(c);
+            if (need > (size_t)c->N * 4u) return fail(c, LIETS_E_CAPACITY, "dense spacing: the bit rows do not fit the seeding scratch (4 N bytes)");
+            LIETS_CUDA_TRY(c, launch_spacing_dense(c, spacing_s, n_cand, nullptr));
+        } else if (c->spacing_order == LIETS_ORDER_KEYED) {
+            LIETS_CUDA_TRY(c, launch_spacing_keyed(c, spacing_s));
+        } else {
+            LIETS_CUDA_TRY(c, launch_spacing(c, spacing_s));
+        }
+    }
     LIETS_CUDA_TRY(c, launch_seed_finalize(c, !accept_all));
     LIETS_CUDA_TRY(c, cudaEventRecord(c->ev1, c->stream));
     if (int rc = readback(c)) return rc;
     LIETS_CUDA_TRY(c, cudaEventElapsedTime(&c->seed_ms, c->ev0, c->ev1));
     c->seeded = true;
     if (n_seeds_out) *n_seeds_out = c->pinned->n_solid;
+    return LIETS_OK;
+}
+
+int liets_set_spacing(liets_ctx* c, int order, int method) {
+    if (!c) return LIETS_E_ARG;
+    if ((order != LIETS_ORDER_INDEX && order != LIETS_ORDER_KEYED) || (method != LIETS_SPACING_SPARSE && method != LIETS_SPACING_DENSE))
+        return fail(c, LIETS_E_ARG, "unknown spacing order or method");
+    if (method == LIETS_SPACING_DENSE && order != LIETS_ORDER_INDEX)
+        return fail(c, LIETS_E_ARG, "the dense dilation works in ascending index order only");
+    if (method == LIETS_SPACING_DENSE && c->periodic)
+        return fail(c, LIETS_E_ARG, "the dense dilation is built for LIETS_BOUNDARY_WALL only");
+    c->spacing_order = order;
+    c->spacing_method = method;
     return LIETS_OK;
 }
 
@@ -541,6 +566,14 @@ int liets_seed_info(liets_ctx* c, uint32_t* n_candidates, uint32_t* slow_path) {
     if (int rc = readback(c)) return rc;
     if (n_candidates) *n_candidates = c->pinned->n_cand;
     if (slow_path) *slow_path = c->pinned->spacing_slow;
+    return LIETS_OK;
+}
+
+int liets_spacing_rounds(liets_ctx* c, uint32_t* rounds) {
+    if (!c || !rounds) return LIETS_E_ARG;
+    if (!c->seeded) return fail(c, LIETS_E_STATE, "liets_spacing_rounds before liets_seed");
+    if (int rc = readback(c)) return rc;
+    *rounds = c->pinned->spacing_rounds;
     return LIETS_OK;
 }
 

@@ -125,6 +125,7 @@ struct Control {
     uint32_t n_cand;                 // seeding: candidates
     uint32_t pend3[3];               // seeding: pending candidates after round r, at index r % 3
     uint32_t spacing_slow;           // seeding: the adjacency lists do not fit the fast resolve -> rescan rounds
+    uint32_t spacing_rounds;         // seeding: rounds of the keyed-order / dense-dilation spacing (0 for the default path)
     uint32_t items;                  // Philox blocks evaluated by the live step (profiling counter)
     uint32_t items0;                 // front voxels with a void target in the live step (= level-0 blocks)
     // STORAGE_TILE keeps the active set as a voxel list while it is small (grow_vox.cu) and as a tile list afterwards

@@ -53,6 +53,8 @@ struct liets_ctx {
     uint64_t n_blocked;
     uint32_t host_step;               // step counter as of the last read-back (selects the current grid copy)
     int resolve_grid;                 // CTAs of the cooperative spacing kernel (0 = not sized yet)
+    int resolve_keyed_grid;           // ... of the keyed-order one
+    int spacing_order, spacing_method;   // liets_set_spacing: LIETS_ORDER_*, LIETS_SPACING_*
     uint32_t spacing_ring, spacing_head;  // test hook (liets_debug_spacing_ring): 0 = the built-in sizes
     int tile_grid;                    // CTAs of the tile growth kernel
     int vox_grid;                     // CTAs of the cooperative voxel-list loop (0 = not sized yet)
@@ -140,6 +142,9 @@ int grow_tile_ctas_per_sm();
 cudaError_t launch_seed_reset(liets_ctx* c);
 cudaError_t launch_seed_candidates(liets_ctx* c, uint64_t t_core, int accept_all);
 cudaError_t launch_spacing(liets_ctx* c, int s);
+cudaError_t launch_spacing_keyed(liets_ctx* c, int s);
+cudaError_t launch_spacing_dense(liets_ctx* c, int s, uint32_t n_cand, uint32_t* rounds_out);
+size_t spacing_dense_bytes(const liets_ctx* c);
 cudaError_t launch_seed_finalize(liets_ctx* c, int spaced);
 cudaError_t launch_seed_explicit(liets_ctx* c, uint64_t n);
 cudaError_t seed_kernel_attributes();

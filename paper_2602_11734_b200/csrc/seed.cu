@@ -33,7 +33,7 @@ __device__ __forceinline__ uint32_t ld_cg(const uint32_t* p) {
 __global__ void k_seed_reset(Control* c) {
     c->n_solid = 0; c->step = 0; c->steps_done = 0; c->active = 0; c->status = 0; c->cur = 0;
     c->count[0] = 0; c->count[1] = 0; c->count_back[0] = 0; c->count_back[1] = 0; c->claims = 0; c->n_cand = 0;
-    c->pool_head = 0; c->pend3[0] = 0; c->pend3[1] = 0; c->pend3[2] = 0; c->spacing_slow = 0;
+    c->pool_head = 0; c->pend3[0] = 0; c->pend3[1] = 0; c->pend3[2] = 0; c->spacing_slow = 0; c->spacing_rounds = 0;
     c->vox_count[0] = 0; c->vox_count[1] = 0; c->vox_overflow = 0; c->pending = 0;
 }
 
@@ -171,9 +171,11 @@ __device__ __forceinline__ void scan_segment(const uint32_t* status2, unsigned l
     }
 }
 
+// whole = true walks every voxel of the diamond (limit = N: no index cut), v itself included
 template <class F>
 __device__ __forceinline__ void scan_diamond(const uint32_t* status2, uint32_t v, const Dims& g, int s,
-                                             uint32_t lane, F& on_word) {
+                                             uint32_t lane, F& on_word, bool whole = false, unsigned long long n_all = 0ull) {
+    const unsigned long long limit = whole ? n_all : (unsigned long long)v;
     const int x = (int)(v % (uint32_t)g.nx);
     const uint32_t rest = v / (uint32_t)g.nx;
     const int y = (int)(rest % (uint32_t)g.ny), z = (int)(rest / (uint32_t)g.ny);
@@ -182,33 +184,33 @@ __device__ __forceinline__ void scan_diamond(const uint32_t* status2, uint32_t v
     // without any wrap-around, lower-index voxels have dz < 0, or dz = 0 and dy <= 0; with a periodic axis the whole
     // diamond is walked and `limit` (on_word sees indices below v only) keeps the lower ones
     const int px = g.periodic & 1, py = g.periodic & 2, pz = g.periodic & 4;
-    const int n_rows = g.periodic ? side * side : (r + 1) * side;
+    const int n_rows = (g.periodic || whole) ? side * side : (r + 1) * side;
     for (int j = (int)lane; j < n_rows; j += 32) {
         const int dz = j / side - r, dy = j % side - r;
         const int rem = r - abs(dz) - abs(dy);
         if (rem < 0) continue;
         int Y = y + dy, Z = z + dz;
-        if (!g.periodic && dz == 0 && dy > 0) continue;
+        if (!g.periodic && !whole && dz == 0 && dy > 0) continue;
         if (py) { Y %= g.ny; if (Y < 0) Y += g.ny; } else if (Y < 0 || Y >= g.ny) continue;
         if (pz) { Z %= g.nz; if (Z < 0) Z += g.nz; } else if (Z < 0 || Z >= g.nz) continue;
         const unsigned long long row = ((unsigned long long)Z * g.ny + Y) * (unsigned long long)g.nx;
         int xa = x - rem, xb = x + rem;
         if (px && 2 * rem + 1 >= g.nx) {                    // the range covers the whole row
-            scan_segment(status2, row, row + g.nx - 1, v, on_word);
+            scan_segment(status2, row, row + g.nx - 1, limit, on_word);
         } else if (!px) {                                   // clipped at the walls
             xa = xa < 0 ? 0 : xa;
             xb = xb >= g.nx ? g.nx - 1 : xb;
-            scan_segment(status2, row + xa, row + xb, v, on_word);
+            scan_segment(status2, row + xa, row + xb, limit, on_word);
         } else {                                            // wrapped range, at most two segments
             if (xa < 0) {
-                scan_segment(status2, row + (xa + g.nx), row + g.nx - 1, v, on_word);
+                scan_segment(status2, row + (xa + g.nx), row + g.nx - 1, limit, on_word);
                 xa = 0;
             }
             if (xb >= g.nx) {
-                scan_segment(status2, row, row + (xb - g.nx), v, on_word);
+                scan_segment(status2, row, row + (xb - g.nx), limit, on_word);
                 xb = g.nx - 1;
             }
-            scan_segment(status2, row + xa, row + xb, v, on_word);
+            scan_segment(status2, row + xa, row + xb, limit, on_word);
         }
     }
 }
@@ -457,6 +459,163 @@ __global__ void __launch_bounds__(1024) k_spacing_resolve(Control* ctl, uint32_t
     }
 }
 
+// --- keyed acceptance order (R19) ---------------------------------------------------------
+// The same candidates, tried in ascending (key, index), key(v) = word v % 4 of Philox at counter (v / 4, 0, 1, 2^32 - 1): a
+// random order fixed by the seed.  The order has no spatial structure, so there are no rank windows to exploit: every
+// pending candidate rescans its WHOLE diamond in the global status map each round and evaluates the key of every
+// candidate it meets; the dependency chains are short (a handful of rounds instead of a sweep through the grid).
+__device__ __forceinline__ uint32_t seed_priority(uint32_t v, const PhiloxKey& key) {
+    const uint4 r = philox4x32_10(v >> 2, 0u, 1u, 0xFFFFFFFFu, key);
+    const uint32_t w = v & 3u;
+    return w == 0u ? r.x : w == 1u ? r.y : w == 2u ? r.z : r.w;
+}
+
+__global__ void __launch_bounds__(1024) k_spacing_resolve_keyed(Control* ctl, uint32_t* status2, uint32_t* cand,
+                                                                 Dims g, int s, unsigned long long N, PhiloxKey key) {
+    cg::grid_group grid = cg::this_grid();
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, n_threads = gridDim.x * blockDim.x;
+    const uint32_t n = ctl->n_cand;
+    if (tid == 0) ctl->spacing_slow = 1u;                   // the result is read from the status map, by voxel
+    for (uint32_t round = 0;; ++round) {
+        uint32_t still = 0;
+        for (uint32_t i = tid >> 5; i < n; i += n_threads >> 5) {      // one warp per candidate
+            const uint32_t v = cand[i];
+            if (status_of(status2, v) != 1u) continue;
+            const uint32_t kv = seed_priority(v, key);
+            bool accepted = false, pending = false;
+            auto look = [&](uint32_t word, unsigned long long lo) {
+                uint32_t f = word & 0x55555555u;            // candidates that are pending or accepted
+                while (f) {
+                    const uint32_t b = (uint32_t)__ffs(f) - 1u;
+                    f &= f - 1u;
+                    const uint32_t w = (uint32_t)lo + (b >> 1);
+                    if (w == v) continue;
+                    const uint32_t kw = seed_priority(w, key);
+                    if (kw < kv || (kw == kv && w < v)) {   // w is tried before v
+                        if ((word >> (b + 1u)) & 1u) accepted = true;
+                        else pending = true;
+                    }
+                }
+            };
+            scan_diamond(status2, v, g, s, lane, look, true, N);
+            accepted = __any_sync(0xffffffffu, accepted);
+            pending = __any_sync(0xffffffffu, pending);
+            if (lane == 0) {
+                if (accepted) atomicAnd(status2 + (v >> 4), ~(1u << (2 * (v & 15u))));
+                else if (!pending) atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u)));
+                else still++;
+            }
+        }
+        if (lane == 0 && still) atomicAdd(&ctl->pend3[round % 3u], still);
+        grid.sync();
+        const uint32_t left = ld_cg(&ctl->pend3[round % 3u]);
+        if (tid == 0) { ctl->pend3[(round + 2u) % 3u] = 0; ctl->spacing_rounds = round + 1u; }
+        if (left == 0) break;
+    }
+}
+
+// --- the spacing filter by dense diamond dilation (Fig. 1(D)) ------------------
+// The paper's mechanism -- repeated passes of a small kernel over the whole grid -- on bit rows (x-rows of Wp 64-bit
+// words), giving exactly the seeds of the ascending-index rule (R12) between walls.  Per round:
+//   LB  = the pending cells dilated by the "later half" of the diamond, D+ = { d != 0 : L1(d) <= s-1, d after 0 in index
+//         order } = (e_z + (s-2) passes of {0, +-x, +-y, +z}) U (e_y + (s-2) passes of {0, +-x, +y}) U (e_x + (s-2) passes of
+//         {0, +x}): a cell of LB has a pending candidate of lower index within its diamond;
+//   NEW = pending & ~LB: nothing of lower index can still cover them -- accepted;
+//   BL  = NEW dilated by s-1 passes of the full 6-neighbour kernel; pending &= ~BL.
+// A round costs 2 (s-1) + 2 sweeps of the bit grid, and the number of rounds is the length of the longest dependency
+// chain in index order: this is the cost the candidate-list form (k_spacing_adjacency / k_spacing_resolve_cta) avoids.
+struct DenseGeom { int nx, ny, nz, Wp; };
+enum : uint32_t { kDilC = 1u, kDilXm = 2u, kDilXp = 4u, kDilYm = 8u, kDilYp = 16u, kDilZm = 32u, kDilZp = 64u };   // out(u) |= in(u), in(u - ex), in(u + ex), ..
+struct DensePass { int n; const unsigned long long* in[3]; unsigned long long* out[3]; uint32_t flags[3]; };
+
+__global__ void __launch_bounds__(256) k_dense_pass(DensePass p, DenseGeom g) {
+    const unsigned long long n_words = (unsigned long long)g.Wp * g.ny * g.nz;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_words;
+         i += (unsigned long long)gridDim.x * blockDim.x) {
+        const int w = (int)(i % (unsigned long long)g.Wp);
+        const unsigned long long rowi = i / (unsigned long long)g.Wp;
+        const int y = (int)(rowi % (unsigned long long)g.ny), z = (int)(rowi / (unsigned long long)g.ny);
+        const int nvalid = min(64, g.nx - 64 * w);
+        const unsigned long long valid = nvalid >= 64 ? ~0ull : (nvalid <= 0 ? 0ull : ~(~0ull << nvalid));
+        const unsigned long long slice = (unsigned long long)g.Wp * g.ny;
+        for (int c = 0; c < p.n; ++c) {
+            const unsigned long long* in = p.in[c];
+            const uint32_t f = p.flags[c];
+            const unsigned long long me = in[i];
+            unsigned long long o = (f & kDilC) ? me : 0ull;
+            if (f & kDilXm) o |= (me << 1) | (w > 0 ? in[i - 1] >> 63 : 0ull);              // in(u - ex)
+            if (f & kDilXp) o |= (me >> 1) | (w + 1 < g.Wp ? in[i + 1] << 63 : 0ull);       // in(u + ex)
+            if ((f & kDilYm) && y > 0) o |= in[i - g.Wp];
+            if ((f & kDilYp) && y + 1 < g.ny) o |= in[i + g.Wp];
+            if ((f & kDilZm) && z > 0) o |= in[i - slice];
+            if ((f & kDilZp) && z + 1 < g.nz) o |= in[i + slice];
+            p.out[c][i] = o & valid;
+        }
+    }
+}
+
+// pending candidates (status 01) as bit rows; the accepted set starts empty
+__global__ void __launch_bounds__(256) k_dense_init(const uint32_t* __restrict__ status2, DenseGeom g, unsigned long long* P,
+                                                     unsigned long long* ACC) {
+    const unsigned long long n_words = (unsigned long long)g.Wp * g.ny * g.nz;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_words;
+         i += (unsigned long long)gridDim.x * blockDim.x) {
+        const int w = (int)(i % (unsigned long long)g.Wp);
+        const unsigned long long rowi = i / (unsigned long long)g.Wp;
+        const int nvalid = min(64, g.nx - 64 * w);
+        unsigned long long bits = 0ull;
+        for (int b = 0; b < nvalid; ++b) {
+            const unsigned long long v = rowi * (unsigned long long)g.nx + (unsigned long long)(64 * w + b);
+            if (((status2[v >> 4] >> (2u * (uint32_t)(v & 15ull))) & 3u) == 1u) bits |= 1ull << b;
+        }
+        P[i] = bits;
+        ACC[i] = 0ull;
+    }
+}
+
+// NEW = P & ~(LBz | LBy | LBx); ACC |= NEW
+__global__ void __launch_bounds__(256) k_dense_accept(const unsigned long long* P, const unsigned long long* LBz,
+                                                       const unsigned long long* LBy, const unsigned long long* LBx,
+                                                       unsigned long long* NEW, unsigned long long* ACC, unsigned long long n_words) {
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_words;
+         i += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long nw = P[i] & ~(LBz[i] | LBy[i] | LBx[i]);
+        NEW[i] = nw;
+        if (nw) ACC[i] |= nw;
+    }
+}
+
+// P &= ~BL; *left += popc(P)
+__global__ void __launch_bounds__(256) k_dense_prune(unsigned long long* P, const unsigned long long* BL, unsigned long long n_words,
+                                                      uint32_t* left) {
+    uint32_t cnt = 0;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_words;
+         i += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long v = P[i] & ~BL[i];
+        P[i] = v;
+        cnt += (uint32_t)__popcll(v);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((threadIdx.x & 31u) == 0u && cnt) atomicAdd(left, cnt);
+}
+
+// the accepted set back into the status map (11 accepted, 00 rejected), by candidate
+__global__ void __launch_bounds__(256) k_dense_finish(Control* ctl, uint32_t* status2, const uint32_t* cand, DenseGeom g,
+                                                       const unsigned long long* ACC, uint32_t rounds) {
+    const uint32_t n = ctl->n_cand;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { ctl->spacing_slow = 1u; ctl->spacing_rounds = rounds; }
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t v = cand[i];
+        const uint32_t x = v % (uint32_t)g.nx;
+        const unsigned long long rowi = v / (uint32_t)g.nx;
+        const bool acc = (ACC[rowi * (unsigned long long)g.Wp + (x >> 6)] >> (x & 63u)) & 1ull;
+        if (acc) atomicOr(status2 + (v >> 4), 2u << (2 * (v & 15u)));
+        else atomicAnd(status2 + (v >> 4), ~(3u << (2 * (v & 15u))));
+    }
+}
+
 // --- finalize: accepted candidates -> grid + initial front A_0 = seeds (R3) ---------------------
 // accepted = status 11: by rank in the spacing fast path's st_rank, else by voxel in the global status map
 __device__ __forceinline__ bool seed_accepted(const Control* ctl, const uint32_t* status2, const uint32_t* cand,
@@ -609,6 +768,95 @@ cudaError_t launch_spacing(liets_ctx* c, int s) {
     e = cudaLaunchCooperativeKernel((const void*)k_spacing_resolve, dim3(c->resolve_grid), dim3(1024), args, 0, c->stream);
     c->launches++;
     return e;
+}
+
+// R19: the keyed order, all rounds in one cooperative launch
+cudaError_t launch_spacing_keyed(liets_ctx* c, int s) {
+    Dims g{ c->nx, c->ny, c->nz, c->periodic };
+    unsigned long long N = c->N;
+    PhiloxKey key = philox_make_key(c->rng_seed);
+    if (c->resolve_keyed_grid == 0) {
+        int per_sm = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spacing_resolve_keyed, 1024, 0);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+        c->resolve_keyed_grid = c->sm_count;
+    }
+    void* args[] = { &c->ctl, &c->status2, &c->cand, &g, &s, &N, &key };
+    cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_spacing_resolve_keyed, dim3(c->resolve_keyed_grid), dim3(1024), args, 0, c->stream);
+    c->launches++;
+    return e;
+}
+
+// NEXT-1: the dense diamond dilation (walls only, ascending index order).  n_cand: the candidate count (read back by the
+// caller); the bit rows live behind the candidate list.  Synchronises once per round (the pending count).
+size_t spacing_dense_bytes(const liets_ctx* c) {
+    return (size_t)((c->nx + 63) / 64) * 8u * (size_t)c->ny * (size_t)c->nz;
+}
+
+cudaError_t launch_spacing_dense(liets_ctx* c, int s, uint32_t n_cand, uint32_t* rounds_out) {
+    DenseGeom g{ c->nx, c->ny, c->nz, (c->nx + 63) / 64 };
+    const unsigned long long n_words = (unsigned long long)g.Wp * g.ny * g.nz;
+    const size_t plane = (size_t)n_words * 8u;
+    uint8_t* base = reinterpret_cast<uint8_t*>(c->cand) + (((size_t)n_cand * 4u + 255u) & ~(size_t)255u);
+    unsigned long long* B[8];
+    for (int k = 0; k < 8; ++k) B[k] = reinterpret_cast<unsigned long long*>(base + (size_t)k * plane);
+    unsigned long long *P = B[0], *ACC = B[1];
+    const int r = s - 1;
+    const int grid = c->sm_count * 8;
+    uint32_t* left = &c->ctl->pend3[0];
+    k_dense_init<<<grid, 256, 0, c->stream>>>(c->status2, g, P, ACC);
+    c->launches++;
+    uint32_t rounds = 0;
+    for (;;) {
+        // the three chains of the later half of the diamond, one sweep per pass: ping-pong between B[2..4] and B[5..7]
+        DensePass p;
+        p.n = 3;
+        p.flags[0] = kDilZm; p.flags[1] = kDilYm; p.flags[2] = kDilXm;                       // the first step of each chain
+        for (int k = 0; k < 3; ++k) { p.in[k] = P; p.out[k] = B[2 + k]; }
+        k_dense_pass<<<grid, 256, 0, c->stream>>>(p, g);
+        c->launches++;
+        int cur = 0;                                        // chains now in B[2 + 3 cur ..]
+        p.flags[0] = kDilC | kDilXm | kDilXp | kDilYm | kDilYp | kDilZm;
+        p.flags[1] = kDilC | kDilXm | kDilXp | kDilYm;
+        p.flags[2] = kDilC | kDilXm;
+        for (int pass = 1; pass < r; ++pass) {
+            for (int k = 0; k < 3; ++k) { p.in[k] = B[2 + 3 * cur + k]; p.out[k] = B[2 + 3 * (cur ^ 1) + k]; }
+            k_dense_pass<<<grid, 256, 0, c->stream>>>(p, g);
+            c->launches++;
+            cur ^= 1;
+        }
+        unsigned long long* NEW = B[2 + 3 * (cur ^ 1)];
+        k_dense_accept<<<grid, 256, 0, c->stream>>>(P, B[2 + 3 * cur], B[2 + 3 * cur + 1], B[2 + 3 * cur + 2], NEW, ACC, n_words);
+        c->launches++;
+        // the accepted cells cover their diamonds: s-1 passes of the full kernel
+        DensePass q;
+        q.n = 1;
+        q.flags[0] = kDilC | kDilXm | kDilXp | kDilYm | kDilYp | kDilZm | kDilZp;
+        unsigned long long* a = NEW;
+        unsigned long long* b = B[2 + 3 * cur];
+        for (int pass = 0; pass < r; ++pass) {
+            q.in[0] = a; q.out[0] = b;
+            k_dense_pass<<<grid, 256, 0, c->stream>>>(q, g);
+            c->launches++;
+            unsigned long long* t = a; a = b; b = t;
+        }
+        cudaError_t e = cudaMemsetAsync(left, 0, sizeof(uint32_t), c->stream);
+        if (e != cudaSuccess) return e;
+        k_dense_prune<<<grid, 256, 0, c->stream>>>(P, a, n_words, left);
+        c->launches++;
+        ++rounds;
+        uint32_t h_left = 0;
+        e = cudaMemcpyAsync(&h_left, left, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream);
+        if (e != cudaSuccess) return e;
+        e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) return e;
+        if (h_left == 0) break;
+    }
+    k_dense_finish<<<grid, 256, 0, c->stream>>>(c->ctl, c->status2, c->cand, g, ACC, rounds);
+    c->launches++;
+    if (rounds_out) *rounds_out = rounds;
+    return cudaGetLastError();
 }
 
 // per-device function attributes, set once per context at liets_create (they are per device, not per process)

@@ -14,11 +14,13 @@ STORAGE_U8, STORAGE_TILE, STORAGE_FULL = 0, 1, 2
 LAW_CONSTANT, LAW_EQ1 = 0, 1
 FORMAT_U8, FORMAT_BITS = 0, 1
 S2_STATIC_MAX_LAGS = 4096
+ORDER_INDEX, ORDER_KEYED = 0, 1
+SPACING_SPARSE, SPACING_DENSE = 0, 1
 
 # every symbol include/liets.h declares
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
            "liets_set_target", "liets_set_blocked", "liets_step", "liets_generate", "liets_grid", "liets_s2", "liets_s2_static", "liets_step_log", "liets_timings",
-           "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info",
+           "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info", "liets_set_spacing", "liets_spacing_rounds",
            "liets_create_batch", "liets_batch_ctx", "liets_generate_batch", "liets_destroy_batch",
            "liets_batch_last_error", "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_debug_thresholds", "liets_probe", "liets_destroy", "liets_last_error")
 PROBE_PHILOX, PROBE_LOP3, PROBE_IMAD, PROBE_MIX, PROBE_L2_READ, PROBE_HBM_READ = range(6)
@@ -71,6 +73,10 @@ def lib():
     L.liets_grid.restype = ci
     L.liets_s2.argtypes = [vp, ci, ci, P(u64), P(u64)]
     L.liets_s2.restype = ci
+    L.liets_set_spacing.argtypes = [vp, ci, ci]
+    L.liets_set_spacing.restype = ci
+    L.liets_spacing_rounds.argtypes = [vp, P(u32)]
+    L.liets_spacing_rounds.restype = ci
     L.liets_s2_static.argtypes = [vp, ci, ci, P(u64), P(u64)]
     L.liets_s2_static.restype = ci
     L.liets_step_log.argtypes = [vp, P(u64), P(u64), P(u64), P(u64), u32]
@@ -199,6 +205,15 @@ class Liets:
         n = ctypes.c_uint64(0)
         self._check(self._L.liets_seed(self._h, core_prob, spacing_s, rng_seed, ctypes.byref(n)))
         return int(n.value)
+
+    def set_spacing(self, order=ORDER_INDEX, method=SPACING_SPARSE):
+        """Variant of the spacing filter used by the next seed(): acceptance order and sparse / dense mechanism."""
+        self._check(self._L.liets_set_spacing(self._h, order, method))
+
+    def spacing_rounds(self):
+        r = ctypes.c_uint32(0)
+        self._check(self._L.liets_spacing_rounds(self._h, ctypes.byref(r)))
+        return int(r.value)
 
     def seed_explicit(self, idx, rng_seed=0):
         a = np.ascontiguousarray(idx, dtype=np.uint64)
