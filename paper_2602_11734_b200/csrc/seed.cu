@@ -251,12 +251,28 @@ __global__ void __launch_bounds__(256) k_seed_rows(const Control* ctl, const uin
         rowoff[rho] = rho < n_rows ? rank_of(status2, coff, (uint32_t)(rho * g.nx)) : ctl->n_cand;
 }
 
+// key of voxel v in the keyed acceptance order (R19): word v % 4 of Philox at counter (v / 4, 0, 1, 2^32 - 1)
+__device__ __forceinline__ uint32_t seed_priority(uint32_t v, const PhiloxKey& key) {
+    const uint4 r = philox4x32_10(v >> 2, 0u, 1u, 0xFFFFFFFFu, key);
+    const uint32_t w = v & 3u;
+    return w == 0u ? r.x : w == 1u ? r.y : w == 2u ? r.z : r.w;
+}
+
+// w is tried before v in the keyed order
+__device__ __forceinline__ bool keyed_before(uint32_t kw, uint32_t w, uint32_t kv, uint32_t v) {
+    return kw < kv || (kw == kv && w < v);
+}
+
 // Pass 1: one warp per candidate (rank i, ascending index order) lists the RANKS of the lower-index candidates
 // within L1 < s, once: one lane per z-slice of the diamond, which walks the candidates of the slice's rows
 // (consecutive ranks) and keeps those in range.  Sets ctl->spacing_slow if a list does not fit or a neighbour is
 // too far back in rank for the ring of k_spacing_resolve_cta.
+// KEYED (R19): the candidates that come BEFORE i in the keyed order, anywhere in the diamond (no rank window: the
+// lists go to k_spacing_resolve_lists).
+template <bool KEYED>
 __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const uint32_t* __restrict__ rowoff, uint32_t* cand,
-                                                            Dims g, int s, unsigned long long N, uint32_t ring, uint32_t head) {
+                                                            Dims g, int s, unsigned long long N, uint32_t ring, uint32_t head,
+                                                            PhiloxKey key) {
     __shared__ uint32_t s_buf[8][kAdjBuf];
     __shared__ uint32_t s_cnt[8];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -269,9 +285,10 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
     // slices to visit: dz = -r..0 between walls (lower index = lower z, or same z and lower row), all slices within r
     // on the torus (each once)
     const int px = g.periodic & 1, py = g.periodic & 2, pz = g.periodic & 4;
-    const int n_slices = pz ? min(2 * r + 1, g.nz) : r + 1;
+    const int n_slices = pz ? min(2 * r + 1, g.nz) : (KEYED ? 2 * r + 1 : r + 1);
     for (uint32_t i = warp_global; i < n; i += n_warps) {
         const uint32_t v = cand[i];
+        const uint32_t kv = KEYED ? seed_priority(v, key) : 0u;
         const int x = (int)(v % (uint32_t)g.nx);
         const uint32_t rest = v / (uint32_t)g.nx;
         const int y = (int)(rest % (uint32_t)g.ny), z = (int)(rest / (uint32_t)g.ny);
@@ -284,8 +301,8 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
                 Z %= g.nz; if (Z < 0) Z += g.nz;
                 dz = abs(Z - z); dz = min(dz, g.nz - dz);
             } else {
-                if (Z < 0) continue;
-                dz = z - Z;
+                if (Z < 0 || Z >= g.nz) continue;
+                dz = abs(z - Z);
             }
             const int rho = r - dz;                         // rows y - rho .. y + rho of slice Z can hold neighbours
             if (rho < 0) continue;
@@ -293,7 +310,7 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
             int run_lo[2], run_hi[2], n_runs = 1;           // row runs [lo, hi] inside the slice
             if (!py) {
                 run_lo[0] = max(ya, 0); run_hi[0] = min(yb, g.ny - 1);
-                if (Z == z && !g.periodic) run_hi[0] = min(run_hi[0], y);   // same slice, no wrap anywhere: only rows up to the candidate's own
+                if (!KEYED && Z == z && !g.periodic) run_hi[0] = min(run_hi[0], y);   // same slice, no wrap anywhere: only rows up to the candidate's own
             } else if (2 * rho + 1 >= g.ny) {
                 run_lo[0] = 0; run_hi[0] = g.ny - 1;
             } else {
@@ -303,7 +320,8 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
             }
             for (int q = 0; q < n_runs; ++q) {
                 const uint32_t row0 = (uint32_t)Z * (uint32_t)g.ny;
-                const uint32_t r0 = rowoff[row0 + run_lo[q]], r1 = min(rowoff[row0 + run_hi[q] + 1], i);   // ranks below i only
+                const uint32_t r0 = rowoff[row0 + run_lo[q]];
+                const uint32_t r1 = KEYED ? rowoff[row0 + run_hi[q] + 1] : min(rowoff[row0 + run_hi[q] + 1], i);   // (index order: ranks below i only)
                 for (uint32_t k = r0; k < r1; ++k) {
                     const uint32_t w = cand[k];
                     const int wx = (int)(w % (uint32_t)g.nx);
@@ -312,6 +330,7 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
                     if (px) dx = min(dx, g.nx - dx);
                     if (py) dy = min(dy, g.ny - dy);
                     if (dx + dy + dz <= r) {
+                        if (KEYED && (k == i || !keyed_before(seed_priority(w, key), w, kv, v))) continue;
                         const uint32_t slot = atomicAdd(&s_cnt[warp], 1u);
                         if (slot < (uint32_t)kAdjBuf) s_buf[warp][slot] = k;
                     }
@@ -335,7 +354,7 @@ __global__ void __launch_bounds__(256) k_spacing_adjacency(Control* ctl, const u
                 if (e < 8u) a.first8[(unsigned long long)e * n + i] = rk;
                 // the resolve re-arms the ring slots of a whole pass (1024 ranks) at once: rk's slot must survive until
                 // the END of i's pass, not just until i
-                far = far || ((i | 1023u) - rk >= ring && rk >= head);
+                if (!KEYED) far = far || ((i | 1023u) - rk >= ring && rk >= head);
             }
             if (far) ctl->spacing_slow = 1u;
             if (lane == 0) { a.off[i] = (uint32_t)base; a.cnt[i] = k; }
@@ -464,19 +483,51 @@ __global__ void __launch_bounds__(1024) k_spacing_resolve(Control* ctl, uint32_t
 // random order fixed by the seed.  The order has no spatial structure, so there are no rank windows to exploit: every
 // pending candidate rescans its WHOLE diamond in the global status map each round and evaluates the key of every
 // candidate it meets; the dependency chains are short (a handful of rounds instead of a sweep through the grid).
-__device__ __forceinline__ uint32_t seed_priority(uint32_t v, const PhiloxKey& key) {
-    const uint4 r = philox4x32_10(v >> 2, 0u, 1u, 0xFFFFFFFFu, key);
-    const uint32_t w = v & 3u;
-    return w == 0u ? r.x : w == 1u ? r.y : w == 2u ? r.z : r.w;
+// Keyed order, fast path: the lists of k_spacing_adjacency<true> hold, for every candidate, the candidates tried before it
+// within its diamond.  Rounds over all candidates with the statuses by rank in global memory (1 pending, 3 accepted,
+// 0 rejected; the layout seed_accepted reads): the chains are a handful of links long, so a link may cost an L2 round trip.
+__global__ void __launch_bounds__(1024) k_spacing_resolve_lists(Control* ctl, uint32_t* cand, unsigned long long N) {
+    cg::grid_group grid = cg::this_grid();
+    if (ctl->spacing_slow) return;
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, n_threads = gridDim.x * blockDim.x;
+    const uint32_t n = ctl->n_cand;
+    const AdjView a = adj_view(cand, n, N);
+    uint8_t* const st = reinterpret_cast<uint8_t*>(a.st_rank);
+    for (uint32_t i = tid; i < n; i += n_threads) st[i] = 1u;
+    grid.sync();
+    for (uint32_t round = 0;; ++round) {
+        uint32_t still = 0;
+        for (uint32_t i = tid; i < n; i += n_threads) {
+            if (__ldcg(st + i) != 1u) continue;
+            const uint32_t k = a.cnt[i], off = a.off[i];
+            bool accepted = false, pending = false;
+            for (uint32_t e = 0; e < k; ++e) {
+                const uint32_t sv = __ldcg(st + a.pool[off + e]);
+                accepted = accepted || sv == 3u;
+                pending = pending || sv == 1u;
+            }
+            if (accepted) st[i] = 0u;
+            else if (!pending) st[i] = 3u;
+            else still++;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) still += __shfl_xor_sync(0xffffffffu, still, o);
+        if (lane == 0 && still) atomicAdd(&ctl->pend3[round % 3u], still);
+        grid.sync();
+        const uint32_t left = ld_cg(&ctl->pend3[round % 3u]);
+        if (tid == 0) { ctl->pend3[(round + 2u) % 3u] = 0; ctl->spacing_rounds = round + 1u; }
+        if (left == 0) break;
+    }
 }
 
 __global__ void __launch_bounds__(1024) k_spacing_resolve_keyed(Control* ctl, uint32_t* status2, uint32_t* cand,
                                                                  Dims g, int s, unsigned long long N, PhiloxKey key) {
     cg::grid_group grid = cg::this_grid();
+    if (!ctl->spacing_slow) return;                         // the lists fitted: k_spacing_resolve_lists has done it
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, n_threads = gridDim.x * blockDim.x;
     const uint32_t n = ctl->n_cand;
-    if (tid == 0) ctl->spacing_slow = 1u;                   // the result is read from the status map, by voxel
     for (uint32_t round = 0;; ++round) {
         uint32_t still = 0;
         for (uint32_t i = tid >> 5; i < n; i += n_threads >> 5) {      // one warp per candidate
@@ -748,7 +799,7 @@ cudaError_t launch_spacing(liets_ctx* c, int s) {
     k_seed_rows<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->coff, c->rowoff, g);
     c->launches++;
     const uint32_t ring = c->spacing_ring ? c->spacing_ring : kRing, head = c->spacing_ring ? c->spacing_head : kHead;
-    k_spacing_adjacency<<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->rowoff, c->cand, g, s, N, ring, head);
+    k_spacing_adjacency<false><<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->rowoff, c->cand, g, s, N, ring, head, PhiloxKey{});
     c->launches++;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -776,14 +827,27 @@ cudaError_t launch_spacing_keyed(liets_ctx* c, int s) {
     unsigned long long N = c->N;
     PhiloxKey key = philox_make_key(c->rng_seed);
     if (c->resolve_keyed_grid == 0) {
-        int per_sm = 0;
+        int per_sm = 0, per_sm_lists = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spacing_resolve_keyed, 1024, 0);
         if (e != cudaSuccess) return e;
-        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_lists, k_spacing_resolve_lists, 1024, 0);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1 || per_sm_lists < 1) return cudaErrorLaunchOutOfResources;
         c->resolve_keyed_grid = c->sm_count;
     }
+    // the candidates tried before each candidate, listed once; rounds over the lists; the rescan rounds only if they did not fit
+    k_seed_rows<<<c->sm_count * 4, 256, 0, c->stream>>>(c->ctl, c->status2, c->coff, c->rowoff, g);
+    c->launches++;
+    k_spacing_adjacency<true><<<c->sm_count * 8, 256, 0, c->stream>>>(c->ctl, c->rowoff, c->cand, g, s, N, 0u, 0u, key);
+    c->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    void* largs[] = { &c->ctl, &c->cand, &N };
+    e = cudaLaunchCooperativeKernel((const void*)k_spacing_resolve_lists, dim3(c->resolve_keyed_grid), dim3(1024), largs, 0, c->stream);
+    c->launches++;
+    if (e != cudaSuccess) return e;
     void* args[] = { &c->ctl, &c->status2, &c->cand, &g, &s, &N, &key };
-    cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_spacing_resolve_keyed, dim3(c->resolve_keyed_grid), dim3(1024), args, 0, c->stream);
+    e = cudaLaunchCooperativeKernel((const void*)k_spacing_resolve_keyed, dim3(c->resolve_keyed_grid), dim3(1024), args, 0, c->stream);
     c->launches++;
     return e;
 }
