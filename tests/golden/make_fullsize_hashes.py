@@ -6,6 +6,7 @@ phase array (N bytes, x fastest).  The GPU tests compare the CUDA path's outputs
 
     python tests/golden/make_fullsize_hashes.py cfg3_400 --target 0.80 [--seed 7] [--s 20]
     python tests/golden/make_fullsize_hashes.py cfg5_1024 --seeds-only          # seeding + spacing only
+    python tests/golden/make_fullsize_hashes.py cfg3_400 --seeds-only --order keyed   # ... in the keyed acceptance order (R19)
     python tests/golden/make_fullsize_hashes.py cfg5_1024 --target 0.80 --trace --hash-every 4
 
 Each run appends one JSON line to fullsize_hashes.jsonl; runs take minutes to hours of one CPU core
@@ -51,6 +52,7 @@ def main():
     ap.add_argument("--seed", type=int, default=None)
     ap.add_argument("--s", type=int, default=None)
     ap.add_argument("--omp", action="store_true")
+    ap.add_argument("--order", default="index", choices=["index", "keyed"], help="acceptance order of the spacing filter (R12 / R19)")
     a = ap.parse_args()
     c = CONFIGS[a.config]
     seed = a.seed if a.seed is not None else c["seeds"][0]
@@ -59,10 +61,16 @@ def main():
     t0 = time.time()
     o = oracle.Oracle(nx, ny, nz, c["periodic"], omp=a.omp)
     o.set_growth(*c["g"], 1)
+    if a.order == "keyed":
+        o.set_spacing_order(1)
     n_seeds = o.seed(c["core"], s, seed)
     t_seed = time.time() - t0
     base = dict(config=a.config, dims=[nx, ny, nz], periodic=c["periodic"], core=c["core"], s=s, rng_seed=seed,
                 g=list(c["g"]))
+    if a.order == "keyed":
+        base["order"] = "keyed"
+        if not a.seeds_only:
+            ap.error("--order keyed is recorded for --seeds-only runs")
     if a.seeds_only:
         h = hashlib.sha256(o.grid().tobytes()).hexdigest()
         rec = dict(base, kind="seeds", n_seeds=n_seeds, sha256=h, oracle_seconds=round(time.time() - t0, 1))

@@ -32,7 +32,7 @@ def records(kind=None):
 
 
 def ident(r):
-    return "%s-s%d-seed%d" % (r["config"], r["s"], r["rng_seed"]) + ("-phi%.2f" % r["target"] if "target" in r else "")
+    return "%s-s%d-seed%d" % (r["config"], r["s"], r["rng_seed"]) + ("-phi%.2f" % r["target"] if "target" in r else "") + ("-keyed" if r.get("order") == "keyed" else "")
 
 
 def traces():
@@ -59,11 +59,17 @@ def test_fullsize_seeds_match_oracle_hash(liets, rec):
     2^17-rank status ring of the spacing resolve): seed count and SHA-256 of the grid right after liets_seed."""
     nx, ny, nz = rec["dims"]
     L = liets.Liets(nx, ny, nz, int(rec["periodic"]), 1)
+    keyed = rec.get("order") == "keyed"                      # R19: the keyed acceptance order (another set of seeds)
+    L.set_spacing(liets.ORDER_KEYED if keyed else liets.ORDER_INDEX, liets.SPACING_SPARSE)
     assert L.seed(rec["core"], rec["s"], rec["rng_seed"]) == rec["n_seeds"]
     n_cand, slow = L.seed_info()
     g = L.grid()
     assert int(g.sum(dtype=np.uint64)) == rec["n_seeds"]
     assert hashlib.sha256(g.tobytes()).hexdigest() == rec["sha256"], "candidates %d, slow path %d" % (n_cand, slow)
+    if not keyed and not rec["periodic"]:                    # the dense diamond dilation gives the same seeds (walls only)
+        L.set_spacing(liets.ORDER_INDEX, liets.SPACING_DENSE)
+        assert L.seed(rec["core"], rec["s"], rec["rng_seed"]) == rec["n_seeds"]
+        assert hashlib.sha256(L.grid().tobytes()).hexdigest() == rec["sha256"], "dense dilation, %d rounds" % L.spacing_rounds()
     L.close()
 
 
