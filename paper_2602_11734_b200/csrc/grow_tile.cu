@@ -350,6 +350,34 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
             claim(last ? le : (le & ~eq), x, rr);
             return last ? 0u : eq;
         };
+        // The same for the rounds AFTER the tile's last voxel, when the ring no longer fills: two nibble levels at once.  The
+        // blocks k and k + 1 of the entry are evaluated side by side (one latency for both chains), so a direction that ties
+        // again is settled in the same round; only a tie at both levels goes back into the ring.  The chain of dependent
+        // partial rounds at the end of every tile (it sits on the tile's critical path) shrinks from one round per level to
+        // one per two levels.  Only the blocks the draws need are counted.
+        auto resolve2 = [&](uint32_t vk, uint32_t tie) -> uint32_t {
+            const uint32_t x = (vk & 0x7Fu) ^ 15u, rr = (vk >> 7) & 0x1FFu, k = vk >> 16, k1 = min(k + 1u, 7u);
+            const uint32_t p = lds_u32(ptab_addr + 4u * rr) + x;
+            const uint4 B = philox_growth_block(p, k, ps, key);
+            const uint4 B1 = philox_growth_block(p, k1, ps, key);
+            ++n_items;
+            const uint4 hk = lds_u128(hpat_addr + 16u * k);
+            const uint32_t h[4] = { hk.x, hk.y, hk.z, hk.w };
+            uint32_t le, eq, still = 0;
+            level_compare(B, h, tie, &le, &eq);
+            uint32_t fire = k == 7u ? le : (le & ~eq);                          // last nibble: draw <= U
+            if (k < 7u && eq) {
+                ++n_items;
+                const uint4 hk1 = lds_u128(hpat_addr + 16u * k1);
+                const uint32_t h1[4] = { hk1.x, hk1.y, hk1.z, hk1.w };
+                uint32_t le1, eq1;
+                level_compare(B1, h1, eq, &le1, &eq1);
+                if (k1 == 7u) fire |= le1;
+                else { fire |= le1 & ~eq1; still = eq1; }
+            }
+            claim(fire, x, rr);
+            return still;
+        };
         uint32_t qh = 0, qn = 0;            // ring head and fill (warp-uniform)
         auto round = [&](uint32_t n_take) {
             constexpr uint32_t kMask = (uint32_t)kQueueCap - 1u;
@@ -361,6 +389,19 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
             qh = (qh + n_take) & kMask;
             qn -= n_take;
             if (still) sts_u64(queue_addr + 8u * ((qh + qn + __popc(have & ((1u << lane) - 1u))) & kMask), vk + (1u << 16), still);
+            qn += __popc(have);
+            __syncwarp();
+        };
+        auto round2 = [&](uint32_t n_take) {
+            constexpr uint32_t kMask = (uint32_t)kQueueCap - 1u;
+            uint32_t vk = 0, tie = 0, still = 0;
+            if (lane < n_take) lds_u64(queue_addr + 8u * ((qh + lane) & kMask), vk, tie);
+            __syncwarp();
+            if (tie) still = resolve2(vk, tie);
+            const uint32_t have = __ballot_sync(0xffffffffu, still != 0u);
+            qh = (qh + n_take) & kMask;
+            qn -= n_take;
+            if (still) sts_u64(queue_addr + 8u * ((qh + qn + __popc(have & ((1u << lane) - 1u))) & kMask), vk + (2u << 16), still);
             qn += __popc(have);
             __syncwarp();
         };
@@ -485,6 +526,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                 }
             };
 #endif
+#ifdef LIETS_OLD_C
             auto settle = [&](uint32_t v, uint32_t tie, uint32_t fire) {       // level-0 hits to the claim volume, ties to the ring
                 if (h0_any && __ballot_sync(0xffffffffu, fire != 0u)) claim(fire, (v & 0x7Fu) ^ 15u, (v >> 7) & 0x1FFu);
                 const uint32_t have = __ballot_sync(0xffffffffu, tie != 0u);
@@ -494,6 +536,25 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                     qn += __popc(have);
                 }
             };
+#else
+            // level-0 hits to the claim volume, ties to the ring: both entries of the pair behind one capacity test
+            auto settle2 = [&](const uint32_t* v, const uint32_t* tie, const uint32_t* fire) {
+                if (h0_any) {
+#pragma unroll
+                    for (int u = 0; u < 2; ++u)
+                        if (__ballot_sync(0xffffffffu, fire[u] != 0u)) claim(fire[u], (v[u] & 0x7Fu) ^ 15u, (v[u] >> 7) & 0x1FFu);
+                }
+                const uint32_t have0 = __ballot_sync(0xffffffffu, tie[0] != 0u), have1 = __ballot_sync(0xffffffffu, tie[1] != 0u);
+                if (have0 | have1) {
+                    constexpr uint32_t kMask = (uint32_t)kQueueCap - 1u;
+                    if (qn + 64u > (uint32_t)kQueueCap) do round(32u); while (qn >= 32u);
+                    const uint32_t n0 = __popc(have0);
+                    if (tie[0]) sts_u64(queue_addr + 8u * ((qh + qn + __popc(have0 & lanes_below)) & kMask), v[0] | (1u << 16), tie[0]);
+                    if (tie[1]) sts_u64(queue_addr + 8u * ((qh + qn + n0 + __popc(have1 & lanes_below)) & kMask), v[1] | (1u << 16), tie[1]);
+                    qn += n0 + __popc(have1);
+                }
+            };
+#endif
 #ifdef LIETS_OLD_C
             for (uint32_t i0 = 0; i0 < n_pass; i0 += kVoxPerThread * kThreads) {
                 uint32_t v[kVoxPerThread], tie[kVoxPerThread], fire[kVoxPerThread];
@@ -507,12 +568,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
             for (uint32_t i0 = 0; i0 < n_pass; i0 += 2u * kThreads) {
                 uint32_t v[2] = { 0u, 0u }, tie[2] = { 0u, 0u }, fire[2] = { 0u, 0u };
                 if (i0 + 64u * warp < n_pass) level0_pair(i0 + 2u * tid, v, tie, fire);     // warp-uniform
-#pragma unroll
-                for (int u = 0; u < 2; ++u) settle(v[u], tie[u], fire[u]);
+                settle2(v, tie, fire);
             }
         }
 #endif
-        while (qn) round(min(qn, 32u));
+        while (qn >= 32u) round(32u);
+        while (qn) round2(qn);              // fewer than 32 entries left
         if (tid == 0) { S.tile[(kt + 1u) & 1u] = next_li; S.tile_id[(kt + 1u) & 1u] = next_id; }   // read after the next barrier but one
         __syncthreads();                    // all claims are in shared memory
 
