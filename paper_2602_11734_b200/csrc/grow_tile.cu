@@ -225,6 +225,16 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
     constexpr uint32_t kM8 = 0x88888888u;
     const uint32_t h0m[4] = { h0[0] & kM8, h0[1] & kM8, h0[2] & kM8, h0[3] & kM8 };     // level-0 compare: uniform parts
     const uint32_t h08[4] = { h0[0] | kM8, h0[1] | kM8, h0[2] | kM8, h0[3] | kM8 };
+    // every leading nibble below 8 (no class at probability >= 1/2): the three-instruction compares of level0_compare_small
+    const bool h0_small = ((h0[0] | h0[1] | h0[2] | h0[3]) & kM8) == 0u;
+    uint32_t h0cle[4], h0clt[4], h0nz[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t nz = (((h0[w] & 0x77777777u) + 0x77777777u) | h0[w]) & kM8;      // 0x8 where the nibble is not zero
+        h0nz[w] = nz;
+        h0cle[w] = 0x77777777u - (h0[w] & 0x77777777u);
+        h0clt[w] = 0x77777777u - ((h0[w] - (nz >> 3)) & 0x77777777u);
+    }
     uint32_t new_solid = 0;                 // per thread: bits this thread flipped 0 -> 1
     uint32_t n_items = 0, n_items0 = 0;     // per thread: Philox blocks evaluated, front voxels with a void target
     // shared-window address of the voxel list, kept in a register: left to itself the compiler rebuilds it (S2R
@@ -514,11 +524,16 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                     n_items0 += void26[u] ? 1u : 0u;
                 }
                 if (h0_any) {               // some leading threshold nibble is non-zero: a draw can fire at level 0
+                    if (h0_small) {
 #pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        uint32_t le;
-                        level0_compare(B0[u], h0, h0m, h08, void26[u], &le, &tie[u]);
-                        fire[u] = le & ~tie[u];
+                        for (int u = 0; u < 2; ++u) level0_compare_small(B0[u], h0cle, h0clt, h0nz, void26[u], &fire[u], &tie[u]);
+                    } else {
+#pragma unroll
+                        for (int u = 0; u < 2; ++u) {
+                            uint32_t le;
+                            level0_compare(B0[u], h0, h0m, h08, void26[u], &le, &tie[u]);
+                            fire[u] = le & ~tie[u];
+                        }
                     }
                 } else {                    // all leading nibbles are 0: "<=" and "==" coincide with "== 0"
 #pragma unroll

@@ -248,6 +248,25 @@ __device__ __forceinline__ void level0_compare(const uint4& B, const uint32_t* h
     *eq = interleave_dirs(e[0], e[1], e[2], e[3]) & mask;
 }
 
+// Level 0 when every leading threshold nibble is below 8 (every class has probability < 1/2 in this step): with the top bit
+// of h clear, a <= h  <=>  a's top bit is clear and its low three bits do not exceed h's, i.e. bit 3 of a | ((a & 7) + (7 - h))
+// is clear -- three instructions per word, like the zero test.  a < h is the same test against h - 1 in the nibbles
+// where h != 0.  cle = 0x777.. - h, clt = 0x777.. - (h - 1 where h != 0), hnz = 0x8 in the nibbles where h != 0: uniform.
+__device__ __forceinline__ void level0_compare_small(const uint4& B, const uint32_t* cle, const uint32_t* clt, const uint32_t* hnz,
+                                                     uint32_t mask, uint32_t* lt, uint32_t* eq) {
+    const uint32_t a[4] = { B.x, B.y, B.z, B.w };
+    uint32_t l[4], t[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t al = a[w] & 0x77777777u;
+        l[w] = ~(a[w] | (al + cle[w])) & 0x88888888u;                           // a <= h
+        t[w] = ~(a[w] | (al + clt[w])) & hnz[w];                                // a < h
+    }
+    const uint32_t le = interleave_dirs(l[0], l[1], l[2], l[3]);
+    *lt = interleave_dirs(t[0], t[1], t[2], t[3]) & mask;
+    *eq = le & ~*lt & mask;
+}
+
 // all-zero thresholds nibbles (every class has probability < 1/16): "<=" is "== 0"; flag at bit 3 of zero nibbles
 __device__ __forceinline__ uint32_t nib_is_zero(uint32_t a) {
 #ifdef LIETS_ZERO_MUL
