@@ -562,7 +562,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                 const uint32_t have0 = __ballot_sync(0xffffffffu, tie[0] != 0u), have1 = __ballot_sync(0xffffffffu, tie[1] != 0u);
                 if (have0 | have1) {
                     constexpr uint32_t kMask = (uint32_t)kQueueCap - 1u;
-                    if (qn + 64u > (uint32_t)kQueueCap) do round(32u); while (qn >= 32u);
+                    while (qn >= 32u) round(32u);           // a full round as soon as there is one: little is left at the tile's end
                     const uint32_t n0 = __popc(have0);
                     if (tie[0]) sts_u64(queue_addr + 8u * ((qh + qn + __popc(have0 & lanes_below)) & kMask), v[0] | (1u << 16), tie[0]);
                     if (tie[1]) sts_u64(queue_addr + 8u * ((qh + qn + n0 + __popc(have1 & lanes_below)) & kMask), v[1] | (1u << 16), tie[1]);
