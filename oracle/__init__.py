@@ -75,6 +75,8 @@ def lib(omp=False):
     L.oracle_set_target.restype = ci
     L.oracle_seed.argtypes = [vp, dbl, ci, u64]
     L.oracle_seed.restype = i64
+    L.oracle_set_interaction.argtypes = [vp, dbl, dbl, dbl]
+    L.oracle_set_interaction.restype = ci
     L.oracle_seed_by_dilation.argtypes = [vp, dbl, ci, u64]
     L.oracle_seed_by_dilation.restype = i64
     L.oracle_set_spacing_order.argtypes = [vp, ci]
@@ -208,6 +210,11 @@ class Oracle:
         if n < 0:
             raise ValueError("bad seed parameters")
         return int(n)
+
+    def set_interaction(self, i_face, i_edge, i_corner):
+        """R20: growth of this phase at its interface with the earlier phases (set_blocked), probabilities per class."""
+        if self._L.oracle_set_interaction(self._h, i_face, i_edge, i_corner) != 0:
+            raise ValueError("bad interaction probabilities")
 
     def set_spacing_order(self, order):
         """0 = ascending index (R12), 1 = ascending (seed_priority, index) (R19); used by the next seed()."""

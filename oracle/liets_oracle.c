@@ -135,6 +135,8 @@ struct oracle_state {
     uint64_t n_t;
     uint64_t attempts[26], successes[26];
     int spacing_order;        /* 0: candidates are tried in ascending index (R12); 1: in ascending (key, index) (R19) */
+    int interact;             /* R20: cells of the earlier phases are sources too, with the thresholds RI */
+    uint64_t RI[4];           /* RI[class]: floor(I 2^32 + 0.5), constant over the run */
 };
 
 oracle_state* oracle_new(int nx, int ny, int nz, int periodic) {
@@ -217,6 +219,29 @@ int oracle_set_blocked(oracle_state* o, const uint8_t* mask) {
     return 0;
 }
 
+/* Interacting phases (PAPER.md:40 step 4, R20): the growing phase n also grows at its interface with the earlier phases m --
+ * a still unassigned cell q next to a cell p of an earlier phase (q = p + e_d) is taken by phase n with the
+ * phase-interaction probability I_d^{n,m}, one per direction class, constant over the run.  In the words of the list
+ * algorithm: the cells of the earlier phases that have a void neighbour are sources beside the front of phase n, with
+ * I in place of G; the draw of (p, t, d) is the same keyed draw.  All three 0 switches it off.  Takes effect at the next
+ * seeding. */
+int oracle_set_interaction(oracle_state* o, double i_face, double i_edge, double i_corner) {
+    if (i_face < 0 || i_face > 1 || i_edge < 0 || i_edge > 1 || i_corner < 0 || i_corner > 1) return -1;
+    o->RI[1] = oracle_prob_to_threshold(i_face);
+    o->RI[2] = oracle_prob_to_threshold(i_edge);
+    o->RI[3] = oracle_prob_to_threshold(i_corner);
+    o->interact = (o->RI[1] | o->RI[2] | o->RI[3]) != 0;
+    o->seeded = 0;
+    return 0;
+}
+
+/* R20: after the seeds, the interface cells of the earlier phases join the sources (ascending index) */
+static void push_interface_sources(oracle_state* o) {
+    if (!o->interact || !o->blocked) return;
+    for (uint64_t v = 0; v < o->N; ++v)
+        if (o->grid[v] == 2 && has_void_neighbour(o, v)) front_push(o, v);
+}
+
 static void reset_run(oracle_state* o, uint64_t rng_seed) {
     memset(o->grid, 0, o->N);
     if (o->blocked)
@@ -291,6 +316,7 @@ int64_t oracle_seed(oracle_state* o, double core_prob, int spacing_s, uint64_t r
         free(c);
         qsort(o->front, o->n_front, sizeof(uint64_t), u64_cmp);             /* A_0 listed in ascending index, as always */
         o->n_solid = o->n_front;
+        push_interface_sources(o);
         return (int64_t)o->n_solid;
     }
     for (uint64_t v = 0; v < o->N; ++v) {
@@ -305,6 +331,7 @@ int64_t oracle_seed(oracle_state* o, double core_prob, int spacing_s, uint64_t r
         if (ok) { o->grid[v] = 1; front_push(o, v); }
     }
     o->n_solid = o->n_front;       /* A_0 = seeds (R3) */
+    push_interface_sources(o);
     return (int64_t)o->n_solid;
 }
 
@@ -346,6 +373,7 @@ int64_t oracle_seed_by_dilation(oracle_state* o, double core_prob, int spacing_s
     }
     free(covered); free(wave);
     o->n_solid = o->n_front;
+    push_interface_sources(o);
     return (int64_t)o->n_solid;
 }
 
@@ -356,6 +384,7 @@ int64_t oracle_seed_explicit(oracle_state* o, const uint64_t* idx, uint64_t n, u
         if (o->grid[idx[i]] == 0) { o->grid[idx[i]] = 1; front_push(o, idx[i]); }
     }
     o->n_solid = o->n_front;
+    push_interface_sources(o);
     return (int64_t)o->n_solid;
 }
 
@@ -380,14 +409,15 @@ int oracle_step_full(oracle_state* o) {
     uint8_t* next = (uint8_t*)malloc(o->N);
     memcpy(next, o->grid, o->N);
     for (uint64_t p = 0; p < o->N; ++p) {
-        if (o->grid[p] != 1) continue;
+        if (o->grid[p] != 1 && !(o->interact && o->grid[p] == 2)) continue;     /* sources: phase n, and (R20) the earlier phases */
+        const uint64_t* Tp = o->grid[p] == 1 ? T : o->RI;
         for (int d = 0; d < 26; ++d) {
             uint64_t q;
             if (!neighbour(o, p, d, &q)) continue;
             if (o->grid[q] != 0) continue;
             int cls = abs(ORACLE_DIRS[d][0]) + abs(ORACLE_DIRS[d][1]) + abs(ORACLE_DIRS[d][2]);
             o->attempts[d]++;
-            if ((uint64_t)oracle_growth_draw(o->rng_seed, o->step, p, d) < T[cls]) {
+            if ((uint64_t)oracle_growth_draw(o->rng_seed, o->step, p, d) < Tp[cls]) {
                 o->successes[d]++;
                 next[q] = 1;
             }
@@ -399,7 +429,7 @@ int oracle_step_full(oracle_state* o) {
     o->n_solid = 0; o->n_front = 0;
     for (uint64_t p = 0; p < o->N; ++p) o->n_solid += (o->grid[p] == 1);
     for (uint64_t p = 0; p < o->N; ++p)
-        if (o->grid[p] == 1 && has_void_neighbour(o, p)) front_push(o, p);
+        if ((o->grid[p] == 1 || (o->interact && o->grid[p] == 2)) && has_void_neighbour(o, p)) front_push(o, p);
     o->step++;
     return 0;
 }
@@ -419,7 +449,8 @@ int oracle_step_list(oracle_state* o) {
             uint64_t p = o->front[i], q;
             if (!neighbour(o, p, d, &q)) continue;     /* line 5: N_d inside domain          */
             if (o->grid[q] != 0) continue;             /* line 6: C_d, still void            */
-            if ((uint64_t)oracle_growth_draw(o->rng_seed, o->step, p, d) < T[cls]) { /* line 8 */
+            const uint64_t* Tp = o->grid[p] == 1 ? T : o->RI;                   /* (R20: a source of an earlier phase uses I) */
+            if ((uint64_t)oracle_growth_draw(o->rng_seed, o->step, p, d) < Tp[cls]) { /* line 8 */
                 o->grid[q] = 1;                        /* line 9                             */
                 front_push(o, q);                      /* line 10: A_new U {q}, once per q   */
                 o->n_solid++;
@@ -454,7 +485,8 @@ int oracle_step_list(oracle_state* o) {
                 uint64_t p = o->front[i], q;
                 if (!neighbour(o, p, d, &q)) continue;                                   /* line 5 */
                 if (__atomic_load_n(&o->grid[q], __ATOMIC_RELAXED) != 0) continue;       /* line 6 */
-                if ((uint64_t)oracle_growth_draw(o->rng_seed, o->step, p, d) < T[cls]) { /* line 8 */
+                const uint64_t* Tp = o->grid[p] == 1 ? T : o->RI;
+                if ((uint64_t)oracle_growth_draw(o->rng_seed, o->step, p, d) < Tp[cls]) { /* line 8 */
                     if (__atomic_exchange_n(&o->grid[q], 1, __ATOMIC_RELAXED) == 0) {    /* line 9 */
                         if (nbuf[me] == cbuf[me]) {                                      /* line 10 */
                             cbuf[me] = cbuf[me] ? 2 * cbuf[me] : 1024;

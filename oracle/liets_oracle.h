@@ -85,6 +85,10 @@ int oracle_threads(void);
 /* cells of earlier growing phases (N bytes, non-zero = taken; NULL clears): not void, not of this phase (PAPER.md:40 step 4,
  * independent phases).  oracle_grid then holds 2 in those cells.  Takes effect at the next oracle_seed. */
 int oracle_set_blocked(oracle_state* o, const uint8_t* mask);
+/* R20 (PAPER.md:40 step 4, interacting phases): the cells of the earlier phases that have a void neighbour are sources too,
+ * with the phase-interaction probabilities I (face, edge, corner; constant) in place of G.  0, 0, 0 switches it off.
+ * Takes effect at the next oracle_seed*. */
+int oracle_set_interaction(oracle_state* o, double i_face, double i_edge, double i_corner);
 const uint8_t* oracle_grid(const oracle_state* o);          /* N bytes in {0,1}, x fastest */
 uint64_t oracle_n_solid(const oracle_state* o);
 uint64_t oracle_n_front_exact(const oracle_state* o);       /* #solid cells with a void neighbour */

@@ -691,3 +691,104 @@ def test_p5k_keyed_order_equals_the_greedy_in_key_order(periodic, s):
     o.step(use_list=True)
     a.step(use_list=False)
     assert (o.grid() == a.grid()).all()
+
+
+# ------------------------------------------------------------------------------- R20: interacting phases
+def _dilate26(m, periodic):
+    """3x3x3 dilation of a boolean (nz, ny, nx) array: walls (nothing comes in from outside) or wrap."""
+    out = m.copy()
+    for dz, dy, dx in itertools.product((-1, 0, 1), repeat=3):
+        r = np.roll(m, (dz, dy, dx), axis=(0, 1, 2))
+        if not periodic:
+            for ax, sh in ((0, dz), (1, dy), (2, dx)):
+                if sh:
+                    sl = [slice(None)] * 3
+                    sl[ax] = 0 if sh == 1 else -1
+                    r[tuple(sl)] = False
+        out |= r
+    return out
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+@pytest.mark.parametrize("use_list", [True, False])
+def test_interaction_with_probability_one_coats_the_earlier_phase(periodic, use_list):
+    """PAPER.md:40 step 4, R20: with I = 1 in every direction and G = 0, one step turns exactly the unassigned cells
+    that touch the earlier phase (its 3x3x3 dilation minus itself) into the new phase, and a second step adds nothing:
+    the interface is covered and the new phase itself does not grow."""
+    nx, ny, nz = 19, 14, 11
+    rng = np.random.default_rng(5)
+    m = np.zeros((nz, ny, nx), bool)
+    m[3:6, 4:9, 5:12] = True
+    m[8, 2, 1] = True
+    m[0, 0, 0] = True                                            # a corner cell: the boundary mode shows
+    o = oracle.Oracle(nx, ny, nz, periodic)
+    o.set_growth(0.0, 0.0, 0.0, 0)
+    o.set_blocked(m.astype(np.uint8))
+    o.set_interaction(1.0, 1.0, 1.0)
+    o.seed_explicit([], 3)
+    o.step(use_list=use_list)
+    coat = _dilate26(m, periodic) & ~m
+    g = o.phase_map()
+    assert ((g == 1) == coat).all() and ((g == 2) == m).all()
+    assert o.n_solid == int(coat.sum())
+    o.step(use_list=use_list)
+    assert ((o.grid() == 1) == coat).all()
+    # face probabilities only: the 6-neighbourhood
+    o2 = oracle.Oracle(nx, ny, nz, periodic)
+    o2.set_growth(0.0, 0.0, 0.0, 0)
+    o2.set_blocked(m.astype(np.uint8))
+    o2.set_interaction(1.0, 0.0, 0.0)
+    o2.seed_explicit([], 3)
+    o2.step(use_list=use_list)
+    face = m.copy()
+    for ax in range(3):
+        for sh in (1, -1):
+            r = np.roll(m, sh, axis=ax)
+            if not periodic:
+                sl = [slice(None)] * 3
+                sl[ax] = 0 if sh == 1 else -1
+                r[tuple(sl)] = False
+            face |= r
+    assert ((o2.grid() == 1) == (face & ~m)).all()
+
+
+def test_interaction_zero_is_the_independent_phase_and_list_equals_full():
+    nx, ny, nz = 24, 17, 13
+    a = oracle.Oracle(nx, ny, nz, False)
+    a.set_growth(0.2, 0.1, 0.05, 0)
+    a.seed(0.01, 0, 4)
+    for _ in range(3):
+        a.step()
+    m = (a.grid() == 1).astype(np.uint8)
+    runs = []
+    for inter, use_list in ((None, True), ((0.0, 0.0, 0.0), True), ((0.3, 0.1, 0.02), True), ((0.3, 0.1, 0.02), False)):
+        o = oracle.Oracle(nx, ny, nz, False)
+        o.set_growth(0.1, 0.05, 0.01, 1)
+        o.set_blocked(m)
+        if inter is not None:
+            o.set_interaction(*inter)
+        o.seed(0.005, 3, 8)
+        rc, steps = o.generate(0.3, use_list=use_list)
+        runs.append((o.grid().copy(), o.n_solid, steps))
+    assert (runs[0][0] == runs[1][0]).all() and runs[0][1:] == runs[1][1:]       # I = 0: the independent phase (R18)
+    assert (runs[2][0] == runs[3][0]).all() and runs[2][1:] == runs[3][1:]       # list == full field with interface sources
+    assert (runs[2][0] != runs[0][0]).any()                                      # and the interface does grow
+    assert not (runs[2][0] & m).any()                                            # the earlier phase keeps its cells
+
+
+def test_interaction_rate_at_the_interface():
+    """One step from a flat wall of the earlier phase with I_face = 0.25 and nothing else: every unassigned cell of the
+    next plane has exactly one source (the wall cell below it), so the taken fraction is binomial around 0.25."""
+    nx, ny, nz = 64, 64, 4
+    m = np.zeros((nz, ny, nx), np.uint8)
+    m[0] = 1
+    o = oracle.Oracle(nx, ny, nz, False)
+    o.set_growth(0.0, 0.0, 0.0, 0)
+    o.set_blocked(m)
+    o.set_interaction(0.25, 0.0, 0.0)
+    o.seed_explicit([], 11)
+    o.step()
+    g = o.grid()
+    assert (g[2:] == 0).all()
+    k, n = int((g[1] == 1).sum()), nx * ny
+    assert abs(k - 0.25 * n) < 5 * math.sqrt(n * 0.25 * 0.75)
