@@ -100,9 +100,18 @@ int liets_seed_explicit(liets_ctx* ctx, const uint64_t* idx, uint64_t n, uint64_
  * The target fraction stays a fraction of all N cells.  mask = NULL clears.  Takes effect at the next liets_seed /
  * liets_seed_explicit (E_STATE from step / generate / grid until then).  A front that dies inside an enclosure of taken
  * cells may be found empty one (claim-less) step after the serial algorithm would: status and grid are the same.
- * Phase-interaction probabilities I_i^{n,m} (growth of a phase ON the surface of another) are not provided.
+ * Phase-interaction probabilities I_i^{n,m} (growth of a phase ON the surface of another): liets_set_interaction.
  * Errors: E_ARG (format), E_CAPACITY (mask_bytes), E_CUDA.  Synchronises. */
 int liets_set_blocked(liets_ctx* ctx, const void* mask, size_t mask_bytes, int format, int mask_is_device);
+
+/* Interacting phases (PAPER.md:40 step 4; R20): the phase being grown also grows at its interface with the
+ * phases handed over by liets_set_blocked -- a still unassigned cell q = p + e_d next to a cell p of an earlier phase is
+ * taken with the phase-interaction probability I of d's class (face, edge, corner; constant over the run, the same keyed
+ * draw of (p, t, d) compared with I instead of G).  The cells of the earlier phases that have a void neighbour are sources
+ * beside the phase's own front; they keep their cells.  0, 0, 0 (the default) switches it off: independent phases (R18).
+ * Bit-row storages only (E_ARG for LIETS_STORAGE_U8); batches run without it.  Seed again afterwards (E_STATE until
+ * then); a run with interaction keeps its active set as tiles from the first step. */
+int liets_set_interaction(liets_ctx* ctx, double i_face, double i_edge, double i_corner);
 
 /* Target solid volume fraction phi_s in (0,1]: n_t = ceil(phi_s*N) (R7). Used by Eq. (1) and by
  * the stopping rule. */

@@ -78,6 +78,27 @@ __global__ void k_set_params(Control* c, unsigned long long R0, unsigned long lo
     c->vox_cap = vox_cap; c->vox_thr = vox_thr;
 }
 
+// R20: the interaction thresholds RI (floor(I 2^32 + 0.5) per class, constant), laid out nibble by nibble like hpat
+__global__ void k_set_interaction(Control* c, unsigned long long RI0, unsigned long long RI1, unsigned long long RI2) {
+    const unsigned long long RI[3] = { RI0, RI1, RI2 };
+    uint32_t U[3], en26 = 0;
+    for (int k = 0; k < 3; ++k) {
+        U[k] = RI[k] >= 1ull ? (uint32_t)(RI[k] - 1ull) : 0u;
+        if (RI[k] >= 1ull) en26 |= class_dir_mask(k);
+    }
+    for (uint32_t lv = 0; lv < 8u; ++lv)
+        for (int w = 0; w < 4; ++w) {
+            uint32_t h = 0;
+            for (int k = 0; k < 3; ++k) {
+                const uint32_t ones = w == 0 ? class_nibble_ones(0, k) : w == 1 ? class_nibble_ones(1, k) : w == 2 ? class_nibble_ones(2, k) : class_nibble_ones(3, k);
+                h += ((U[k] >> (28u - 4u * lv)) & 15u) * ones;
+            }
+            c->hpatI[lv][w] = h;
+        }
+    c->enI26 = en26;
+    c->interact = en26 != 0u;
+}
+
 // test aid: eq1_threshold on the device for n (R, n_t, n_solid) triples (liets_debug_thresholds)
 __global__ void k_eq1_thresholds(const unsigned long long* R, const unsigned long long* n_t, const unsigned long long* n_solid,
                                  unsigned long long* T, uint32_t n) {
@@ -98,6 +119,12 @@ cudaError_t launch_control(liets_ctx* c, uint32_t flags) {
 
 cudaError_t launch_begin(liets_ctx* c, int generate, uint32_t max_steps) {
     k_begin<<<1, 1, 0, c->stream>>>(c->ctl, generate, max_steps);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_set_interaction(liets_ctx* c) {
+    k_set_interaction<<<1, 1, 0, c->stream>>>(c->ctl, c->RI[0], c->RI[1], c->RI[2]);
     c->launches++;
     return cudaGetLastError();
 }

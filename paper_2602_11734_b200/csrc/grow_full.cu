@@ -59,12 +59,15 @@ __global__ void __launch_bounds__(kFullThreads) k_grow_full(Control* __restrict_
                                                              unsigned long long* G1, const unsigned long long* __restrict__ P,
                                                              PhiloxKey key) {
     if (!ctl->active) return;
-    __shared__ __align__(16) uint32_t s_hpat[8][4];
+    __shared__ __align__(16) uint32_t s_hpat[2][8][4];      // [1]: the interaction thresholds (R20), used by sources of earlier phases
     const uint32_t t = ctl->step;
     const unsigned long long* __restrict__ Gc = (t & 1u) ? G1 : G0;
     unsigned long long* Gn = (t & 1u) ? G0 : G1;
-    if (threadIdx.x < 32) s_hpat[threadIdx.x >> 2][threadIdx.x & 3] = ctl->hpat[threadIdx.x >> 2][threadIdx.x & 3];
+    if (threadIdx.x < 32) s_hpat[0][threadIdx.x >> 2][threadIdx.x & 3] = ctl->hpat[threadIdx.x >> 2][threadIdx.x & 3];
+    else if (threadIdx.x < 64) s_hpat[1][(threadIdx.x - 32) >> 2][threadIdx.x & 3] = ctl->hpatI[(threadIdx.x - 32) >> 2][threadIdx.x & 3];
     const uint32_t en26 = ctl->en26;
+    const bool interact = P != nullptr && ctl->interact != 0u;
+    const uint32_t enI26 = ctl->enI26;
     const PhiloxStep ps = philox_step_uniform(t, key);
     __syncthreads();
     const uint32_t lane = threadIdx.x & 31u;
@@ -98,7 +101,8 @@ __global__ void __launch_bounds__(kFullThreads) k_grow_full(Control* __restrict_
         uint32_t solid32 = own32 & in_row;
         // carry g_t into g_{t+1} (one atomic per segment that holds solid cells)
         if (lane == 0 && solid32) atomicOr(Gn + own_word_idx, (unsigned long long)solid32 << (x0 & 63));
-        if (P) solid32 &= ~(uint32_t)(__ldg(P + own_word_idx) >> (x0 & 63));   // cells of earlier phases are carried, but are no sources
+        uint32_t other32 = 0;                               // cells of earlier phases: carried; sources only at an interacting interface (R20)
+        if (P) { other32 = (uint32_t)(__ldg(P + own_word_idx) >> (x0 & 63)) & solid32; if (!interact) solid32 &= ~other32; }
         // nothing solid in the centre row's cells, or no void cell anywhere around: no attempt can exist here
         if (solid32 == 0u || all_and == 0x3FFFFFFFFull || all_or == 0ull) continue;
         const int x = x0 + (int)lane;
@@ -108,16 +112,17 @@ __global__ void __launch_bounds__(kFullThreads) k_grow_full(Control* __restrict_
 #pragma unroll
             for (int e = 0; e < 9; ++e) nb27 |= ((uint32_t)(win[e] >> lane) & 7u) << (3 * e);
             const uint32_t v27 = ~nb27;
-            const uint32_t mask = ((v27 & 0x1FFFu) | ((v27 >> 14) << 13)) & 0x3FFFFFFu & en26;     // C_d (Algorithm 2 line 6), the centre skipped
+            const uint32_t kind = (other32 >> lane) & 1u;   // 1: a cell of an earlier phase, it uses I
+            const uint32_t mask = ((v27 & 0x1FFFu) | ((v27 >> 14) << 13)) & 0x3FFFFFFu & (kind ? enI26 : en26);     // C_d (Algorithm 2 line 6), the centre skipped
             if (mask) {
                 const uint32_t p = (uint32_t)x + (uint32_t)g.nx * ((uint32_t)y + (uint32_t)g.ny * (uint32_t)z);
                 ++my_items;
                 ++my_items0;
                 const uint4 B0 = philox_growth_block(p, 0u, ps, key);      // R_d for all directions (line 7), nibble level 0
                 uint32_t le, eq;
-                level_compare(B0, s_hpat[0], mask, &le, &eq);
+                level_compare(B0, s_hpat[kind][0], mask, &le, &eq);
                 fire = le & ~eq;
-                if (eq) fire |= resolve_ties(p, t, eq, s_hpat, key, &my_items);
+                if (eq) fire |= resolve_ties(p, t, eq, s_hpat[kind], key, &my_items);
             }
         }
         while (fire) {                                      // line 8: phase_new[mask] = 1, "counted once" by the atomic's old value (:77)

@@ -65,7 +65,7 @@ struct Smem {
     unsigned long long own[64][kTileW];         // the tile's own not-void words (row y + 8 z)
     uint32_t claims[100][2 * kRowWords];        // cells claimed in this step: row as in win, bit 64 + x of the row (32-bit view)
     uint32_t queue[kWarps][2 * kQueueCap];      // ring of (list entry | nibble level << 16, tied directions)
-    uint32_t hpat[8][4];
+    uint32_t hpat[2][8][4];                     // [1]: the interaction thresholds (R20; only loaded when INTERACT)
     uint32_t dir[28];                           // direction d: claim-word offset 8 (10 dz + dy + 11) | (dx + 1) << 16
     uint32_t ptab[100];                         // voxel index of tile x = 0 of each own row
     uint32_t tile[2], tile_id[2];               // list entry handed to the CTA, double-buffered by tile parity
@@ -175,7 +175,9 @@ struct TileBatch {
     PhiloxKey key[MAXB];
 };
 
-template <int MAXB>
+// INTERACT (R20): cells of the earlier phases (plane P) that have a void neighbour are sources too, with the thresholds
+// Control::hpatI; bit 15 of a list entry says which kind of source the voxel is.
+template <int MAXB, bool INTERACT>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid_constant__ TileBatch<MAXB> B, const TileGeom g) {
     __shared__ __align__(16) Smem S;        // static (< 48 KB): shared-memory addresses are immediates, not generic pointers
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -212,15 +214,16 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
     const PhiloxStep ps = philox_step_uniform(t, key);
     const unsigned long long* __restrict__ Gc = (t & 1u) ? G1 : G0;     // g_t (read only)
     unsigned long long* Gn = (t & 1u) ? G0 : G1;                        // g_{t+1} (OR target)
-    if (tid < 32) S.hpat[tid >> 2][tid & 3] = ctl->hpat[tid >> 2][tid & 3];
+    if (tid < 32) S.hpat[0][tid >> 2][tid & 3] = ctl->hpat[tid >> 2][tid & 3];
+    else if (INTERACT && tid < 64) S.hpat[1][(tid - 32u) >> 2][tid & 3] = ctl->hpatI[(tid - 32u) >> 2][tid & 3];
     if (tid < 28) {
         const int d = tid < 26 ? (int)tid : 25;
         const int raw = d + (d >= 13 ? 1 : 0);
         const int dx = raw % 3 - 1, dy = (raw / 3) % 3 - 1, dz = raw / 9 - 1;
         S.dir[tid] = (uint32_t)(2 * kRowWords * (dz * 10 + dy + 11)) | ((uint32_t)(dx + 1) << 16);
     }
-    const uint32_t en26 = ctl->en26;
-    const bool h0_any = ctl->h0_any != 0u;
+    const uint32_t en26 = ctl->en26, enI26 = INTERACT ? ctl->enI26 : 0u;
+    const bool h0_any = INTERACT || ctl->h0_any != 0u;      // (with two kinds of sources level 0 always takes the general compare)
     const uint32_t h0[4] = { ctl->hpat[0][0], ctl->hpat[0][1], ctl->hpat[0][2], ctl->hpat[0][3] };
     constexpr uint32_t kM8 = 0x88888888u;
     const uint32_t h0m[4] = { h0[0] & kM8, h0[1] & kM8, h0[2] & kM8, h0[3] & kM8 };     // level-0 compare: uniform parts
@@ -301,6 +304,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
         // ---- B: front voxels of the tile ------------------------------------------------------------
         uint32_t n_front = 0, off0 = 0;
         unsigned long long F = 0ull;        // this thread's word (row tid / kTileW, word tid % kTileW): its front voxels
+        unsigned long long Pw = 0ull;       // ... and which of its cells belong to earlier phases
         const int f_row = (int)tid / kTileW, f_j = (int)tid - f_row * kTileW;
         {
             static_assert(64 * kTileW == kThreads, "one tile word per thread");
@@ -309,7 +313,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
             if (y < tc.wcy && z < tc.wcz && xbase < g.nx) {
                 unsigned long long src = S.own[f_row][f_j];
                 if (xbase + 64 > g.nx) src &= ~(~0ull << (g.nx - xbase));               // padding is not a source
-                if (P) src &= ~__ldg(P + (unsigned long long)g.Wp * ((unsigned long long)(tc.y0 + y) + (unsigned long long)g.ny * (unsigned long long)(tc.z0 + z)) + (unsigned long long)(tc.w0 + f_j));   // nor is a cell of an earlier phase
+                if (P) {                                                                // nor is a cell of an earlier phase -- unless it interacts (R20)
+                    Pw = __ldg(P + (unsigned long long)g.Wp * ((unsigned long long)(tc.y0 + y) + (unsigned long long)g.ny * (unsigned long long)(tc.z0 + z)) + (unsigned long long)(tc.w0 + f_j));
+                    if (!INTERACT) src &= ~Pw;
+                }
                 if (src) {                                                              // (sparse early steps: most words hold no solid)
                     unsigned long long anyvoid = 0ull;
 #pragma unroll
@@ -348,11 +355,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
         // fire are claimed, the ones that tie again are returned.  round() takes the 32 oldest entries of the ring, one lane
         // each, and appends the entries that still tie one level deeper; while the tile is being listed only full rounds run.
         auto resolve = [&](uint32_t vk, uint32_t tie) -> uint32_t {
-            const uint32_t x = (vk & 0x7Fu) ^ 15u, rr = (vk >> 7) & 0x1FFu, k = vk >> 16;
+            const uint32_t x = (vk & 0x7Fu) ^ 15u, rr = (vk >> 7) & 0x7Fu, k = vk >> 16;
             const uint32_t p = lds_u32(ptab_addr + 4u * rr) + x;
             const uint4 B = philox_growth_block(p, k, ps, key);
             ++n_items;
-            const uint4 hk = lds_u128(hpat_addr + 16u * k);
+            const uint4 hk = lds_u128(hpat_addr + 16u * k + (INTERACT ? ((vk >> 15) & 1u) * 128u : 0u));
             const uint32_t h[4] = { hk.x, hk.y, hk.z, hk.w };
             uint32_t le, eq;
             level_compare(B, h, tie, &le, &eq);
@@ -366,19 +373,20 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
         // partial rounds at the end of every tile (it sits on the tile's critical path) shrinks from one round per level to
         // one per two levels.  Only the blocks the draws need are counted.
         auto resolve2 = [&](uint32_t vk, uint32_t tie) -> uint32_t {
-            const uint32_t x = (vk & 0x7Fu) ^ 15u, rr = (vk >> 7) & 0x1FFu, k = vk >> 16, k1 = min(k + 1u, 7u);
+            const uint32_t x = (vk & 0x7Fu) ^ 15u, rr = (vk >> 7) & 0x7Fu, k = vk >> 16, k1 = min(k + 1u, 7u);
             const uint32_t p = lds_u32(ptab_addr + 4u * rr) + x;
             const uint4 B = philox_growth_block(p, k, ps, key);
             const uint4 B1 = philox_growth_block(p, k1, ps, key);
             ++n_items;
-            const uint4 hk = lds_u128(hpat_addr + 16u * k);
+            const uint32_t hk_addr = hpat_addr + (INTERACT ? ((vk >> 15) & 1u) * 128u : 0u);
+            const uint4 hk = lds_u128(hk_addr + 16u * k);
             const uint32_t h[4] = { hk.x, hk.y, hk.z, hk.w };
             uint32_t le, eq, still = 0;
             level_compare(B, h, tie, &le, &eq);
             uint32_t fire = k == 7u ? le : (le & ~eq);                          // last nibble: draw <= U
             if (k < 7u && eq) {
                 ++n_items;
-                const uint4 hk1 = lds_u128(hpat_addr + 16u * k1);
+                const uint4 hk1 = lds_u128(hk_addr + 16u * k1);
                 const uint32_t h1[4] = { hk1.x, hk1.y, hk1.z, hk1.w };
                 uint32_t le1, eq1;
                 level_compare(B1, h1, eq, &le1, &eq1);
@@ -429,7 +437,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                         for (uint32_t m = (uint32_t)(F >> (32 * half)); m; addr += 2u) {
                             const uint32_t b = 31u - __clz(m);
                             m ^= 1u << b;
-                            asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((uint16_t)(hh ^ b)) : "memory");
+                            uint32_t ent = hh ^ b;
+                            if (INTERACT) ent |= ((uint32_t)(Pw >> (32 * half)) >> b & 1u) << 15;
+                            asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((uint16_t)ent) : "memory");
                         }
                     }
                 } else {                    // list the front voxels pass0 .. pass0 + kFrontCap - 1
@@ -441,7 +451,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                             const uint32_t b = 31u - __clz(m);
                             m ^= 1u << b;
                             if (off - pass0 < (uint32_t)kFrontCap)
-                                asm volatile("st.shared.u16 [%0], %1;" ::"r"(flist_addr + 2u * (off - pass0)), "h"((uint16_t)(hh ^ b)) : "memory");
+                            {
+                                uint32_t ent = hh ^ b;
+                                if (INTERACT) ent |= ((uint32_t)(Pw >> (32 * half)) >> b & 1u) << 15;
+                                asm volatile("st.shared.u16 [%0], %1;" ::"r"(flist_addr + 2u * (off - pass0)), "h"((uint16_t)ent) : "memory");
+                            }
                         }
                     }
                 }
@@ -462,7 +476,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                     // the nine rows of the neighbourhood: one window each, aligned so that x+1, x, x-1 are bits 31..29 (a multiply:
                     // FMA pipe) and pushed into the mask three bits at a time (row dz = +1, dy = +1 first):
                     // bit 9(dz+1) + 3(dy+1) + (dx+1) = not void
-                    const uint32_t wa = win_addr + ((v >> 2) & 0xFFFCu) - 4u * kWin * 11u;
+                    const uint32_t wa = win_addr + ((v >> 2) & 0x0FFCu) - 4u * kWin * 11u;
                     const uint32_t mult = 1u << (v & 15u);
                     uint32_t nb27 = 0;
 #define LIETS_ROW(E) nb27 = __funnelshift_l(mul_lo_u32(lds_u32_at<4 * kWin * (((E) / 3) * 10 + (E) % 3)>(wa), mult), nb27, 3)
@@ -495,7 +509,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                 // the nine rows of the neighbourhood: one window each, aligned so that x+1, x, x-1 are bits 31..29 (a multiply:
                 // FMA pipe) and pushed into the mask three bits at a time (row dz = +1, dy = +1 first):
                 // bit 9(dz+1) + 3(dy+1) + (dx+1) = not void
-                const uint32_t wa = win_addr + ((v >> 2) & 0xFFFCu) - 4u * kWin * 11u;
+                const uint32_t wa = win_addr + ((v >> 2) & 0x0FFCu) - 4u * kWin * 11u;
                 const uint32_t mult = 1u << (v & 15u);
                 uint32_t nb27 = 0;
 #define LIETS_ROW(E) nb27 = __funnelshift_l(mul_lo_u32(lds_u32_at<4 * kWin * (((E) / 3) * 10 + (E) % 3)>(wa), mult), nb27, 3)
@@ -503,7 +517,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
 #undef LIETS_ROW
                 // the centre (bit 13) is solid, so ~nb27 has bit 13 clear: closing the gap is (v + (v & 0x1FFF)) >> 1
                 const uint32_t lo13 = ~nb27 & 0x1FFFu;
-                return ((~nb27 + lo13) >> 1) & en26;
+                return (~nb27 + lo13) >> 1;
             };
             constexpr uint32_t kSafeEntry = (8u * 11u) << 4;        // row (0, 0), window 0: a list entry that is always addressable
             auto level0_pair = [&](uint32_t i, uint32_t* v, uint32_t* tie, uint32_t* fire) {
@@ -514,16 +528,25 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                 uint32_t void26[2];
                 uint4 B0[2];
 #pragma unroll
-                for (int u = 0; u < 2; ++u) void26[u] = gather26(v[u]);
+                for (int u = 0; u < 2; ++u) void26[u] = gather26(v[u]) & ((INTERACT && (v[u] >> 15)) ? enI26 : en26);
                 void26[0] = live0 ? void26[0] : 0u;
                 void26[1] = live1 ? void26[1] : 0u;
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
-                    const uint32_t p = lds_u32(ptab_addr + ((v[u] >> 5) & 0x3FCu)) + ((v[u] & 0x7Fu) ^ 15u);
+                    const uint32_t p = lds_u32(ptab_addr + ((v[u] >> 5) & 0x1FCu)) + ((v[u] & 0x7Fu) ^ 15u);
                     B0[u] = philox_growth_block(p, 0u, ps, key);
                     n_items0 += void26[u] ? 1u : 0u;
                 }
-                if (h0_any) {               // some leading threshold nibble is non-zero: a draw can fire at level 0
+                if (INTERACT) {             // two kinds of sources: the voxel's own thresholds, general compare
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const uint4 hk = lds_u128(hpat_addr + (v[u] >> 15) * 128u);
+                        const uint32_t hsel[4] = { hk.x, hk.y, hk.z, hk.w };
+                        uint32_t le;
+                        level_compare(B0[u], hsel, void26[u], &le, &tie[u]);
+                        fire[u] = le & ~tie[u];
+                    }
+                } else if (h0_any) {        // some leading threshold nibble is non-zero: a draw can fire at level 0
                     if (h0_small) {
 #pragma unroll
                         for (int u = 0; u < 2; ++u) level0_compare_small(B0[u], h0cle, h0clt, h0nz, void26[u], &fire[u], &tie[u]);
@@ -557,7 +580,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                 if (h0_any) {
 #pragma unroll
                     for (int u = 0; u < 2; ++u)
-                        if (__ballot_sync(0xffffffffu, fire[u] != 0u)) claim(fire[u], (v[u] & 0x7Fu) ^ 15u, (v[u] >> 7) & 0x1FFu);
+                        if (__ballot_sync(0xffffffffu, fire[u] != 0u)) claim(fire[u], (v[u] & 0x7Fu) ^ 15u, (v[u] >> 7) & 0x7Fu);
                 }
                 const uint32_t have0 = __ballot_sync(0xffffffffu, tie[0] != 0u), have1 = __ballot_sync(0xffffffffu, tie[1] != 0u);
                 if (have0 | have1) {
@@ -736,9 +759,11 @@ int grow_tile_max_batch() { return kMaxBatch; }
 // per-device function attribute, set once per context at liets_create: the SM's shared memory to the CTAs
 cudaError_t grow_tile_attributes() {
     static_assert(sizeof(Smem) <= 48 * 1024, "static shared memory");
-    cudaError_t e = cudaFuncSetAttribute(k_grow_tile<1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    cudaError_t e = cudaFuncSetAttribute(k_grow_tile<1, false>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_grow_tile<kMaxBatch>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    e = cudaFuncSetAttribute(k_grow_tile<1, true>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_grow_tile<kMaxBatch, false>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
 }
 
 template <int MAXB>
@@ -755,7 +780,8 @@ static void fill_batch(TileBatch<MAXB>* b, liets_ctx* const* ctx, int n) {
 cudaError_t launch_grow_tile(liets_ctx* c) {
     TileBatch<1> b;
     fill_batch(&b, &c, 1);
-    k_grow_tile<1><<<c->tile_grid, kThreads, 0, c->stream>>>(b, c->geom);
+    if (c->interact && c->has_blocked) k_grow_tile<1, true><<<c->tile_grid, kThreads, 0, c->stream>>>(b, c->geom);
+    else k_grow_tile<1, false><<<c->tile_grid, kThreads, 0, c->stream>>>(b, c->geom);
     c->launches++;
     return cudaGetLastError();
 }
@@ -767,7 +793,7 @@ cudaError_t grow_tile_node(liets_ctx* c, cudaGraph_t graph, cudaGraphExec_t exec
     fill_batch(&b, &c, 1);
     void* args[] = { &b, &c->geom };
     cudaKernelNodeParams p = {};
-    p.func = reinterpret_cast<void*>(k_grow_tile<1>);
+    p.func = (c->interact && c->has_blocked) ? reinterpret_cast<void*>(k_grow_tile<1, true>) : reinterpret_cast<void*>(k_grow_tile<1, false>);
     p.gridDim = dim3(c->tile_grid); p.blockDim = dim3(kThreads); p.sharedMemBytes = 0; p.kernelParams = args;
     return exec ? cudaGraphExecKernelNodeSetParams(exec, *node, &p) : cudaGraphAddKernelNode(node, graph, nullptr, 0, &p);
 }
@@ -779,7 +805,7 @@ cudaError_t grow_tile_batch_node(liets_ctx* const* ctx, int n, cudaGraph_t graph
     fill_batch(&b, ctx, n);
     void* args[] = { &b, &ctx[0]->geom };
     cudaKernelNodeParams p = {};
-    p.func = reinterpret_cast<void*>(k_grow_tile<kMaxBatch>);
+    p.func = reinterpret_cast<void*>(k_grow_tile<kMaxBatch, false>);
     p.gridDim = dim3(ctx[0]->tile_grid); p.blockDim = dim3(kThreads); p.sharedMemBytes = 0; p.kernelParams = args;
     return exec ? cudaGraphExecKernelNodeSetParams(exec, *node, &p) : cudaGraphAddKernelNode(node, graph, nullptr, 0, &p);
 }

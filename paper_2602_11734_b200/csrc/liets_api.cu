@@ -133,11 +133,12 @@ bool add_loop(liets_ctx* c, cudaGraph_t g, const cudaGraphNode_t* after, int whi
 
 bool ensure_loop_graph(liets_ctx* c) {
     if (c->loop_exec) {
-        if (c->loop_seed == c->rng_seed && c->loop_blocked == c->has_blocked) return true;
+        const bool inter = c->interact && c->has_blocked;
+        if (c->loop_seed == c->rng_seed && c->loop_blocked == c->has_blocked && c->loop_interact == inter) return true;
         cudaError_t e = c->storage == LIETS_STORAGE_U8 ? grow_u8_node(c, nullptr, c->loop_exec, &c->loop_grow_node)
                       : c->storage == LIETS_STORAGE_FULL ? grow_full_node(c, nullptr, c->loop_exec, &c->loop_grow_node)
                                                          : grow_tile_node(c, nullptr, c->loop_exec, &c->loop_grow_node);
-        if (e == cudaSuccess) { c->loop_seed = c->rng_seed; c->loop_blocked = c->has_blocked; return true; }
+        if (e == cudaSuccess) { c->loop_seed = c->rng_seed; c->loop_blocked = c->has_blocked; c->loop_interact = inter; return true; }
         cudaGetLastError();
         cudaGraphExecDestroy(c->loop_exec); cudaGraphDestroy(c->loop_graph);        // rebuild below
         c->loop_exec = nullptr; c->loop_graph = nullptr; c->loop_tried = false;
@@ -162,7 +163,7 @@ bool ensure_loop_graph(liets_ctx* c) {
         if (g) cudaGraphDestroy(g);
         return false;
     }
-    c->loop_graph = g; c->loop_exec = exec; c->loop_grow_node = grow_node; c->loop_seed = c->rng_seed; c->loop_blocked = c->has_blocked;
+    c->loop_graph = g; c->loop_exec = exec; c->loop_grow_node = grow_node; c->loop_seed = c->rng_seed; c->loop_blocked = c->has_blocked; c->loop_interact = c->interact && c->has_blocked;
     return true;
 }
 
@@ -353,6 +354,20 @@ int liets_seed(liets_ctx* c, double core_prob, int spacing_s, uint64_t rng_seed,
     LIETS_CUDA_TRY(c, cudaEventElapsedTime(&c->seed_ms, c->ev0, c->ev1));
     c->seeded = true;
     if (n_seeds_out) *n_seeds_out = c->pinned->n_solid;
+    return LIETS_OK;
+}
+
+int liets_set_interaction(liets_ctx* c, double i_face, double i_edge, double i_corner) {
+    if (!c) return LIETS_E_ARG;
+    const double I[3] = { i_face, i_edge, i_corner };
+    for (int k = 0; k < 3; ++k)
+        if (!(I[k] >= 0.0 && I[k] <= 1.0)) return fail(c, LIETS_E_ARG, "interaction probability outside [0,1]");
+    const bool on = I[0] > 0.0 || I[1] > 0.0 || I[2] > 0.0;
+    if (on && c->storage == LIETS_STORAGE_U8) return fail(c, LIETS_E_ARG, "phase interaction needs a bit-row storage (LIETS_STORAGE_TILE or _FULL)");
+    for (int k = 0; k < 3; ++k) c->RI[k] = prob_to_threshold(I[k]);
+    c->interact = (c->RI[0] | c->RI[1] | c->RI[2]) != 0;
+    LIETS_CUDA_TRY(c, launch_set_interaction(c));
+    c->seeded = false;                                      // the sources change: seed again
     return LIETS_OK;
 }
 

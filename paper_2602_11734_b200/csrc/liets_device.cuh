@@ -126,6 +126,9 @@ struct Control {
     uint32_t pend3[3];               // seeding: pending candidates after round r, at index r % 3
     uint32_t spacing_slow;           // seeding: the adjacency lists do not fit the fast resolve -> rescan rounds
     uint32_t spacing_rounds;         // seeding: rounds of the keyed-order / dense-dilation spacing (0 for the default path)
+    uint32_t interact;               // R20: cells of the earlier phases with a void neighbour are sources, with thresholds I
+    uint32_t enI26;                  // ... directions whose interaction class can fire at all
+    uint32_t hpatI[8][4];            // ... the interaction thresholds nibble by nibble, laid out like hpat (constant over the run)
     uint32_t items;                  // Philox blocks evaluated by the live step (profiling counter)
     uint32_t items0;                 // front voxels with a void target in the live step (= level-0 blocks)
     // STORAGE_TILE keeps the active set as a voxel list while it is small (grow_vox.cu) and as a tile list afterwards
@@ -330,8 +333,9 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     uint32_t mode = __ldcg(&c->mode), pending = __ldcg(&c->pending);
     const uint32_t vox_thr = __ldcg(&c->vox_thr), vox_overflow = __ldcg(&c->vox_overflow);
     uint32_t count[2];
+    const uint32_t interact = __ldcg(&c->interact);
     if (mode == 0u && !pending) { count[0] = __ldcg(&c->vox_count[0]); count[1] = __ldcg(&c->vox_count[1]); }
-    else if (mode == 2u) { count[0] = count[1] = (n_solid != 0ull) ? 1u : 0u; }      // the full-field sweep keeps no list
+    else if (mode == 2u) { count[0] = count[1] = (n_solid != 0ull || interact) ? 1u : 0u; }      // the full-field sweep keeps no list
     else { count[0] = __ldcg(&c->count[0]) + __ldcg(&c->count_back[0]); count[1] = __ldcg(&c->count[1]) + __ldcg(&c->count_back[1]); }
     const uint32_t law = __ldcg(&c->law), max_steps = __ldcg(&c->max_steps);
     uint32_t step = __ldcg(&c->step), steps_done = __ldcg(&c->steps_done), cur = __ldcg(&c->cur);
@@ -358,7 +362,7 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
     if (!(flags & kCtlForce)) {                          // stop rule, between whole steps only
         if (status != kStatusRunning) return;
         if (n_solid >= n_t) status = 0;                                      // LIETS_OK
-        else if (count[cur] == 0 || n_solid == N) status = 1;                // FRONT_EMPTY
+        else if ((count[cur] == 0 && !(interact && mode == 0u)) || n_solid == N) status = 1;   // FRONT_EMPTY (R20: the interface sources are listed with the tiles)
         else if (steps_done >= max_steps) status = 2;                        // MAX_STEPS
         if (status != kStatusRunning) { if (lead) c->status = status; return; }
     }
@@ -390,7 +394,7 @@ static __device__ __noinline__ void control_step(Control* c, uint32_t flags) {
         c->hpat[lv][w] = ((U[0] >> (28u - 4u * lv)) & 15u) * ones[0] + ((U[1] >> (28u - 4u * lv)) & 15u) * ones[1] +
                          ((U[2] >> (28u - 4u * lv)) & 15u) * ones[2];
     }
-    if (mode == 0u && (count[cur] > vox_thr || vox_overflow)) pending = 2u;  // the front has outgrown the voxel list: this step
+    if (mode == 0u && (count[cur] > vox_thr || vox_overflow || interact)) pending = 2u;  // the front has outgrown the voxel list: this step
                                                                              // runs on tiles (2: handed over in this very call)
     if (lead) {
         c->en26 = en26;

@@ -65,6 +65,8 @@ struct liets_ctx {
     bool seeded, has_target, growth_set;
     uint64_t rng_seed;
     uint64_t R[3];
+    uint64_t RI[3];                   // R20: interaction thresholds per class (all 0: off)
+    bool interact;
     int law;
     uint64_t n_t;
     float seed_ms, gen_ms;
@@ -78,6 +80,7 @@ struct liets_ctx {
     cudaGraphNode_t loop_grow_node;
     uint64_t loop_seed;               // rng_seed whose Philox key the graph's growth node holds
     bool loop_blocked;                // ... and whether it holds the blocked-cell plane
+    bool loop_interact;               // ... and whether its growth node is the interacting variant (R20)
     bool loop_tried;                  // graph creation attempted (on failure generate keeps enqueueing batches)
     char err[256];
 };
@@ -115,6 +118,7 @@ constexpr size_t kControlScalarBytes = offsetof(Control, log_front);
 cudaError_t launch_control(liets_ctx* c, uint32_t flags);
 cudaError_t launch_begin(liets_ctx* c, int generate, uint32_t max_steps);
 cudaError_t launch_set_params(liets_ctx* c);
+cudaError_t launch_set_interaction(liets_ctx* c);
 cudaError_t launch_eq1_thresholds(const unsigned long long* dev_in, unsigned long long* dev_out, uint32_t n, cudaStream_t stream);
 cudaError_t control_loop_node(liets_ctx* c, cudaGraph_t graph, cudaGraphNode_t after, cudaGraphConditionalHandle loop,
                               cudaGraphNode_t* node);

@@ -19,7 +19,7 @@ SPACING_SPARSE, SPACING_DENSE = 0, 1
 
 # every symbol include/liets.h declares
 EXPORTS = ("liets_workspace_bytes", "liets_create", "liets_set_growth", "liets_seed", "liets_seed_explicit",
-           "liets_set_target", "liets_set_blocked", "liets_step", "liets_generate", "liets_grid", "liets_s2", "liets_s2_static", "liets_step_log", "liets_timings",
+           "liets_set_target", "liets_set_blocked", "liets_set_interaction", "liets_step", "liets_generate", "liets_grid", "liets_s2", "liets_s2_static", "liets_step_log", "liets_timings",
            "liets_set_profiling", "liets_step_times", "liets_launch_count", "liets_seed_info", "liets_set_spacing", "liets_spacing_rounds",
            "liets_create_batch", "liets_batch_ctx", "liets_generate_batch", "liets_destroy_batch",
            "liets_batch_last_error", "liets_debug_spacing_ring", "liets_debug_vox_list", "liets_debug_thresholds", "liets_probe", "liets_destroy", "liets_last_error")
@@ -73,6 +73,8 @@ def lib():
     L.liets_grid.restype = ci
     L.liets_s2.argtypes = [vp, ci, ci, P(u64), P(u64)]
     L.liets_s2.restype = ci
+    L.liets_set_interaction.argtypes = [vp, dbl, dbl, dbl]
+    L.liets_set_interaction.restype = ci
     L.liets_set_spacing.argtypes = [vp, ci, ci]
     L.liets_set_spacing.restype = ci
     L.liets_spacing_rounds.argtypes = [vp, P(u32)]
@@ -205,6 +207,10 @@ class Liets:
         n = ctypes.c_uint64(0)
         self._check(self._L.liets_seed(self._h, core_prob, spacing_s, rng_seed, ctypes.byref(n)))
         return int(n.value)
+
+    def set_interaction(self, i_face, i_edge, i_corner):
+        """Growth at the interface with the earlier phases (set_blocked) with probabilities I per class; seed again afterwards."""
+        self._check(self._L.liets_set_interaction(self._h, i_face, i_edge, i_corner))
 
     def set_spacing(self, order=ORDER_INDEX, method=SPACING_SPARSE):
         """Variant of the spacing filter used by the next seed(): acceptance order and sparse / dense mechanism."""
