@@ -5,7 +5,7 @@
  * The calls follow the paper's statement of the problem (PAPER.md:38-39 seeding and growth,
  * :110-116 / Algorithm 3 :133-169 the list-indexed step, :122 seed spacing, Eq. (1) :126 the
  * volume-fraction dependent growth probability, :140 the stopping rule).  Readings of points
- * where the paper is silent are listed in DESIGN.md ("Readings", R1..R19).
+ * where the paper is silent are listed in DESIGN.md ("Readings", R1..R20).
  *
  * Conventions
  *   - Every call returns >= 0 (a status) or < 0 (an error); nothing throws or aborts across the
