@@ -109,7 +109,7 @@ int liets_set_blocked(liets_ctx* ctx, const void* mask, size_t mask_bytes, int f
  * taken with the phase-interaction probability I of d's class (face, edge, corner; constant over the run, the same keyed
  * draw of (p, t, d) compared with I instead of G).  The cells of the earlier phases that have a void neighbour are sources
  * beside the phase's own front; they keep their cells.  0, 0, 0 (the default) switches it off: independent phases (R18).
- * Bit-row storages only (E_ARG for LIETS_STORAGE_U8); batches run without it.  Seed again afterwards (E_STATE until
+ * Bit-row storages only (E_ARG for LIETS_STORAGE_U8); liets_generate_batch refuses such a grid (E_ARG).  Seed again afterwards (E_STATE until
  * then); a run with interaction keeps its active set as tiles from the first step. */
 int liets_set_interaction(liets_ctx* ctx, double i_face, double i_edge, double i_corner);
 

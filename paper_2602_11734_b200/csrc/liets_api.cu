@@ -692,6 +692,7 @@ int liets_generate_batch(liets_batch* b, const double* target_solid_fraction, ui
         liets_ctx* c = b->ctx[i];
         if (!(target_solid_fraction[i] > 0.0 && target_solid_fraction[i] <= 1.0)) { snprintf(b->err, sizeof(b->err), "target solid fraction of grid %d outside (0,1]", i); return LIETS_E_ARG; }
         if (!c->seeded) { snprintf(b->err, sizeof(b->err), "liets_generate_batch before liets_seed of grid %d", i); return LIETS_E_STATE; }
+        if (c->interact && c->has_blocked) { snprintf(b->err, sizeof(b->err), "grid %d: phase interaction (liets_set_interaction) is not provided in batches", i); return LIETS_E_ARG; }
     }
     LIETS_BATCH_TRY(b, cudaEventRecord(b->ev0, b->stream));
     for (int i = 0; i < b->n; ++i) {

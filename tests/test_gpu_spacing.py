@@ -99,3 +99,28 @@ def test_spacing_variant_arguments(liets):
     with pytest.raises(liets.LietsError) as e:
         T.seed(0.1, 3, 1)
     assert e.value.code == liets.E_CAPACITY
+
+
+def test_spacing_variants_and_interaction_inside_a_batch(liets):
+    """The generators of a batch take the spacing variants like any other; a grid with phase interaction is refused."""
+    dims = (96, 40, 24)
+    B = liets.LietsBatch(3, *dims)
+    singles = []
+    for i, (order, method) in enumerate(((0, 0), (1, 0), (0, 1))):
+        for L in (B[i], liets.Liets(*dims, 0, 1)):
+            L.set_spacing(order, method)
+            L.set_growth(0.08, 0.03, 0.01, liets.LAW_EQ1)
+            n = L.seed(0.01, 5, 40 + i)
+        singles.append(L)
+        assert B[i].seed_info()[0] == L.seed_info()[0] and n > 0
+    res = B.generate(0.4)
+    for i, L in enumerate(singles):
+        rc, steps, n_solid = L.generate(0.4)
+        assert (rc, steps, n_solid) == tuple(res[i]) and (B[i].grid() == L.grid()).all()
+    m = singles[0].grid().ravel()
+    B[1].set_blocked(m)
+    B[1].set_interaction(0.1, 0.0, 0.0)
+    B[1].seed(0.01, 5, 41)
+    with pytest.raises(liets.LietsError) as e:
+        B.generate(0.4)
+    assert e.value.code == liets.E_ARG
