@@ -14,8 +14,13 @@
  * full-field definition == the list algorithm; binomial acceptance rates; one-step claim
  * probability.  "Parity unpinned" (conventions of this repo that the paper does
  * not fix, so nothing outside the repo can pin them): the Philox counter layout (R9), the
- * rounding of phi_s*N to n_t (R7), the rounding of probabilities to 32-bit thresholds (R8) and
- * the ascending-index acceptance order of seed spacing (R12).
+ * rounding of phi_s*N to n_t (R7), the rounding of probabilities to 32-bit thresholds (R8),
+ * the ascending-index acceptance order of seed spacing (R12), the key of the optional keyed
+ * acceptance order (R19: word v % 4 of the Philox block at counter (v / 4, 0, 1, 2^32 - 1)) and
+ * which of the two statements of PAPER.md:40 step 4 about interacting phases is meant (R20: the
+ * growing phase takes unassigned cells only, also at its interface with the earlier phases, with
+ * the probability I of the direction's class).  Further pins: P5d (seeding by literal dilation
+ * passes), P5k (the keyed order against an independent greedy), the closed forms of R20.
  */
 #ifndef LIETS_ORACLE_H
 #define LIETS_ORACLE_H
