@@ -16,17 +16,20 @@
 //   B  front voxels: solid cells with a void neighbour, 64 cells per bit operation;
 //      their ids are compacted into a shared-memory list (popc + CTA-wide prefix sum).  A list entry is
 //      (15 - (x & 15)) | (8 row + x / 16) << 4: the shift count and the window index, ready to use
-//   C  one thread per front voxel: its 26 void-target bits (Algorithm 3 lines 5-6) from nine window loads, each
-//      aligned by one multiply and pushed into the mask by one funnel shift; ONE Philox4x32-10 block = the
-//      leading nibble of all 26 draws (R9), one carry-free per-nibble compare = the directions that fire or tie
-//      with the threshold (line 8); voxels with hits or ties go to a per-warp queue
-//   D  one lane per queued voxel: its hits are set in a shared-memory claim volume (atomicOr); for tied
-//      directions the next block decides, one direction at a time (there is almost always exactly one)
+//   C  one thread per front voxel, two consecutive list entries per thread in one branch-free block: the voxel's 26
+//      void-target bits (Algorithm 3 lines 5-6) from nine window loads, each aligned by one multiply and pushed into the
+//      mask by one funnel shift; ONE Philox4x32-10 block = the leading nibble of all 26 draws (R9), one carry-free
+//      per-nibble compare (zero test / thresholds below 8 / general, chosen per launch) = the directions that fire or tie
+//      with the threshold (line 8); level-0 hits go to a shared-memory claim volume, ties to a per-warp ring
+//   D  one lane per ring entry and nibble level: the next block decides all tied directions of the voxel at once; a
+//      round runs as soon as 32 entries wait, the few left at the tile's end are resolved two levels per round
 //   E  claim + compact: own rows are OR-ed into G[next] together with the carried state, halo hits
-//      go to the neighbour tiles' rows with atomicOr; the returned old word tells who flipped the bit
-//      (line 9-10, "counted once" PAPER.md:77) for the solid count; a per-tile step stamp
+//      go to the neighbour tiles' rows with atomicOr (all of a row's atomics in one batch); the returned old word tells
+//      who flipped the bit (line 9-10, "counted once" PAPER.md:77) for the solid count; a per-tile step stamp
 //      (atomicMax) makes every tile enter the next list exactly once; tiles without front voxels
 //      are not re-emitted (lazy retirement).
+// With INTERACT (liets_set_interaction, R20) the cells of earlier phases that have a void neighbour are front
+// voxels too (bit 15 of their list entry), compared against the interaction thresholds.
 #include "liets_host.h"
 
 namespace liets {
@@ -40,12 +43,6 @@ constexpr int kThreads = 128;
 #endif
 constexpr int kCtasPerSm = LIETS_TILE_CTAS;       // resident CTAs per SM the kernel is compiled for (registers) and launched with
 constexpr int kWarps = kThreads / 32;
-#ifdef LIETS_OLD_C
-#ifndef LIETS_VOX_PER_THREAD
-#define LIETS_VOX_PER_THREAD 2
-#endif
-constexpr int kVoxPerThread = LIETS_VOX_PER_THREAD;     // front voxels a thread handles per trip of phase C
-#endif
 constexpr int kMaxBatch = 16;                   // grids per launch of the batched kernel (kernel parameters: 2.2 KB)
 constexpr int kRowWords = kTileW + 2;           // left halo word | tile words | right halo word
 constexpr int kWin = 64 * kTileW / 16;          // 18-bit windows per row, one per 16 voxels
@@ -462,44 +459,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
             }
             __syncthreads();                // flist (and win) complete
             const uint32_t n_pass = min((uint32_t)kFrontCap, n_front - pass0);
-#ifdef LIETS_OLD_C
-            // C: one thread per front voxel, kVoxPerThread voxels per thread and trip (their Philox chains interleave, the loop
-            // and ring bookkeeping is shared)
-            auto level0 = [&](uint32_t i, uint32_t& v, uint32_t& tie, uint32_t& fire) {
-                tie = 0; fire = 0; v = 0;
-                if (i < n_pass) {
-                    {
-                        uint16_t v16;
-                        asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v16) : "r"(flist_addr + 2u * i) : "memory");
-                        v = v16;
-                    }
-                    // the nine rows of the neighbourhood: one window each, aligned so that x+1, x, x-1 are bits 31..29 (a multiply:
-                    // FMA pipe) and pushed into the mask three bits at a time (row dz = +1, dy = +1 first):
-                    // bit 9(dz+1) + 3(dy+1) + (dx+1) = not void
-                    const uint32_t wa = win_addr + ((v >> 2) & 0x0FFCu) - 4u * kWin * 11u;
-                    const uint32_t mult = 1u << (v & 15u);
-                    uint32_t nb27 = 0;
-#define LIETS_ROW(E) nb27 = __funnelshift_l(mul_lo_u32(lds_u32_at<4 * kWin * (((E) / 3) * 10 + (E) % 3)>(wa), mult), nb27, 3)
-                    LIETS_ROW(8); LIETS_ROW(7); LIETS_ROW(6); LIETS_ROW(5); LIETS_ROW(4); LIETS_ROW(3); LIETS_ROW(2); LIETS_ROW(1); LIETS_ROW(0);
-#undef LIETS_ROW
-                    // the centre (bit 13) is solid, so ~nb27 has bit 13 clear: closing the gap is (v + (v & 0x1FFF)) >> 1
-                    const uint32_t lo13 = ~nb27 & 0x1FFFu;
-                    const uint32_t void26 = ((~nb27 + lo13) >> 1) & en26;
-                    if (void26) {
-                        const uint32_t p = lds_u32(ptab_addr + ((v >> 5) & 0x3FCu)) + ((v & 0x7Fu) ^ 15u);
-                        const uint4 B0 = philox_growth_block(p, 0u, ps, key);
-                        ++n_items0;
-                        if (h0_any) {       // some leading threshold nibble is non-zero: a draw can fire at level 0
-                            uint32_t le;
-                            level0_compare(B0, h0, h0m, h08, void26, &le, &tie);
-                            fire = le & ~tie;
-                        } else {            // all leading nibbles are 0: "<=" and "==" coincide with "== 0"
-                            tie = level_zero(B0, void26);
-                        }
-                    }
-                }
-            };
-#else
             // C: front voxels, two CONSECUTIVE list entries per thread and trip (one 32-bit load), worked without a branch in
             // one basic block: the two Philox chains interleave and share the round keys.  A warp covers 64 entries, so the
             // test that skips a warp beyond the list's end is warp-uniform; a lane beyond the end works on a harmless
@@ -563,18 +522,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                     for (int u = 0; u < 2; ++u) tie[u] = level_zero(B0[u], void26[u]);
                 }
             };
-#endif
-#ifdef LIETS_OLD_C
-            auto settle = [&](uint32_t v, uint32_t tie, uint32_t fire) {       // level-0 hits to the claim volume, ties to the ring
-                if (h0_any && __ballot_sync(0xffffffffu, fire != 0u)) claim(fire, (v & 0x7Fu) ^ 15u, (v >> 7) & 0x1FFu);
-                const uint32_t have = __ballot_sync(0xffffffffu, tie != 0u);
-                if (have) {
-                    if (qn + 32u > (uint32_t)kQueueCap) do round(32u); while (qn >= 32u);
-                    if (tie) sts_u64(queue_addr + 8u * ((qh + qn + __popc(have & lanes_below)) & ((uint32_t)kQueueCap - 1u)), v | (1u << 16), tie);
-                    qn += __popc(have);
-                }
-            };
-#else
             // level-0 hits to the claim volume, ties to the ring: both entries of the pair behind one capacity test
             auto settle2 = [&](const uint32_t* v, const uint32_t* tie, const uint32_t* fire) {
                 if (h0_any) {
@@ -592,24 +539,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_grow_tile(const __grid
                     qn += n0 + __popc(have1);
                 }
             };
-#endif
-#ifdef LIETS_OLD_C
-            for (uint32_t i0 = 0; i0 < n_pass; i0 += kVoxPerThread * kThreads) {
-                uint32_t v[kVoxPerThread], tie[kVoxPerThread], fire[kVoxPerThread];
-#pragma unroll
-                for (int u = 0; u < kVoxPerThread; ++u) level0(i0 + (uint32_t)u * kThreads + tid, v[u], tie[u], fire[u]);
-#pragma unroll
-                for (int u = 0; u < kVoxPerThread; ++u) settle(v[u], tie[u], fire[u]);
-            }
-        }
-#else
             for (uint32_t i0 = 0; i0 < n_pass; i0 += 2u * kThreads) {
                 uint32_t v[2] = { 0u, 0u }, tie[2] = { 0u, 0u }, fire[2] = { 0u, 0u };
                 if (i0 + 64u * warp < n_pass) level0_pair(i0 + 2u * tid, v, tie, fire);     // warp-uniform
                 settle2(v, tie, fire);
             }
         }
-#endif
         while (qn >= 32u) round(32u);
         while (qn) round2(qn);              // fewer than 32 entries left
         if (tid == 0) { S.tile[(kt + 1u) & 1u] = next_li; S.tile_id[(kt + 1u) & 1u] = next_id; }   // read after the next barrier but one
